@@ -1,0 +1,276 @@
+#!/usr/bin/env python
+"""bench.py -- two-component D3Q19 MLUPS on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+A "step" is one pass of the whole hot path (SURVEY.md §8a rows a0-a7 except on-demand
+diagnostics) over all fluid nodes of the workload.  Default workload: BASELINE.json config 4, the
+256^3 sandstone-like mask the north_star quotes its roofline target on.  Inputs are seeded and
+synthetic (workloads/generators.py); they stand in for the paper's Bentheimer image.
+
+N > 1: the path is single-GPU by the north_star ("no sharding"): ranks run independent replicas
+(DESIGN.md "Multi-GPU: replicas only"), no data-path collective; value = all ranks' updates / max
+time over ranks.
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the
+same workload on the host cores; it is a deliberately slow program, reported as a baseline.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+BYTES_PER_UPDATE_STEP = 472      # 3 x 152 B populations + 8 B psi write + 8 B read
+BYTES_PER_UPDATE_COLLIDE = 312   # fused pass alone: 152 read + 8 psi + 152 write
+BYTES_PER_UPDATE_DENSITY = 160   # density pass alone: 152 read + 8 write
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--size", type=int, default=None, help="override the box edge (debugging)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            with open(path) as fh:
+                return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def workload(args):
+    from workloads import make_config
+    c = make_config(args.config, size=args.size)
+    if args.config in (1,):
+        c["params"]["storage_bits"] = 32  # throughput is quoted on the fp32 production build
+    return c
+
+
+def cpu_sample(cfg, edge=128):
+    """Bounded sample of the workload for the CPU oracle: the leading edge^3 corner of the same
+    mask and state (end layers re-cleared when z is open so the crop is a valid open box)."""
+    m = cfg["mask"]
+    e = min(edge, m.shape[0])
+    sl = (slice(0, e),) * 3
+    mask = np.ascontiguousarray(m[sl]).copy()
+    rA = np.ascontiguousarray(cfg["rhoA"][sl]).copy()
+    rB = np.ascontiguousarray(cfg["rhoB"][sl]).copy()
+    if cfg["params"]["z_open"] and e < m.shape[0]:
+        rA[-8:] = np.where(mask[-8:] == 0, rA[-8:], rA[-9].max())
+        rB[-8:] = np.where(mask[-8:] == 0, rB[-8:], rB[-9].min())
+        mask[-8:] = 0
+    return mask, rA, rB, f"leading {e}^3 corner of the {m.shape[0]}^3 mask"
+
+
+def time_oracle(cfg, steps, warmup, budget_s=25.0):
+    from oracle import LbmRef, threads
+    mask, rA, rB, what = cpu_sample(cfg)
+    p = dict(cfg["params"])
+    o = LbmRef(mask, p)
+    o.set_density(rA, rB)
+    t0 = time.perf_counter()
+    o.step(max(1, warmup))
+    per = (time.perf_counter() - t0) / max(1, warmup)
+    n = steps if steps is not None else max(1, min(20, int(budget_s / max(per, 1e-3))))
+    t0 = time.perf_counter()
+    o.step(n)
+    dt = time.perf_counter() - t0
+    mlups = o.num_fluid * n / dt / 1e6
+    return dict(value=mlups, unit="MLUPS", cores=threads(), kind="oracle",
+                sample=f"{what}: {o.num_fluid} fluid nodes x {n} steps, fp64 dense, OpenMP",
+                ms_per_step=1e3 * dt / n, steps=n)
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.samples, self.reasons, self.max_mhz = index, False, [], set(), None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def result(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, on the host cores, rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    cfg = workload(args)
+    steps = args.steps if args.steps is not None else None
+    warm = args.warmup if args.warmup is not None else 1
+    r = time_oracle(cfg, steps, warm)
+    line = {"impl": "reference", "metric": "two_component_d3q19_mlups", "value": r["value"],
+            "unit": "MLUPS", "n_gpus": args.gpus, "steps": r["steps"], "warmup": warm,
+            "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "sample": r["sample"]},
+            "cpu_baseline": {"value": r["value"], "unit": "MLUPS", "cores": r["cores"],
+                             "kind": "oracle", "sample": r["sample"]},
+            "e2e": {"value": r["value"], "unit": "MLUPS", "h2d_bytes_per_step": 0,
+                    "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2207_01534_b200 import Lbm
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    K = args.steps if args.steps is not None else 500
+    W = args.warmup if args.warmup is not None else 20
+    cfg = workload(args)
+    sim = Lbm(cfg["mask"], cfg["params"])
+    sim.set_density(cfg["rhoA"], cfg["rhoB"])
+    nf = sim.num_fluid
+    mem = sim.memory_bytes()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K steps between events
+    sim.step(W)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    sim.step(K)
+    e1.record()
+    barrier()
+    sampler.stop_flag = True
+    sampler.join()
+    ms = torch.tensor([e0.elapsed_time(e1)], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_total = float(ms.item())
+    _, launches = sim.last_step_profile()
+    mass, _ = sim.diagnostics()          # fails loudly on a non-finite state
+    value = world * nf * K / (ms_total * 1e-3) / 1e6
+
+    # ---- per-kernel durations: a second pass of K steps with CUDA events around every launch
+    sim.set_profiling(True)
+    sim.step(K)
+    kms, _ = sim.last_step_profile()
+    sim.set_profiling(False)
+    peak, peak_src = measured_peaks()
+    t_col = kms["collide_stream"] / K * 1e-3
+    achieved = BYTES_PER_UPDATE_COLLIDE * nf / t_col / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_collide_stream", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": BYTES_PER_UPDATE_COLLIDE * nf,
+                "kernel_ms_per_launch": {k: v / K for k, v in kms.items()},
+                "step_algorithmic_gbs": BYTES_PER_UPDATE_STEP * nf / (ms_total / K * 1e-3) / 1e9,
+                "step_frac_of_peak": BYTES_PER_UPDATE_STEP * nf / (ms_total / K * 1e-3) / 1e9 / peak,
+                "step_frac_of_8TBs": BYTES_PER_UPDATE_STEP * nf / (ms_total / K * 1e-3) / 1e9 / 8000.0}
+
+    # ---- end to end through the public API with HOST buffers: upload the initial state, run
+    # K steps, download both density fields; copies are inside the timed region.
+    e2e = None
+    if not args.no_e2e:
+        out = {k: np.empty(cfg["mask"].shape, np.float64) for k in ("rhoA", "rhoB")}
+        barrier()
+        t0 = time.perf_counter()
+        sim.set_density(cfg["rhoA"], cfg["rhoB"])
+        sim.step(K)
+        sim.get_macroscopic(fields=("rhoA", "rhoB"), out=out)
+        torch.cuda.synchronize()
+        dt = torch.tensor([time.perf_counter() - t0], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        nbytes = 2 * cfg["mask"].size * 8
+        e2e = {"value": world * nf * K / float(dt.item()) / 1e6, "unit": "MLUPS",
+               "h2d_bytes_per_step": nbytes / K, "d2h_bytes_per_step": nbytes / K,
+               "job": f"lbm_set_density (host f64) + lbm_step({K}) + lbm_get_macroscopic(rhoA,rhoB)"
+                      f" to host; {nbytes} B each way per job"}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        r = time_oracle(cfg, None, 1)
+        cpu = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+
+    if rank == 0:
+        line = {"metric": "two_component_d3q19_mlups", "value": value, "unit": "MLUPS",
+                "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_total / K,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32" if cfg["params"]["storage_bits"] == 32 else "f64",
+                "data": "synthetic",
+                "config": {"workload": cfg["name"], "box": list(cfg["mask"].shape[::-1]),
+                           "fluid_nodes": nf, "wall_solid_nodes": sim.num_wall_solid,
+                           "porosity": cfg["porosity"], "parallelism": f"replicas x{world}",
+                           "l2": "populations (2 x %.0f MB) exceed the 126 MB L2; no flush needed"
+                                 % (mem["populations"] / 2e6),
+                           "device_bytes": mem},
+                "clocks": sampler.result(), "e2e": e2e, "gpu_launches": launches,
+                "roofline": roofline, "cpu_baseline": cpu,
+                "mass_check": [float(mass[0]), float(mass[1])]}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

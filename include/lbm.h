@@ -1,0 +1,130 @@
+/* lbm.h -- C ABI of the B200-native two-component pseudopotential D3Q19 lattice Boltzmann step
+ * of arXiv 2207.01534 (Eq. 1-15, boundary treatment PAPER.md L107-113 / L147-157).
+ *
+ * One lbm_ctx is one simulation on one GPU (the current CUDA device at lbm_create time).
+ * Every step of the hot path runs in hand-written sm_100a kernels;
+ * PyTorch is used only for device memory (its CUDA caching allocator) and for the stream
+ * (torch's current CUDA stream).  There is NO CPU fallback: without a CUDA device lbm_create
+ * fails with LBM_ECUDA.
+ *
+ * Conventions
+ *  - All pointers are HOST pointers unless a parameter says "device".  The caller owns every
+ *    host buffer; the library copies during the call and never retains a caller pointer.  The
+ *    library owns all device memory and releases it in lbm_destroy.
+ *  - Dense arrays are indexed idx = x + nx*(y + ny*z) (x fastest).  Values at solid voxels are
+ *    written as 0 on output and ignored on input.
+ *  - Populations use the canonical D3Q19 order (reading R1 of PAPER.md
+ *    L65-67, whose velocity table is missing):
+ *      0:(0,0,0) 1:(+,0,0) 2:(-,0,0) 3:(0,+,0) 4:(0,-,0) 5:(0,0,+) 6:(0,0,-) 7:(+,+,0) 8:(-,+,0)
+ *      9:(+,-,0) 10:(-,-,0) 11:(+,0,+) 12:(-,0,+) 13:(+,0,-) 14:(-,0,-) 15:(0,+,+) 16:(0,-,+)
+ *      17:(0,+,-) 18:(0,-,-);  w = 1/3, 1/18 (1-6), 1/36 (7-18)
+ *  - Every function returns LBM_OK (0) or a negative LBM_E* code; no C++ exception crosses the
+ *    ABI; lbm_last_error() returns a thread-local message for the last failure.
+ *  - x and y are always periodic; z is periodic (z_open=0) or carries an inlet plane z=0 and an
+ *    outlet plane z=nz-1 (z_open=1).  Walls are solid voxels of the mask.
+ *  - lbm_step is asynchronous (enqueued on torch's current CUDA stream); every getter and
+ *    diagnostic synchronises that stream before returning.
+ */
+#ifndef LBM_B200_H
+#define LBM_B200_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  LBM_OK = 0,
+  LBM_EINVAL = -1,   /* NULL pointer, bad size, tau <= 1/2, bad enum value, bad z-range           */
+  LBM_ENOFLUID = -2, /* the mask has no fluid voxel (or the z-range of a query has none)          */
+  LBM_ESOLIDOPEN = -3, /* z_open=1 and a solid voxel lies on z in {0,1,nz-2,nz-1} (reading R12)   */
+  LBM_ENOMEM = -4,   /* host or device allocation failed                                          */
+  LBM_ECUDA = -5,    /* CUDA runtime error, or no CUDA device                                     */
+  LBM_ENONFINITE = -6 /* a diagnostic found a non-finite state                                    */
+};
+
+typedef struct lbm_ctx lbm_ctx; /* opaque */
+
+/* Parameters (plain data, copied by lbm_create). */
+typedef struct {
+  double G;          /* G_coh of Eq. (11)/(13); positive = inter-component
+                        repulsion; the same value couples fluid-fluid and fluid-solid (L124)     */
+  double tau[2];     /* tau^(sigma) of Eq. (7), each > 1/2 (reading R2)            */
+  double xi;         /* wettability: chi_1 = 1+xi, chi_2 = 1-xi               */
+  double accel[3];   /* g; body force F^b_sigma = rho_sigma g (reading R8)        */
+  int z_open;        /* 0: periodic in z.  1: inlet plane z=0, outlet plane z=nz-1               */
+  int inlet_kind;    /* 1: density Dirichlet (NEEM), 2: velocity Dirichlet (NEEM); L149, L223    */
+  int inlet_comp;    /* component (0 or 1) that receives the Dirichlet condition at the inlet;
+                        the other keeps its inward populations frozen        */
+  double inlet_rho;  /* density imposed when inlet_kind == 1                                     */
+  double inlet_uz;   /* velocity imposed when inlet_kind == 2                                    */
+  int outlet_kind;   /* 1: density Dirichlet (NEEM)                                              */
+  int outlet_comp;
+  double outlet_rho;
+  int storage_bits;  /* 64: fp64 storage and arithmetic (validation build);
+                        32: fp32 storage and arithmetic (production build)                       */
+  int half_force;    /* 1: u_eq carries F/2 (reading R3); 0: literal Eq. (4) (negative control)  */
+} lbm_params;
+
+/* Build a simulation from a geometry mask (binary rock image).
+ *  solid: nx*ny*nz bytes, nonzero = solid.  Classifies voxels, compacts the fluid nodes,
+ *  builds the neighbour index, allocates and uploads.  Populations start at zero: call
+ *  lbm_set_density or lbm_set_populations next.  *out is written only on success. */
+int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, const lbm_params* p);
+void lbm_destroy(lbm_ctx* c); /* NULL is allowed */
+
+/* f_i^sigma = w_i * rho_sigma (reading R11); dense double arrays of nx*ny*nz.  Also records the
+ * frozen inlet/outlet populations (reading R27). */
+int lbm_set_density(lbm_ctx* c, const double* rhoA, const double* rhoB);
+/* Checkpoint interface: dense [19][nz][ny][nx] doubles of one component, canonical order. */
+int lbm_set_populations(lbm_ctx* c, int comp, const double* f);
+int lbm_get_populations(lbm_ctx* c, int comp, double* f);
+/* Change the imposed inlet value (density or velocity, by inlet_kind) and the outlet density
+ * between steps (pressure ramps of PAPER.md L223). */
+int lbm_set_boundary(lbm_ctx* c, double inlet_value, double outlet_rho);
+
+/* Advance n time steps (SURVEY.md §8c steps 1-7 per step): density pass (Eq. 3), virtual solid
+ * density (Eq. 14-15), forces (Eq. 10, 11, 13), tau_s and u_eq (Eq. 5-8), collision (Eq. 1, 2,
+ * 9), streaming with halfway bounce-back, open-plane fix (L147-157).
+ * Asynchronous; n >= 0. */
+int lbm_step(lbm_ctx* c, int n);
+int lbm_sync(lbm_ctx* c);
+
+/* rho_sigma (Eq. 3), u = u_eq (Eq. 8) and P (Eq. 12, reading R13) of the current
+ * state; any output pointer may be NULL. */
+int lbm_get_macroscopic(lbm_ctx* c, double* rhoA, double* rhoB, double* ux, double* uy,
+                        double* uz, double* P);
+/* mass[sigma] = sum_x rho_sigma; momentum = sum_x sum_sigma sum_i e_i f_i (bare). fp64 sums in
+ * a fixed order (deterministic). */
+int lbm_diagnostics(lbm_ctx* c, double mass[2], double momentum[3]);
+/* Saturation of component comp in z in [z0,z1): fraction of fluid nodes with rho_comp greater
+ * than the other density (tie -> component 1) (reading R14). */
+int lbm_saturation(lbm_ctx* c, int comp, int z0, int z1, double* S);
+/* Trapped volume (reading R15): phase-comp nodes in [z0,z1) whose 6-connected same-phase
+ * cluster (periodic in x,y; not across z) touches neither z=0 nor z=nz-1. */
+int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, double* mass);
+
+long long lbm_num_fluid(lbm_ctx* c);       /* N_f, or -1 */
+long long lbm_num_wall_solid(lbm_ctx* c);  /* N_w: solid voxels with >= 1 fluid D3Q19 neighbour */
+/* Device bytes the context holds, split as [0] populations, [1] psi, [2] index tables, [3] other. */
+int lbm_memory_bytes(lbm_ctx* c, long long bytes[4]);
+/* Device time (ms) of the kernels of the last lbm_step call, by kind, measured with CUDA events
+ * on the launching stream when profiling is enabled with lbm_set_profiling(c, 1):
+ * ms[0] density pass, [1] virtual-solid pass, [2] collide+stream, [3] open-plane fix; launches =
+ * number of kernel launches of that call.  Synchronises. */
+int lbm_set_profiling(lbm_ctx* c, int on);
+int lbm_last_step_profile(lbm_ctx* c, double ms[4], long long* launches);
+const char* lbm_last_error(void);
+
+/* Host-only helper (no GPU needed): builds the compact index exactly as lbm_create does and
+ * returns it for inspection.  vox2id (nx*ny*nz int32, caller-allocated): fluid id in [0,N_f),
+ * N_f + wall id for wall solids, -1 for buried solids.  nbr (18*N_f int32, caller-allocated,
+ * may be NULL; pass capacity in nbr_cap as a count of int32): nbr[(i-1)*N_f + n] for direction
+ * i = 1..18: id of x+e_i (fluid id, or N_f + wall id), or -(m+1) with m the mirror node when
+ * x+e_i lies beyond an open plane.  Returns N_f through *nf and N_w through *nw. */
+int lbm_build_index(const uint8_t* solid, int nx, int ny, int nz, int z_open, int32_t* vox2id,
+                    int32_t* nbr, long long nbr_cap, long long* nf, long long* nw);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

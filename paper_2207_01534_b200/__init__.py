@@ -1,0 +1,6 @@
+"""B200-native two-component pseudopotential D3Q19 lattice Boltzmann step (arXiv 2207.01534).
+
+The product is the C-ABI library `liblbm_b200.so` (include/lbm.h, csrc/); `Lbm` is its thin
+ctypes binding.  Nothing in this package imports `oracle/`.
+"""
+from .lbm import Lbm, LbmError, lbm_build_index, lbm_params, load, make_params, SYMBOLS  # noqa: F401

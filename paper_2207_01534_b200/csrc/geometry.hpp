@@ -1,0 +1,38 @@
+// geometry.hpp -- host-side classification and compaction of the voxel mask (product code;
+// shares nothing with oracle/).  See DESIGN.md "Data layout in HBM".
+//
+// Voxels are classified as fluid, wall solid (solid with >= 1 fluid D3Q19 neighbour: the only
+// solids Eq. (15) of PAPER.md L132 is ever evaluated on, reading R7) or buried solid.  Fluid
+// nodes get compact ids [0, N_f) in x-fastest raster order, wall solids ids [N_f, N_f+N_w).
+#pragma once
+#include <cstdint>
+#include <vector>
+
+namespace lbmgeo {
+
+// Direction table in the canonical order of include/lbm.h (reading R1).
+constexpr int kQ = 19;
+extern const int kE[kQ][3];
+extern const int kOpp[kQ];
+
+struct Geometry {
+  int nx = 0, ny = 0, nz = 0, z_open = 0;
+  long long nvox = 0, nf = 0, nw = 0;
+  std::vector<int32_t> vox2id;    // [nvox]  fluid id | nf + wall id | -1
+  std::vector<int32_t> node_vox;  // [nf]    voxel index of fluid node n
+  std::vector<int32_t> wall_vox;  // [nw]    voxel index of wall solid w
+  // nbr[(i-1)*nf + n], i = 1..18: id of x+e_i: fluid id, nf + wall id, or -(m+1) where m is the
+  // id of the mirror node when x+e_i lies beyond an open plane (reading R12 iv).
+  std::vector<int32_t> nbr;
+  // wall_nbr[(i-1)*nw + w]: fluid id of x_w+e_i (mirror across open planes), or -1 if not fluid.
+  std::vector<int32_t> wall_nbr;
+  // 1 / sum_i w_i (1 - phi(x_w+e_i)): the denominator of Eq. (15).
+  std::vector<double> wall_inv_den;
+};
+
+// Returns 0, or -1 bad arguments, -2 no fluid voxel, -3 solid on an open plane or its interior
+// neighbour plane (z in {0,1,nz-2,nz-1}), -4 out of memory.  `with_tables` = also fill nbr,
+// wall_nbr, wall_inv_den.
+int build(Geometry& g, const uint8_t* solid, int nx, int ny, int nz, int z_open, bool with_tables);
+
+}  // namespace lbmgeo

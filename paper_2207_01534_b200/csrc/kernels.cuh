@@ -1,0 +1,468 @@
+// kernels.cuh -- sm_100a kernels of the two-component D3Q19 pseudopotential LBM step.
+// Product code: written from PAPER.md (arXiv 2207.01534) Eq. (1)-(15); shares nothing with
+// oracle/.  Layout and byte counts: DESIGN.md "Data layout in HBM" and "Kernels".
+//
+// Storage (T = float or double):
+//   f   [2 comps][19 dirs][npad]   populations at time t (post-streaming), node id fastest
+//   psi [nf + nw] of Vec2<T>       (rho_A, rho_B) on fluid ids, (rho~_A, rho~_B) on wall ids
+//   nbr [18][npad] int32           id of x+e_i (see geometry.hpp)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace lbmk {
+
+constexpr int Q = 19;
+
+// D3Q19 in the canonical order of include/lbm.h (reading R1 of PAPER.md L65-67).
+__host__ __device__ constexpr int ex(int i) {
+  constexpr int t[Q] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
+  return t[i];
+}
+__host__ __device__ constexpr int ey(int i) {
+  constexpr int t[Q] = {0, 0, 0, 1, -1, 0, 0, 1, 1, -1, -1, 0, 0, 0, 0, 1, -1, 1, -1};
+  return t[i];
+}
+__host__ __device__ constexpr int ez(int i) {
+  constexpr int t[Q] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, 1, -1, -1, 1, 1, -1, -1};
+  return t[i];
+}
+__host__ __device__ constexpr int opp(int i) {
+  constexpr int t[Q] = {0, 2, 1, 4, 3, 6, 5, 10, 9, 8, 7, 14, 13, 12, 11, 18, 17, 16, 15};
+  return t[i];
+}
+// w_i
+template <typename T>
+__host__ __device__ constexpr T wgt(int i) {
+  return i == 0 ? T(1.0 / 3.0) : (i < 7 ? T(1.0 / 18.0) : T(1.0 / 36.0));
+}
+// the 5 directions with e_z = +1 (inward at the inlet) and with e_z = -1 (inward at the outlet)
+__host__ __device__ constexpr int inward(int plane, int k) {
+  constexpr int t[2][5] = {{5, 11, 12, 15, 16}, {6, 13, 14, 17, 18}};
+  return t[plane][k];
+}
+
+template <typename T> struct Vec2;
+template <> struct __align__(8) Vec2<float> { float a, b; };
+template <> struct __align__(16) Vec2<double> { double a, b; };
+
+template <typename T>
+struct Consts {
+  T G;            // G_coh, Eq. (11)/(13)
+  T tauA, tauB;   // Eq. (7)
+  T gx, gy, gz;   // body acceleration (R8)
+  T hf;           // 0.5 (reading R3) or 0 (literal Eq. 4)
+  T chiA, chiB;   // 1+xi, 1-xi
+};
+
+// ---------------------------------------------------------------------------------------------
+// a1  density / psi pass: rho_sigma = sum_i f_i^sigma (Eq. 3); psi = rho (L105).
+// One thread per fluid node; every load is a fully coalesced row read.
+template <typename T>
+__global__ void __launch_bounds__(256) k_density(const T* __restrict__ f, Vec2<T>* __restrict__ psi,
+                                                 int nf, size_t npad) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= nf) return;
+  T a[Q], b[Q];
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    a[i] = f[(size_t)i * npad + n];
+    b[i] = f[(size_t)(Q + i) * npad + n];
+  }
+  T ra = a[0], rb = b[0];
+#pragma unroll
+  for (int i = 1; i < Q; ++i) { ra += a[i]; rb += b[i]; }
+  Vec2<T> o; o.a = ra; o.b = rb;
+  psi[n] = o;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2  virtual solid density on wall solids (improved virtual solid density scheme):
+//   rho~_sigma(x) = chi_sigma * sum_i w_i rho_sigma(x+e_i)(1-phi(x+e_i)) / sum_i w_i (1-phi)
+// Eq. (14)-(15) PAPER.md L128-133; chi: L141-143.  wall_nbr < 0 means "not fluid".
+template <typename T>
+__global__ void __launch_bounds__(256) k_wallpsi(Vec2<T>* __restrict__ psi,
+                                                 const int* __restrict__ wall_nbr,
+                                                 const T* __restrict__ inv_den, int nf, int nw,
+                                                 size_t nwpad, T chiA, T chiB) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= nw) return;
+  T na = T(0), nb = T(0);
+#pragma unroll
+  for (int i = 1; i < Q; ++i) {
+    const int id = wall_nbr[(size_t)(i - 1) * nwpad + w];
+    if (id >= 0) {
+      const Vec2<T> p = psi[id];
+      na += wgt<T>(i) * p.a;
+      nb += wgt<T>(i) * p.b;
+    }
+  }
+  const T s = inv_den[w];
+  Vec2<T> o; o.a = chiA * na * s; o.b = chiB * nb * s;
+  psi[(size_t)nf + w] = o;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Per-node mixture quantities shared by the collide kernel and the macroscopic getter.
+// a3: F_sigma = -G rho_sigma sum_i w_i Psi_sigmabar(x+e_i) e_i + rho_sigma g
+//     (Eq. 10, 11, 13; one combined 18-term sum, reading R6)
+// a4: rho = rho_A + rho_B; tau_s = (rho_A tau_A + rho_B tau_B)/rho (Eq. 5-7, R2);
+//     u_eq = (sum_sigma sum_i e_i f_i + hf * sum_sigma F_sigma)/rho (Eq. 8, R3, R4)
+template <typename T>
+struct NodeState {
+  T rhoA, rhoB;
+  T FA[3], FB[3];
+  T u[3];
+  T om;  // 1/tau_s
+};
+
+template <typename T>
+__device__ __forceinline__ void gather_force_sums(const Vec2<T>* __restrict__ psi,
+                                                  const int (&id)[Q], T (&SA)[3], T (&SB)[3]) {
+  // axis neighbours (w = 1/18) and diagonal neighbours (w = 1/36) summed separately
+  T a1[3] = {T(0), T(0), T(0)}, b1[3] = {T(0), T(0), T(0)};
+  T a2[3] = {T(0), T(0), T(0)}, b2[3] = {T(0), T(0), T(0)};
+#pragma unroll
+  for (int i = 1; i < Q; ++i) {
+    const int k = id[i] >= 0 ? id[i] : -id[i] - 1;  // mirror node beyond an open plane (R12 iv)
+    const Vec2<T> p = psi[k];
+    if (i < 7) {
+      if (ex(i)) { a1[0] += T(ex(i)) * p.a; b1[0] += T(ex(i)) * p.b; }
+      if (ey(i)) { a1[1] += T(ey(i)) * p.a; b1[1] += T(ey(i)) * p.b; }
+      if (ez(i)) { a1[2] += T(ez(i)) * p.a; b1[2] += T(ez(i)) * p.b; }
+    } else {
+      if (ex(i)) { a2[0] += T(ex(i)) * p.a; b2[0] += T(ex(i)) * p.b; }
+      if (ey(i)) { a2[1] += T(ey(i)) * p.a; b2[1] += T(ey(i)) * p.b; }
+      if (ez(i)) { a2[2] += T(ez(i)) * p.a; b2[2] += T(ez(i)) * p.b; }
+    }
+  }
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    SA[d] = wgt<T>(1) * a1[d] + wgt<T>(7) * a2[d];
+    SB[d] = wgt<T>(1) * b1[d] + wgt<T>(7) * b2[d];
+  }
+}
+
+template <typename T>
+__device__ __forceinline__ void node_state(const T (&fa)[Q], const T (&fb)[Q],
+                                           const Vec2<T>* __restrict__ psi, const int (&id)[Q],
+                                           const Consts<T>& c, NodeState<T>& s) {
+  T ra = fa[0], rb = fb[0];
+  T j[3] = {T(0), T(0), T(0)};
+#pragma unroll
+  for (int i = 1; i < Q; ++i) {
+    ra += fa[i];
+    rb += fb[i];
+    const T t = fa[i] + fb[i];
+    if (ex(i)) j[0] += T(ex(i)) * t;
+    if (ey(i)) j[1] += T(ey(i)) * t;
+    if (ez(i)) j[2] += T(ez(i)) * t;
+  }
+  T SA[3], SB[3];
+  gather_force_sums<T>(psi, id, SA, SB);
+  const T g[3] = {c.gx, c.gy, c.gz};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    s.FA[d] = -c.G * ra * SB[d] + ra * g[d];
+    s.FB[d] = -c.G * rb * SA[d] + rb * g[d];
+  }
+  const T inv = T(1) / (ra + rb);
+#pragma unroll
+  for (int d = 0; d < 3; ++d) s.u[d] = (j[d] + c.hf * (s.FA[d] + s.FB[d])) * inv;
+  s.om = (ra + rb) / (ra * c.tauA + rb * c.tauB);
+  s.rhoA = ra;
+  s.rhoB = rb;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3-a6 fused: forces, tau_s/u_eq, collision, push-streaming with halfway bounce-back.
+//   f*_i = f_i - (f_i - feq_i)/tau_s + (1 - 1/(2 tau_s)) S_i                     Eq. (1)
+//   feq_i = w_i rho_sigma [1 + 3 e.u + 4.5 (e.u)^2 - 1.5 u.u]                     Eq. (2)
+//   S_i  = w_i [3 (e_i - u).F_sigma + 9 (e_i.u)(e_i.F_sigma)]                     Eq. (9)
+//   f_i(x+e_i, t+1) = f*_i(x,t);  x+e_i solid -> f_opp(i)(x, t+1) = f*_i(x,t)     L191, L215 (R10)
+// REMAINDER (fp32 build): the rest population is written as rho_sigma - sum_{i>=1} f*_i, which
+// equals Eq. (1) for i=0 exactly in exact arithmetic (sum_i feq = rho, sum_i S_i = 0) and removes
+// the 1.5e-8-per-step mass drift that the fp32-rounded weights (sum = 1 + 1.49e-8) would inject
+// (DESIGN.md "fp32 build").
+template <typename T, bool REMAINDER>
+__device__ __forceinline__ void collide_component(const T (&f)[Q], T rho, const T (&F)[3],
+                                                  const T (&u)[3], T om, T (&out)[Q]) {
+  const T uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+  const T uF = u[0] * F[0] + u[1] * F[1] + u[2] * F[2];
+  const T c1 = T(1) - om;
+  const T cS = T(1) - T(0.5) * om;
+  T acc = T(0);
+#pragma unroll
+  for (int i = Q - 1; i >= 0; --i) {
+    T eu = T(0), eF = T(0);
+    if (ex(i)) { eu += T(ex(i)) * u[0]; eF += T(ex(i)) * F[0]; }
+    if (ey(i)) { eu += T(ey(i)) * u[1]; eF += T(ey(i)) * F[1]; }
+    if (ez(i)) { eu += T(ez(i)) * u[2]; eF += T(ez(i)) * F[2]; }
+    const T feq = wgt<T>(i) * rho * (T(1) + T(3) * eu + T(4.5) * eu * eu - T(1.5) * uu);
+    const T S = wgt<T>(i) * (T(3) * (eF - uF) + T(9) * eu * eF);
+    T v = c1 * f[i] + om * feq + cS * S;
+    if (REMAINDER && i == 0) v = rho - acc;
+    if (i > 0) acc += v;
+    out[i] = v;
+  }
+}
+
+template <typename T>
+__device__ __forceinline__ void push_component(T* __restrict__ fo, const T (&v)[Q],
+                                               const int (&id)[Q], int n, int nf, size_t npad) {
+  fo[n] = v[0];
+#pragma unroll
+  for (int i = 1; i < Q; ++i) {
+    const int k = id[i];
+    if ((unsigned)k < (unsigned)nf) fo[(size_t)i * npad + k] = v[i];        // fluid neighbour
+    else if (k >= nf) fo[(size_t)opp(i) * npad + n] = v[i];                  // halfway bounce-back
+    // k < 0: the population leaves through an open plane
+  }
+}
+
+template <typename T, bool REMAINDER>
+__global__ void __launch_bounds__(256) k_collide_stream(const T* __restrict__ fin,
+                                                        T* __restrict__ fout,
+                                                        const Vec2<T>* __restrict__ psi,
+                                                        const int* __restrict__ nbr, int nf,
+                                                        size_t npad, Consts<T> c) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= nf) return;
+  int id[Q];
+  id[0] = n;
+#pragma unroll
+  for (int i = 1; i < Q; ++i) id[i] = nbr[(size_t)(i - 1) * npad + n];
+  T fa[Q], fb[Q];
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    fa[i] = fin[(size_t)i * npad + n];
+    fb[i] = fin[(size_t)(Q + i) * npad + n];
+  }
+  NodeState<T> s;
+  node_state<T>(fa, fb, psi, id, c, s);
+  T v[Q];
+  collide_component<T, REMAINDER>(fa, s.rhoA, s.FA, s.u, s.om, v);
+  push_component<T>(fout, v, id, n, nf, npad);
+  collide_component<T, REMAINDER>(fb, s.rhoB, s.FB, s.u, s.om, v);
+  push_component<T>(fout + (size_t)Q * npad, v, id, n, nf, npad);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a0  open-plane fix on the new buffer (reading R12 of PAPER.md L147-157, L223): planes z=0 and
+// z=nz-1 are all fluid, so their ids are q, nf-np+q and their interior neighbours np+q,
+// nf-2np+q.  Dirichlet component: all 19 populations <- feq(rho_b,u_b) + [f(x_f) - feq(rho(x_f),
+// u_f)] (non-equilibrium extrapolation); other component: its 5 inward populations <- frozen.
+template <typename T>
+struct OpenPlane {
+  int dc[2];       // Dirichlet component at inlet / outlet
+  int kind[2];     // 1 density, 2 velocity
+  T rho[2];        // imposed density (kind 1)
+  T uz[2];         // imposed velocity (kind 2)
+};
+
+template <typename T>
+__device__ __forceinline__ T feq_of(int i, T rho, const T (&u)[3]) {
+  T eu = T(0);
+  if (ex(i)) eu += T(ex(i)) * u[0];
+  if (ey(i)) eu += T(ey(i)) * u[1];
+  if (ez(i)) eu += T(ez(i)) * u[2];
+  const T uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+  return wgt<T>(i) * rho * (T(1) + T(3) * eu + T(4.5) * eu * eu - T(1.5) * uu);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128) k_open_planes(T* __restrict__ f,
+                                                     const T* __restrict__ frozen, int nf, int np,
+                                                     size_t npad, OpenPlane<T> op) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= 2 * np) return;
+  const int plane = t / np, q = t - plane * np;
+  const int vb = plane == 0 ? q : nf - np + q;
+  const int vf = plane == 0 ? np + q : nf - 2 * np + q;
+  T ff[2][Q];
+  T rf[2] = {T(0), T(0)}, j[3] = {T(0), T(0), T(0)};
+#pragma unroll
+  for (int s = 0; s < 2; ++s)
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+      const T v = f[(size_t)(s * Q + i) * npad + vf];
+      ff[s][i] = v;
+      rf[s] += v;
+      if (ex(i)) j[0] += T(ex(i)) * v;
+      if (ey(i)) j[1] += T(ey(i)) * v;
+      if (ez(i)) j[2] += T(ez(i)) * v;
+    }
+  const T inv = T(1) / (rf[0] + rf[1]);
+  const T uf[3] = {j[0] * inv, j[1] * inv, j[2] * inv};  // R12 iii: bare mixture velocity
+  const int dc = op.dc[plane];
+  const T rfd = dc == 0 ? rf[0] : rf[1];
+  T rho_b, ub[3];
+  if (op.kind[plane] == 1) {
+    rho_b = op.rho[plane];
+    ub[0] = uf[0]; ub[1] = uf[1]; ub[2] = uf[2];
+  } else {
+    rho_b = rfd;
+    ub[0] = T(0); ub[1] = T(0); ub[2] = op.uz[plane];
+  }
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    const T fi = dc == 0 ? ff[0][i] : ff[1][i];
+    f[(size_t)(dc * Q + i) * npad + vb] = feq_of<T>(i, rho_b, ub) + (fi - feq_of<T>(i, rfd, uf));
+  }
+  const int oc = 1 - dc;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const int i = plane == 0 ? inward(0, k) : inward(1, k);
+    f[(size_t)(oc * Q + i) * npad + vb] = frozen[((size_t)(plane * 2 + oc) * 5 + k) * np + q];
+  }
+}
+
+// frozen[plane][comp][k][q] <- f[comp][inward(plane,k)][plane node q]   (reading R27)
+template <typename T>
+__global__ void k_record_frozen(const T* __restrict__ f, T* __restrict__ frozen, int comp, int nf,
+                                int np, size_t npad) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= 2 * np) return;
+  const int plane = t / np, q = t - plane * np;
+  const int vb = plane == 0 ? q : nf - np + q;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const int i = plane == 0 ? inward(0, k) : inward(1, k);
+    frozen[((size_t)(plane * 2 + comp) * 5 + k) * np + q] = f[(size_t)(comp * Q + i) * npad + vb];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Initialisation and I/O between dense host-ordered double arrays (device copies) and the
+// compact store.  node_vox[n] = dense voxel index of fluid node n.
+template <typename T>
+__global__ void k_init_density(const double* __restrict__ rhoA, const double* __restrict__ rhoB,
+                               const int* __restrict__ node_vox, T* __restrict__ f, int nf,
+                               size_t npad) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= nf) return;
+  const int v = node_vox[n];
+  const double ra = rhoA[v], rb = rhoB[v];
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {  // f_i = w_i rho (reading R11)
+    f[(size_t)i * npad + n] = (T)(wgt<double>(i) * ra);
+    f[(size_t)(Q + i) * npad + n] = (T)(wgt<double>(i) * rb);
+  }
+}
+
+template <typename T>
+__global__ void k_dense_to_compact(const double* __restrict__ dense,
+                                   const int* __restrict__ node_vox, T* __restrict__ row, int nf) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n < nf) row[n] = (T)dense[node_vox[n]];
+}
+
+template <typename T>
+__global__ void k_compact_to_dense(const T* __restrict__ row, const int* __restrict__ node_vox,
+                                   double* __restrict__ dense, int nf) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n < nf) dense[node_vox[n]] = (double)row[n];
+}
+
+// rho_sigma, u = u_eq, P = (rho_A+rho_B)/3 + (G/3) rho_A rho_B (Eq. 12, R13) into
+// compact double rows out[q][nf], q = rhoA, rhoB, ux, uy, uz, P.  Needs psi of the current state.
+template <typename T>
+__global__ void __launch_bounds__(256) k_macroscopic(const T* __restrict__ fin,
+                                                     const Vec2<T>* __restrict__ psi,
+                                                     const int* __restrict__ nbr,
+                                                     double* __restrict__ out, int nf, size_t npad,
+                                                     Consts<T> c) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= nf) return;
+  int id[Q];
+  id[0] = n;
+#pragma unroll
+  for (int i = 1; i < Q; ++i) id[i] = nbr[(size_t)(i - 1) * npad + n];
+  T fa[Q], fb[Q];
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    fa[i] = fin[(size_t)i * npad + n];
+    fb[i] = fin[(size_t)(Q + i) * npad + n];
+  }
+  NodeState<T> s;
+  node_state<T>(fa, fb, psi, id, c, s);
+  out[n] = (double)s.rhoA;
+  out[(size_t)nf + n] = (double)s.rhoB;
+  out[(size_t)2 * nf + n] = (double)s.u[0];
+  out[(size_t)3 * nf + n] = (double)s.u[1];
+  out[(size_t)4 * nf + n] = (double)s.u[2];
+  out[(size_t)5 * nf + n] =
+      (double)((s.rhoA + s.rhoB) / T(3) + (c.G / T(3)) * s.rhoA * s.rhoB);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a7  diagnostics: warp-shuffle block reductions into one fp64 partial per block, then a
+// single-block fixed-order second stage: the sums are deterministic.
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  return v;
+}
+
+constexpr int kDiagVals = 6;  // mass A, mass B, momentum x,y,z, non-finite count
+constexpr int kDiagBlock = 256;
+
+template <typename T>
+__global__ void __launch_bounds__(kDiagBlock) k_diag_partial(const T* __restrict__ f,
+                                                             double* __restrict__ partial, int nf,
+                                                             size_t npad) {
+  double acc[kDiagVals] = {0, 0, 0, 0, 0, 0};
+  for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < nf; n += gridDim.x * blockDim.x) {
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+#pragma unroll
+      for (int i = 0; i < Q; ++i) {
+        const double v = (double)f[(size_t)(s * Q + i) * npad + n];
+        acc[s] += v;
+        if (ex(i)) acc[2] += ex(i) * v;
+        if (ey(i)) acc[3] += ey(i) * v;
+        if (ez(i)) acc[4] += ez(i) * v;
+        if (!isfinite(v)) acc[5] += 1.0;
+      }
+  }
+  __shared__ double sm[kDiagVals][kDiagBlock / 32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < kDiagVals; ++k) {
+    const double v = warp_sum(acc[k]);
+    if (lane == 0) sm[k][wid] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < kDiagVals) {
+    double t = 0.0;
+    for (int w = 0; w < kDiagBlock / 32; ++w) t += sm[threadIdx.x][w];
+    partial[(size_t)blockIdx.x * kDiagVals + threadIdx.x] = t;
+  }
+}
+
+__global__ void k_diag_final(const double* __restrict__ partial, double* __restrict__ out,
+                             int nblocks) {
+  const int k = threadIdx.x;
+  if (k >= kDiagVals) return;
+  double t = 0.0;
+  for (int b = 0; b < nblocks; ++b) t += partial[(size_t)b * kDiagVals + k];
+  out[k] = t;
+}
+
+// Saturation (reading R14): count nodes in the id range [n0,n1) whose
+// rho_comp exceeds the other density (tie -> component 1).  Integer atomics: deterministic.
+template <typename T>
+__global__ void k_count_phase(const Vec2<T>* __restrict__ psi, int n0, int n1, int comp,
+                              unsigned long long* __restrict__ count) {
+  const int n = n0 + blockIdx.x * blockDim.x + threadIdx.x;
+  int mine = 0;
+  if (n < n1) {
+    const Vec2<T> p = psi[n];
+    const int owner = p.a > p.b ? 0 : 1;
+    mine = owner == comp;
+  }
+  const unsigned b = __ballot_sync(0xffffffffu, mine);
+  if ((threadIdx.x & 31) == 0 && b) atomicAdd(count, (unsigned long long)__popc(b));
+}
+
+}  // namespace lbmk

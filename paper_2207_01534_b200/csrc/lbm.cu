@@ -1,0 +1,616 @@
+// lbm.cu -- the C ABI of include/lbm.h: host orchestration of the sm_100a kernels.
+// Product code; no CPU fallback; shares nothing with oracle/.
+#include "../../include/lbm.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "geometry.hpp"
+#include "kernels.cuh"
+
+extern "C" void* lbm_shim_alloc(size_t bytes);
+extern "C" void lbm_shim_free(void* p);
+extern "C" void* lbm_shim_stream(void);
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return code;
+}
+
+#define CU(call)                                                                         \
+  do {                                                                                   \
+    cudaError_t e_ = (call);                                                             \
+    if (e_ != cudaSuccess)                                                               \
+      return fail(LBM_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_),     \
+                  __FILE__, __LINE__);                                                   \
+  } while (0)
+
+inline unsigned blocks(long long n, int b) { return (unsigned)((n + b - 1) / b); }
+inline size_t pad64(long long n) { return (size_t)((n + 63) / 64 * 64); }
+
+struct ProfEvent {
+  int kind;
+  cudaEvent_t a, b;
+};
+
+// RAII for temporary device buffers from torch's caching allocator
+struct DevBuf {
+  void* p = nullptr;
+  explicit DevBuf(size_t bytes) { p = lbm_shim_alloc(bytes ? bytes : 1); }
+  ~DevBuf() { lbm_shim_free(p); }
+  DevBuf(const DevBuf&) = delete;
+  DevBuf& operator=(const DevBuf&) = delete;
+};
+
+}  // namespace
+
+struct lbm_ctx {
+  lbm_params p{};
+  int nx = 0, ny = 0, nz = 0, np = 0, bits = 32, device = 0;
+  long long nvox = 0;
+  int nf = 0, nw = 0;
+  size_t npad = 0, nwpad = 0, esz = 4;
+  std::vector<int32_t> vox2id, node_vox, zstart;  // host copies used by queries
+  void* f[2] = {nullptr, nullptr};                // [2][19][npad] T
+  void* psi = nullptr;                            // [nf+nw] Vec2<T>
+  int* nbr = nullptr;                             // [18][npad]
+  int* wall_nbr = nullptr;                        // [18][nwpad]
+  void* wall_inv_den = nullptr;                   // [nw] T
+  int* node_vox_d = nullptr;                      // [nf]
+  void* frozen = nullptr;                         // [2 planes][2 comps][5][np] T
+  double* partial = nullptr;                      // [diag blocks][6]
+  double* diag_out = nullptr;                     // [6] + count
+  int diag_blocks = 0;
+  int cur = 0;
+  long long bytes[4] = {0, 0, 0, 0};
+  bool prof = false;
+  std::vector<ProfEvent> prof_events;
+  double prof_ms[4] = {0, 0, 0, 0};
+  long long prof_launches = 0;
+
+  ~lbm_ctx() {
+    for (auto& e : prof_events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    lbm_shim_free(f[0]); lbm_shim_free(f[1]); lbm_shim_free(psi); lbm_shim_free(nbr);
+    lbm_shim_free(wall_nbr); lbm_shim_free(wall_inv_den); lbm_shim_free(node_vox_d);
+    lbm_shim_free(frozen); lbm_shim_free(partial); lbm_shim_free(diag_out);
+  }
+};
+
+namespace {
+
+using namespace lbmk;
+
+template <typename T>
+Consts<T> make_consts(const lbm_params& p) {
+  Consts<T> c;
+  c.G = (T)p.G; c.tauA = (T)p.tau[0]; c.tauB = (T)p.tau[1];
+  c.gx = (T)p.accel[0]; c.gy = (T)p.accel[1]; c.gz = (T)p.accel[2];
+  c.hf = p.half_force ? (T)0.5 : (T)0;
+  c.chiA = (T)(1.0 + p.xi); c.chiB = (T)(1.0 - p.xi);
+  return c;
+}
+
+template <typename T>
+OpenPlane<T> make_open(const lbm_params& p) {
+  OpenPlane<T> o;
+  o.dc[0] = p.inlet_comp; o.dc[1] = p.outlet_comp;
+  o.kind[0] = p.inlet_kind; o.kind[1] = p.outlet_kind;
+  o.rho[0] = (T)p.inlet_rho; o.rho[1] = (T)p.outlet_rho;
+  o.uz[0] = (T)p.inlet_uz; o.uz[1] = (T)0;
+  return o;
+}
+
+cudaStream_t cur_stream() { return (cudaStream_t)lbm_shim_stream(); }
+
+struct Timed {  // brackets one launch with events when profiling is on
+  lbm_ctx* c; cudaStream_t st; int kind; ProfEvent ev{};
+  Timed(lbm_ctx* c_, cudaStream_t st_, int kind_) : c(c_), st(st_), kind(kind_) {
+    if (c->prof) {
+      ev.kind = kind;
+      cudaEventCreate(&ev.a); cudaEventCreate(&ev.b);
+      cudaEventRecord(ev.a, st);
+    }
+  }
+  ~Timed() {
+    if (c->prof) { cudaEventRecord(ev.b, st); c->prof_events.push_back(ev); }
+    ++c->prof_launches;
+  }
+};
+
+// a1 + a2 on the current buffer
+template <typename T>
+void launch_psi(lbm_ctx* c, cudaStream_t st) {
+  const T* fin = (const T*)c->f[c->cur];
+  {
+    Timed t(c, st, 0);
+    k_density<T><<<blocks(c->nf, 256), 256, 0, st>>>(fin, (Vec2<T>*)c->psi, c->nf, c->npad);
+  }
+  if (c->nw > 0) {
+    Timed t(c, st, 1);
+    k_wallpsi<T><<<blocks(c->nw, 256), 256, 0, st>>>((Vec2<T>*)c->psi, c->wall_nbr,
+                                                     (const T*)c->wall_inv_den, c->nf, c->nw,
+                                                     c->nwpad, (T)(1.0 + c->p.xi),
+                                                     (T)(1.0 - c->p.xi));
+  }
+}
+
+template <typename T>
+int step_T(lbm_ctx* c, int n, cudaStream_t st) {
+  const Consts<T> k = make_consts<T>(c->p);
+  const OpenPlane<T> op = make_open<T>(c->p);
+  constexpr bool kRemainder = sizeof(T) == 4;
+  for (int it = 0; it < n; ++it) {
+    const T* fin = (const T*)c->f[c->cur];
+    T* fout = (T*)c->f[c->cur ^ 1];
+    launch_psi<T>(c, st);
+    {
+      Timed t(c, st, 2);
+      k_collide_stream<T, kRemainder><<<blocks(c->nf, 256), 256, 0, st>>>(
+          fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->npad, k);
+    }
+    if (c->p.z_open) {
+      Timed t(c, st, 3);
+      k_open_planes<T><<<blocks(2LL * c->np, 128), 128, 0, st>>>(fout, (const T*)c->frozen, c->nf,
+                                                                 c->np, c->npad, op);
+    }
+    c->cur ^= 1;
+  }
+  CU(cudaPeekAtLastError());
+  return LBM_OK;
+}
+
+template <typename T>
+int record_frozen_T(lbm_ctx* c, int comp, cudaStream_t st) {
+  if (!c->p.z_open) return LBM_OK;
+  k_record_frozen<T><<<blocks(2LL * c->np, 128), 128, 0, st>>>((const T*)c->f[c->cur],
+                                                               (T*)c->frozen, comp, c->nf, c->np,
+                                                               c->npad);
+  CU(cudaPeekAtLastError());
+  return LBM_OK;
+}
+
+int check_ctx(lbm_ctx* c) {
+  if (!c) return fail(LBM_EINVAL, "NULL context");
+  cudaError_t e = cudaSetDevice(c->device);
+  if (e != cudaSuccess) return fail(LBM_ECUDA, "cudaSetDevice: %s", cudaGetErrorString(e));
+  return LBM_OK;
+}
+
+int validate_params(const lbm_params* p, int nz) {
+  if (!(p->tau[0] > 0.5) || !(p->tau[1] > 0.5) || !std::isfinite(p->tau[0]) ||
+      !std::isfinite(p->tau[1]))
+    return fail(LBM_EINVAL, "relaxation times must be finite and > 1/2");
+  if (!std::isfinite(p->G) || !std::isfinite(p->xi))
+    return fail(LBM_EINVAL, "G and xi must be finite");
+  if (p->storage_bits != 32 && p->storage_bits != 64)
+    return fail(LBM_EINVAL, "storage_bits must be 32 or 64");
+  if (p->z_open) {
+    if (nz < 4) return fail(LBM_EINVAL, "z_open needs nz >= 4");
+    if (p->inlet_kind != 1 && p->inlet_kind != 2)
+      return fail(LBM_EINVAL, "inlet_kind must be 1 (density) or 2 (velocity)");
+    if (p->outlet_kind != 1) return fail(LBM_EINVAL, "outlet_kind must be 1 (density)");
+    if (p->inlet_comp < 0 || p->inlet_comp > 1 || p->outlet_comp < 0 || p->outlet_comp > 1)
+      return fail(LBM_EINVAL, "inlet_comp / outlet_comp must be 0 or 1");
+  }
+  return LBM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* lbm_last_error(void) { return g_err.c_str(); }
+
+int lbm_build_index(const uint8_t* solid, int nx, int ny, int nz, int z_open, int32_t* vox2id,
+                    int32_t* nbr, long long nbr_cap, long long* nf, long long* nw) {
+  if (!solid || !vox2id || !nf || !nw) return fail(LBM_EINVAL, "NULL argument");
+  lbmgeo::Geometry g;
+  const int rc = lbmgeo::build(g, solid, nx, ny, nz, z_open, nbr != nullptr);
+  if (rc) return fail(rc, "geometry build failed (%d)", rc);
+  std::memcpy(vox2id, g.vox2id.data(), sizeof(int32_t) * g.nvox);
+  *nf = g.nf;
+  *nw = g.nw;
+  if (nbr) {
+    if (nbr_cap < 18 * g.nf) return fail(LBM_EINVAL, "nbr capacity too small");
+    std::memcpy(nbr, g.nbr.data(), sizeof(int32_t) * 18 * g.nf);
+  }
+  return LBM_OK;
+}
+
+int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, const lbm_params* p) {
+  if (!out || !solid || !p) return fail(LBM_EINVAL, "NULL argument");
+  if (nx < 1 || ny < 1 || nz < 1) return fail(LBM_EINVAL, "box dimensions must be positive");
+  if (int rc = validate_params(p, nz)) return rc;
+  lbmgeo::Geometry g;
+  {
+    const int rc = lbmgeo::build(g, solid, nx, ny, nz, p->z_open, true);
+    if (rc == -2) return fail(LBM_ENOFLUID, "the mask has no fluid voxel");
+    if (rc == -3) return fail(LBM_ESOLIDOPEN, "solid voxel on an open plane or its neighbour plane");
+    if (rc == -4) return fail(LBM_ENOMEM, "host allocation failed");
+    if (rc) return fail(LBM_EINVAL, "bad geometry arguments");
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail(LBM_ECUDA, "no CUDA device: this library has no CPU fallback");
+  }
+  lbm_ctx* c = new (std::nothrow) lbm_ctx;
+  if (!c) return fail(LBM_ENOMEM, "host allocation failed");
+  CU(cudaGetDevice(&c->device));
+  c->p = *p;
+  c->nx = nx; c->ny = ny; c->nz = nz; c->np = nx * ny; c->nvox = g.nvox;
+  c->nf = (int)g.nf; c->nw = (int)g.nw;
+  c->bits = p->storage_bits; c->esz = p->storage_bits / 8;
+  c->npad = pad64(g.nf); c->nwpad = pad64(g.nw);
+  if ((size_t)2 * 19 * c->npad >= ((size_t)1 << 31)) {
+    delete c;
+    return fail(LBM_EINVAL, "too many fluid nodes for 32-bit slot indices");
+  }
+  c->zstart.assign(nz + 1, 0);
+  for (long long n = 0; n < g.nf; ++n) ++c->zstart[g.node_vox[n] / c->np + 1];
+  for (int z = 0; z < nz; ++z) c->zstart[z + 1] += c->zstart[z];
+  cudaStream_t st = cur_stream();
+  const size_t fbytes = (size_t)2 * 19 * c->npad * c->esz;
+  const size_t psibytes = (size_t)(g.nf + g.nw) * 2 * c->esz;
+  const size_t nbrbytes = (size_t)18 * c->npad * sizeof(int);
+  const size_t wnbrbytes = (size_t)18 * c->nwpad * sizeof(int);
+  const size_t frozenbytes = p->z_open ? (size_t)2 * 2 * 5 * c->np * c->esz : 0;
+  c->diag_blocks = 148 * 8;
+  c->f[0] = lbm_shim_alloc(fbytes);
+  c->f[1] = lbm_shim_alloc(fbytes);
+  c->psi = lbm_shim_alloc(psibytes);
+  c->nbr = (int*)lbm_shim_alloc(nbrbytes);
+  c->wall_nbr = (int*)lbm_shim_alloc(wnbrbytes ? wnbrbytes : 4);
+  c->wall_inv_den = lbm_shim_alloc(g.nw ? g.nw * c->esz : 4);
+  c->node_vox_d = (int*)lbm_shim_alloc(g.nf * sizeof(int));
+  c->frozen = lbm_shim_alloc(frozenbytes ? frozenbytes : 4);
+  c->partial = (double*)lbm_shim_alloc((size_t)c->diag_blocks * kDiagVals * sizeof(double));
+  c->diag_out = (double*)lbm_shim_alloc(8 * sizeof(double));
+  if (!c->f[0] || !c->f[1] || !c->psi || !c->nbr || !c->wall_nbr || !c->wall_inv_den ||
+      !c->node_vox_d || !c->frozen || !c->partial || !c->diag_out) {
+    delete c;
+    return fail(LBM_ENOMEM, "device allocation failed (populations need %zu bytes per buffer)",
+                fbytes);
+  }
+  c->bytes[0] = 2 * (long long)fbytes;
+  c->bytes[1] = (long long)psibytes;
+  c->bytes[2] = (long long)(nbrbytes + wnbrbytes + g.nw * c->esz + g.nf * sizeof(int));
+  c->bytes[3] = (long long)(frozenbytes + c->diag_blocks * kDiagVals * 8 + 64);
+  cudaError_t e = cudaSuccess;
+  auto up = [&](void* dst, const void* src, size_t bytes) {
+    if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st);
+  };
+  e = cudaMemsetAsync(c->f[0], 0, fbytes, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->f[1], 0, fbytes, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->psi, 0, psibytes, st);
+  if (e == cudaSuccess && frozenbytes) e = cudaMemsetAsync(c->frozen, 0, frozenbytes, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->nbr, 0, nbrbytes, st);
+  for (int i = 0; i < 18; ++i) {
+    up(c->nbr + (size_t)i * c->npad, g.nbr.data() + (size_t)i * g.nf, g.nf * sizeof(int));
+    up(c->wall_nbr + (size_t)i * c->nwpad, g.wall_nbr.data() + (size_t)i * g.nw,
+       g.nw * sizeof(int));
+  }
+  up(c->node_vox_d, g.node_vox.data(), g.nf * sizeof(int));
+  std::vector<float> invf;
+  if (c->bits == 32) {
+    invf.assign(g.wall_inv_den.begin(), g.wall_inv_den.end());
+    up(c->wall_inv_den, invf.data(), g.nw * sizeof(float));
+  } else {
+    up(c->wall_inv_den, g.wall_inv_den.data(), g.nw * sizeof(double));
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);  // host sources die with this scope
+  if (e != cudaSuccess) {
+    delete c;
+    return fail(LBM_ECUDA, "upload failed: %s", cudaGetErrorString(e));
+  }
+  c->vox2id.swap(g.vox2id);
+  c->node_vox.swap(g.node_vox);
+  *out = c;
+  return LBM_OK;
+}
+
+void lbm_destroy(lbm_ctx* c) {
+  if (!c) return;
+  cudaSetDevice(c->device);
+  cudaStreamSynchronize(cur_stream());
+  delete c;
+}
+
+long long lbm_num_fluid(lbm_ctx* c) { return c ? c->nf : -1; }
+long long lbm_num_wall_solid(lbm_ctx* c) { return c ? c->nw : -1; }
+
+int lbm_memory_bytes(lbm_ctx* c, long long bytes[4]) {
+  if (!c || !bytes) return fail(LBM_EINVAL, "NULL argument");
+  for (int k = 0; k < 4; ++k) bytes[k] = c->bytes[k];
+  return LBM_OK;
+}
+
+int lbm_set_boundary(lbm_ctx* c, double inlet_value, double outlet_rho) {
+  if (!c) return fail(LBM_EINVAL, "NULL context");
+  if (!c->p.z_open) return fail(LBM_EINVAL, "z is periodic: no boundary values to set");
+  if (!std::isfinite(inlet_value) || !std::isfinite(outlet_rho))
+    return fail(LBM_EINVAL, "boundary values must be finite");
+  if (c->p.inlet_kind == 1) c->p.inlet_rho = inlet_value; else c->p.inlet_uz = inlet_value;
+  c->p.outlet_rho = outlet_rho;
+  return LBM_OK;
+}
+
+int lbm_sync(lbm_ctx* c) {
+  if (int rc = check_ctx(c)) return rc;
+  CU(cudaStreamSynchronize(cur_stream()));
+  return LBM_OK;
+}
+
+int lbm_step(lbm_ctx* c, int n) {
+  if (int rc = check_ctx(c)) return rc;
+  if (n < 0) return fail(LBM_EINVAL, "n must be >= 0");
+  cudaStream_t st = cur_stream();
+  if (c->prof) {
+    for (auto& e : c->prof_events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    c->prof_events.clear();
+  }
+  c->prof_launches = 0;
+  return c->bits == 64 ? step_T<double>(c, n, st) : step_T<float>(c, n, st);
+}
+
+int lbm_set_profiling(lbm_ctx* c, int on) {
+  if (!c) return fail(LBM_EINVAL, "NULL context");
+  c->prof = on != 0;
+  return LBM_OK;
+}
+
+int lbm_last_step_profile(lbm_ctx* c, double ms[4], long long* launches) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!ms || !launches) return fail(LBM_EINVAL, "NULL argument");
+  CU(cudaStreamSynchronize(cur_stream()));
+  for (int k = 0; k < 4; ++k) ms[k] = 0.0;
+  for (auto& e : c->prof_events) {
+    float t = 0.f;
+    CU(cudaEventElapsedTime(&t, e.a, e.b));
+    ms[e.kind] += t;
+  }
+  *launches = c->prof_launches;
+  return LBM_OK;
+}
+
+int lbm_set_density(lbm_ctx* c, const double* rhoA, const double* rhoB) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!rhoA || !rhoB) return fail(LBM_EINVAL, "NULL argument");
+  cudaStream_t st = cur_stream();
+  const size_t bytes = (size_t)c->nvox * sizeof(double);
+  DevBuf a(bytes), b(bytes);
+  if (!a.p || !b.p) return fail(LBM_ENOMEM, "device staging allocation failed");
+  CU(cudaMemcpyAsync(a.p, rhoA, bytes, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(b.p, rhoB, bytes, cudaMemcpyHostToDevice, st));
+  if (c->bits == 64)
+    k_init_density<double><<<blocks(c->nf, 256), 256, 0, st>>>(
+        (const double*)a.p, (const double*)b.p, c->node_vox_d, (double*)c->f[c->cur], c->nf, c->npad);
+  else
+    k_init_density<float><<<blocks(c->nf, 256), 256, 0, st>>>(
+        (const double*)a.p, (const double*)b.p, c->node_vox_d, (float*)c->f[c->cur], c->nf, c->npad);
+  CU(cudaPeekAtLastError());
+  for (int s = 0; s < 2; ++s)
+    if (int rc = c->bits == 64 ? record_frozen_T<double>(c, s, st) : record_frozen_T<float>(c, s, st))
+      return rc;
+  CU(cudaStreamSynchronize(st));
+  return LBM_OK;
+}
+
+int lbm_set_populations(lbm_ctx* c, int comp, const double* f) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!f || comp < 0 || comp > 1) return fail(LBM_EINVAL, "bad argument");
+  cudaStream_t st = cur_stream();
+  const size_t bytes = (size_t)c->nvox * sizeof(double);
+  DevBuf d(bytes);
+  if (!d.p) return fail(LBM_ENOMEM, "device staging allocation failed");
+  for (int i = 0; i < Q; ++i) {
+    CU(cudaMemcpyAsync(d.p, f + (size_t)i * c->nvox, bytes, cudaMemcpyHostToDevice, st));
+    const size_t row = (size_t)(comp * Q + i) * c->npad;
+    if (c->bits == 64)
+      k_dense_to_compact<double><<<blocks(c->nf, 256), 256, 0, st>>>(
+          (const double*)d.p, c->node_vox_d, (double*)c->f[c->cur] + row, c->nf);
+    else
+      k_dense_to_compact<float><<<blocks(c->nf, 256), 256, 0, st>>>(
+          (const double*)d.p, c->node_vox_d, (float*)c->f[c->cur] + row, c->nf);
+    CU(cudaStreamSynchronize(st));  // pageable source: keep the staging buffer reuse ordered
+  }
+  CU(cudaPeekAtLastError());
+  if (int rc = c->bits == 64 ? record_frozen_T<double>(c, comp, st)
+                             : record_frozen_T<float>(c, comp, st))
+    return rc;
+  CU(cudaStreamSynchronize(st));
+  return LBM_OK;
+}
+
+int lbm_get_populations(lbm_ctx* c, int comp, double* f) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!f || comp < 0 || comp > 1) return fail(LBM_EINVAL, "bad argument");
+  cudaStream_t st = cur_stream();
+  const size_t bytes = (size_t)c->nvox * sizeof(double);
+  DevBuf d(bytes);
+  if (!d.p) return fail(LBM_ENOMEM, "device staging allocation failed");
+  for (int i = 0; i < Q; ++i) {
+    CU(cudaMemsetAsync(d.p, 0, bytes, st));
+    const size_t row = (size_t)(comp * Q + i) * c->npad;
+    if (c->bits == 64)
+      k_compact_to_dense<double><<<blocks(c->nf, 256), 256, 0, st>>>(
+          (const double*)c->f[c->cur] + row, c->node_vox_d, (double*)d.p, c->nf);
+    else
+      k_compact_to_dense<float><<<blocks(c->nf, 256), 256, 0, st>>>(
+          (const float*)c->f[c->cur] + row, c->node_vox_d, (double*)d.p, c->nf);
+    CU(cudaMemcpyAsync(f + (size_t)i * c->nvox, d.p, bytes, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+  }
+  return LBM_OK;
+}
+
+int lbm_get_macroscopic(lbm_ctx* c, double* rhoA, double* rhoB, double* ux, double* uy,
+                        double* uz, double* P) {
+  if (int rc = check_ctx(c)) return rc;
+  cudaStream_t st = cur_stream();
+  const bool was = c->prof;
+  c->prof = false;
+  DevBuf m((size_t)6 * c->nf * sizeof(double));
+  const size_t bytes = (size_t)c->nvox * sizeof(double);
+  DevBuf d(bytes);
+  if (!m.p || !d.p) { c->prof = was; return fail(LBM_ENOMEM, "device staging allocation failed"); }
+  if (c->bits == 64) {
+    launch_psi<double>(c, st);
+    k_macroscopic<double><<<blocks(c->nf, 256), 256, 0, st>>>(
+        (const double*)c->f[c->cur], (const Vec2<double>*)c->psi, c->nbr, (double*)m.p, c->nf,
+        c->npad, make_consts<double>(c->p));
+  } else {
+    launch_psi<float>(c, st);
+    k_macroscopic<float><<<blocks(c->nf, 256), 256, 0, st>>>(
+        (const float*)c->f[c->cur], (const Vec2<float>*)c->psi, c->nbr, (double*)m.p, c->nf,
+        c->npad, make_consts<float>(c->p));
+  }
+  c->prof = was;
+  CU(cudaPeekAtLastError());
+  double* outs[6] = {rhoA, rhoB, ux, uy, uz, P};
+  for (int q = 0; q < 6; ++q) {
+    if (!outs[q]) continue;
+    CU(cudaMemsetAsync(d.p, 0, bytes, st));
+    k_compact_to_dense<double><<<blocks(c->nf, 256), 256, 0, st>>>(
+        (const double*)m.p + (size_t)q * c->nf, c->node_vox_d, (double*)d.p, c->nf);
+    CU(cudaMemcpyAsync(outs[q], d.p, bytes, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+  }
+  CU(cudaStreamSynchronize(st));
+  return LBM_OK;
+}
+
+int lbm_diagnostics(lbm_ctx* c, double mass[2], double momentum[3]) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!mass || !momentum) return fail(LBM_EINVAL, "NULL argument");
+  cudaStream_t st = cur_stream();
+  const int nb = c->diag_blocks;
+  if (c->bits == 64)
+    k_diag_partial<double><<<nb, kDiagBlock, 0, st>>>((const double*)c->f[c->cur], c->partial,
+                                                      c->nf, c->npad);
+  else
+    k_diag_partial<float><<<nb, kDiagBlock, 0, st>>>((const float*)c->f[c->cur], c->partial, c->nf,
+                                                     c->npad);
+  k_diag_final<<<1, 32, 0, st>>>(c->partial, c->diag_out, nb);
+  CU(cudaPeekAtLastError());
+  double h[kDiagVals];
+  CU(cudaMemcpyAsync(h, c->diag_out, sizeof h, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  mass[0] = h[0]; mass[1] = h[1];
+  momentum[0] = h[2]; momentum[1] = h[3]; momentum[2] = h[4];
+  if (h[5] != 0.0 || !std::isfinite(h[0]) || !std::isfinite(h[1]))
+    return fail(LBM_ENONFINITE, "non-finite populations detected");
+  return LBM_OK;
+}
+
+int lbm_saturation(lbm_ctx* c, int comp, int z0, int z1, double* S) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!S || comp < 0 || comp > 1 || z0 < 0 || z1 > c->nz || z0 >= z1)
+    return fail(LBM_EINVAL, "bad argument");
+  const int n0 = c->zstart[z0], n1 = c->zstart[z1];
+  if (n1 <= n0) return fail(LBM_ENOFLUID, "no fluid node in the z-range");
+  cudaStream_t st = cur_stream();
+  const bool was = c->prof;
+  c->prof = false;
+  unsigned long long* cnt = (unsigned long long*)(c->diag_out + 7);
+  CU(cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), st));
+  if (c->bits == 64) {
+    launch_psi<double>(c, st);
+    k_count_phase<double><<<blocks(n1 - n0, 256), 256, 0, st>>>((const Vec2<double>*)c->psi, n0,
+                                                                n1, comp, cnt);
+  } else {
+    launch_psi<float>(c, st);
+    k_count_phase<float><<<blocks(n1 - n0, 256), 256, 0, st>>>((const Vec2<float>*)c->psi, n0, n1,
+                                                               comp, cnt);
+  }
+  c->prof = was;
+  CU(cudaPeekAtLastError());
+  unsigned long long h = 0;
+  CU(cudaMemcpyAsync(&h, cnt, sizeof h, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  *S = (double)h / (double)(n1 - n0);
+  return LBM_OK;
+}
+
+int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, double* mass) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!nodes || !mass || comp < 0 || comp > 1 || z0 < 0 || z1 > c->nz || z0 >= z1)
+    return fail(LBM_EINVAL, "bad argument");
+  cudaStream_t st = cur_stream();
+  const bool was = c->prof;
+  c->prof = false;
+  if (c->bits == 64) launch_psi<double>(c, st); else launch_psi<float>(c, st);
+  c->prof = was;
+  CU(cudaPeekAtLastError());
+  const int nf = c->nf;
+  std::vector<double> rho;  // rho_comp per fluid node
+  std::vector<uint8_t> state;
+  try {
+    rho.resize(nf);
+    state.resize(nf);
+    if (c->bits == 64) {
+      std::vector<double> h((size_t)2 * nf);
+      CU(cudaMemcpyAsync(h.data(), c->psi, h.size() * 8, cudaMemcpyDeviceToHost, st));
+      CU(cudaStreamSynchronize(st));
+      for (int n = 0; n < nf; ++n) {
+        state[n] = ((h[2 * n] > h[2 * n + 1]) ? 0 : 1) == comp;
+        rho[n] = h[2 * n + comp];
+      }
+    } else {
+      std::vector<float> h((size_t)2 * nf);
+      CU(cudaMemcpyAsync(h.data(), c->psi, h.size() * 4, cudaMemcpyDeviceToHost, st));
+      CU(cudaStreamSynchronize(st));
+      for (int n = 0; n < nf; ++n) {
+        state[n] = ((h[2 * n] > h[2 * n + 1]) ? 0 : 1) == comp;
+        rho[n] = h[2 * n + comp];
+      }
+    }
+    // flood from both end planes through same-phase 6-neighbours (periodic x,y; not across z)
+    std::vector<int32_t> stack;
+    for (int z : {0, c->nz - 1})
+      for (int n = c->zstart[z]; n < c->zstart[z + 1]; ++n)
+        if (state[n] == 1) { state[n] = 2; stack.push_back(n); }
+    const int nx = c->nx, ny = c->ny, nz = c->nz;
+    const int d6[6][3] = {{1, 0, 0}, {-1, 0, 0}, {0, 1, 0}, {0, -1, 0}, {0, 0, 1}, {0, 0, -1}};
+    while (!stack.empty()) {
+      const int n = stack.back();
+      stack.pop_back();
+      const long long v = c->node_vox[n];
+      const int x = (int)(v % nx), y = (int)((v / nx) % ny), z = (int)(v / c->np);
+      for (int k = 0; k < 6; ++k) {
+        const int zn = z + d6[k][2];
+        if (zn < 0 || zn >= nz) continue;
+        const int xn = (x + d6[k][0] + nx) % nx, yn = (y + d6[k][1] + ny) % ny;
+        const int32_t m = c->vox2id[(long long)xn + (long long)nx * (yn + (long long)ny * zn)];
+        if (m >= 0 && m < nf && state[m] == 1) { state[m] = 2; stack.push_back(m); }
+      }
+    }
+  } catch (const std::bad_alloc&) {
+    return fail(LBM_ENOMEM, "host allocation failed");
+  }
+  long long cnt = 0;
+  double msum = 0.0;
+  for (int n = c->zstart[z0]; n < c->zstart[z1]; ++n)
+    if (state[n] == 1) { ++cnt; msum += rho[n]; }
+  *nodes = cnt;
+  *mass = msum;
+  return LBM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,259 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Run with `-m gpu` on a B200.
+
+Tolerances (BASELINE.json north_star; norms are reading R22, stated here):
+  fp64 build : every population, relative  abs(a-b)/abs(b) <= 1e-10 after 200 steps;
+  fp32 build : component densities element-wise relative <= 1e-4 after 100 steps; velocities
+               max-norm of the difference / max-norm of the oracle field <= 1e-4;
+               total mass per component relative <= 1e-6.
+"""
+import numpy as np
+import pytest
+
+from oracle import LbmRef
+from paper_2207_01534_b200 import Lbm
+from workloads import default_params, make_config
+
+pytestmark = pytest.mark.gpu
+
+
+def _pair(mask, rhoA, rhoB, params):
+    o = LbmRef(mask, params)
+    g = Lbm(mask, params)
+    o.set_density(rhoA, rhoB)
+    g.set_density(rhoA, rhoB)
+    return o, g
+
+
+def _pop_rel(o, g, mask):
+    fl = mask == 0
+    worst = 0.0
+    for s in (0, 1):
+        a, b = g.get_populations(s), o.get_populations(s)
+        assert np.all(a[:, ~fl] == 0.0)
+        rel = np.abs(a[:, fl] - b[:, fl]) / np.abs(b[:, fl])
+        worst = max(worst, float(rel.max()))
+    return worst
+
+
+def _check_fp32(o, g, mask, rho_tol=1e-4, u_tol=1e-4, mass_tol=1e-6):
+    fl = mask == 0
+    mo, mg = o.get_macroscopic(), g.get_macroscopic()
+    for k in ("rhoA", "rhoB"):
+        rel = np.abs(mg[k][fl] - mo[k][fl]) / np.abs(mo[k][fl])
+        assert rel.max() <= rho_tol, (k, rel.max())
+        assert np.all(mg[k][~fl] == 0.0)
+    uo = np.stack([mo[k][fl] for k in ("ux", "uy", "uz")])
+    ug = np.stack([mg[k][fl] for k in ("ux", "uy", "uz")])
+    assert np.abs(ug - uo).max() <= u_tol * np.abs(uo).max(), np.abs(ug - uo).max() / np.abs(uo).max()
+    rel = np.abs(mg["P"][fl] - mo["P"][fl]) / np.abs(mo["P"][fl])
+    assert rel.max() <= 1e-4
+    m_o, _ = o.diagnostics()
+    m_g, _ = g.diagnostics()
+    assert np.max(np.abs(m_g - m_o) / m_o) <= mass_tol, np.abs(m_g - m_o) / m_o
+
+
+# ------------------------------------------------------------------ config 1: fp64, 1e-10
+
+def test_cfg1_fp64_every_population_200_steps():
+    c = make_config(1)
+    assert c["params"]["storage_bits"] == 64
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    assert _pop_rel(o, g, c["mask"]) == 0.0            # identical initial state
+    o.step(200)
+    g.step(200)
+    assert _pop_rel(o, g, c["mask"]) <= 1e-10
+    m_o, j_o = o.diagnostics()
+    m_g, j_g = g.diagnostics()
+    assert np.max(np.abs(m_g - m_o) / m_o) < 1e-13 and np.max(np.abs(j_g - j_o)) < 1e-11
+
+
+def test_cfg1_fp32_build():
+    c = make_config(1, storage_bits=32)
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    o.step(100)
+    g.step(100)
+    _check_fp32(o, g, c["mask"])
+
+
+# ------------------------------------------------------------------ all features, fp64, ragged sizes
+
+@pytest.mark.parametrize("shape,seed", [((5, 6, 8), 1), ((9, 33, 67), 2), ((23, 17, 130), 3)])
+def test_random_porous_fp64_all_features(shape, seed):
+    """Random solids (bounce-back + IVSD), unequal tau, wetting, body force; sizes that are not
+    multiples of the block size and span several blocks."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    mask = (rng.uniform(size=shape) < 0.3).astype(np.uint8)
+    rA = np.where(mask == 0, rng.uniform(0.05, 1.0, shape), 0.0)
+    rB = np.where(mask == 0, rng.uniform(0.05, 1.0, shape), 0.0)
+    p = default_params(G=3.5, tau=(1.2, 0.7), xi=0.25, accel=(1e-5, -2e-5, 3e-5), storage_bits=64)
+    o, g = _pair(mask, rA, rB, p)
+    o.step(20)
+    g.step(20)
+    assert _pop_rel(o, g, mask) <= 1e-10
+    mo, mg = o.get_macroscopic(), g.get_macroscopic()
+    for k in mo:
+        assert np.max(np.abs(mo[k] - mg[k])) <= 1e-12, k
+
+
+def test_worked_example_on_gpu():
+    """SURVEY.md App. C set-up (the oracle is pinned to its printed values in the CPU suite)."""
+    nx, ny, nz = 8, 6, 5
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    mask = ((x + 2 * y + 3 * z) % 7 == 0).astype(np.uint8)
+    rA = 0.5 + 0.4 * np.sin(2 * np.pi * x / 8) * np.cos(2 * np.pi * y / 6) + 0.05 * np.cos(2 * np.pi * z / 5)
+    p = default_params(G=3.5, tau=(1.0, 0.7), xi=0.2, accel=(0.0, 0.0, 1e-5), storage_bits=64)
+    o, g = _pair(mask, rA, 1.03 - rA, p)
+    o.step(5)
+    g.step(5)
+    assert _pop_rel(o, g, mask) <= 1e-12
+    m, j = g.diagnostics()
+    assert abs(m[0] - 1.032080772877051e+02) < 1e-11 and abs(j[0] - 1.316643580760437e-01) < 1e-12
+
+
+def test_half_force_off_negative_control_matches_too():
+    c = make_config(1, size=16, half_force=0)
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    o.step(30)
+    g.step(30)
+    assert _pop_rel(o, g, c["mask"]) <= 1e-11
+
+
+# ------------------------------------------------------------------ config 2: walls + wetting, fp32
+
+@pytest.mark.parametrize("xi", [-0.3, 0.0, 0.3])
+def test_cfg2_contact_fp32_100_steps(xi):
+    c = make_config(2, size=32, xi=xi)
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    o.step(100)
+    g.step(100)
+    _check_fp32(o, g, c["mask"])
+
+
+def test_cfg2_contact_fp64():
+    c = make_config(2, size=24, xi=-0.3, storage_bits=64)
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    o.step(100)
+    g.step(100)
+    assert _pop_rel(o, g, c["mask"]) <= 1e-10
+
+
+# ------------------------------------------------------------------ configs 3, 4: open planes
+
+def test_cfg3_drainage_open_fp64():
+    c = make_config(3, size=32, storage_bits=64)
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    o.step(60)
+    g.step(60)
+    assert _pop_rel(o, g, c["mask"]) <= 1e-10
+
+
+def test_cfg3_drainage_open_fp32():
+    c = make_config(3, size=48)
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    o.step(100)
+    g.step(100)
+    _check_fp32(o, g, c["mask"])
+
+
+@pytest.mark.parametrize("G", [3.5, 3.0])
+def test_cfg4_imbibition_open_fp32(G):
+    c = make_config(4, size=48, G=G)
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    o.step(100)
+    g.step(100)
+    _check_fp32(o, g, c["mask"])
+    for comp in (0, 1):
+        assert abs(o.saturation(comp, 8, 40) - g.saturation(comp, 8, 40)) < 1e-12
+        assert o.trapped_volume(comp, 8, 40)[0] == g.trapped_volume(comp, 8, 40)[0]
+
+
+def test_cfg4_imbibition_open_fp64():
+    c = make_config(4, size=32, storage_bits=64)
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    o.step(60)
+    g.step(60)
+    assert _pop_rel(o, g, c["mask"]) <= 1e-10
+
+
+# ------------------------------------------------------------------ config 5: periodic pack + body force
+
+def test_cfg5_spherepack_bodyforce_fp32():
+    c = make_config(5, size=64)
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    o.step(100)
+    g.step(100)
+    _check_fp32(o, g, c["mask"])
+
+
+# ------------------------------------------------------------------ interfaces and edge cases
+
+def test_checkpoint_roundtrip_and_restart():
+    c = make_config(3, size=24, storage_bits=64)
+    a = Lbm(c["mask"], c["params"])
+    a.set_density(c["rhoA"], c["rhoB"])
+    a.step(7)
+    b = Lbm(c["mask"], c["params"])
+    for s in (0, 1):
+        b.set_populations(s, a.get_populations(s))
+    a.step(5)
+    b.step(5)
+    for s in (0, 1):
+        assert np.array_equal(a.get_populations(s), b.get_populations(s))
+
+
+def test_step_zero_and_split_steps_are_identical():
+    c = make_config(1, size=16)
+    a = Lbm(c["mask"], c["params"])
+    b = Lbm(c["mask"], c["params"])
+    a.set_density(c["rhoA"], c["rhoB"])
+    b.set_density(c["rhoA"], c["rhoB"])
+    a.step(0)
+    a.step(6)
+    for n in (1, 2, 3):
+        b.step(n)
+    for s in (0, 1):
+        assert np.array_equal(a.get_populations(s), b.get_populations(s))   # deterministic
+
+
+def test_single_fluid_voxel_and_single_component():
+    mask = np.ones((3, 3, 3), np.uint8)
+    mask[1, 1, 1] = 0
+    p = default_params(G=3.5, tau=(1.0, 0.8), xi=0.1, storage_bits=64)
+    rA = np.where(mask == 0, 0.7, 0.0)
+    o, g = _pair(mask, rA, np.zeros_like(rA), p)          # rho_B = 0 everywhere (R4)
+    o.step(5)
+    g.step(5)
+    a, b = g.get_populations(0), o.get_populations(0)
+    assert np.max(np.abs(a - b)) <= 1e-15 and np.isfinite(a).all()
+    assert np.all(g.get_populations(1) == 0.0)
+
+
+def test_diagnostics_saturation_trapped_volume_match_oracle():
+    rng = np.random.Generator(np.random.PCG64(9))
+    shape = (14, 10, 12)
+    mask = (rng.uniform(size=shape) < 0.3).astype(np.uint8)
+    rA = np.where(mask == 0, rng.uniform(0.0, 1.0, shape), 0.0)
+    rB = np.where(mask == 0, rng.uniform(0.0, 1.0, shape), 0.0)
+    p = default_params(storage_bits=64)
+    o, g = _pair(mask, rA, rB, p)
+    m_o, j_o = o.diagnostics()
+    m_g, j_g = g.diagnostics()
+    assert np.allclose(m_o, m_g, rtol=1e-14) and np.allclose(j_o, j_g, atol=1e-13)
+    for comp in (0, 1):
+        for z0, z1 in ((0, 14), (3, 9)):
+            assert abs(o.saturation(comp, z0, z1) - g.saturation(comp, z0, z1)) < 1e-15
+            no, mo = o.trapped_volume(comp, z0, z1)
+            ng, mg = g.trapped_volume(comp, z0, z1)
+            assert no == ng and abs(mo - mg) < 1e-12 * max(1.0, mo)
+
+
+def test_set_boundary_changes_inlet_density():
+    c = make_config(4, size=24, storage_bits=64)
+    g = Lbm(c["mask"], c["params"])
+    g.set_density(c["rhoA"], c["rhoB"])
+    g.set_boundary(1.05, 0.98)
+    g.step(3)
+    m = g.get_macroscopic(fields=("rhoA", "rhoB"))
+    assert np.allclose(m["rhoB"][0], 1.05, atol=1e-12)      # inlet Dirichlet on B (config 4)
+    assert np.allclose(m["rhoA"][-1], 0.98, atol=1e-12)     # outlet Dirichlet on A
