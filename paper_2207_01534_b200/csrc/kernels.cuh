@@ -248,6 +248,188 @@ __global__ void __launch_bounds__(256) k_collide_stream(const T* __restrict__ fi
 }
 
 // ---------------------------------------------------------------------------------------------
+// Bulk-async (TMA engine) staging for the fused pass.  One CTA owns a tile of TN consecutive
+// node ids; its 38 population rows and 18 neighbour-index rows are TN-element contiguous,
+// 16-byte-aligned segments of the SoA arrays, so the whole tile arrives in shared memory through
+// 56 cp.async.bulk copies (SASS UBLKCP) that complete on one mbarrier.  Registers then hold only
+// the working set, so several CTAs per SM keep >100 KB of loads in flight per SM with no
+// register cost -- what the one-node-per-thread register version (167 registers, 12 % occupancy,
+// 34 % of HBM peak; profiles/r1_v1_collide.md) could not do.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+               "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes,
+                                         uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+          "r"(smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
+
+template <typename T, int TN>
+constexpr size_t collide_smem_bytes() {
+  return (size_t)2 * Q * TN * sizeof(T) + (size_t)18 * TN * sizeof(int);
+}
+
+template <typename T, int TN, int MINB, bool REMAINDER>
+__global__ void __launch_bounds__(TN, MINB)
+    k_collide_stream_bulk(const T* __restrict__ fin, T* __restrict__ fout,
+                          const Vec2<T>* __restrict__ psi, const int* __restrict__ nbr, int nf,
+                          size_t npad, Consts<T> c) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* sf = reinterpret_cast<T*>(smem_raw);                                   // [38][TN]
+  int* sid = reinterpret_cast<int*>(smem_raw + (size_t)2 * Q * TN * sizeof(T));  // [18][TN]
+  __shared__ uint64_t bar;
+  const int tid = threadIdx.x;
+  const size_t t0 = (size_t)blockIdx.x * TN;
+  if (tid == 0) mbar_init(&bar, 1);
+  __syncthreads();
+  if (tid < 32) {
+    if (tid == 0) mbar_expect_tx(&bar, (uint32_t)collide_smem_bytes<T, TN>());
+    __syncwarp();
+    for (int r = tid; r < 2 * Q + 18; r += 32) {
+      if (r < 2 * Q)
+        bulk_g2s(sf + (size_t)r * TN, fin + (size_t)r * npad + t0, TN * sizeof(T), &bar);
+      else
+        bulk_g2s(sid + (size_t)(r - 2 * Q) * TN, nbr + (size_t)(r - 2 * Q) * npad + t0,
+                 TN * sizeof(int), &bar);
+    }
+  }
+  mbar_wait(&bar, 0);
+  const int n = (int)t0 + tid;
+  if (n >= nf) return;
+
+  // a3 inputs: psi gathers through the staged neighbour ids (ids are re-read from shared memory
+  // at store time instead of being held in registers)
+  T SA[3], SB[3];
+  {
+    T a1[3] = {T(0), T(0), T(0)}, b1[3] = {T(0), T(0), T(0)};
+    T a2[3] = {T(0), T(0), T(0)}, b2[3] = {T(0), T(0), T(0)};
+#pragma unroll
+    for (int i = 1; i < Q; ++i) {
+      const int k0 = sid[(i - 1) * TN + tid];
+      const int k = k0 >= 0 ? k0 : -k0 - 1;  // mirror node beyond an open plane (R12 iv)
+      const Vec2<T> p = psi[k];
+      if (i < 7) {
+        if (ex(i)) { a1[0] += T(ex(i)) * p.a; b1[0] += T(ex(i)) * p.b; }
+        if (ey(i)) { a1[1] += T(ey(i)) * p.a; b1[1] += T(ey(i)) * p.b; }
+        if (ez(i)) { a1[2] += T(ez(i)) * p.a; b1[2] += T(ez(i)) * p.b; }
+      } else {
+        if (ex(i)) { a2[0] += T(ex(i)) * p.a; b2[0] += T(ex(i)) * p.b; }
+        if (ey(i)) { a2[1] += T(ey(i)) * p.a; b2[1] += T(ey(i)) * p.b; }
+        if (ez(i)) { a2[2] += T(ez(i)) * p.a; b2[2] += T(ez(i)) * p.b; }
+      }
+    }
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      SA[d] = wgt<T>(1) * a1[d] + wgt<T>(7) * a2[d];
+      SB[d] = wgt<T>(1) * b1[d] + wgt<T>(7) * b2[d];
+    }
+  }
+  // a1 (recomputed locally) + bare momentum
+  T ra = sf[tid], rb = sf[Q * TN + tid];
+  T j[3] = {T(0), T(0), T(0)};
+#pragma unroll
+  for (int i = 1; i < Q; ++i) {
+    const T a = sf[i * TN + tid], b = sf[(Q + i) * TN + tid];
+    ra += a;
+    rb += b;
+    const T t = a + b;
+    if (ex(i)) j[0] += T(ex(i)) * t;
+    if (ey(i)) j[1] += T(ey(i)) * t;
+    if (ez(i)) j[2] += T(ez(i)) * t;
+  }
+  const T g[3] = {c.gx, c.gy, c.gz};
+  T FA[3], FB[3], u[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    FA[d] = -c.G * ra * SB[d] + ra * g[d];
+    FB[d] = -c.G * rb * SA[d] + rb * g[d];
+  }
+  const T inv = T(1) / (ra + rb);
+#pragma unroll
+  for (int d = 0; d < 3; ++d) u[d] = (j[d] + c.hf * (FA[d] + FB[d])) * inv;
+  const T om = (ra + rb) / (ra * c.tauA + rb * c.tauB);
+  // Collision in opposite-direction pairs (i, opp(i)): with A = 1 + 4.5 (e.u)^2 - 1.5 u.u and
+  // B = 9 (e.u)(e.F) - 3 u.F, Eq. (1),(2),(9) give
+  //   f*_i      = (1-om) f_i      + [om w rho A + cS w B] + 3 [om w rho (e.u) + cS w (e.F)]
+  //   f*_opp(i) = (1-om) f_opp(i) + [om w rho A + cS w B] - 3 [om w rho (e.u) + cS w (e.F)]
+  // (the bracketed even/odd parts are shared by the pair), cS = 1 - om/2.
+  const T k0 = T(1) - T(1.5) * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+  const T c1 = T(1) - om, cS = T(1) - T(0.5) * om;
+  const unsigned np32 = (unsigned)npad;  // 38 * npad < 2^31: 32-bit slot indices
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+    const T rho = s == 0 ? ra : rb;
+    const T F0 = s == 0 ? FA[0] : FB[0], F1 = s == 0 ? FA[1] : FB[1], F2 = s == 0 ? FA[2] : FB[2];
+    const T m3uF = T(-3) * (u[0] * F0 + u[1] * F1 + u[2] * F2);
+    const T* sfs = sf + (size_t)s * Q * TN + tid;
+    T* fo = fout + (size_t)s * Q * npad;
+    T acc = T(0);
+#pragma unroll
+    for (int i = 1; i < Q; i += 2) {  // canonical order: opp(i) == i + 1 for odd i
+      static_assert(opp(1) == 2 && opp(7) == 10 && opp(9) == 8, "pairing below relies on the table");
+      const int ip = i, im = opp(i);
+      const T w = wgt<T>(ip);
+      T eu = T(0), eF = T(0);
+      if (ex(ip)) { eu += T(ex(ip)) * u[0]; eF += T(ex(ip)) * F0; }
+      if (ey(ip)) { eu += T(ey(ip)) * u[1]; eF += T(ey(ip)) * F1; }
+      if (ez(ip)) { eu += T(ez(ip)) * u[2]; eF += T(ez(ip)) * F2; }
+      const T kA = om * w * rho, kB = cS * w;
+      const T A = T(4.5) * eu * eu + k0;
+      const T B = T(9) * eu * eF + m3uF;
+      const T X = kA * A + kB * B;
+      const T Y = T(3) * (kA * eu + kB * eF);
+      const T vp = c1 * sfs[ip * TN] + X + Y;
+      const T vm = c1 * sfs[im * TN] + X - Y;
+      acc += vp + vm;
+      {
+        const int k = sid[(ip - 1) * TN + tid];
+        if ((unsigned)k < (unsigned)nf) fo[(unsigned)ip * np32 + (unsigned)k] = vp;  // fluid neighbour
+        else if (k >= nf) fo[(unsigned)im * np32 + (unsigned)n] = vp;  // halfway bounce-back
+      }
+      {
+        const int k = sid[(im - 1) * TN + tid];
+        if ((unsigned)k < (unsigned)nf) fo[(unsigned)im * np32 + (unsigned)k] = vm;
+        else if (k >= nf) fo[(unsigned)ip * np32 + (unsigned)n] = vm;
+      }
+    }
+    // rest population: Eq. (1) with e_0 = 0, or the remainder rho - sum_{i>=1} f*_i (fp32 build)
+    T v0;
+    if (REMAINDER) {
+      v0 = rho - acc;
+    } else {
+      const T w0 = wgt<T>(0);
+      v0 = c1 * sfs[0] + om * w0 * rho * k0 + cS * w0 * m3uF;
+    }
+    fo[n] = v0;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // a0  open-plane fix on the new buffer (reading R12 of PAPER.md L147-157, L223): planes z=0 and
 // z=nz-1 are all fluid, so their ids are q, nf-np+q and their interior neighbours np+q,
 // nf-2np+q.  Dirichlet component: all 19 populations <- feq(rho_b,u_b) + [f(x_f) - feq(rho(x_f),

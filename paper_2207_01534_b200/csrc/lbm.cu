@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -43,6 +44,9 @@ int fail(int code, const char* fmt, ...) {
 
 inline unsigned blocks(long long n, int b) { return (unsigned)((n + b - 1) / b); }
 inline size_t pad64(long long n) { return (size_t)((n + 63) / 64 * 64); }
+// population / neighbour rows are padded to whole 256-node tiles so that every bulk copy of the
+// fused pass is a full, 1 KB-aligned segment
+inline size_t pad256(long long n) { return (size_t)((n + 255) / 256 * 256); }
 
 struct ProfEvent {
   int kind;
@@ -78,6 +82,8 @@ struct lbm_ctx {
   double* diag_out = nullptr;                     // [6] + count
   int diag_blocks = 0;
   int cur = 0;
+  int collide_variant = 1;  // 0: register kernel, 1: bulk-async staged (default); env LBM_B200_COLLIDE
+  int tile = 1285;          // fp32 bulk kernel variant: tile nodes * 10 + min CTAs/SM; env LBM_B200_TILE
   long long bytes[4] = {0, 0, 0, 0};
   bool prof = false;
   std::vector<ProfEvent> prof_events;
@@ -150,19 +156,55 @@ void launch_psi(lbm_ctx* c, cudaStream_t st) {
   }
 }
 
+
+// a3-a6: the fused pass.  Production = bulk-async staged tiles; the register kernel is kept as
+// an A/B reference (LBM_B200_COLLIDE=simple).
+template <typename T, int TN, int MINB>
+void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
+  constexpr bool kRemainder = sizeof(T) == 4;
+  constexpr size_t smem = collide_smem_bytes<T, TN>();
+  static bool configured = false;
+  if (!configured) {
+    cudaFuncSetAttribute(k_collide_stream_bulk<T, TN, MINB, kRemainder>,
+                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configured = true;
+  }
+  k_collide_stream_bulk<T, TN, MINB, kRemainder><<<blocks(c->nf, TN), TN, smem, st>>>(
+      fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->npad, k);
+}
+
+template <typename T>
+void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
+  constexpr bool kRemainder = sizeof(T) == 4;
+  if (c->collide_variant == 0) {
+    k_collide_stream<T, kRemainder><<<blocks(c->nf, 256), 256, 0, st>>>(
+        fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->npad, k);
+    return;
+  }
+  if constexpr (sizeof(T) == 4) {
+    switch (c->tile) {
+      case 1282: launch_bulk<T, 128, 4>(c, fin, fout, k, st); break;
+      case 1286: launch_bulk<T, 128, 6>(c, fin, fout, k, st); break;
+      case 2562: launch_bulk<T, 256, 2>(c, fin, fout, k, st); break;
+      case 2563: launch_bulk<T, 256, 3>(c, fin, fout, k, st); break;
+      default: launch_bulk<T, 128, 5>(c, fin, fout, k, st); break;
+    }
+  } else {
+    launch_bulk<T, 128, 2>(c, fin, fout, k, st);
+  }
+}
+
 template <typename T>
 int step_T(lbm_ctx* c, int n, cudaStream_t st) {
   const Consts<T> k = make_consts<T>(c->p);
   const OpenPlane<T> op = make_open<T>(c->p);
-  constexpr bool kRemainder = sizeof(T) == 4;
   for (int it = 0; it < n; ++it) {
     const T* fin = (const T*)c->f[c->cur];
     T* fout = (T*)c->f[c->cur ^ 1];
     launch_psi<T>(c, st);
     {
       Timed t(c, st, 2);
-      k_collide_stream<T, kRemainder><<<blocks(c->nf, 256), 256, 0, st>>>(
-          fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->npad, k);
+      launch_collide<T>(c, fin, fout, k, st);
     }
     if (c->p.z_open) {
       Timed t(c, st, 3);
@@ -257,7 +299,9 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   c->nx = nx; c->ny = ny; c->nz = nz; c->np = nx * ny; c->nvox = g.nvox;
   c->nf = (int)g.nf; c->nw = (int)g.nw;
   c->bits = p->storage_bits; c->esz = p->storage_bits / 8;
-  c->npad = pad64(g.nf); c->nwpad = pad64(g.nw);
+  if (const char* e = std::getenv("LBM_B200_COLLIDE")) c->collide_variant = std::strcmp(e, "simple") ? 1 : 0;
+  if (const char* e = std::getenv("LBM_B200_TILE")) c->tile = std::atoi(e);
+  c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
   if ((size_t)2 * 19 * c->npad >= ((size_t)1 << 31)) {
     delete c;
     return fail(LBM_EINVAL, "too many fluid nodes for 32-bit slot indices");
