@@ -267,18 +267,22 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
                "r"(bytes)
                : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
-      "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\n"
-      "bra WAIT_%=;\n"
-      "DONE_%=:\n"
-      "}\n" ::"r"(smem_u32(bar)),
-      "r"(parity)
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
       : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) {
+  }
 }
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes,
                                          uint64_t* bar) {
@@ -287,6 +291,17 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
           "r"(smem_u32(dst)),
       "l"(src), "r"(bytes), "r"(smem_u32(bar))
       : "memory");
+}
+
+// e_i . (x,y,z) without a zero-initialised accumulator (0 + x cannot be folded under IEEE rules)
+template <typename T>
+__device__ __forceinline__ T edot(int i, T x, T y, T z) {
+  T r = T(0);
+  bool init = false;
+  if (ex(i)) { r = T(ex(i)) * x; init = true; }
+  if (ey(i)) { r = init ? r + T(ey(i)) * y : T(ey(i)) * y; init = true; }
+  if (ez(i)) { r = init ? r + T(ez(i)) * z : T(ez(i)) * z; init = true; }
+  return r;
 }
 
 template <typename T, int TN>
@@ -317,10 +332,18 @@ __global__ void __launch_bounds__(TN, MINB)
         bulk_g2s(sid + (size_t)(r - 2 * Q) * TN, nbr + (size_t)(r - 2 * Q) * npad + t0,
                  TN * sizeof(int), &bar);
     }
+    // Only the producer warp spins on the mbarrier; everyone else joins at the block barrier.
+    // (A data-dependent spin executed by all warps makes ptxas treat the rest of the kernel as
+    // divergent: it then re-materialises the global-memory descriptor with an R2UR pair in front
+    // of every load/store -- 104 extra XU-pipe instructions per thread; profiles/r1_v2_collide.md.)
+    mbar_wait(&bar, 0);
   }
-  mbar_wait(&bar, 0);
+  __syncthreads();
+  // No early exit: threads of the ragged last tile compute on the zero padding and only their
+  // stores are predicated off, so control flow stays warp-uniform (keeps the memory descriptors
+  // in uniform registers instead of one R2UR pair per store).
   const int n = (int)t0 + tid;
-  if (n >= nf) return;
+  const bool valid = n < nf;
 
   // a3 inputs: psi gathers through the staged neighbour ids (ids are re-read from shared memory
   // at store time instead of being held in registers)
@@ -394,10 +417,8 @@ __global__ void __launch_bounds__(TN, MINB)
       static_assert(opp(1) == 2 && opp(7) == 10 && opp(9) == 8, "pairing below relies on the table");
       const int ip = i, im = opp(i);
       const T w = wgt<T>(ip);
-      T eu = T(0), eF = T(0);
-      if (ex(ip)) { eu += T(ex(ip)) * u[0]; eF += T(ex(ip)) * F0; }
-      if (ey(ip)) { eu += T(ey(ip)) * u[1]; eF += T(ey(ip)) * F1; }
-      if (ez(ip)) { eu += T(ez(ip)) * u[2]; eF += T(ez(ip)) * F2; }
+      const T eu = edot<T>(ip, u[0], u[1], u[2]);
+      const T eF = edot<T>(ip, F0, F1, F2);
       const T kA = om * w * rho, kB = cS * w;
       const T A = T(4.5) * eu * eu + k0;
       const T B = T(9) * eu * eF + m3uF;
@@ -406,15 +427,19 @@ __global__ void __launch_bounds__(TN, MINB)
       const T vp = c1 * sfs[ip * TN] + X + Y;
       const T vm = c1 * sfs[im * TN] + X - Y;
       acc += vp + vm;
+      // push-streaming with halfway bounce-back, branch-free: one predicated store per
+      // population (k < 0: the population leaves through an open plane and is dropped)
       {
         const int k = sid[(ip - 1) * TN + tid];
-        if ((unsigned)k < (unsigned)nf) fo[(unsigned)ip * np32 + (unsigned)k] = vp;  // fluid neighbour
-        else if (k >= nf) fo[(unsigned)im * np32 + (unsigned)n] = vp;  // halfway bounce-back
+        const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)ip * np32 + (unsigned)k
+                                                         : (unsigned)im * np32 + (unsigned)n;
+        if (valid && k >= 0) fo[slot] = vp;
       }
       {
         const int k = sid[(im - 1) * TN + tid];
-        if ((unsigned)k < (unsigned)nf) fo[(unsigned)im * np32 + (unsigned)k] = vm;
-        else if (k >= nf) fo[(unsigned)ip * np32 + (unsigned)n] = vm;
+        const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)im * np32 + (unsigned)k
+                                                         : (unsigned)ip * np32 + (unsigned)n;
+        if (valid && k >= 0) fo[slot] = vm;
       }
     }
     // rest population: Eq. (1) with e_0 = 0, or the remainder rho - sum_{i>=1} f*_i (fp32 build)
@@ -425,7 +450,7 @@ __global__ void __launch_bounds__(TN, MINB)
       const T w0 = wgt<T>(0);
       v0 = c1 * sfs[0] + om * w0 * rho * k0 + cS * w0 * m3uF;
     }
-    fo[n] = v0;
+    if (valid) fo[n] = v0;
   }
 }
 
