@@ -280,9 +280,33 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
+// Warp-uniform wait: lane 0 polls, the result is broadcast with a shuffle, so the spin loop's
+// exit condition is a warp-uniform value.  (A spin whose exit depends on a per-thread asm result
+// makes ptxas treat everything after it as divergent: it then re-materialises the global-memory
+// descriptor with an R2UR pair in front of every load/store -- ~100 extra XU-pipe instructions per
+// thread, measured in profiles/r1_v2_collide.md.)  Must be called by all 32 lanes of a warp.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  while (!mbar_try_wait(bar, parity)) {
+  const bool leader = (threadIdx.x & 31) == 0;
+  while (true) {
+    uint32_t ok = 0;
+    if (leader) ok = mbar_try_wait(bar, parity) ? 1u : 0u;
+    if (__shfl_sync(0xffffffffu, ok, 0)) break;
   }
+}
+// One lane of a converged warp, chosen by hardware (elect.sync): the compiler keeps the guarded
+// code on the uniform datapath, so cp.async.bulk is issued as a single UBLKCP per copy.  (Issuing
+// one copy per lane instead compiles to a VOTEU/R2UR.BROADCAST loop that serialises the 56 copies
+// of a tile at ~50 cycles each: profiles/r1_v2_collide.md.)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n"
+      ".reg .pred P;\n"
+      "elect.sync _|P, 0xffffffff;\n"
+      "selp.u32 %0, 1, 0, P;\n"
+      "}\n"
+      : "=r"(pred));
+  return pred != 0;
 }
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes,
                                          uint64_t* bar) {
@@ -309,41 +333,17 @@ constexpr size_t collide_smem_bytes() {
   return (size_t)2 * Q * TN * sizeof(T) + (size_t)18 * TN * sizeof(int);
 }
 
-template <typename T, int TN, int MINB, bool REMAINDER>
-__global__ void __launch_bounds__(TN, MINB)
-    k_collide_stream_bulk(const T* __restrict__ fin, T* __restrict__ fout,
-                          const Vec2<T>* __restrict__ psi, const int* __restrict__ nbr, int nf,
-                          size_t npad, Consts<T> c) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  T* sf = reinterpret_cast<T*>(smem_raw);                                   // [38][TN]
-  int* sid = reinterpret_cast<int*>(smem_raw + (size_t)2 * Q * TN * sizeof(T));  // [18][TN]
-  __shared__ uint64_t bar;
-  const int tid = threadIdx.x;
-  const size_t t0 = (size_t)blockIdx.x * TN;
-  if (tid == 0) mbar_init(&bar, 1);
-  __syncthreads();
-  if (tid < 32) {
-    if (tid == 0) mbar_expect_tx(&bar, (uint32_t)collide_smem_bytes<T, TN>());
-    __syncwarp();
-    for (int r = tid; r < 2 * Q + 18; r += 32) {
-      if (r < 2 * Q)
-        bulk_g2s(sf + (size_t)r * TN, fin + (size_t)r * npad + t0, TN * sizeof(T), &bar);
-      else
-        bulk_g2s(sid + (size_t)(r - 2 * Q) * TN, nbr + (size_t)(r - 2 * Q) * npad + t0,
-                 TN * sizeof(int), &bar);
-    }
-    // Only the producer warp spins on the mbarrier; everyone else joins at the block barrier.
-    // (A data-dependent spin executed by all warps makes ptxas treat the rest of the kernel as
-    // divergent: it then re-materialises the global-memory descriptor with an R2UR pair in front
-    // of every load/store -- 104 extra XU-pipe instructions per thread; profiles/r1_v2_collide.md.)
-    mbar_wait(&bar, 0);
-  }
-  __syncthreads();
-  // No early exit: threads of the ragged last tile compute on the zero padding and only their
-  // stores are predicated off, so control flow stays warp-uniform (keeps the memory descriptors
-  // in uniform registers instead of one R2UR pair per store).
-  const int n = (int)t0 + tid;
-  const bool valid = n < nf;
+// Per-thread work of the fused pass on a staged tile: sf = [38][TN] populations, sid = [18][TN]
+// neighbour ids in shared memory; lt = column of this thread in the tile; n = its node id.
+// Threads of the ragged last tile (valid = false) compute on the zero padding and only their
+// stores are predicated off, so control flow stays warp-uniform.
+template <typename T, int TN, bool REMAINDER>
+__device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
+                                                    const int* __restrict__ sid, const int tid,
+                                                    const int n, const bool valid,
+                                                    T* __restrict__ fout,
+                                                    const Vec2<T>* __restrict__ psi, const int nf,
+                                                    const size_t npad, const Consts<T>& c) {
 
   // a3 inputs: psi gathers through the staged neighbour ids (ids are re-read from shared memory
   // at store time instead of being held in registers)
@@ -453,6 +453,45 @@ __global__ void __launch_bounds__(TN, MINB)
     if (valid) fo[n] = v0;
   }
 }
+
+// Stage one tile: 38 population rows + 18 neighbour-index rows of TN nodes -> shared memory,
+// completion on `bar`.  Call from one converged warp.
+template <typename T, int TN>
+__device__ __forceinline__ void load_tile(T* sf, int* sid, const T* __restrict__ fin,
+                                          const int* __restrict__ nbr, size_t npad, size_t t0,
+                                          uint64_t* bar) {
+  if (elect_one()) {
+    mbar_expect_tx(bar, (uint32_t)collide_smem_bytes<T, TN>());
+#pragma unroll
+    for (int r = 0; r < 2 * Q; ++r)
+      bulk_g2s(sf + (size_t)r * TN, fin + (size_t)r * npad + t0, TN * sizeof(T), bar);
+#pragma unroll
+    for (int r = 0; r < 18; ++r)
+      bulk_g2s(sid + (size_t)r * TN, nbr + (size_t)r * npad + t0, TN * sizeof(int), bar);
+  }
+  __syncwarp();
+}
+
+template <typename T, int TN, int MINB, bool REMAINDER>
+__global__ void __launch_bounds__(TN, MINB)
+    k_collide_stream_bulk(const T* __restrict__ fin, T* __restrict__ fout,
+                          const Vec2<T>* __restrict__ psi, const int* __restrict__ nbr, int nf,
+                          size_t npad, Consts<T> c) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* sf = reinterpret_cast<T*>(smem_raw);                                   // [38][TN]
+  int* sid = reinterpret_cast<int*>(smem_raw + (size_t)2 * Q * TN * sizeof(T));  // [18][TN]
+  __shared__ uint64_t bar;
+  const int tid = threadIdx.x;
+  const size_t t0 = (size_t)blockIdx.x * TN;
+  if (tid == 0) mbar_init(&bar, 1);
+  __syncthreads();
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // compiler-visible warp-uniform value
+  if (warp == 0) load_tile<T, TN>(sf, sid, fin, nbr, npad, t0, &bar);
+  mbar_wait(&bar, 0);
+  const int n = (int)t0 + tid;
+  collide_tile_thread<T, TN, REMAINDER>(sf, sid, tid, n, n < nf, fout, psi, nf, npad, c);
+}
+
 
 // ---------------------------------------------------------------------------------------------
 // a0  open-plane fix on the new buffer (reading R12 of PAPER.md L147-157, L223): planes z=0 and

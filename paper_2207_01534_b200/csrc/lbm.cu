@@ -82,8 +82,10 @@ struct lbm_ctx {
   double* diag_out = nullptr;                     // [6] + count
   int diag_blocks = 0;
   int cur = 0;
-  int collide_variant = 1;  // 0: register kernel, 1: bulk-async staged (default); env LBM_B200_COLLIDE
-  int tile = 1285;          // fp32 bulk kernel variant: tile nodes * 10 + min CTAs/SM; env LBM_B200_TILE
+  int collide_variant = 1;  // 0: register kernel (A/B reference), 1: bulk-async staged tiles
+                            // (production); env LBM_B200_COLLIDE=simple|bulk
+  int num_sms = 148;
+  int tile = 1286;          // fp32 bulk kernel variant: tile nodes * 10 + min CTAs/SM; env LBM_B200_TILE
   long long bytes[4] = {0, 0, 0, 0};
   bool prof = false;
   std::vector<ProfEvent> prof_events;
@@ -183,11 +185,9 @@ void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaS
   }
   if constexpr (sizeof(T) == 4) {
     switch (c->tile) {
-      case 1282: launch_bulk<T, 128, 4>(c, fin, fout, k, st); break;
-      case 1286: launch_bulk<T, 128, 6>(c, fin, fout, k, st); break;
-      case 2562: launch_bulk<T, 256, 2>(c, fin, fout, k, st); break;
+      case 1285: launch_bulk<T, 128, 5>(c, fin, fout, k, st); break;
       case 2563: launch_bulk<T, 256, 3>(c, fin, fout, k, st); break;
-      default: launch_bulk<T, 128, 5>(c, fin, fout, k, st); break;
+      default: launch_bulk<T, 128, 6>(c, fin, fout, k, st); break;
     }
   } else {
     launch_bulk<T, 128, 2>(c, fin, fout, k, st);
@@ -295,11 +295,12 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   lbm_ctx* c = new (std::nothrow) lbm_ctx;
   if (!c) return fail(LBM_ENOMEM, "host allocation failed");
   CU(cudaGetDevice(&c->device));
+  cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
   c->p = *p;
   c->nx = nx; c->ny = ny; c->nz = nz; c->np = nx * ny; c->nvox = g.nvox;
   c->nf = (int)g.nf; c->nw = (int)g.nw;
   c->bits = p->storage_bits; c->esz = p->storage_bits / 8;
-  if (const char* e = std::getenv("LBM_B200_COLLIDE")) c->collide_variant = std::strcmp(e, "simple") ? 1 : 0;
+  if (const char* e = std::getenv("LBM_B200_COLLIDE")) c->collide_variant = !std::strcmp(e, "simple") ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_TILE")) c->tile = std::atoi(e);
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
   if ((size_t)2 * 19 * c->npad >= ((size_t)1 << 31)) {
