@@ -333,8 +333,66 @@ constexpr size_t collide_smem_bytes() {
   return (size_t)2 * Q * TN * sizeof(T) + (size_t)18 * TN * sizeof(int);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Component pairs.  The two fluid components go through identical arithmetic with different
+// (rho, F) and the same u, so the fused pass carries every per-component quantity as a pair
+// (A, B).  For fp32 the pair operations are Blackwell's packed FP32x2 instructions (PTX
+// add/sub/mul/fma .f32x2 -> SASS FADD2/FMUL2/FFMA2, two FP32 results per issue slot; a scalar
+// broadcast operand and the half-swap are free operand modifiers); for fp64 they are two plain
+// operations.  This halves the floating-point issue slots of an issue-bound kernel.
+template <typename T> struct Pr { T a, b; };
+
+__device__ __forceinline__ Pr<double> padd(Pr<double> x, Pr<double> y) { return {x.a + y.a, x.b + y.b}; }
+__device__ __forceinline__ Pr<double> psub(Pr<double> x, Pr<double> y) { return {x.a - y.a, x.b - y.b}; }
+__device__ __forceinline__ Pr<double> pmul(Pr<double> x, Pr<double> y) { return {x.a * y.a, x.b * y.b}; }
+__device__ __forceinline__ Pr<double> pfma(Pr<double> x, Pr<double> y, Pr<double> z) {
+  return {x.a * y.a + z.a, x.b * y.b + z.b};
+}
+__device__ __forceinline__ Pr<float> padd(Pr<float> x, Pr<float> y) {
+  Pr<float> d;
+  asm("{.reg .b64 ra,rb,rd; mov.b64 ra,{%2,%3}; mov.b64 rb,{%4,%5}; add.rn.f32x2 rd,ra,rb; "
+      "mov.b64 {%0,%1},rd;}"
+      : "=f"(d.a), "=f"(d.b) : "f"(x.a), "f"(x.b), "f"(y.a), "f"(y.b));
+  return d;
+}
+__device__ __forceinline__ Pr<float> psub(Pr<float> x, Pr<float> y) {
+  Pr<float> d;
+  asm("{.reg .b64 ra,rb,rd; mov.b64 ra,{%2,%3}; mov.b64 rb,{%4,%5}; sub.rn.f32x2 rd,ra,rb; "
+      "mov.b64 {%0,%1},rd;}"
+      : "=f"(d.a), "=f"(d.b) : "f"(x.a), "f"(x.b), "f"(y.a), "f"(y.b));
+  return d;
+}
+__device__ __forceinline__ Pr<float> pmul(Pr<float> x, Pr<float> y) {
+  Pr<float> d;
+  asm("{.reg .b64 ra,rb,rd; mov.b64 ra,{%2,%3}; mov.b64 rb,{%4,%5}; mul.rn.f32x2 rd,ra,rb; "
+      "mov.b64 {%0,%1},rd;}"
+      : "=f"(d.a), "=f"(d.b) : "f"(x.a), "f"(x.b), "f"(y.a), "f"(y.b));
+  return d;
+}
+__device__ __forceinline__ Pr<float> pfma(Pr<float> x, Pr<float> y, Pr<float> z) {
+  Pr<float> d;
+  asm("{.reg .b64 ra,rb,rc,rd; mov.b64 ra,{%2,%3}; mov.b64 rb,{%4,%5}; mov.b64 rc,{%6,%7}; "
+      "fma.rn.f32x2 rd,ra,rb,rc; mov.b64 {%0,%1},rd;}"
+      : "=f"(d.a), "=f"(d.b)
+      : "f"(x.a), "f"(x.b), "f"(y.a), "f"(y.b), "f"(z.a), "f"(z.b));
+  return d;
+}
+template <typename T> __device__ __forceinline__ Pr<T> pbc(T s) { return {s, s}; }       // broadcast
+template <typename T> __device__ __forceinline__ Pr<T> pswap(Pr<T> x) { return {x.b, x.a}; }
+
+// e_i . (X, Y, Z) on pairs, no zero-initialised accumulator
+template <typename T>
+__device__ __forceinline__ Pr<T> edot2(int i, Pr<T> x, Pr<T> y, Pr<T> z) {
+  Pr<T> r = {T(0), T(0)};
+  bool init = false;
+  if (ex(i)) { r = ex(i) > 0 ? x : psub(r, x); init = true; }
+  if (ey(i)) { r = !init ? (ey(i) > 0 ? y : psub(r, y)) : (ey(i) > 0 ? padd(r, y) : psub(r, y)); init = true; }
+  if (ez(i)) { r = !init ? (ez(i) > 0 ? z : psub(r, z)) : (ez(i) > 0 ? padd(r, z) : psub(r, z)); init = true; }
+  return r;
+}
+
 // Per-thread work of the fused pass on a staged tile: sf = [38][TN] populations, sid = [18][TN]
-// neighbour ids in shared memory; lt = column of this thread in the tile; n = its node id.
+// neighbour ids in shared memory; tid = column of this thread in the tile; n = its node id.
 // Threads of the ragged last tile (valid = false) compute on the zero padding and only their
 // stores are predicated off, so control flow stays warp-uniform.
 template <typename T, int TN, bool REMAINDER>
@@ -344,114 +402,113 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
                                                     T* __restrict__ fout,
                                                     const Vec2<T>* __restrict__ psi, const int nf,
                                                     const size_t npad, const Consts<T>& c) {
+  using P = Pr<T>;
+  const T* sfa = sf + tid;                   // component A column
+  const T* sfb = sf + (size_t)Q * TN + tid;  // component B column
+  const int* sidc = sid + tid;
 
-  // a3 inputs: psi gathers through the staged neighbour ids (ids are re-read from shared memory
-  // at store time instead of being held in registers)
-  T SA[3], SB[3];
+  // a3 inputs: Psi gathers through the staged neighbour ids.  S[d] = sum_i w_i e_id Psi(x+e_i) as
+  // a pair (A, B); axis (w=1/18) and diagonal (w=1/36) neighbours are summed separately.
+  P S[3];
   {
-    T a1[3] = {T(0), T(0), T(0)}, b1[3] = {T(0), T(0), T(0)};
-    T a2[3] = {T(0), T(0), T(0)}, b2[3] = {T(0), T(0), T(0)};
+    P a1[3] = {{T(0), T(0)}, {T(0), T(0)}, {T(0), T(0)}};
+    P a2[3] = {{T(0), T(0)}, {T(0), T(0)}, {T(0), T(0)}};
 #pragma unroll
     for (int i = 1; i < Q; ++i) {
-      const int k0 = sid[(i - 1) * TN + tid];
+      const int k0 = sidc[(i - 1) * TN];
       const int k = k0 >= 0 ? k0 : -k0 - 1;  // mirror node beyond an open plane (R12 iv)
-      const Vec2<T> p = psi[k];
-      if (i < 7) {
-        if (ex(i)) { a1[0] += T(ex(i)) * p.a; b1[0] += T(ex(i)) * p.b; }
-        if (ey(i)) { a1[1] += T(ey(i)) * p.a; b1[1] += T(ey(i)) * p.b; }
-        if (ez(i)) { a1[2] += T(ez(i)) * p.a; b1[2] += T(ez(i)) * p.b; }
-      } else {
-        if (ex(i)) { a2[0] += T(ex(i)) * p.a; b2[0] += T(ex(i)) * p.b; }
-        if (ey(i)) { a2[1] += T(ey(i)) * p.a; b2[1] += T(ey(i)) * p.b; }
-        if (ez(i)) { a2[2] += T(ez(i)) * p.a; b2[2] += T(ez(i)) * p.b; }
-      }
+      const Vec2<T> v = psi[k];
+      const P p = {v.a, v.b};
+      P* acc = i < 7 ? a1 : a2;
+      if (ex(i)) acc[0] = ex(i) > 0 ? padd(acc[0], p) : psub(acc[0], p);
+      if (ey(i)) acc[1] = ey(i) > 0 ? padd(acc[1], p) : psub(acc[1], p);
+      if (ez(i)) acc[2] = ez(i) > 0 ? padd(acc[2], p) : psub(acc[2], p);
     }
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      SA[d] = wgt<T>(1) * a1[d] + wgt<T>(7) * a2[d];
-      SB[d] = wgt<T>(1) * b1[d] + wgt<T>(7) * b2[d];
-    }
+    for (int d = 0; d < 3; ++d)
+      S[d] = pfma(pbc(wgt<T>(1)), a1[d], pmul(pbc(wgt<T>(7)), a2[d]));
   }
-  // a1 (recomputed locally) + bare momentum
-  T ra = sf[tid], rb = sf[Q * TN + tid];
-  T j[3] = {T(0), T(0), T(0)};
+  // a1 (recomputed locally): R = (rho_A, rho_B); J[d] = per-component bare momentum
+  P R = {sfa[0], sfb[0]};
+  P J[3] = {{T(0), T(0)}, {T(0), T(0)}, {T(0), T(0)}};
 #pragma unroll
   for (int i = 1; i < Q; ++i) {
-    const T a = sf[i * TN + tid], b = sf[(Q + i) * TN + tid];
-    ra += a;
-    rb += b;
-    const T t = a + b;
-    if (ex(i)) j[0] += T(ex(i)) * t;
-    if (ey(i)) j[1] += T(ey(i)) * t;
-    if (ez(i)) j[2] += T(ez(i)) * t;
+    const P f = {sfa[i * TN], sfb[i * TN]};
+    R = padd(R, f);
+    if (ex(i)) J[0] = ex(i) > 0 ? padd(J[0], f) : psub(J[0], f);
+    if (ey(i)) J[1] = ey(i) > 0 ? padd(J[1], f) : psub(J[1], f);
+    if (ez(i)) J[2] = ez(i) > 0 ? padd(J[2], f) : psub(J[2], f);
   }
+  // a3: F_sigma = rho_sigma (-G S_sigmabar + g)   (Eq. 10, 11, 13; body force R8)
   const T g[3] = {c.gx, c.gy, c.gz};
-  T FA[3], FB[3], u[3];
+  P F[3];
+  T u[3];
+  const T rho = R.a + R.b;
+  const T inv = T(1) / rho;
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    FA[d] = -c.G * ra * SB[d] + ra * g[d];
-    FB[d] = -c.G * rb * SA[d] + rb * g[d];
+    F[d] = pmul(R, pfma(pbc(-c.G), pswap(S[d]), pbc(g[d])));
+    // a4: u_eq = (sum_sigma j_sigma + hf * sum_sigma F_sigma) / rho   (Eq. 8, R3)
+    u[d] = ((J[d].a + J[d].b) + c.hf * (F[d].a + F[d].b)) * inv;
   }
-  const T inv = T(1) / (ra + rb);
-#pragma unroll
-  for (int d = 0; d < 3; ++d) u[d] = (j[d] + c.hf * (FA[d] + FB[d])) * inv;
-  const T om = (ra + rb) / (ra * c.tauA + rb * c.tauB);
-  // Collision in opposite-direction pairs (i, opp(i)): with A = 1 + 4.5 (e.u)^2 - 1.5 u.u and
+  const T om = rho / (R.a * c.tauA + R.b * c.tauB);  // 1/tau_s, Eq. (6)-(7)
+  // a5 in opposite-direction pairs (i, opp(i)): with A = 1 + 4.5 (e.u)^2 - 1.5 u.u and
   // B = 9 (e.u)(e.F) - 3 u.F, Eq. (1),(2),(9) give
   //   f*_i      = (1-om) f_i      + [om w rho A + cS w B] + 3 [om w rho (e.u) + cS w (e.F)]
   //   f*_opp(i) = (1-om) f_opp(i) + [om w rho A + cS w B] - 3 [om w rho (e.u) + cS w (e.F)]
-  // (the bracketed even/odd parts are shared by the pair), cS = 1 - om/2.
+  // with cS = 1 - om/2; both components at once as pairs.
   const T k0 = T(1) - T(1.5) * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
   const T c1 = T(1) - om, cS = T(1) - T(0.5) * om;
+  const P M3UF = pmul(pbc(T(-3)), pfma(pbc(u[0]), F[0], pfma(pbc(u[1]), F[1], pmul(pbc(u[2]), F[2]))));
+  const P KA1 = pmul(pbc(om * wgt<T>(1)), R), KA2 = pmul(pbc(om * wgt<T>(7)), R);
+  const T kB1 = cS * wgt<T>(1), kB2 = cS * wgt<T>(7);
   const unsigned np32 = (unsigned)npad;  // 38 * npad < 2^31: 32-bit slot indices
+  T* foa = fout;
+  T* fob = fout + (size_t)Q * npad;
+  P acc = {T(0), T(0)};
 #pragma unroll
-  for (int s = 0; s < 2; ++s) {
-    const T rho = s == 0 ? ra : rb;
-    const T F0 = s == 0 ? FA[0] : FB[0], F1 = s == 0 ? FA[1] : FB[1], F2 = s == 0 ? FA[2] : FB[2];
-    const T m3uF = T(-3) * (u[0] * F0 + u[1] * F1 + u[2] * F2);
-    const T* sfs = sf + (size_t)s * Q * TN + tid;
-    T* fo = fout + (size_t)s * Q * npad;
-    T acc = T(0);
-#pragma unroll
-    for (int i = 1; i < Q; i += 2) {  // canonical order: opp(i) == i + 1 for odd i
-      static_assert(opp(1) == 2 && opp(7) == 10 && opp(9) == 8, "pairing below relies on the table");
-      const int ip = i, im = opp(i);
-      const T w = wgt<T>(ip);
-      const T eu = edot<T>(ip, u[0], u[1], u[2]);
-      const T eF = edot<T>(ip, F0, F1, F2);
-      const T kA = om * w * rho, kB = cS * w;
-      const T A = T(4.5) * eu * eu + k0;
-      const T B = T(9) * eu * eF + m3uF;
-      const T X = kA * A + kB * B;
-      const T Y = T(3) * (kA * eu + kB * eF);
-      const T vp = c1 * sfs[ip * TN] + X + Y;
-      const T vm = c1 * sfs[im * TN] + X - Y;
-      acc += vp + vm;
-      // push-streaming with halfway bounce-back, branch-free: one predicated store per
-      // population (k < 0: the population leaves through an open plane and is dropped)
-      {
-        const int k = sid[(ip - 1) * TN + tid];
-        const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)ip * np32 + (unsigned)k
-                                                         : (unsigned)im * np32 + (unsigned)n;
-        if (valid && k >= 0) fo[slot] = vp;
-      }
-      {
-        const int k = sid[(im - 1) * TN + tid];
-        const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)im * np32 + (unsigned)k
-                                                         : (unsigned)ip * np32 + (unsigned)n;
-        if (valid && k >= 0) fo[slot] = vm;
-      }
+  for (int i = 1; i < Q; i += 2) {  // canonical order: the opposite of an odd i is its partner
+    static_assert(opp(1) == 2 && opp(7) == 10 && opp(9) == 8, "pairing below relies on the table");
+    const int ip = i, im = opp(i);
+    const P KA = ip < 7 ? KA1 : KA2;
+    const T kB = ip < 7 ? kB1 : kB2;
+    const T eu = edot<T>(ip, u[0], u[1], u[2]);
+    const P EF = edot2<T>(ip, F[0], F[1], F[2]);
+    const T A = T(4.5) * eu * eu + k0;
+    const P B = pfma(pbc(T(9) * eu), EF, M3UF);
+    const P X = pfma(KA, pbc(A), pmul(pbc(kB), B));
+    const P Y = pfma(KA, pbc(eu), pmul(pbc(kB), EF));
+    const P fp = {sfa[ip * TN], sfb[ip * TN]};
+    const P fm = {sfa[im * TN], sfb[im * TN]};
+    const P vp = pfma(pbc(c1), fp, pfma(Y, pbc(T(3)), X));
+    const P vm = pfma(pbc(c1), fm, pfma(Y, pbc(T(-3)), X));
+    acc = padd(acc, padd(vp, vm));
+    // a6: push-streaming with halfway bounce-back, branch-free: the slot is computed once per
+    // direction and used for both components; one predicated store per population
+    // (k < 0: the population leaves through an open plane and is dropped).
+    {
+      const int k = sidc[(ip - 1) * TN];
+      const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)ip * np32 + (unsigned)k
+                                                       : (unsigned)im * np32 + (unsigned)n;
+      if (valid && k >= 0) { foa[slot] = vp.a; fob[slot] = vp.b; }
     }
-    // rest population: Eq. (1) with e_0 = 0, or the remainder rho - sum_{i>=1} f*_i (fp32 build)
-    T v0;
-    if (REMAINDER) {
-      v0 = rho - acc;
-    } else {
-      const T w0 = wgt<T>(0);
-      v0 = c1 * sfs[0] + om * w0 * rho * k0 + cS * w0 * m3uF;
+    {
+      const int k = sidc[(im - 1) * TN];
+      const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)im * np32 + (unsigned)k
+                                                       : (unsigned)ip * np32 + (unsigned)n;
+      if (valid && k >= 0) { foa[slot] = vm.a; fob[slot] = vm.b; }
     }
-    if (valid) fo[n] = v0;
   }
+  // rest population: Eq. (1) with e_0 = 0, or the remainder rho - sum_{i>=1} f*_i (fp32 build)
+  P v0;
+  if (REMAINDER) {
+    v0 = psub(R, acc);
+  } else {
+    const T w0 = wgt<T>(0);
+    const P f0 = {sfa[0], sfb[0]};
+    v0 = pfma(pbc(c1), f0, pfma(pbc(om * w0 * k0), R, pmul(pbc(cS * w0), M3UF)));
+  }
+  if (valid) { foa[n] = v0.a; fob[n] = v0.b; }
 }
 
 // Stage one tile: 38 population rows + 18 neighbour-index rows of TN nodes -> shared memory,
