@@ -124,6 +124,15 @@ const char* lbm_last_error(void);
 int lbm_build_index(const uint8_t* solid, int nx, int ny, int nz, int z_open, int32_t* vox2id,
                     int32_t* nbr, long long nbr_cap, long long* nf, long long* nw);
 
+/* Host-only helper (no GPU needed): the work schedule of the fused single-kernel step exactly as
+ * lbm_create builds it.  records: caller-allocated, cap_items*16 int32;
+ * item k is records[16k..16k+15] = {type<<30 | tile, 3 x (lo,cnt) D-tile dependency ranges,
+ * 3 x (lo,cnt) W-tile dependency ranges, 0, 0, 0}, type 0 = density pass on a fluid tile, 1 =
+ * virtual-solid pass on a wall tile, 2 = fused collide+stream pass on a fluid tile; tiles are
+ * `tile` consecutive ids.  *n_items receives the item count (2*ceil(N_f/tile)+ceil(N_w/tile)). */
+int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open, int tile,
+                       int lead, int32_t* records, long long cap_items, long long* n_items);
+
 #ifdef __cplusplus
 }
 #endif

@@ -1,7 +1,9 @@
 // geometry.cpp -- see geometry.hpp.  Host only, O(voxels), not on the timed path.
 #include "geometry.hpp"
 
+#include <algorithm>
 #include <new>
+#include <utility>
 
 namespace lbmgeo {
 
@@ -109,6 +111,146 @@ int build(Geometry& g, const uint8_t* solid, int nx, int ny, int nz, int z_open,
       }
       g.wall_inv_den[w] = 1.0 / den;
     }
+  } catch (const std::bad_alloc&) {
+    return -4;
+  }
+  return 0;
+}
+
+namespace {
+
+// Compress a sorted list of distinct tile ids into at most kDepRanges (lo,cnt) ranges by closing
+// the smallest gaps first (a range may then cover tiles that are not strictly needed).
+void to_ranges(std::vector<int32_t>& ids, int32_t* out /* 2*kDepRanges */) {
+  for (int k = 0; k < 2 * kDepRanges; ++k) out[k] = 0;
+  if (ids.empty()) return;
+  std::sort(ids.begin(), ids.end());
+  ids.erase(std::unique(ids.begin(), ids.end()), ids.end());
+  std::vector<std::pair<int32_t, int32_t>> r;  // [lo, hi]
+  for (int32_t v : ids) {
+    if (!r.empty() && v == r.back().second + 1) r.back().second = v;
+    else r.emplace_back(v, v);
+  }
+  while ((int)r.size() > kDepRanges) {
+    size_t best = 0;
+    int32_t gap = r[1].first - r[0].second;
+    for (size_t k = 1; k + 1 < r.size(); ++k)
+      if (r[k + 1].first - r[k].second < gap) { gap = r[k + 1].first - r[k].second; best = k; }
+    r[best].second = r[best + 1].second;
+    r.erase(r.begin() + best + 1);
+  }
+  for (size_t k = 0; k < r.size(); ++k) {
+    out[2 * k] = r[k].first;
+    out[2 * k + 1] = r[k].second - r[k].first + 1;
+  }
+}
+
+}  // namespace
+
+int build_schedule(const Geometry& g, int tile, int lead, Schedule& s) {
+  if (tile < 32 || g.nf <= 0 || g.nbr.empty()) return -1;
+  const long long nf = g.nf, nw = g.nw;
+  s.tile = tile;
+  s.ntf = (int)((nf + tile - 1) / tile);
+  s.ntw = (int)((nw + tile - 1) / tile);
+  const int ntf = s.ntf, ntw = s.ntw;
+  try {
+    // dependency ranges
+    std::vector<int32_t> dep_c((size_t)ntf * 4 * kDepRanges), dep_w((size_t)ntw * 2 * kDepRanges);
+#pragma omp parallel
+    {
+      std::vector<int32_t> ds, ws;
+#pragma omp for schedule(static)
+      for (int t = 0; t < ntf; ++t) {
+        ds.clear(); ws.clear();
+        const long long n1 = std::min<long long>(nf, (long long)(t + 1) * tile);
+        for (int i = 0; i < 18; ++i)
+          for (long long n = (long long)t * tile; n < n1; ++n) {
+            int32_t id = g.nbr[(size_t)i * nf + n];
+            if (id < 0) id = -id - 1;
+            const int32_t k = id < nf ? id / tile : (int32_t)((id - nf) / tile);
+            std::vector<int32_t>& v = id < nf ? ds : ws;
+            if (v.empty() || v.back() != k) v.push_back(k);
+          }
+        to_ranges(ds, &dep_c[(size_t)t * 4 * kDepRanges]);
+        to_ranges(ws, &dep_c[(size_t)t * 4 * kDepRanges + 2 * kDepRanges]);
+      }
+#pragma omp for schedule(static)
+      for (int j = 0; j < ntw; ++j) {
+        ds.clear();
+        const long long w1 = std::min<long long>(nw, (long long)(j + 1) * tile);
+        for (int i = 0; i < 18; ++i)
+          for (long long w = (long long)j * tile; w < w1; ++w) {
+            const int32_t id = g.wall_nbr[(size_t)i * nw + w];
+            if (id < 0) continue;
+            const int32_t k = id / tile;
+            if (ds.empty() || ds.back() != k) ds.push_back(k);
+          }
+        to_ranges(ds, &dep_w[(size_t)j * 2 * kDepRanges]);
+      }
+    }
+    // one global order in which dependencies always come first
+    s.records.clear();
+    s.records.reserve(((size_t)2 * ntf + ntw) * kRecordInts);
+    std::vector<uint8_t> done_d(ntf, 0), done_w(ntw, 0);
+    auto push = [&](int type, int t, const int32_t* d, const int32_t* w) {
+      const size_t base = s.records.size();
+      s.records.resize(base + kRecordInts, 0);
+      s.records[base] = (int32_t)(((uint32_t)type << 30) | (uint32_t)t);
+      for (int k = 0; k < 2 * kDepRanges; ++k) {
+        s.records[base + 1 + k] = d ? d[k] : 0;
+        s.records[base + 1 + 2 * kDepRanges + k] = w ? w[k] : 0;
+      }
+    };
+    auto emit_d = [&](int t) {
+      if (t < 0 || t >= ntf || done_d[t]) return;
+      done_d[t] = 1;
+      push(0, t, nullptr, nullptr);
+    };
+    auto emit_w = [&](int j) {
+      if (j < 0 || j >= ntw || done_w[j]) return;
+      done_w[j] = 1;
+      const int32_t* d = &dep_w[(size_t)j * 2 * kDepRanges];
+      for (int k = 0; k < kDepRanges; ++k)
+        for (int q = 0; q < d[2 * k + 1]; ++q) emit_d(d[2 * k] + q);
+      push(1, j, d, nullptr);
+    };
+    // Producers are issued ahead of need (lead D tiles, lead/4 W tiles beyond the furthest
+    // non-wrapping dependency), so that a consumer normally finds its flags set and never waits.
+    const int lead_w = lead / 4;
+    int cur_d = 0, cur_w = 0;
+    auto d_upto = [&](int x) {  // all D tiles <= x, in natural order
+      for (; cur_d <= std::min(ntf - 1, x); ++cur_d) emit_d(cur_d);
+    };
+    // furthest tile of 3 ranges that is not a periodic wrap-around seen from `from` (-1 if none)
+    auto far_of = [&](const int32_t* r, int from, int n) {
+      int far = -1;
+      for (int k = 0; k < kDepRanges; ++k) {
+        const int hi = r[2 * k] + r[2 * k + 1] - 1;
+        if (r[2 * k + 1] > 0 && hi > far && hi - from < n / 2 + 1) far = hi;
+      }
+      return far;
+    };
+    int want_w = -1;  // furthest W tile any C tile so far depends on
+    for (int t = 0; t < ntf; ++t) {
+      const int32_t* d = &dep_c[(size_t)t * 4 * kDepRanges];
+      const int32_t* w = d + 2 * kDepRanges;
+      want_w = std::max(want_w, far_of(w, std::max(want_w, 0), ntw));
+      for (; want_w >= 0 && cur_w <= std::min(ntw - 1, want_w + lead_w); ++cur_w) {
+        // the D tiles a W item reads are issued `lead` tiles before it
+        const int fd = far_of(&dep_w[(size_t)cur_w * 2 * kDepRanges], t, ntf);
+        if (fd >= 0) d_upto(fd + lead);
+        emit_w(cur_w);
+      }
+      d_upto(far_of(d, t, ntf) + lead);
+      for (int k = 0; k < kDepRanges; ++k) {
+        for (int q = 0; q < w[2 * k + 1]; ++q) emit_w(w[2 * k] + q);
+        for (int q = 0; q < d[2 * k + 1]; ++q) emit_d(d[2 * k] + q);
+      }
+      push(2, t, d, w);
+    }
+    for (int j = 0; j < ntw; ++j) emit_w(j);
+    for (int t = 0; t < ntf; ++t) emit_d(t);
   } catch (const std::bad_alloc&) {
     return -4;
   }

@@ -30,6 +30,24 @@ struct Geometry {
   std::vector<double> wall_inv_den;
 };
 
+// Work schedule of the fused single-kernel step.  The step is cut into
+// items -- D(t): density pass on fluid tile t, W(j): virtual-solid pass on wall tile j, C(t):
+// fused force+collide+stream pass on fluid tile t, tiles of `tile` consecutive ids -- and the items
+// are put in one global order in which every item comes after the items whose psi it reads.
+// Dependencies are explicit: each item lists up to kDepRanges ranges of D tiles and of W tiles
+// whose completion flags it must see (the psi stencil of a tile touches ~10 D tiles in three id
+// ranges, one per z-plane); there is no global watermark.
+constexpr int kDepRanges = 3;
+constexpr int kRecordInts = 16;  // {type<<30|tile, D: 3 x (lo,cnt), W: 3 x (lo,cnt), 0, 0, 0}
+struct Schedule {
+  int tile = 128;
+  int ntf = 0, ntw = 0;           // fluid / wall tiles
+  std::vector<int32_t> records;   // [nitems * kRecordInts]; type 0 = D, 1 = W, 2 = C
+  size_t nitems() const { return records.size() / kRecordInts; }
+};
+// lead = how many D tiles (lead/4 W tiles) beyond the strict need are issued ahead of each C tile
+int build_schedule(const Geometry& g, int tile, int lead, Schedule& s);
+
 // Returns 0, or -1 bad arguments, -2 no fluid voxel, -3 solid on an open plane or its interior
 // neighbour plane (z in {0,1,nz-2,nz-1}), -4 out of memory.  `with_tables` = also fill nbr,
 // wall_nbr, wall_inv_den.

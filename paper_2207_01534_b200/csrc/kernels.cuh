@@ -4,8 +4,10 @@
 //
 // Storage (T = float or double):
 //   f   [2 comps][19 dirs][npad]   populations at time t (post-streaming), node id fastest
-//   psi [nf + nw] of Vec2<T>       (rho_A, rho_B) on fluid ids, (rho~_A, rho~_B) on wall ids
-//   nbr [18][npad] int32           id of x+e_i (see geometry.hpp)
+//   psi [npad + nwpad] of Vec2<T>  (rho_A, rho_B) at fluid id n; (rho~_A, rho~_B) of wall solid w at
+//                                  npad + w (both parts start on a tile boundary)
+//   nbr [18][npad] int32           psi index of x+e_i: < nf fluid id; >= npad wall solid;
+//                                  -(m+1) beyond an open plane, m = mirror node (see geometry.hpp)
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -83,8 +85,9 @@ __global__ void __launch_bounds__(256) k_density(const T* __restrict__ f, Vec2<T
 template <typename T>
 __global__ void __launch_bounds__(256) k_wallpsi(Vec2<T>* __restrict__ psi,
                                                  const int* __restrict__ wall_nbr,
-                                                 const T* __restrict__ inv_den, int nf, int nw,
-                                                 size_t nwpad, T chiA, T chiB) {
+                                                 const T* __restrict__ inv_den,
+                                                 size_t wall_base, int nw, size_t nwpad, T chiA,
+                                                 T chiB) {
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
   if (w >= nw) return;
   T na = T(0), nb = T(0);
@@ -99,7 +102,7 @@ __global__ void __launch_bounds__(256) k_wallpsi(Vec2<T>* __restrict__ psi,
   }
   const T s = inv_den[w];
   Vec2<T> o; o.a = chiA * na * s; o.b = chiB * nb * s;
-  psi[(size_t)nf + w] = o;
+  psi[wall_base + w] = o;  // wall ids are stored at wall_base = npad (tile-aligned)
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -549,6 +552,170 @@ __global__ void __launch_bounds__(TN, MINB)
   collide_tile_thread<T, TN, REMAINDER>(sf, sid, tid, n, n < nf, fout, psi, nf, npad, c);
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Fused single-kernel step (production).  The two grid-wide dependencies of a step -- every
+// node's force needs its neighbours' rho(t), every wall solid's rho~(t) needs its fluid
+// neighbours' rho(t) -- are resolved INSIDE one persistent kernel instead of by kernel
+// boundaries, so that the density pass runs only a short distance ahead of the fused pass and the
+// populations it has just read are still in the 126 MB L2 when the fused pass reads them again
+// (saves the second 152 B/node DRAM read of the two-pass method).
+//
+// Work items (tiles of TN consecutive ids): D(t) density, W(j) virtual solid density, C(t) fused
+// force+collide+stream; host-built global order `sched` in which every item follows the items
+// whose psi it reads (geometry.hpp Schedule).  CTAs take items with an atomic ticket.  D and W
+// items publish a per-tile completion flag; a consumer polls exactly the ~10 tiles its psi stencil
+// touches (wait_ranges).  All CTAs are co-resident (cooperative launch), tickets are handed
+// out in schedule order and every wait is on an earlier item: the item with the smallest ticket
+// can always finish, so the scheme cannot deadlock.
+__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
+  int v;
+  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_gpu(int* p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// Completion tracking.  D(t) / W(j) publish flags[t] = epoch with a gpu-scope release store after
+// the CTA barrier that follows their psi stores (release is cumulative over the barrier).  A
+// consumer checks exactly the tiles it depends on, given as up to 3 (lo,cnt) ranges: one warp
+// polls 32 flags per round with relaxed gpu-scope loads (served by L2) until all carry this
+// step's epoch; the CTA barrier that follows orders every thread's psi loads after the poll.
+// No acquire fence is used: a gpu-scope acquire invalidates the SM's whole L1 (CCTL.IVALL), which
+// six co-resident CTAs pay for on every item, and it is not needed here -- a psi line can only
+// enter an L1 after its tile's flag was seen set (tiles are line-aligned), i.e. with final data,
+// and L1 does not survive a kernel boundary.  Call from all 32 lanes of one warp.
+__device__ __forceinline__ void wait_ranges(const int* __restrict__ flags, const int* rng,
+                                            int epoch) {
+  const int lane = threadIdx.x & 31;
+#pragma unroll
+  for (int r = 0; r < 3; ++r) {
+    const int lo = rng[2 * r], cnt = rng[2 * r + 1];
+    for (int b = 0; b < cnt; b += 32) {
+      const int k = b + lane;
+      while (true) {
+        const int ok = k >= cnt || ld_relaxed_gpu(flags + lo + k) == epoch;
+        if (__all_sync(0xffffffffu, ok)) break;
+        __nanosleep(64);
+      }
+    }
+  }
+}
+
+struct FusedSched {
+  int* flags_d;        // [ntf] epoch of the last step in which D(t) completed
+  int* flags_w;        // [ntw]
+  int epoch;           // this step's epoch (> 0, increases by one per step)
+  const int4* items;   // [nitems][4] = 16 ints per item (geometry.hpp kRecordInts):
+                       //   {type << 30 | tile, D deps 3 x (lo,cnt), W deps 3 x (lo,cnt), 0, 0, 0}
+  int nitems;
+};
+
+template <typename T, int TN, int MINB, bool REMAINDER>
+__global__ void __launch_bounds__(TN, MINB)
+    k_step_fused(const T* __restrict__ fin, T* __restrict__ fout, Vec2<T>* __restrict__ psi,
+                 const int* __restrict__ nbr, const int* __restrict__ wall_nbr,
+                 const T* __restrict__ inv_den, int nf, int nw, size_t npad, size_t nwpad,
+                 Consts<T> c, FusedSched sc, int* __restrict__ ctr, int* __restrict__ ctr_next) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* sf = reinterpret_cast<T*>(smem_raw);                                        // [38][TN]
+  int* sid = reinterpret_cast<int*>(smem_raw + (size_t)2 * Q * TN * sizeof(T));  // [18][TN]
+  __shared__ uint64_t bar;
+  const int tid = threadIdx.x;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // compiler-visible warp-uniform value
+  if (tid == 0) {
+    mbar_init(&bar, 1);
+    if (blockIdx.x == 0) {  // the other watermark set is idle during this launch: reset it
+    }
+  }
+  __syncthreads();
+  uint32_t phase = 0;
+  // Items are handed out in schedule order by an atomic ticket (fast CTAs take more items, so no
+  // CTA falls behind the others).  A ticket holder waits only on items with smaller tickets,
+  // which are finished or running on co-resident CTAs: progress is guaranteed.  Thread 0 draws
+  // the NEXT ticket and fetches its record while the CTA works on the current item.
+  __shared__ __align__(16) int s_rec[2][16];  // double-buffered item record
+  if (tid < 4) {
+    int k = 0;
+    if (tid == 0) k = atomicAdd(&ctr[0], 1);
+    k = __shfl_sync(0xfu, k, 0);
+    reinterpret_cast<int4*>(s_rec[0])[tid] =
+        k < sc.nitems ? __ldg(sc.items + (size_t)4 * k + tid) : make_int4(-1, 0, 0, 0);
+    if (blockIdx.x == 0 && tid == 0) ctr_next[0] = 0;
+  }
+  __syncthreads();
+  int buf = 0;
+  while (true) {
+    const int* rec = s_rec[buf];
+    const int head = __shfl_sync(0xffffffffu, rec[0], 0);
+    if (head == -1) break;
+    // draw the next ticket and fetch its record into the other buffer (read next iteration)
+    if (tid < 4) {
+      int k = 0;
+      if (tid == 0) k = atomicAdd(&ctr[0], 1);
+      k = __shfl_sync(0xfu, k, 0);
+      reinterpret_cast<int4*>(s_rec[buf ^ 1])[tid] =
+          k < sc.nitems ? __ldg(sc.items + (size_t)4 * k + tid) : make_int4(-1, 0, 0, 0);
+    }
+    const int type = (int)((unsigned)head >> 30), t = head & 0x3fffffff;
+    if (type == 0) {
+      // ---- D(t): a1 on fluid tile t
+      const int n = t * TN + tid;
+      T ra = T(0), rb = T(0);
+#pragma unroll
+      for (int i = 0; i < Q; ++i) {
+        ra += fin[(size_t)i * npad + n];
+        rb += fin[(size_t)(Q + i) * npad + n];
+      }
+      Vec2<T> o; o.a = ra; o.b = rb;
+      psi[n] = o;  // n < npad always; the padding holds zeros
+      __syncthreads();
+      if (tid == 0) st_release_gpu(sc.flags_d + t, sc.epoch);
+    } else if (type == 1) {
+      // ---- W(j): a2 on wall tile t
+      if (warp == 0) wait_ranges(sc.flags_d, rec + 1, sc.epoch);
+      __syncthreads();
+      const int w = t * TN + tid;
+      if (w < nw) {
+        T na = T(0), nb = T(0);
+#pragma unroll
+        for (int i = 1; i < Q; ++i) {
+          const int id = wall_nbr[(size_t)(i - 1) * nwpad + w];
+          if (id >= 0) {
+            const Vec2<T> p = psi[id];
+            na += wgt<T>(i) * p.a;
+            nb += wgt<T>(i) * p.b;
+          }
+        }
+        const T s = inv_den[w];
+        Vec2<T> o; o.a = c.chiA * na * s; o.b = c.chiB * nb * s;
+        psi[npad + w] = o;
+      }
+      __syncthreads();
+      if (tid == 0) st_release_gpu(sc.flags_w + t, sc.epoch);
+    } else {
+      // ---- C(t): a3-a6 on fluid tile t.  The tile's populations and ids do not depend on psi:
+      // their bulk copies are issued before the dependency wait.
+      if (warp == 0) {
+        load_tile<T, TN>(sf, sid, fin, nbr, npad, (size_t)t * TN, &bar);
+        wait_ranges(sc.flags_d, rec + 1, sc.epoch);
+        wait_ranges(sc.flags_w, rec + 7, sc.epoch);
+      }
+      __syncthreads();
+      mbar_wait(&bar, phase);
+      phase ^= 1u;
+      const int n = t * TN + tid;
+      collide_tile_thread<T, TN, REMAINDER>(sf, sid, tid, n, n < nf, fout, psi, nf, npad, c);
+    }
+    buf ^= 1;
+    __syncthreads();  // next record is in place; the stage is free for the next C item
+  }
+}
 
 // ---------------------------------------------------------------------------------------------
 // a0  open-plane fix on the new buffer (reading R12 of PAPER.md L147-157, L223): planes z=0 and

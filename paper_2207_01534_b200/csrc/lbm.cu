@@ -85,6 +85,15 @@ struct lbm_ctx {
   int collide_variant = 1;  // 0: register kernel (A/B reference), 1: bulk-async staged tiles
                             // (production); env LBM_B200_COLLIDE=simple|bulk
   int num_sms = 148;
+  int step_variant = 0;     // 0: one kernel per pass (split, default), 1: fused persistent step kernel
+                            // (experimental); env LBM_B200_STEP=split|fused
+  int fused_grid = 0;       // co-resident CTAs of the fused kernel
+  int4* sched_items = nullptr;       // fused-step schedule records (geometry.hpp Schedule)
+  int sched_nitems = 0, sched_ntf = 0, sched_ntw = 0;
+  int* fused_ctr = nullptr;          // [2][4] ticket / D watermark / W watermark, alternating per step
+  int* fused_flags = nullptr;        // [ntf+32 | ntw+32] per-rank completion epochs
+  int fused_epoch = 0;
+  int fused_parity = 0;
   int tile = 1286;          // fp32 bulk kernel variant: tile nodes * 10 + min CTAs/SM; env LBM_B200_TILE
   long long bytes[4] = {0, 0, 0, 0};
   bool prof = false;
@@ -97,6 +106,8 @@ struct lbm_ctx {
     lbm_shim_free(f[0]); lbm_shim_free(f[1]); lbm_shim_free(psi); lbm_shim_free(nbr);
     lbm_shim_free(wall_nbr); lbm_shim_free(wall_inv_den); lbm_shim_free(node_vox_d);
     lbm_shim_free(frozen); lbm_shim_free(partial); lbm_shim_free(diag_out);
+    lbm_shim_free(sched_items); lbm_shim_free(fused_ctr);
+    lbm_shim_free(fused_flags);
   }
 };
 
@@ -152,7 +163,7 @@ void launch_psi(lbm_ctx* c, cudaStream_t st) {
   if (c->nw > 0) {
     Timed t(c, st, 1);
     k_wallpsi<T><<<blocks(c->nw, 256), 256, 0, st>>>((Vec2<T>*)c->psi, c->wall_nbr,
-                                                     (const T*)c->wall_inv_den, c->nf, c->nw,
+                                                     (const T*)c->wall_inv_den, c->npad, c->nw,
                                                      c->nwpad, (T)(1.0 + c->p.xi),
                                                      (T)(1.0 - c->p.xi));
   }
@@ -194,6 +205,45 @@ void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaS
   }
 }
 
+// One cooperative launch of the fused persistent step kernel (a1-a6 in one kernel).
+template <typename T, int MINB>
+int launch_fused(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
+  constexpr int TN = 128;
+  constexpr bool kRemainder = sizeof(T) == 4;
+  constexpr size_t smem = collide_smem_bytes<T, TN>();
+  auto kern = k_step_fused<T, TN, MINB, kRemainder>;
+  static int grid_cache = 0;
+  if (grid_cache == 0) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TN, smem));
+    if (per_sm < 1) return fail(LBM_ECUDA, "fused kernel does not fit on an SM");
+    grid_cache = per_sm * c->num_sms;
+  }
+  c->fused_grid = grid_cache;
+  FusedSched sc;
+  sc.flags_d = c->fused_flags;
+  sc.flags_w = c->fused_flags + c->sched_ntf;
+  sc.epoch = ++c->fused_epoch;
+  sc.items = c->sched_items;
+  sc.nitems = c->sched_nitems;
+  Vec2<T>* psi = (Vec2<T>*)c->psi;
+  const int* nbr = c->nbr;
+  const int* wall_nbr = c->wall_nbr;
+  const T* inv_den = (const T*)c->wall_inv_den;
+  int nf = c->nf, nw = c->nw;
+  size_t npad = c->npad, nwpad = c->nwpad;
+  Consts<T> kk = k;
+  int* ctr = c->fused_ctr + 4 * c->fused_parity;
+  int* ctr_next = c->fused_ctr + 4 * (c->fused_parity ^ 1);
+  c->fused_parity ^= 1;
+  void* args[] = {(void*)&fin, (void*)&fout, (void*)&psi, (void*)&nbr, (void*)&wall_nbr,
+                  (void*)&inv_den, (void*)&nf, (void*)&nw, (void*)&npad, (void*)&nwpad,
+                  (void*)&kk, (void*)&sc, (void*)&ctr, (void*)&ctr_next};
+  CU(cudaLaunchCooperativeKernel((const void*)kern, dim3(grid_cache), dim3(TN), args, smem, st));
+  return LBM_OK;
+}
+
 template <typename T>
 int step_T(lbm_ctx* c, int n, cudaStream_t st) {
   const Consts<T> k = make_consts<T>(c->p);
@@ -201,8 +251,14 @@ int step_T(lbm_ctx* c, int n, cudaStream_t st) {
   for (int it = 0; it < n; ++it) {
     const T* fin = (const T*)c->f[c->cur];
     T* fout = (T*)c->f[c->cur ^ 1];
-    launch_psi<T>(c, st);
-    {
+    if (c->step_variant == 1) {
+      Timed t(c, st, 2);
+      int rc;
+      if constexpr (sizeof(T) == 4) rc = launch_fused<T, 6>(c, fin, fout, k, st);
+      else rc = launch_fused<T, 2>(c, fin, fout, k, st);
+      if (rc) return rc;
+    } else {
+      launch_psi<T>(c, st);
       Timed t(c, st, 2);
       launch_collide<T>(c, fin, fout, k, st);
     }
@@ -275,6 +331,21 @@ int lbm_build_index(const uint8_t* solid, int nx, int ny, int nz, int z_open, in
   return LBM_OK;
 }
 
+int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open, int tile,
+                       int lead, int32_t* records, long long cap_items, long long* n_items) {
+  if (!solid || !records || !n_items) return fail(LBM_EINVAL, "NULL argument");
+  lbmgeo::Geometry g;
+  const int rc = lbmgeo::build(g, solid, nx, ny, nz, z_open, true);
+  if (rc) return fail(rc, "geometry build failed (%d)", rc);
+  lbmgeo::Schedule s;
+  if (lbmgeo::build_schedule(g, tile, lead < 0 ? 0 : lead, s) != 0)
+    return fail(LBM_EINVAL, "schedule build failed");
+  *n_items = (long long)s.nitems();
+  if ((long long)s.nitems() > cap_items) return fail(LBM_EINVAL, "records capacity too small");
+  std::memcpy(records, s.records.data(), s.records.size() * sizeof(int32_t));
+  return LBM_OK;
+}
+
 int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, const lbm_params* p) {
   if (!out || !solid || !p) return fail(LBM_EINVAL, "NULL argument");
   if (nx < 1 || ny < 1 || nz < 1) return fail(LBM_EINVAL, "box dimensions must be positive");
@@ -302,6 +373,7 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   c->bits = p->storage_bits; c->esz = p->storage_bits / 8;
   if (const char* e = std::getenv("LBM_B200_COLLIDE")) c->collide_variant = !std::strcmp(e, "simple") ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_TILE")) c->tile = std::atoi(e);
+  if (const char* e = std::getenv("LBM_B200_STEP")) c->step_variant = !std::strcmp(e, "split") ? 0 : 1;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
   if ((size_t)2 * 19 * c->npad >= ((size_t)1 << 31)) {
     delete c;
@@ -312,7 +384,7 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   for (int z = 0; z < nz; ++z) c->zstart[z + 1] += c->zstart[z];
   cudaStream_t st = cur_stream();
   const size_t fbytes = (size_t)2 * 19 * c->npad * c->esz;
-  const size_t psibytes = (size_t)(g.nf + g.nw) * 2 * c->esz;
+  const size_t psibytes = (c->npad + c->nwpad) * 2 * c->esz;  // wall part starts at npad
   const size_t nbrbytes = (size_t)18 * c->npad * sizeof(int);
   const size_t wnbrbytes = (size_t)18 * c->nwpad * sizeof(int);
   const size_t frozenbytes = p->z_open ? (size_t)2 * 2 * 5 * c->np * c->esz : 0;
@@ -346,6 +418,23 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   if (e == cudaSuccess) e = cudaMemsetAsync(c->psi, 0, psibytes, st);
   if (e == cudaSuccess && frozenbytes) e = cudaMemsetAsync(c->frozen, 0, frozenbytes, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->nbr, 0, nbrbytes, st);
+  // Fused-step schedule (built from the raw ids), then re-base wall ids from nf+w to npad+w so
+  // that the wall part of psi starts on a tile boundary.
+  lbmgeo::Schedule sch;
+  {
+    int lead = 256;
+    if (const char* e = std::getenv("LBM_B200_LEAD")) lead = std::atoi(e);
+    if (lbmgeo::build_schedule(g, 128, lead < 0 ? 0 : lead, sch) != 0) {
+      delete c;
+      return fail(LBM_ENOMEM, "schedule build failed");
+    }
+  }
+  {
+    const int32_t shift = (int32_t)(c->npad - (size_t)g.nf);
+    const int32_t nf32 = (int32_t)g.nf;
+    for (auto& v : g.nbr)
+      if (v >= nf32) v += shift;
+  }
   for (int i = 0; i < 18; ++i) {
     up(c->nbr + (size_t)i * c->npad, g.nbr.data() + (size_t)i * g.nf, g.nf * sizeof(int));
     up(c->wall_nbr + (size_t)i * c->nwpad, g.wall_nbr.data() + (size_t)i * g.nw,
@@ -358,6 +447,24 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
     up(c->wall_inv_den, invf.data(), g.nw * sizeof(float));
   } else {
     up(c->wall_inv_den, g.wall_inv_den.data(), g.nw * sizeof(double));
+  }
+  // fused-step schedule records, completion flags and counters
+  {
+    c->sched_nitems = (int)sch.nitems();
+    c->sched_ntf = sch.ntf;
+    c->sched_ntw = sch.ntw;
+    const size_t nflags = (size_t)sch.ntf + sch.ntw;
+    c->sched_items = (int4*)lbm_shim_alloc(sch.records.size() * sizeof(int32_t));
+    c->fused_ctr = (int*)lbm_shim_alloc(8 * sizeof(int));
+    c->fused_flags = (int*)lbm_shim_alloc(nflags * sizeof(int));
+    if (!c->sched_items || !c->fused_ctr || !c->fused_flags) {
+      delete c;
+      return fail(LBM_ENOMEM, "device allocation failed (schedule)");
+    }
+    up(c->sched_items, sch.records.data(), sch.records.size() * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->fused_ctr, 0, 8 * sizeof(int), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->fused_flags, 0, nflags * sizeof(int), st);
+    c->bytes[2] += (long long)(sch.records.size() * 4 + nflags * 4);
   }
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);  // host sources die with this scope
   if (e != cudaSuccess) {

@@ -22,7 +22,7 @@ SYMBOLS = [
     "lbm_set_boundary", "lbm_step", "lbm_sync", "lbm_get_macroscopic", "lbm_diagnostics",
     "lbm_saturation", "lbm_trapped_volume", "lbm_num_fluid", "lbm_num_wall_solid",
     "lbm_memory_bytes", "lbm_set_profiling", "lbm_last_step_profile", "lbm_last_error",
-    "lbm_build_index",
+    "lbm_build_index", "lbm_build_schedule",
 ]
 
 
@@ -82,10 +82,12 @@ def load():
     lib.lbm_last_error.argtypes = []
     lib.lbm_last_error.restype = C.c_char_p
     lib.lbm_build_index.argtypes = [V, I, I, I, I, V, V, LL, C.POINTER(LL), C.POINTER(LL)]
+    lib.lbm_build_schedule.argtypes = [V, I, I, I, I, I, I, V, LL, C.POINTER(LL)]
     for fn in ("lbm_create", "lbm_set_density", "lbm_set_populations", "lbm_get_populations",
                "lbm_set_boundary", "lbm_step", "lbm_sync", "lbm_get_macroscopic",
                "lbm_diagnostics", "lbm_saturation", "lbm_trapped_volume", "lbm_memory_bytes",
-               "lbm_set_profiling", "lbm_last_step_profile", "lbm_build_index"):
+               "lbm_set_profiling", "lbm_last_step_profile", "lbm_build_index",
+               "lbm_build_schedule"):
         getattr(lib, fn).restype = I
     _lib = lib
     return lib
@@ -126,6 +128,20 @@ def lbm_build_index(mask, z_open=0, with_nbr=True):
                              nbr.ctypes.data if with_nbr else None, 18 * max(nfluid, 1),
                              C.byref(nf), C.byref(nw)), "lbm_build_index")
     return vox2id, (nbr[:, :nf.value] if with_nbr else None), nf.value, nw.value
+
+
+def lbm_build_schedule(mask, z_open=0, tile=128, lead=256):
+    """Host-only: the fused-step work schedule lbm_create builds. Returns records[n_items, 16]."""
+    lib = load()
+    mask = np.ascontiguousarray(mask, np.uint8)
+    nz, ny, nx = mask.shape
+    nf = int((mask == 0).sum())
+    cap = 2 * (nf // tile + 1) + (int((mask != 0).sum()) // tile + 1)
+    rec = np.zeros((cap, 16), np.int32)
+    n = C.c_longlong()
+    _chk(lib.lbm_build_schedule(mask.ctypes.data, nx, ny, nz, int(z_open), int(tile), int(lead),
+                                rec.ctypes.data, cap, C.byref(n)), "lbm_build_schedule")
+    return rec[:n.value]
 
 
 class Lbm:

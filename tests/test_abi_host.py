@@ -148,3 +148,45 @@ def test_compact_index_on_config_geometries():
     ids, nbr_ref, nf_ref, nw_ref = _brute_index(c["mask"], 1)
     assert (nf, nw) == (nf_ref, nw_ref) and np.array_equal(nbr, nbr_ref)
     assert nf == int((c["mask"] == 0).sum())
+
+
+# ------------------------------------------------------------------ fused-step schedule (host)
+
+@pytest.mark.parametrize("z_open,lead", [(0, 0), (1, 4), (0, 16)])
+def test_fused_schedule_is_a_valid_topological_order(z_open, lead):
+    """Every D/W/C item appears exactly once and every tile an item waits for (its dependency
+    ranges) was issued earlier in the schedule; the ranges cover the true psi stencil."""
+    rng = np.random.Generator(np.random.PCG64(23))
+    mask = (rng.uniform(size=(12, 20, 24)) < 0.35).astype(np.uint8)
+    if z_open:
+        mask[:2] = 0
+        mask[-2:] = 0
+    tile = 32
+    rec = lbm.lbm_build_schedule(mask, z_open, tile, lead)
+    vox2id, nbr, nf, nw = lbm.lbm_build_index(mask, z_open)
+    ntf, ntw = -(-nf // tile), -(-nw // tile)
+    typ = rec[:, 0].astype(np.uint32) >> 30
+    til = rec[:, 0] & 0x3FFFFFFF
+    assert len(rec) == 2 * ntf + ntw
+    for k, n in ((0, ntf), (1, ntw), (2, ntf)):
+        assert sorted(til[typ == k]) == list(range(n))
+    pos_d = np.empty(ntf, np.int64)
+    pos_d[til[typ == 0]] = np.nonzero(typ == 0)[0]
+    pos_w = np.empty(max(ntw, 1), np.int64)
+    pos_w[til[typ == 1]] = np.nonzero(typ == 1)[0]
+
+    def covered(r):
+        out = set()
+        for q in range(3):
+            out.update(range(r[2 * q], r[2 * q] + r[2 * q + 1]))
+        return out
+
+    ids = np.where(nbr < 0, -nbr - 1, nbr)                  # mirror ids beyond open planes
+    for k in range(len(rec)):
+        d, w = covered(rec[k, 1:7]), covered(rec[k, 7:13])
+        assert all(pos_d[t] < k for t in d) and all(pos_w[j] < k for j in w)
+        if typ[k] == 2:                                      # C item: ranges cover its psi stencil
+            cols = ids[:, til[k] * tile:(til[k] + 1) * tile]
+            need_d = set((cols[cols < nf] // tile).tolist())
+            need_w = set(((cols[cols >= nf] - nf) // tile).tolist())
+            assert need_d <= d and need_w <= w
