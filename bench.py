@@ -140,6 +140,22 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons), "samples": len(s)}
 
 
+def aggregate_over_ranks(local_ms, units_per_rank, world, device):
+    """Max-over-ranks time and whole-job throughput (units of all ranks / that time)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    return ms, world * units_per_rank / (ms * 1e-3) / 1e6
+
+
+# DRAM bytes per launch of the fused pass from the committed `ncu --set full` capture
+# (profiles/r1_v4_step.md): dram__bytes_read.sum + dram__bytes_write.sum on config 4.
+NCU_TRAFFIC_CFG4_COLLIDE = 1.677e9
+
+
 def run_reference(args):
     """--impl reference: the oracle as it stands, on the host cores, rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -199,13 +215,9 @@ def run_ours(args):
     barrier()
     sampler.stop_flag = True
     sampler.join()
-    ms = torch.tensor([e0.elapsed_time(e1)], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-    ms_total = float(ms.item())
+    ms_total, value = aggregate_over_ranks(e0.elapsed_time(e1), nf * K, world, "cuda")
     _, launches = sim.last_step_profile()
     mass, _ = sim.diagnostics()          # fails loudly on a non-finite state
-    value = world * nf * K / (ms_total * 1e-3) / 1e6
 
     # ---- per-kernel durations: a second pass of K steps with CUDA events around every launch
     sim.set_profiling(True)
@@ -216,7 +228,9 @@ def run_ours(args):
     t_col = kms["collide_stream"] / K * 1e-3
     achieved = BYTES_PER_UPDATE_COLLIDE * nf / t_col / 1e9
     roofline = {"bound": "hbm", "kernel": "k_collide_stream", "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "unit": "GB/s", "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_CFG4_COLLIDE if (args.config == 4 and args.size is None) else None,
+                "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": BYTES_PER_UPDATE_COLLIDE * nf,
                 "kernel_ms_per_launch": {k: v / K for k, v in kms.items()},
                 "step_algorithmic_gbs": BYTES_PER_UPDATE_STEP * nf / (ms_total / K * 1e-3) / 1e9,
