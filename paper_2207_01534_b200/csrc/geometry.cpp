@@ -257,4 +257,49 @@ int build_schedule(const Geometry& g, int tile, int lead, Schedule& s) {
   return 0;
 }
 
+int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Index16& out) {
+  if (g.nf <= 0 || g.nbr.empty()) return -1;
+  const long long nf = g.nf;
+  const int ntf = (int)((nf + kIdxTile - 1) / kIdxTile);
+  if (stride < (size_t)ntf * kIdxTile) return -1;
+  try {
+    out.stride = stride;
+    out.nbr16.assign((size_t)18 * stride, 0);
+    out.meta.assign((size_t)ntf * kIdxMeta, 0);
+    long long wide = 0;
+#pragma omp parallel for schedule(static) reduction(+ : wide)
+    for (int t = 0; t < ntf; ++t) {
+      const long long n0 = (long long)t * kIdxTile, n1 = std::min<long long>(nf, n0 + kIdxTile);
+      int32_t* m = &out.meta[(size_t)t * kIdxMeta];
+      bool is_wide = false;
+      for (int i = 0; i < 18; ++i) {
+        long long fmin = -1, fmax = -1, wmin = -1, wmax = -1;
+        for (long long n = n0; n < n1; ++n) {
+          int32_t id = g.nbr[(size_t)i * nf + n];
+          if (id < 0) id = -id - 1;
+          if (id < nf) { if (fmin < 0 || id < fmin) fmin = id; if (id > fmax) fmax = id; }
+          else { const long long w = id - nf; if (wmin < 0 || w < wmin) wmin = w; if (w > wmax) wmax = w; }
+        }
+        if (fmax - fmin > 0x7fff || wmax - wmin > 0x7fff) is_wide = true;
+        m[i] = (int32_t)std::max<long long>(fmin, 0);
+        m[18 + i] = (int32_t)(psi_wall_base + std::max<long long>(wmin, 0));
+        for (long long n = n0; n < n1; ++n) {
+          int32_t id = g.nbr[(size_t)i * nf + n];
+          if (id < 0) id = -id - 1;
+          uint16_t e;
+          if (id < nf) e = (uint16_t)((id - std::max<long long>(fmin, 0)) & 0x7fff);
+          else e = (uint16_t)(0x8000 | (((id - nf) - std::max<long long>(wmin, 0)) & 0x7fff));
+          out.nbr16[(size_t)i * stride + n] = e;
+        }
+      }
+      m[36] = is_wide ? 1 : 0;
+      wide += is_wide ? 1 : 0;
+    }
+    out.wide_tiles = wide;
+  } catch (const std::bad_alloc&) {
+    return -4;
+  }
+  return 0;
+}
+
 }  // namespace lbmgeo

@@ -48,6 +48,24 @@ struct Schedule {
 // lead = how many D tiles (lead/4 W tiles) beyond the strict need are issued ahead of each C tile
 int build_schedule(const Geometry& g, int tile, int lead, Schedule& s);
 
+// 16-bit tile-relative form of the neighbour index (halves the index traffic of the fused pass).
+// For tile t (kIdxTile consecutive fluid ids) and direction i the entries of nbr are written as
+//   bit 15 = 0: fluid id (or mirror node)  = meta[t][i-1]      + (e & 0x7fff)
+//   bit 15 = 1: wall solid, psi index      = meta[t][18 + i-1] + (e & 0x7fff)   (already npad-based)
+// "beyond an open plane" is not stored: the kernel derives it from the node's plane and e_z.
+// meta[t][36] = 1 marks a "wide" tile (some offset range does not fit 15 bits, e.g. a periodic
+// wrap inside the tile): the kernel then reads the tile's int32 rows instead.
+constexpr int kIdxTile = 128;
+constexpr int kIdxMeta = 40;  // ints per tile: 18 fluid bases, 18 wall bases, wide flag, 3 pad
+struct Index16 {
+  std::vector<uint16_t> nbr16;  // [18][stride]
+  std::vector<int32_t> meta;    // [ntf][kIdxMeta]
+  size_t stride = 0;
+  long long wide_tiles = 0;
+};
+// psi_wall_base = psi index of wall solid 0 (npad); stride = row stride of nbr16 (>= ntf*kIdxTile)
+int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Index16& out);
+
 // Returns 0, or -1 bad arguments, -2 no fluid voxel, -3 solid on an open plane or its interior
 // neighbour plane (z in {0,1,nz-2,nz-1}), -4 out of memory.  `with_tables` = also fill nbr,
 // wall_nbr, wall_inv_den.

@@ -532,26 +532,87 @@ __device__ __forceinline__ void load_tile(T* sf, int* sid, const T* __restrict__
   __syncwarp();
 }
 
-template <typename T, int TN, int MINB, bool REMAINDER>
+// 16-bit tile-relative neighbour index (geometry.hpp Index16): per tile 18 rows of TN uint16 plus
+// a 160 B record of bases.  Halves the index bytes of the fused pass (72 -> 37 B per node).
+constexpr int kIdxMeta = 40;
+struct Idx16 {
+  const uint16_t* nbr16;  // [18][npad]
+  const int* meta;        // [tiles][kIdxMeta]
+  int np;                 // nodes per open plane (nx*ny) when z is open, else 0
+};
+
+template <typename T, int TN>
+constexpr size_t collide16_smem_bytes() {
+  return collide_smem_bytes<T, TN>() + (size_t)18 * TN * sizeof(uint16_t) + kIdxMeta * sizeof(int);
+}
+
+template <typename T, int TN, int MINB, bool REMAINDER, bool IDX16>
 __global__ void __launch_bounds__(TN, MINB)
     k_collide_stream_bulk(const T* __restrict__ fin, T* __restrict__ fout,
                           const Vec2<T>* __restrict__ psi, const int* __restrict__ nbr, int nf,
-                          size_t npad, Consts<T> c) {
+                          size_t npad, Consts<T> c, Idx16 ix) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  T* sf = reinterpret_cast<T*>(smem_raw);                                   // [38][TN]
+  T* sf = reinterpret_cast<T*>(smem_raw);                                        // [38][TN]
   int* sid = reinterpret_cast<int*>(smem_raw + (size_t)2 * Q * TN * sizeof(T));  // [18][TN]
+  uint16_t* s16 = reinterpret_cast<uint16_t*>(smem_raw + collide_smem_bytes<T, TN>());  // [18][TN]
+  int* smeta = reinterpret_cast<int*>(smem_raw + collide_smem_bytes<T, TN>() +
+                                      (size_t)18 * TN * sizeof(uint16_t));       // [kIdxMeta]
   __shared__ uint64_t bar;
   const int tid = threadIdx.x;
   const size_t t0 = (size_t)blockIdx.x * TN;
   if (tid == 0) mbar_init(&bar, 1);
   __syncthreads();
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // compiler-visible warp-uniform value
-  if (warp == 0) load_tile<T, TN>(sf, sid, fin, nbr, npad, t0, &bar);
-  mbar_wait(&bar, 0);
   const int n = (int)t0 + tid;
+  if constexpr (!IDX16) {
+    if (warp == 0) load_tile<T, TN>(sf, sid, fin, nbr, npad, t0, &bar);
+    mbar_wait(&bar, 0);
+  } else {
+    if (warp == 0) {
+      if (elect_one()) {
+        mbar_expect_tx(&bar, (uint32_t)((size_t)2 * Q * TN * sizeof(T) +
+                                        (size_t)18 * TN * sizeof(uint16_t) + kIdxMeta * sizeof(int)));
+#pragma unroll
+        for (int r = 0; r < 2 * Q; ++r)
+          bulk_g2s(sf + (size_t)r * TN, fin + (size_t)r * npad + t0, TN * sizeof(T), &bar);
+#pragma unroll
+        for (int r = 0; r < 18; ++r)
+          bulk_g2s(s16 + (size_t)r * TN, ix.nbr16 + (size_t)r * npad + t0, TN * sizeof(uint16_t),
+                   &bar);
+        bulk_g2s(smeta, ix.meta + (size_t)blockIdx.x * kIdxMeta, kIdxMeta * sizeof(int), &bar);
+      }
+      __syncwarp();
+    }
+    mbar_wait(&bar, 0);
+    const int wide = __shfl_sync(0xffffffffu, smeta[36], 0);
+    if (wide) {
+      // rare: an offset range of this tile does not fit 15 bits -> take the int32 rows
+      if (warp == 0) {
+        if (elect_one()) {
+          mbar_expect_tx(&bar, (uint32_t)((size_t)18 * TN * sizeof(int)));
+#pragma unroll
+          for (int r = 0; r < 18; ++r)
+            bulk_g2s(sid + (size_t)r * TN, nbr + (size_t)r * npad + t0, TN * sizeof(int), &bar);
+        }
+        __syncwarp();
+      }
+      mbar_wait(&bar, 1);
+    } else {
+      // decode this thread's column into the int32 form the tile function reads; a neighbour
+      // beyond an open plane (reading R12 iv) is recognised from the node's plane and e_z
+      const bool lo_plane = n < ix.np, hi_plane = n >= nf - ix.np;
+#pragma unroll
+      for (int i = 1; i < Q; ++i) {
+        const int e = s16[(i - 1) * TN + tid];
+        int k = smeta[(e >> 15) * 18 + (i - 1)] + (e & 0x7fff);
+        if (ez(i) < 0) k = lo_plane ? -k - 1 : k;
+        if (ez(i) > 0) k = hi_plane ? -k - 1 : k;
+        sid[(i - 1) * TN + tid] = k;
+      }
+    }
+  }
   collide_tile_thread<T, TN, REMAINDER>(sf, sid, tid, n, n < nf, fout, psi, nf, npad, c);
 }
-
 
 // ---------------------------------------------------------------------------------------------
 // Fused single-kernel step (production).  The two grid-wide dependencies of a step -- every

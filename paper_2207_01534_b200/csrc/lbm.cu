@@ -85,6 +85,10 @@ struct lbm_ctx {
   int collide_variant = 1;  // 0: register kernel (A/B reference), 1: bulk-async staged tiles
                             // (production); env LBM_B200_COLLIDE=simple|bulk
   int num_sms = 148;
+  int idx16 = 1;            // fused pass reads the 16-bit tile-relative index (env LBM_B200_IDX=32: int32)
+  uint16_t* nbr16 = nullptr;         // [18][npad]
+  int* nbr16_meta = nullptr;         // [tiles][kIdxMeta]
+  long long wide_tiles = 0;
   int step_variant = 0;     // 0: one kernel per pass (split, default), 1: fused persistent step kernel
                             // (experimental); env LBM_B200_STEP=split|fused
   int fused_grid = 0;       // co-resident CTAs of the fused kernel
@@ -106,7 +110,8 @@ struct lbm_ctx {
     lbm_shim_free(f[0]); lbm_shim_free(f[1]); lbm_shim_free(psi); lbm_shim_free(nbr);
     lbm_shim_free(wall_nbr); lbm_shim_free(wall_inv_den); lbm_shim_free(node_vox_d);
     lbm_shim_free(frozen); lbm_shim_free(partial); lbm_shim_free(diag_out);
-    lbm_shim_free(sched_items); lbm_shim_free(fused_ctr);
+    lbm_shim_free(sched_items); lbm_shim_free(fused_ctr); lbm_shim_free(nbr16);
+    lbm_shim_free(nbr16_meta);
     lbm_shim_free(fused_flags);
   }
 };
@@ -172,18 +177,22 @@ void launch_psi(lbm_ctx* c, cudaStream_t st) {
 
 // a3-a6: the fused pass.  Production = bulk-async staged tiles; the register kernel is kept as
 // an A/B reference (LBM_B200_COLLIDE=simple).
-template <typename T, int TN, int MINB>
+template <typename T, int TN, int MINB, bool IDX16>
 void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
   constexpr bool kRemainder = sizeof(T) == 4;
-  constexpr size_t smem = collide_smem_bytes<T, TN>();
+  constexpr size_t smem = IDX16 ? collide16_smem_bytes<T, TN>() : collide_smem_bytes<T, TN>();
   static bool configured = false;
   if (!configured) {
-    cudaFuncSetAttribute(k_collide_stream_bulk<T, TN, MINB, kRemainder>,
+    cudaFuncSetAttribute(k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX16>,
                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
-  k_collide_stream_bulk<T, TN, MINB, kRemainder><<<blocks(c->nf, TN), TN, smem, st>>>(
-      fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->npad, k);
+  Idx16 ix;
+  ix.nbr16 = c->nbr16;
+  ix.meta = c->nbr16_meta;
+  ix.np = c->p.z_open ? c->np : 0;
+  k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX16><<<blocks(c->nf, TN), TN, smem, st>>>(
+      fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->npad, k, ix);
 }
 
 template <typename T>
@@ -195,13 +204,19 @@ void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaS
     return;
   }
   if constexpr (sizeof(T) == 4) {
+    if (c->idx16) {
+      if (c->tile == 1285) launch_bulk<T, 128, 5, true>(c, fin, fout, k, st);
+      else launch_bulk<T, 128, 6, true>(c, fin, fout, k, st);
+      return;
+    }
     switch (c->tile) {
-      case 1285: launch_bulk<T, 128, 5>(c, fin, fout, k, st); break;
-      case 2563: launch_bulk<T, 256, 3>(c, fin, fout, k, st); break;
-      default: launch_bulk<T, 128, 6>(c, fin, fout, k, st); break;
+      case 1285: launch_bulk<T, 128, 5, false>(c, fin, fout, k, st); break;
+      case 2563: launch_bulk<T, 256, 3, false>(c, fin, fout, k, st); break;
+      default: launch_bulk<T, 128, 6, false>(c, fin, fout, k, st); break;
     }
   } else {
-    launch_bulk<T, 128, 2>(c, fin, fout, k, st);
+    if (c->idx16) launch_bulk<T, 128, 2, true>(c, fin, fout, k, st);
+    else launch_bulk<T, 128, 2, false>(c, fin, fout, k, st);
   }
 }
 
@@ -373,6 +388,7 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   c->bits = p->storage_bits; c->esz = p->storage_bits / 8;
   if (const char* e = std::getenv("LBM_B200_COLLIDE")) c->collide_variant = !std::strcmp(e, "simple") ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_TILE")) c->tile = std::atoi(e);
+  if (const char* e = std::getenv("LBM_B200_IDX")) c->idx16 = std::atoi(e) == 32 ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_STEP")) c->step_variant = !std::strcmp(e, "split") ? 0 : 1;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
   if ((size_t)2 * 19 * c->npad >= ((size_t)1 << 31)) {
@@ -429,6 +445,12 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
       return fail(LBM_ENOMEM, "schedule build failed");
     }
   }
+  lbmgeo::Index16 i16;
+  if (lbmgeo::build_index16(g, (long long)c->npad, c->npad, i16) != 0) {
+    delete c;
+    return fail(LBM_ENOMEM, "index16 build failed");
+  }
+  c->wide_tiles = i16.wide_tiles;
   {
     const int32_t shift = (int32_t)(c->npad - (size_t)g.nf);
     const int32_t nf32 = (int32_t)g.nf;
@@ -448,6 +470,15 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   } else {
     up(c->wall_inv_den, g.wall_inv_den.data(), g.nw * sizeof(double));
   }
+  c->nbr16 = (uint16_t*)lbm_shim_alloc(i16.nbr16.size() * sizeof(uint16_t));
+  c->nbr16_meta = (int*)lbm_shim_alloc(i16.meta.size() * sizeof(int32_t) + 16);
+  if (!c->nbr16 || !c->nbr16_meta) {
+    delete c;
+    return fail(LBM_ENOMEM, "device allocation failed (index16)");
+  }
+  up(c->nbr16, i16.nbr16.data(), i16.nbr16.size() * sizeof(uint16_t));
+  up(c->nbr16_meta, i16.meta.data(), i16.meta.size() * sizeof(int32_t));
+  c->bytes[2] += (long long)(i16.nbr16.size() * 2 + i16.meta.size() * 4);
   // fused-step schedule records, completion flags and counters
   {
     c->sched_nitems = (int)sch.nitems();
