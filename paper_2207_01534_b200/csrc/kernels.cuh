@@ -539,6 +539,7 @@ struct Idx16 {
   const uint16_t* nbr16;  // [18][npad]
   const int* meta;        // [tiles][kIdxMeta]
   int np;                 // nodes per open plane (nx*ny) when z is open, else 0
+  int reverse;            // 1: CTA b takes tile gridDim-1-b
 };
 
 template <typename T, int TN>
@@ -559,7 +560,11 @@ __global__ void __launch_bounds__(TN, MINB)
                                       (size_t)18 * TN * sizeof(uint16_t));       // [kIdxMeta]
   __shared__ uint64_t bar;
   const int tid = threadIdx.x;
-  const size_t t0 = (size_t)blockIdx.x * TN;
+  // Tiles are taken from the END of the id range first: the density pass that ran just before
+  // walked the range forwards, so the last ~100 MB of populations it read are still in L2, and
+  // this kernel's last writes (the head of the range) are what the next density pass reads first.
+  const unsigned tile = ix.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
+  const size_t t0 = (size_t)tile * TN;
   if (tid == 0) mbar_init(&bar, 1);
   __syncthreads();
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // compiler-visible warp-uniform value
@@ -579,7 +584,7 @@ __global__ void __launch_bounds__(TN, MINB)
         for (int r = 0; r < 18; ++r)
           bulk_g2s(s16 + (size_t)r * TN, ix.nbr16 + (size_t)r * npad + t0, TN * sizeof(uint16_t),
                    &bar);
-        bulk_g2s(smeta, ix.meta + (size_t)blockIdx.x * kIdxMeta, kIdxMeta * sizeof(int), &bar);
+        bulk_g2s(smeta, ix.meta + (size_t)tile * kIdxMeta, kIdxMeta * sizeof(int), &bar);
       }
       __syncwarp();
     }

@@ -89,6 +89,7 @@ struct lbm_ctx {
   uint16_t* nbr16 = nullptr;         // [18][npad]
   int* nbr16_meta = nullptr;         // [tiles][kIdxMeta]
   long long wide_tiles = 0;
+  int reverse = 1;          // fused pass walks the tiles backwards (L2 reuse across passes); env LBM_B200_REVERSE=0
   int step_variant = 0;     // 0: one kernel per pass (split, default), 1: fused persistent step kernel
                             // (experimental); env LBM_B200_STEP=split|fused
   int fused_grid = 0;       // co-resident CTAs of the fused kernel
@@ -191,6 +192,7 @@ void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
   ix.nbr16 = c->nbr16;
   ix.meta = c->nbr16_meta;
   ix.np = c->p.z_open ? c->np : 0;
+  ix.reverse = c->reverse;
   k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX16><<<blocks(c->nf, TN), TN, smem, st>>>(
       fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->npad, k, ix);
 }
@@ -388,6 +390,7 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   c->bits = p->storage_bits; c->esz = p->storage_bits / 8;
   if (const char* e = std::getenv("LBM_B200_COLLIDE")) c->collide_variant = !std::strcmp(e, "simple") ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_TILE")) c->tile = std::atoi(e);
+  if (const char* e = std::getenv("LBM_B200_REVERSE")) c->reverse = std::atoi(e) != 0;
   if (const char* e = std::getenv("LBM_B200_IDX")) c->idx16 = std::atoi(e) == 32 ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_STEP")) c->step_variant = !std::strcmp(e, "split") ? 0 : 1;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
