@@ -1,0 +1,74 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (config 4 at
+256^3, config 5 at 512^3, fp32 production build): sampled outputs that the oracle can compute one
+by one.  After ONE step from f = w_i*rho the state at a node depends only on the densities within
+lattice distance 4 (streaming 1, force stencil 1, virtual-solid stencil 1, its fluid neighbours 1),
+so the oracle run on the 9^3 crop around a sampled node reproduces that node exactly."""
+import numpy as np
+import pytest
+
+from oracle import LbmRef
+from paper_2207_01534_b200 import Lbm
+from workloads import make_config
+
+pytestmark = pytest.mark.gpu
+R = 4
+
+
+def _sampled_one_step_parity(cfg, nsamples, seed, fields):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    mask = cfg["mask"]
+    nz, ny, nx = mask.shape
+    fl = mask == 0
+    # seeded perturbation so that the step is not trivial anywhere
+    rA = np.where(fl, cfg["rhoA"] * (1.0 + 0.05 * rng.uniform(-1, 1, mask.shape)), 0.0)
+    rB = np.where(fl, cfg["rhoB"] * (1.0 + 0.05 * rng.uniform(-1, 1, mask.shape)), 0.0)
+    g = Lbm(mask, cfg["params"])
+    g.set_density(rA, rB)
+    g.step(1)
+    out = g.get_macroscopic(fields=fields)
+    g.close()
+    # samples: fluid nodes away from the z ends (open planes are covered at reduced size), half of
+    # them touching a solid
+    zz, yy, xx = np.nonzero(fl[R + 2:nz - R - 2])
+    zz = zz + R + 2
+    pick = rng.choice(len(zz), size=min(4000, len(zz)), replace=False)
+    near_wall, bulk = [], []
+    for k in pick:
+        z, y, x = zz[k], yy[k], xx[k]
+        nb = mask[z - 1:z + 2, np.arange(y - 1, y + 2) % ny][:, :, np.arange(x - 1, x + 2) % nx]
+        (near_wall if nb.any() else bulk).append((z, y, x))
+    samples = near_wall[:nsamples // 2] + bulk[:nsamples - min(len(near_wall), nsamples // 2)]
+    assert len(samples) >= nsamples // 2
+    p = dict(cfg["params"], z_open=0)
+    worst = {k: 0.0 for k in fields}
+    for z, y, x in samples:
+        zi = np.arange(z - R, z + R + 1)
+        yi = np.arange(y - R, y + R + 1) % ny
+        xi = np.arange(x - R, x + R + 1) % nx
+        sub = np.ix_(zi, yi, xi)
+        o = LbmRef(np.ascontiguousarray(mask[sub]), p)
+        o.set_density(np.ascontiguousarray(rA[sub]), np.ascontiguousarray(rB[sub]))
+        o.step(1)
+        mo = o.get_macroscopic()
+        for k in fields:
+            ref, got = mo[k][R, R, R], out[k][z, y, x]
+            if k in ("rhoA", "rhoB"):
+                err = abs(got - ref) / abs(ref)
+            else:   # velocities: against the scale of the velocity field (R22)
+                err = abs(got - ref) / max(np.abs(out[k]).max(), 1e-30)
+            worst[k] = max(worst[k], err)
+    return worst
+
+
+def test_config4_full_size_sampled_against_oracle():
+    cfg = make_config(4)                                   # 256^3, as bench.py runs it
+    assert cfg["mask"].shape == (256, 256, 256) and cfg["params"]["storage_bits"] == 32
+    worst = _sampled_one_step_parity(cfg, 24, 41, ("rhoA", "rhoB", "ux", "uy", "uz"))
+    assert all(v <= 1e-5 for v in worst.values()), worst
+
+
+def test_config5_full_size_sampled_against_oracle():
+    cfg = make_config(5)                                   # 512^3 sphere pack, 51 M fluid nodes
+    assert cfg["mask"].shape == (512, 512, 512)
+    worst = _sampled_one_step_parity(cfg, 16, 43, ("rhoA", "rhoB", "uz"))
+    assert all(v <= 1e-5 for v in worst.values()), worst
