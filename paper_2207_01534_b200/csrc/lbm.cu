@@ -82,6 +82,8 @@ struct lbm_ctx {
   double* diag_out = nullptr;                     // [6] + count
   int diag_blocks = 0;
   int cur = 0;
+  bool open_pending = false;  // the open-plane fix of the last step has not been applied yet (it
+                              // is folded into the next density pass, or applied by a getter)
   int collide_variant = 1;  // 0: register kernel (A/B reference), 1: bulk-async staged tiles
                             // (production); env LBM_B200_COLLIDE=simple|bulk
   int num_sms = 148;
@@ -161,10 +163,18 @@ struct Timed {  // brackets one launch with events when profiling is on
 // a1 + a2 on the current buffer
 template <typename T>
 void launch_psi(lbm_ctx* c, cudaStream_t st) {
-  const T* fin = (const T*)c->f[c->cur];
+  T* fin = (T*)c->f[c->cur];
   {
     Timed t(c, st, 0);
-    k_density<T><<<blocks(c->nf, 256), 256, 0, st>>>(fin, (Vec2<T>*)c->psi, c->nf, c->npad);
+    if (c->open_pending) {  // a0 of the previous step rides along (k_density_open)
+      const unsigned nbp = blocks(2LL * c->np, 256);
+      k_density_open<T><<<nbp + blocks(c->nf, 256), 256, 0, st>>>(
+          fin, (Vec2<T>*)c->psi, (const T*)c->frozen, c->nf, c->np, c->npad, (int)nbp,
+          make_open<T>(c->p));
+      c->open_pending = false;
+    } else {
+      k_density<T><<<blocks(c->nf, 256), 256, 0, st>>>(fin, (Vec2<T>*)c->psi, c->nf, c->npad);
+    }
   }
   if (c->nw > 0) {
     Timed t(c, st, 1);
@@ -178,6 +188,19 @@ void launch_psi(lbm_ctx* c, cudaStream_t st) {
 
 // a3-a6: the fused pass.  Production = bulk-async staged tiles; the register kernel is kept as
 // an A/B reference (LBM_B200_COLLIDE=simple).
+// Apply a deferred open-plane fix now (getters that read the populations directly).
+template <typename T>
+void apply_pending_T(lbm_ctx* c, cudaStream_t st) {
+  if (!c->open_pending) return;
+  k_open_planes<T><<<blocks(2LL * c->np, 128), 128, 0, st>>>((T*)c->f[c->cur], (const T*)c->frozen,
+                                                             c->nf, c->np, c->npad,
+                                                             make_open<T>(c->p));
+  c->open_pending = false;
+}
+void apply_pending(lbm_ctx* c, cudaStream_t st) {
+  if (c->bits == 64) apply_pending_T<double>(c, st); else apply_pending_T<float>(c, st);
+}
+
 template <typename T, int TN, int MINB, bool IDX16>
 void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
   constexpr bool kRemainder = sizeof(T) == 4;
@@ -269,6 +292,7 @@ int step_T(lbm_ctx* c, int n, cudaStream_t st) {
     const T* fin = (const T*)c->f[c->cur];
     T* fout = (T*)c->f[c->cur ^ 1];
     if (c->step_variant == 1) {
+      apply_pending_T<T>(c, st);
       Timed t(c, st, 2);
       int rc;
       if constexpr (sizeof(T) == 4) rc = launch_fused<T, 6>(c, fin, fout, k, st);
@@ -279,12 +303,16 @@ int step_T(lbm_ctx* c, int n, cudaStream_t st) {
       Timed t(c, st, 2);
       launch_collide<T>(c, fin, fout, k, st);
     }
-    if (c->p.z_open) {
-      Timed t(c, st, 3);
-      k_open_planes<T><<<blocks(2LL * c->np, 128), 128, 0, st>>>(fout, (const T*)c->frozen, c->nf,
-                                                                 c->np, c->npad, op);
-    }
     c->cur ^= 1;
+    if (c->p.z_open) {
+      if (c->step_variant == 1) {
+        Timed t(c, st, 3);
+        k_open_planes<T><<<blocks(2LL * c->np, 128), 128, 0, st>>>(fout, (const T*)c->frozen,
+                                                                   c->nf, c->np, c->npad, op);
+      } else {
+        c->open_pending = true;  // a0 is folded into the next density pass
+      }
+    }
   }
   CU(cudaPeekAtLastError());
   return LBM_OK;
@@ -532,6 +560,8 @@ int lbm_set_boundary(lbm_ctx* c, double inlet_value, double outlet_rho) {
   if (!c->p.z_open) return fail(LBM_EINVAL, "z is periodic: no boundary values to set");
   if (!std::isfinite(inlet_value) || !std::isfinite(outlet_rho))
     return fail(LBM_EINVAL, "boundary values must be finite");
+  if (int rc = check_ctx(c)) return rc;
+  apply_pending(c, cur_stream());  // the last step's fix uses the values it was run with
   if (c->p.inlet_kind == 1) c->p.inlet_rho = inlet_value; else c->p.inlet_uz = inlet_value;
   c->p.outlet_rho = outlet_rho;
   return LBM_OK;
@@ -579,6 +609,7 @@ int lbm_set_density(lbm_ctx* c, const double* rhoA, const double* rhoB) {
   if (int rc = check_ctx(c)) return rc;
   if (!rhoA || !rhoB) return fail(LBM_EINVAL, "NULL argument");
   cudaStream_t st = cur_stream();
+  c->open_pending = false;  // the whole state is replaced
   const size_t bytes = (size_t)c->nvox * sizeof(double);
   DevBuf a(bytes), b(bytes);
   if (!a.p || !b.p) return fail(LBM_ENOMEM, "device staging allocation failed");
@@ -602,6 +633,7 @@ int lbm_set_populations(lbm_ctx* c, int comp, const double* f) {
   if (int rc = check_ctx(c)) return rc;
   if (!f || comp < 0 || comp > 1) return fail(LBM_EINVAL, "bad argument");
   cudaStream_t st = cur_stream();
+  apply_pending(c, st);  // the other component keeps its (completed) state
   const size_t bytes = (size_t)c->nvox * sizeof(double);
   DevBuf d(bytes);
   if (!d.p) return fail(LBM_ENOMEM, "device staging allocation failed");
@@ -628,6 +660,7 @@ int lbm_get_populations(lbm_ctx* c, int comp, double* f) {
   if (int rc = check_ctx(c)) return rc;
   if (!f || comp < 0 || comp > 1) return fail(LBM_EINVAL, "bad argument");
   cudaStream_t st = cur_stream();
+  apply_pending(c, st);
   const size_t bytes = (size_t)c->nvox * sizeof(double);
   DevBuf d(bytes);
   if (!d.p) return fail(LBM_ENOMEM, "device staging allocation failed");
@@ -686,6 +719,7 @@ int lbm_diagnostics(lbm_ctx* c, double mass[2], double momentum[3]) {
   if (int rc = check_ctx(c)) return rc;
   if (!mass || !momentum) return fail(LBM_EINVAL, "NULL argument");
   cudaStream_t st = cur_stream();
+  apply_pending(c, st);
   const int nb = c->diag_blocks;
   if (c->bits == 64)
     k_diag_partial<double><<<nb, kDiagBlock, 0, st>>>((const double*)c->f[c->cur], c->partial,
