@@ -72,3 +72,37 @@ def test_config5_full_size_sampled_against_oracle():
     assert cfg["mask"].shape == (512, 512, 512)
     worst = _sampled_one_step_parity(cfg, 16, 43, ("rhoA", "rhoB", "uz"))
     assert all(v <= 1e-5 for v in worst.values()), worst
+
+
+def _elementwise_fp32(cfg, steps):
+    o = LbmRef(cfg["mask"], cfg["params"])
+    g = Lbm(cfg["mask"], cfg["params"])
+    o.set_density(cfg["rhoA"], cfg["rhoB"])
+    g.set_density(cfg["rhoA"], cfg["rhoB"])
+    o.step(steps)
+    g.step(steps)
+    fl = cfg["mask"] == 0
+    mo, mg = o.get_macroscopic(), g.get_macroscopic()
+    for k in ("rhoA", "rhoB"):
+        assert (np.abs(mg[k][fl] - mo[k][fl]) / np.abs(mo[k][fl])).max() <= 1e-4, k
+    uo = np.stack([mo[k][fl] for k in ("ux", "uy", "uz")])
+    ug = np.stack([mg[k][fl] for k in ("ux", "uy", "uz")])
+    assert np.abs(ug - uo).max() <= 1e-4 * np.abs(uo).max()
+    m_o, _ = o.diagnostics()
+    m_g, _ = g.diagnostics()
+    assert np.max(np.abs(m_g - m_o) / m_o) <= 1e-6
+
+
+def test_config2_full_size_elementwise_100_steps():
+    """BASELINE.json config 2 at its full 64^3 size, fp32, every fluid node, 100 steps."""
+    cfg = make_config(2, xi=-0.3)
+    assert cfg["mask"].shape == (64, 64, 64)
+    _elementwise_fp32(cfg, 100)
+
+
+def test_config3_full_size_elementwise_100_steps():
+    """BASELINE.json config 3 at its full 128^3 size (sphere pack, velocity inlet on A, pressure
+    outlet on B), fp32, every fluid node, 100 steps."""
+    cfg = make_config(3)
+    assert cfg["mask"].shape == (128, 128, 128)
+    _elementwise_fp32(cfg, 100)
