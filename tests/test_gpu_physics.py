@@ -82,3 +82,63 @@ def test_laplace_law_3d():
     gamma = (Pin - P[0, 0, 0]) * R / 2.0
     assert abs(R - r0) < 1.5
     assert 0.068 < gamma < 0.080, gamma
+
+
+def _laplace_3d(n, r0, tau, steps):
+    shape = (n, n, n)
+    c = (n - 1) / 2.0
+    rA = tanh_profile(shape, (c, c, c), r0)                     # Eq. (16)
+    g = Lbm(np.zeros(shape, np.uint8), default_params(G=3.5, tau=tau, storage_bits=32))
+    g.set_density(rA, 1.027 - rA)
+    g.step(steps)
+    m = g.get_macroscopic(fields=("rhoA", "rhoB", "P"))
+    g.close()
+    d = m["rhoA"] - m["rhoB"]
+    h = n // 2
+    row = 0.25 * (d[h - 1, h - 1] + d[h, h] + d[h - 1, h] + d[h, h - 1])
+    i = np.nonzero((row[:-1] > 0) & (row[1:] <= 0))[0][0]
+    R = i + row[i] / (row[i] - row[i + 1]) - c
+    P = m["P"]
+    dP = P[h - 1:h + 1, h - 1:h + 1, h - 1:h + 1].mean() - P[0, 0, 0]
+    return R, dP
+
+
+def test_laplace_paper_size_128_cubed():
+    """PAPER.md Sec. 3.1 at the paper's own size: 128^3 periodic box, droplets up to r0 = 30,
+    G = 3.5.  The regression of dP against 2/R gives the surface tension: the paper reports
+    gamma = 0.071 for M = 1, 25 and 1/25 alike (L175-183)."""
+    pts = [_laplace_3d(128, r0, (1.0, 1.0), 12000) for r0 in (18, 24, 30)]
+    x = np.array([2.0 / R for R, _ in pts])
+    y = np.array([dP for _, dP in pts])
+    slope, icpt = np.polyfit(x, y, 1)
+    assert abs(slope / 0.071 - 1.0) < 0.08, (slope, icpt, pts)
+    assert abs(icpt) < 6e-4                                    # dP -> 0 as R -> infinity
+    # independent of the viscosity ratio: same droplet at M = 25 and M = 1/25
+    g1 = pts[2][1] * pts[2][0] / 2.0
+    for tau in ((3.5, 0.62), (0.62, 3.5)):
+        R, dP = _laplace_3d(128, 30, tau, 12000)
+        assert abs(dP * R / 2.0 / g1 - 1.0) < 0.03, (tau, dP * R / 2.0, g1)
+
+
+def test_contact_angle_calibration_paper_size():
+    """PAPER.md Sec. 3.2 at the paper's own size and viscosity ratio: 200 x 100 x 200 (wall-normal
+    extent 100), droplet r0 = 30 on the bottom wall, M = 25 (tau = 3.5 / 0.62), G = 3.5.  theta
+    (through component 2) against the printed cubic (L199) over xi in [-0.4, 0.4]."""
+    nz, ny, nx = 100, 200, 200
+    shape = (nz, ny, nx)
+    mask = np.zeros(shape, np.uint8)
+    mask[0] = mask[-1] = 1
+    rA = tanh_profile(shape, ((nx - 1) / 2.0, (ny - 1) / 2.0, 0.5), 30.0)
+    rA = np.where(mask == 0, rA, 0.0)
+    rB = np.where(mask == 0, 1.027 - rA, 0.0)
+    got = {}
+    for xi in (-0.4, -0.2, 0.0, 0.2, 0.4):
+        g = Lbm(mask, default_params(G=3.5, tau=(3.5, 0.62), xi=xi, storage_bits=32))
+        g.set_density(rA, rB)
+        g.step(15000)
+        m = g.get_macroscopic(fields=("rhoA", "rhoB"))
+        g.close()
+        assert np.isfinite(m["rhoA"]).all()
+        got[xi] = _cap_angle_through_B(m["rhoA"], m["rhoB"])
+    for xi, th in got.items():
+        assert abs(th - _paper_fit(xi)) < 3.0, got
