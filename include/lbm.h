@@ -85,7 +85,9 @@ int lbm_set_boundary(lbm_ctx* c, double inlet_value, double outlet_rho);
 /* Advance n time steps (SURVEY.md §8c steps 1-7 per step): density pass (Eq. 3), virtual solid
  * density (Eq. 14-15), forces (Eq. 10, 11, 13), tau_s and u_eq (Eq. 5-8), collision (Eq. 1, 2,
  * 9), streaming with halfway bounce-back, open-plane fix (L147-157).
- * Asynchronous; n >= 0. */
+ * Asynchronous; n >= 0.  The open-plane fix of the last step is deferred: it is applied by the
+ * next lbm_step (inside its density pass) or by the next getter, whichever comes first, with the
+ * boundary values that were in force when the step ran; callers always observe a complete state. */
 int lbm_step(lbm_ctx* c, int n);
 int lbm_sync(lbm_ctx* c);
 
@@ -109,8 +111,17 @@ long long lbm_num_wall_solid(lbm_ctx* c);  /* N_w: solid voxels with >= 1 fluid 
 int lbm_memory_bytes(lbm_ctx* c, long long bytes[4]);
 /* Device time (ms) of the kernels of the last lbm_step call, by kind, measured with CUDA events
  * on the launching stream when profiling is enabled with lbm_set_profiling(c, 1):
- * ms[0] density pass, [1] virtual-solid pass, [2] collide+stream, [3] open-plane fix; launches =
- * number of kernel launches of that call.  Synchronises. */
+ * ms[0] density pass (in the default path it carries the open-plane fix of the previous step),
+ * [1] virtual-solid pass, [2] collide+stream (the whole step when LBM_B200_STEP=fused),
+ * [3] open-plane fix when it is launched on its own; launches = number of kernel launches of that
+ * call.  Synchronises.
+ *
+ * Tuning / A-B knobs read from the environment by lbm_create (defaults are the production path):
+ *   LBM_B200_STEP=split|fused      one kernel per pass (default) | experimental single-kernel step
+ *   LBM_B200_COLLIDE=bulk|simple   bulk-async staged fused pass (default) | register kernel
+ *   LBM_B200_IDX=16|32             16-bit tile-relative neighbour index (default) | int32 rows
+ *   LBM_B200_REVERSE=1|0           fused pass walks tiles backwards (default) | forwards
+ *   LBM_B200_TILE, LBM_B200_LEAD   CTA shape of the fused pass; producer lead of the fused step */
 int lbm_set_profiling(lbm_ctx* c, int on);
 int lbm_last_step_profile(lbm_ctx* c, double ms[4], long long* launches);
 const char* lbm_last_error(void);

@@ -408,9 +408,11 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
     cudaGetLastError();
     return fail(LBM_ECUDA, "no CUDA device: this library has no CPU fallback");
   }
+  int device = 0;
+  CU(cudaGetDevice(&device));
   lbm_ctx* c = new (std::nothrow) lbm_ctx;
   if (!c) return fail(LBM_ENOMEM, "host allocation failed");
-  CU(cudaGetDevice(&c->device));
+  c->device = device;
   cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
   c->p = *p;
   c->nx = nx; c->ny = ny; c->nz = nz; c->np = nx * ny; c->nvox = g.nvox;
