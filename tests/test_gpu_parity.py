@@ -292,3 +292,51 @@ def test_fused_single_kernel_step_matches_split_and_oracle(monkeypatch):
         s.step(25)
     for comp in (0, 1):
         assert np.array_equal(a.get_populations(comp), b.get_populations(comp))
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 64), (1, 40, 41), (3, 1, 5), (2, 2, 2)])
+def test_degenerate_box_shapes_fp64(shape):
+    """Boxes that are one voxel thick along one or two axes (a voxel is then its own periodic
+    neighbour) and a 2x2x2 box (every neighbour pair wraps): fp64, with solids and wetting."""
+    rng = np.random.Generator(np.random.PCG64(sum(shape)))
+    mask = (rng.uniform(size=shape) < 0.2).astype(np.uint8)
+    mask.flat[0] = 0
+    rA = np.where(mask == 0, rng.uniform(0.1, 1.0, shape), 0.0)
+    rB = np.where(mask == 0, rng.uniform(0.1, 1.0, shape), 0.0)
+    p = default_params(G=2.0, tau=(0.9, 1.3), xi=-0.2, accel=(1e-5, 2e-5, -1e-5), storage_bits=64)
+    o, g = _pair(mask, rA, rB, p)
+    o.step(15)
+    g.step(15)
+    assert _pop_rel(o, g, mask) <= 1e-10
+
+
+def test_periodic_box_larger_than_15_bit_offsets_fp64():
+    """48^3 periodic box (110 592 nodes): tiles that straddle the z wrap have neighbour-id ranges
+    wider than the 15-bit offsets of the tile-relative index and take the int32 fallback rows."""
+    c = make_config(1, size=48)
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    o.step(8)
+    g.step(8)
+    assert _pop_rel(o, g, c["mask"]) <= 1e-12
+
+
+def test_fp32_run_is_deterministic():
+    c = make_config(4, size=40)
+    res = []
+    for _ in range(2):
+        g = Lbm(c["mask"], c["params"])
+        g.set_density(c["rhoA"], c["rhoB"])
+        g.step(50)
+        res.append([g.get_populations(s) for s in (0, 1)])
+        g.close()
+    for s in (0, 1):
+        assert np.array_equal(res[0][s], res[1][s])
+
+
+def test_velocity_inlet_on_component_b_and_extreme_parameters_fp64():
+    c = make_config(3, size=24, storage_bits=64, inlet_comp=1, outlet_comp=0, inlet_uz=5e-4,
+                    tau=(0.55, 3.5), xi=0.5)
+    o, g = _pair(c["mask"], c["rhoA"], c["rhoB"], c["params"])
+    o.step(40)
+    g.step(40)
+    assert _pop_rel(o, g, c["mask"]) <= 1e-10
