@@ -205,11 +205,11 @@ template <typename T, int TN, int MINB, bool IDX16>
 void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
   constexpr bool kRemainder = sizeof(T) == 4;
   constexpr size_t smem = IDX16 ? collide16_smem_bytes<T, TN>() : collide_smem_bytes<T, TN>();
-  static bool configured = false;
-  if (!configured) {
+  static bool configured[64] = {};  // function attributes are per device
+  if (!configured[c->device & 63]) {
     cudaFuncSetAttribute(k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX16>,
                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = true;
+    configured[c->device & 63] = true;
   }
   Idx16 ix;
   ix.nbr16 = c->nbr16;
@@ -252,7 +252,8 @@ int launch_fused(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
   constexpr bool kRemainder = sizeof(T) == 4;
   constexpr size_t smem = collide_smem_bytes<T, TN>();
   auto kern = k_step_fused<T, TN, MINB, kRemainder>;
-  static int grid_cache = 0;
+  static int grid_cache_dev[64] = {};  // per device
+  int& grid_cache = grid_cache_dev[c->device & 63];
   if (grid_cache == 0) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
