@@ -42,6 +42,9 @@ def test_lattice_identities():
     n2 = (e * e).sum(1)
     assert np.allclose(w[n2 == 0], 1 / 3) and np.allclose(w[n2 == 1], 1 / 18)
     assert np.allclose(w[n2 == 2], 1 / 36) and sorted(np.bincount(n2)) == [1, 6, 12]
+    with open(os.path.join(HERE, "golden", "paper_values.txt")) as fh:
+        printed = [l.split("#")[0].split()[1:] for l in fh if l.startswith("weights")][0]
+    assert np.allclose(sorted(set(np.round(w, 15)), reverse=True), [float(v) for v in printed])
     for i in range(19):
         assert np.array_equal(e[opp[i]], -e[i])
     # what PAPER.md L152-154 and L113 reveal about the numbering (flow axis = z here)
