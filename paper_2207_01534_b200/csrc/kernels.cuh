@@ -620,7 +620,8 @@ __global__ void __launch_bounds__(TN, MINB)
 }
 
 // ---------------------------------------------------------------------------------------------
-// Fused single-kernel step (production).  The two grid-wide dependencies of a step -- every
+// Fused single-kernel step (EXPERIMENTAL, LBM_B200_STEP=fused; slower than the default one kernel
+// per pass on B200).  The two grid-wide dependencies of a step -- every
 // node's force needs its neighbours' rho(t), every wall solid's rho~(t) needs its fluid
 // neighbours' rho(t) -- are resolved INSIDE one persistent kernel instead of by kernel
 // boundaries, so that the density pass runs only a short distance ahead of the fused pass and the
