@@ -3,7 +3,8 @@
 // oracle/.  Layout and byte counts: DESIGN.md "Data layout in HBM" and "Kernels".
 //
 // Storage (T = float or double):
-//   f   [2 comps][19 dirs][npad]   populations at time t (post-streaming), node id fastest
+//   f   [19 dirs][npad][2 comps]   populations at time t (post-streaming): the two components of a
+//                                  population are adjacent (one 8-byte pair in fp32), node id next
 //   psi [npad + nwpad] of Vec2<T>  (rho_A, rho_B) at fluid id n; (rho~_A, rho~_B) of wall solid w at
 //                                  npad + w (both parts start on a tile boundary)
 //   nbr [18][npad] int32           psi index of x+e_i: < nf fluid id; >= npad wall solid;
@@ -44,6 +45,11 @@ __host__ __device__ constexpr int inward(int plane, int k) {
   return t[plane][k];
 }
 
+// index of population (component s, direction i, node n) in f
+__host__ __device__ __forceinline__ size_t pidx(int s, int i, size_t n, size_t npad) {
+  return ((size_t)i * npad + n) * 2 + (size_t)s;
+}
+
 template <typename T> struct Vec2;
 template <> struct __align__(8) Vec2<float> { float a, b; };
 template <> struct __align__(16) Vec2<double> { double a, b; };
@@ -65,15 +71,13 @@ __global__ void __launch_bounds__(256) k_density(const T* __restrict__ f, Vec2<T
                                                  int nf, size_t npad) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
   if (n >= nf) return;
-  T a[Q], b[Q];
+  const Vec2<T>* f2 = reinterpret_cast<const Vec2<T>*>(f);
+  Vec2<T> v[Q];
 #pragma unroll
-  for (int i = 0; i < Q; ++i) {
-    a[i] = f[(size_t)i * npad + n];
-    b[i] = f[(size_t)(Q + i) * npad + n];
-  }
-  T ra = a[0], rb = b[0];
+  for (int i = 0; i < Q; ++i) v[i] = f2[(size_t)i * npad + n];
+  T ra = v[0].a, rb = v[0].b;
 #pragma unroll
-  for (int i = 1; i < Q; ++i) { ra += a[i]; rb += b[i]; }
+  for (int i = 1; i < Q; ++i) { ra += v[i].a; rb += v[i].b; }
   Vec2<T> o; o.a = ra; o.b = rb;
   psi[n] = o;
 }
@@ -211,14 +215,14 @@ __device__ __forceinline__ void collide_component(const T (&f)[Q], T rho, const 
 }
 
 template <typename T>
-__device__ __forceinline__ void push_component(T* __restrict__ fo, const T (&v)[Q],
+__device__ __forceinline__ void push_component(T* __restrict__ fo, int s, const T (&v)[Q],
                                                const int (&id)[Q], int n, int nf, size_t npad) {
-  fo[n] = v[0];
+  fo[pidx(s, 0, n, npad)] = v[0];
 #pragma unroll
   for (int i = 1; i < Q; ++i) {
     const int k = id[i];
-    if ((unsigned)k < (unsigned)nf) fo[(size_t)i * npad + k] = v[i];        // fluid neighbour
-    else if (k >= nf) fo[(size_t)opp(i) * npad + n] = v[i];                  // halfway bounce-back
+    if ((unsigned)k < (unsigned)nf) fo[pidx(s, i, k, npad)] = v[i];         // fluid neighbour
+    else if (k >= nf) fo[pidx(s, opp(i), n, npad)] = v[i];                   // halfway bounce-back
     // k < 0: the population leaves through an open plane
   }
 }
@@ -238,16 +242,16 @@ __global__ void __launch_bounds__(256) k_collide_stream(const T* __restrict__ fi
   T fa[Q], fb[Q];
 #pragma unroll
   for (int i = 0; i < Q; ++i) {
-    fa[i] = fin[(size_t)i * npad + n];
-    fb[i] = fin[(size_t)(Q + i) * npad + n];
+    fa[i] = fin[pidx(0, i, n, npad)];
+    fb[i] = fin[pidx(1, i, n, npad)];
   }
   NodeState<T> s;
   node_state<T>(fa, fb, psi, id, c, s);
   T v[Q];
   collide_component<T, REMAINDER>(fa, s.rhoA, s.FA, s.u, s.om, v);
-  push_component<T>(fout, v, id, n, nf, npad);
+  push_component<T>(fout, 0, v, id, n, nf, npad);
   collide_component<T, REMAINDER>(fb, s.rhoB, s.FB, s.u, s.om, v);
-  push_component<T>(fout + (size_t)Q * npad, v, id, n, nf, npad);
+  push_component<T>(fout, 1, v, id, n, nf, npad);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -343,7 +347,7 @@ constexpr size_t collide_smem_bytes() {
 // add/sub/mul/fma .f32x2 -> SASS FADD2/FMUL2/FFMA2, two FP32 results per issue slot; a scalar
 // broadcast operand and the half-swap are free operand modifiers); for fp64 they are two plain
 // operations.  This halves the floating-point issue slots of an issue-bound kernel.
-template <typename T> struct Pr { T a, b; };
+template <typename T> struct alignas(2 * sizeof(T)) Pr { T a, b; };
 
 __device__ __forceinline__ Pr<double> padd(Pr<double> x, Pr<double> y) { return {x.a + y.a, x.b + y.b}; }
 __device__ __forceinline__ Pr<double> psub(Pr<double> x, Pr<double> y) { return {x.a - y.a, x.b - y.b}; }
@@ -406,8 +410,8 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
                                                     const Vec2<T>* __restrict__ psi, const int nf,
                                                     const size_t npad, const Consts<T>& c) {
   using P = Pr<T>;
-  const T* sfa = sf + tid;                   // component A column
-  const T* sfb = sf + (size_t)Q * TN + tid;  // component B column
+  // staged populations: [19][TN] pairs (A, B); column tid
+  const P* sfp = reinterpret_cast<const P*>(sf) + tid;
   const int* sidc = sid + tid;
 
   // a3 inputs: Psi gathers through the staged neighbour ids.  S[d] = sum_i w_i e_id Psi(x+e_i) as
@@ -432,11 +436,11 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
       S[d] = pfma(pbc(wgt<T>(1)), a1[d], pmul(pbc(wgt<T>(7)), a2[d]));
   }
   // a1 (recomputed locally): R = (rho_A, rho_B); J[d] = per-component bare momentum
-  P R = {sfa[0], sfb[0]};
+  P R = sfp[0];
   P J[3] = {{T(0), T(0)}, {T(0), T(0)}, {T(0), T(0)}};
 #pragma unroll
   for (int i = 1; i < Q; ++i) {
-    const P f = {sfa[i * TN], sfb[i * TN]};
+    const P f = sfp[i * TN];
     R = padd(R, f);
     if (ex(i)) J[0] = ex(i) > 0 ? padd(J[0], f) : psub(J[0], f);
     if (ey(i)) J[1] = ey(i) > 0 ? padd(J[1], f) : psub(J[1], f);
@@ -465,9 +469,8 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
   const P M3UF = pmul(pbc(T(-3)), pfma(pbc(u[0]), F[0], pfma(pbc(u[1]), F[1], pmul(pbc(u[2]), F[2]))));
   const P KA1 = pmul(pbc(om * wgt<T>(1)), R), KA2 = pmul(pbc(om * wgt<T>(7)), R);
   const T kB1 = cS * wgt<T>(1), kB2 = cS * wgt<T>(7);
-  const unsigned np32 = (unsigned)npad;  // 38 * npad < 2^31: 32-bit slot indices
-  T* foa = fout;
-  T* fob = fout + (size_t)Q * npad;
+  const unsigned np32 = (unsigned)npad;  // 19 * npad < 2^31: 32-bit pair-slot indices
+  P* fo = reinterpret_cast<P*>(fout);  // pair (A, B) of population i at node k: fo[i * npad + k]
   P acc = {T(0), T(0)};
 #pragma unroll
   for (int i = 1; i < Q; i += 2) {  // canonical order: the opposite of an odd i is its partner
@@ -481,25 +484,25 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
     const P B = pfma(pbc(T(9) * eu), EF, M3UF);
     const P X = pfma(KA, pbc(A), pmul(pbc(kB), B));
     const P Y = pfma(KA, pbc(eu), pmul(pbc(kB), EF));
-    const P fp = {sfa[ip * TN], sfb[ip * TN]};
-    const P fm = {sfa[im * TN], sfb[im * TN]};
+    const P fp = sfp[ip * TN];
+    const P fm = sfp[im * TN];
     const P vp = pfma(pbc(c1), fp, pfma(Y, pbc(T(3)), X));
     const P vm = pfma(pbc(c1), fm, pfma(Y, pbc(T(-3)), X));
     acc = padd(acc, padd(vp, vm));
     // a6: push-streaming with halfway bounce-back, branch-free: the slot is computed once per
-    // direction and used for both components; one predicated store per population
+    // direction; one predicated 8-byte store carries both components of a population
     // (k < 0: the population leaves through an open plane and is dropped).
     {
       const int k = sidc[(ip - 1) * TN];
       const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)ip * np32 + (unsigned)k
                                                        : (unsigned)im * np32 + (unsigned)n;
-      if (valid && k >= 0) { foa[slot] = vp.a; fob[slot] = vp.b; }
+      if (valid && k >= 0) fo[slot] = vp;
     }
     {
       const int k = sidc[(im - 1) * TN];
       const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)im * np32 + (unsigned)k
                                                        : (unsigned)ip * np32 + (unsigned)n;
-      if (valid && k >= 0) { foa[slot] = vm.a; fob[slot] = vm.b; }
+      if (valid && k >= 0) fo[slot] = vm;
     }
   }
   // rest population: Eq. (1) with e_0 = 0, or the remainder rho - sum_{i>=1} f*_i (fp32 build)
@@ -508,10 +511,10 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
     v0 = psub(R, acc);
   } else {
     const T w0 = wgt<T>(0);
-    const P f0 = {sfa[0], sfb[0]};
+    const P f0 = sfp[0];
     v0 = pfma(pbc(c1), f0, pfma(pbc(om * w0 * k0), R, pmul(pbc(cS * w0), M3UF)));
   }
-  if (valid) { foa[n] = v0.a; fob[n] = v0.b; }
+  if (valid) fo[n] = v0;
 }
 
 // Stage one tile: 38 population rows + 18 neighbour-index rows of TN nodes -> shared memory,
@@ -523,8 +526,8 @@ __device__ __forceinline__ void load_tile(T* sf, int* sid, const T* __restrict__
   if (elect_one()) {
     mbar_expect_tx(bar, (uint32_t)collide_smem_bytes<T, TN>());
 #pragma unroll
-    for (int r = 0; r < 2 * Q; ++r)
-      bulk_g2s(sf + (size_t)r * TN, fin + (size_t)r * npad + t0, TN * sizeof(T), bar);
+    for (int r = 0; r < Q; ++r)  // one row of TN (A, B) pairs per direction
+      bulk_g2s(sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2, 2 * TN * sizeof(T), bar);
 #pragma unroll
     for (int r = 0; r < 18; ++r)
       bulk_g2s(sid + (size_t)r * TN, nbr + (size_t)r * npad + t0, TN * sizeof(int), bar);
@@ -578,8 +581,9 @@ __global__ void __launch_bounds__(TN, MINB)
         mbar_expect_tx(&bar, (uint32_t)((size_t)2 * Q * TN * sizeof(T) +
                                         (size_t)18 * TN * sizeof(uint16_t) + kIdxMeta * sizeof(int)));
 #pragma unroll
-        for (int r = 0; r < 2 * Q; ++r)
-          bulk_g2s(sf + (size_t)r * TN, fin + (size_t)r * npad + t0, TN * sizeof(T), &bar);
+        for (int r = 0; r < Q; ++r)  // one row of TN (A, B) pairs per direction
+          bulk_g2s(sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2, 2 * TN * sizeof(T),
+                   &bar);
 #pragma unroll
         for (int r = 0; r < 18; ++r)
           bulk_g2s(s16 + (size_t)r * TN, ix.nbr16 + (size_t)r * npad + t0, TN * sizeof(uint16_t),
@@ -733,11 +737,14 @@ __global__ void __launch_bounds__(TN, MINB)
     if (type == 0) {
       // ---- D(t): a1 on fluid tile t
       const int n = t * TN + tid;
-      T ra = T(0), rb = T(0);
+      const Vec2<T>* f2 = reinterpret_cast<const Vec2<T>*>(fin);
+      Vec2<T> v0 = f2[n];
+      T ra = v0.a, rb = v0.b;
 #pragma unroll
-      for (int i = 0; i < Q; ++i) {
-        ra += fin[(size_t)i * npad + n];
-        rb += fin[(size_t)(Q + i) * npad + n];
+      for (int i = 1; i < Q; ++i) {
+        const Vec2<T> v = f2[(size_t)i * npad + n];
+        ra += v.a;
+        rb += v.b;
       }
       Vec2<T> o; o.a = ra; o.b = rb;
       psi[n] = o;  // n < npad always; the padding holds zeros
@@ -821,7 +828,7 @@ __device__ __forceinline__ Vec2<T> open_plane_node(T* __restrict__ f, const T* _
   for (int s = 0; s < 2; ++s)
 #pragma unroll
     for (int i = 0; i < Q; ++i) {
-      const T v = f[(size_t)(s * Q + i) * npad + vf];
+      const T v = f[pidx(s, i, vf, npad)];
       ff[s][i] = v;
       rf[s] += v;
       if (ex(i)) j[0] += T(ex(i)) * v;
@@ -845,7 +852,7 @@ __device__ __forceinline__ Vec2<T> open_plane_node(T* __restrict__ f, const T* _
   for (int i = 0; i < Q; ++i) {
     const T fi = dc == 0 ? ff[0][i] : ff[1][i];
     const T v = feq_of<T>(i, rho_b, ub) + (fi - feq_of<T>(i, rfd, uf));
-    f[(size_t)(dc * Q + i) * npad + vb] = v;
+    f[pidx(dc, i, vb, npad)] = v;
     rd = i == 0 ? v : rd + v;
   }
   const int oc = 1 - dc;
@@ -859,9 +866,9 @@ __device__ __forceinline__ Vec2<T> open_plane_node(T* __restrict__ f, const T* _
       for (int kk = 0; kk < 5; ++kk)
         if (inward(0, kk) == i || inward(1, kk) == i) k = kk;
       v = frozen[((size_t)(plane * 2 + oc) * 5 + k) * np + q];
-      f[(size_t)(oc * Q + i) * npad + vb] = v;
+      f[pidx(oc, i, vb, npad)] = v;
     } else {
-      v = f[(size_t)(oc * Q + i) * npad + vb];
+      v = f[pidx(oc, i, vb, npad)];
     }
     ro = i == 0 ? v : ro + v;
   }
@@ -893,12 +900,13 @@ __global__ void __launch_bounds__(256, 4)
   if ((int)blockIdx.x >= nb_planes) {
     const int n = ((int)blockIdx.x - nb_planes) * blockDim.x + threadIdx.x;
     if (n >= nf || n < np || n >= nf - np) return;
-    T ra = f[n], rb = f[(size_t)Q * npad + n];
+    const Vec2<T>* f2 = reinterpret_cast<const Vec2<T>*>(f);
+    Vec2<T> v[Q];
 #pragma unroll
-    for (int i = 1; i < Q; ++i) {
-      ra += f[(size_t)i * npad + n];
-      rb += f[(size_t)(Q + i) * npad + n];
-    }
+    for (int i = 0; i < Q; ++i) v[i] = f2[(size_t)i * npad + n];
+    T ra = v[0].a, rb = v[0].b;
+#pragma unroll
+    for (int i = 1; i < Q; ++i) { ra += v[i].a; rb += v[i].b; }
     Vec2<T> o; o.a = ra; o.b = rb;
     psi[n] = o;
   } else {  // the plane blocks come first so that their dependent chain overlaps the streaming
@@ -920,7 +928,7 @@ __global__ void k_record_frozen(const T* __restrict__ f, T* __restrict__ frozen,
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
     const int i = plane == 0 ? inward(0, k) : inward(1, k);
-    frozen[((size_t)(plane * 2 + comp) * 5 + k) * np + q] = f[(size_t)(comp * Q + i) * npad + vb];
+    frozen[((size_t)(plane * 2 + comp) * 5 + k) * np + q] = f[pidx(comp, i, vb, npad)];
   }
 }
 
@@ -937,23 +945,24 @@ __global__ void k_init_density(const double* __restrict__ rhoA, const double* __
   const double ra = rhoA[v], rb = rhoB[v];
 #pragma unroll
   for (int i = 0; i < Q; ++i) {  // f_i = w_i rho (reading R11)
-    f[(size_t)i * npad + n] = (T)(wgt<double>(i) * ra);
-    f[(size_t)(Q + i) * npad + n] = (T)(wgt<double>(i) * rb);
+    f[pidx(0, i, n, npad)] = (T)(wgt<double>(i) * ra);
+    f[pidx(1, i, n, npad)] = (T)(wgt<double>(i) * rb);
   }
 }
 
 template <typename T>
 __global__ void k_dense_to_compact(const double* __restrict__ dense,
-                                   const int* __restrict__ node_vox, T* __restrict__ row, int nf) {
+                                   const int* __restrict__ node_vox, T* __restrict__ row, int nf,
+                                   int stride) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
-  if (n < nf) row[n] = (T)dense[node_vox[n]];
+  if (n < nf) row[(size_t)n * stride] = (T)dense[node_vox[n]];
 }
 
 template <typename T>
 __global__ void k_compact_to_dense(const T* __restrict__ row, const int* __restrict__ node_vox,
-                                   double* __restrict__ dense, int nf) {
+                                   double* __restrict__ dense, int nf, int stride) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
-  if (n < nf) dense[node_vox[n]] = (double)row[n];
+  if (n < nf) dense[node_vox[n]] = (double)row[(size_t)n * stride];
 }
 
 // rho_sigma, u = u_eq, P = (rho_A+rho_B)/3 + (G/3) rho_A rho_B (Eq. 12, R13) into
@@ -973,8 +982,8 @@ __global__ void __launch_bounds__(256) k_macroscopic(const T* __restrict__ fin,
   T fa[Q], fb[Q];
 #pragma unroll
   for (int i = 0; i < Q; ++i) {
-    fa[i] = fin[(size_t)i * npad + n];
-    fb[i] = fin[(size_t)(Q + i) * npad + n];
+    fa[i] = fin[pidx(0, i, n, npad)];
+    fb[i] = fin[pidx(1, i, n, npad)];
   }
   NodeState<T> s;
   node_state<T>(fa, fb, psi, id, c, s);
@@ -1009,7 +1018,7 @@ __global__ void __launch_bounds__(kDiagBlock) k_diag_partial(const T* __restrict
     for (int s = 0; s < 2; ++s)
 #pragma unroll
       for (int i = 0; i < Q; ++i) {
-        const double v = (double)f[(size_t)(s * Q + i) * npad + n];
+        const double v = (double)f[pidx(s, i, n, npad)];
         acc[s] += v;
         if (ex(i)) acc[2] += ex(i) * v;
         if (ey(i)) acc[3] += ey(i) * v;

@@ -71,7 +71,7 @@ struct lbm_ctx {
   int nf = 0, nw = 0;
   size_t npad = 0, nwpad = 0, esz = 4;
   std::vector<int32_t> vox2id, node_vox, zstart;  // host copies used by queries
-  void* f[2] = {nullptr, nullptr};                // [2][19][npad] T
+  void* f[2] = {nullptr, nullptr};                // two buffers of [19][npad][2 comps] T
   void* psi = nullptr;                            // [nf+nw] Vec2<T>
   int* nbr = nullptr;                             // [18][npad]
   int* wall_nbr = nullptr;                        // [18][nwpad]
@@ -642,13 +642,13 @@ int lbm_set_populations(lbm_ctx* c, int comp, const double* f) {
   if (!d.p) return fail(LBM_ENOMEM, "device staging allocation failed");
   for (int i = 0; i < Q; ++i) {
     CU(cudaMemcpyAsync(d.p, f + (size_t)i * c->nvox, bytes, cudaMemcpyHostToDevice, st));
-    const size_t row = (size_t)(comp * Q + i) * c->npad;
+    const size_t row = pidx(comp, i, 0, c->npad);  // element stride 2: components are interleaved
     if (c->bits == 64)
       k_dense_to_compact<double><<<blocks(c->nf, 256), 256, 0, st>>>(
-          (const double*)d.p, c->node_vox_d, (double*)c->f[c->cur] + row, c->nf);
+          (const double*)d.p, c->node_vox_d, (double*)c->f[c->cur] + row, c->nf, 2);
     else
       k_dense_to_compact<float><<<blocks(c->nf, 256), 256, 0, st>>>(
-          (const double*)d.p, c->node_vox_d, (float*)c->f[c->cur] + row, c->nf);
+          (const double*)d.p, c->node_vox_d, (float*)c->f[c->cur] + row, c->nf, 2);
     CU(cudaStreamSynchronize(st));  // pageable source: keep the staging buffer reuse ordered
   }
   CU(cudaPeekAtLastError());
@@ -669,13 +669,13 @@ int lbm_get_populations(lbm_ctx* c, int comp, double* f) {
   if (!d.p) return fail(LBM_ENOMEM, "device staging allocation failed");
   for (int i = 0; i < Q; ++i) {
     CU(cudaMemsetAsync(d.p, 0, bytes, st));
-    const size_t row = (size_t)(comp * Q + i) * c->npad;
+    const size_t row = pidx(comp, i, 0, c->npad);  // element stride 2: components are interleaved
     if (c->bits == 64)
       k_compact_to_dense<double><<<blocks(c->nf, 256), 256, 0, st>>>(
-          (const double*)c->f[c->cur] + row, c->node_vox_d, (double*)d.p, c->nf);
+          (const double*)c->f[c->cur] + row, c->node_vox_d, (double*)d.p, c->nf, 2);
     else
       k_compact_to_dense<float><<<blocks(c->nf, 256), 256, 0, st>>>(
-          (const float*)c->f[c->cur] + row, c->node_vox_d, (double*)d.p, c->nf);
+          (const float*)c->f[c->cur] + row, c->node_vox_d, (double*)d.p, c->nf, 2);
     CU(cudaMemcpyAsync(f + (size_t)i * c->nvox, d.p, bytes, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
   }
@@ -710,7 +710,7 @@ int lbm_get_macroscopic(lbm_ctx* c, double* rhoA, double* rhoB, double* ux, doub
     if (!outs[q]) continue;
     CU(cudaMemsetAsync(d.p, 0, bytes, st));
     k_compact_to_dense<double><<<blocks(c->nf, 256), 256, 0, st>>>(
-        (const double*)m.p + (size_t)q * c->nf, c->node_vox_d, (double*)d.p, c->nf);
+        (const double*)m.p + (size_t)q * c->nf, c->node_vox_d, (double*)d.p, c->nf, 1);
     CU(cudaMemcpyAsync(outs[q], d.p, bytes, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
   }
