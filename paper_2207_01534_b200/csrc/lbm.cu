@@ -425,7 +425,8 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   if (const char* e = std::getenv("LBM_B200_IDX")) c->idx16 = std::atoi(e) == 32 ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_STEP")) c->step_variant = !std::strcmp(e, "split") ? 0 : 1;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
-  if ((size_t)2 * 19 * c->npad >= ((size_t)1 << 31)) {
+  // pair-slot indices i * npad + k and psi indices npad + w are 32-bit
+  if ((size_t)19 * c->npad >= ((size_t)1 << 31) || c->npad + c->nwpad >= ((size_t)1 << 31)) {
     delete c;
     return fail(LBM_EINVAL, "too many fluid nodes for 32-bit slot indices");
   }
