@@ -101,8 +101,11 @@ int lbm_diagnostics(lbm_ctx* c, double mass[2], double momentum[3]);
 /* Saturation of component comp in z in [z0,z1): fraction of fluid nodes with rho_comp greater
  * than the other density (tie -> component 1) (reading R14). */
 int lbm_saturation(lbm_ctx* c, int comp, int z0, int z1, double* S);
-/* Trapped volume (reading R15): phase-comp nodes in [z0,z1) whose 6-connected same-phase
- * cluster (periodic in x,y; not across z) touches neither z=0 nor z=nz-1. */
+/* Trapped volume (reading R15): phase-comp nodes in [z0,z1) whose 6-connected
+ * same-phase cluster (periodic in x,y; not across z) touches neither z=0 nor z=nz-1; *nodes is
+ * their number, *mass the sum of rho_comp over them.  The phase of a node is decided as in
+ * lbm_saturation.  Runs on the GPU (lock-free union-find over the compact ids, 8 B per fluid
+ * node of temporary device memory); an empty z-range gives 0.  Synchronises. */
 int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, double* mass);
 
 long long lbm_num_fluid(lbm_ctx* c);       /* N_f, or -1 */

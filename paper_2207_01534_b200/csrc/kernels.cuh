@@ -1066,4 +1066,130 @@ __global__ void k_count_phase(const Vec2<T>* __restrict__ psi, int n0, int n1, i
   if ((threadIdx.x & 31) == 0 && b) atomicAdd(count, (unsigned long long)__popc(b));
 }
 
+// ---------------------------------------------------------------------------------------------
+// a7  trapped volume (reading R15): connected components of the phase-comp
+// fluid nodes over the 6-neighbour graph (periodic in x,y; no edge across the z ends), by
+// lock-free union-find on the compact ids.  parent[n] = -1 for nodes of the other phase; a
+// larger root is always hooked under a smaller one, so the root of a cluster is its smallest id
+// and the result does not depend on the interleaving.  Every access to parent[] goes to L2
+// (ld.cg / st.cg / atomics): a stale L1 line could make the hook loop spin.
+template <typename T>
+__global__ void __launch_bounds__(256) k_ccl_init(const Vec2<T>* __restrict__ psi, int nf, int comp,
+                                                  int* __restrict__ parent, int* __restrict__ flag) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= nf) return;
+  const Vec2<T> p = psi[n];
+  const int owner = p.a > p.b ? 0 : 1;  // tie -> component 1, as k_count_phase
+  parent[n] = owner == comp ? n : -1;
+  flag[n] = 0;
+}
+
+__device__ __forceinline__ int ccl_find(int* parent, int x) {
+  int p = __ldcg(parent + x);
+  while (p != x) {  // path halving: x is not a root and never becomes one again
+    const int g = __ldcg(parent + p);
+    if (g != p) __stcg(parent + x, g);
+    x = p;
+    p = g;
+  }
+  return x;
+}
+
+__device__ __forceinline__ void ccl_unite(int* parent, int a, int b) {
+  for (;;) {
+    a = ccl_find(parent, a);
+    b = ccl_find(parent, b);
+    if (a == b) return;
+    if (a < b) { const int t = a; a = b; b = t; }
+    if (atomicCAS(parent + a, a, b) == a) return;  // else a was hooked meanwhile: look again
+  }
+}
+
+// one thread per fluid node: joins it to its +x, +y, +z neighbour of the same phase (each edge of
+// the graph is the forward edge of exactly one of its ends; the periodic wrap in z is the one
+// forward neighbour with a smaller id, and a neighbour beyond an open plane is negative)
+__global__ void __launch_bounds__(256) k_ccl_unite(const int* __restrict__ nbr, int nf, size_t npad,
+                                                   int* parent) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= nf || __ldcg(parent + n) < 0) return;
+#pragma unroll
+  for (int i = 1; i <= 5; i += 2) {
+    static_assert(ex(1) == 1 && ey(3) == 1 && ez(5) == 1, "forward axis directions");
+    const int m = nbr[(size_t)(i - 1) * npad + n];
+    if (m < 0 || m >= nf || (i == 5 && m <= n)) continue;
+    if (__ldcg(parent + m) < 0) continue;
+    ccl_unite(parent, n, m);
+  }
+}
+
+// after the last union: parent[n] <- root.  The walk only reads (a path-halving store by another
+// thread could land after this thread's final store and leave a non-root behind); whatever it
+// meets on the way is either an old ancestor or already the root.
+__global__ void __launch_bounds__(256) k_ccl_flatten(int nf, int* parent) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= nf) return;
+  int x = __ldcg(parent + n);
+  if (x < 0) return;
+  for (int p = __ldcg(parent + x); p != x; p = __ldcg(parent + x)) x = p;
+  __stcg(parent + n, x);
+}
+
+// clusters with a node on z = 0 or z = nz-1 are connected to an end plane; [a0,a1) and [b0,b1)
+// are the id ranges of those two planes
+__global__ void __launch_bounds__(256) k_ccl_mark(const int* __restrict__ parent, int a0, int a1,
+                                                  int b0, int b1, int* __restrict__ flag) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  const int na = a1 - a0;
+  if (k >= na + (b1 - b0)) return;
+  const int n = k < na ? a0 + k : b0 + (k - na);
+  const int r = parent[n];
+  if (r >= 0) flag[r] = 1;
+}
+
+// nodes and mass of the unmarked clusters in the id range [n0,n1); block b takes one contiguous
+// chunk and k_ccl_final adds the per-block results in block order (deterministic)
+constexpr int kCclBlock = 256;
+template <typename T>
+__global__ void __launch_bounds__(kCclBlock) k_ccl_count(const Vec2<T>* __restrict__ psi,
+                                                         const int* __restrict__ parent,
+                                                         const int* __restrict__ flag, int n0, int n1,
+                                                         int comp, int chunk,
+                                                         double* __restrict__ partial) {
+  __shared__ double smass[kCclBlock / 32];
+  __shared__ long long scnt[kCclBlock / 32];
+  const int lo = n0 + blockIdx.x * chunk;
+  const int hi = min(n1, lo + chunk);
+  double mass = 0.0;
+  long long cnt = 0;
+  for (int n = lo + threadIdx.x; n < hi; n += kCclBlock) {
+    const int r = parent[n];
+    if (r >= 0 && flag[r] == 0) {
+      const Vec2<T> p = psi[n];
+      mass += (double)(comp == 0 ? p.a : p.b);
+      ++cnt;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    mass += __shfl_down_sync(0xffffffffu, mass, o);
+    cnt += __shfl_down_sync(0xffffffffu, cnt, o);
+  }
+  if ((threadIdx.x & 31) == 0) { smass[threadIdx.x >> 5] = mass; scnt[threadIdx.x >> 5] = cnt; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < kCclBlock / 32; ++w) { mass += smass[w]; cnt += scnt[w]; }
+    partial[2 * blockIdx.x] = mass;
+    partial[2 * blockIdx.x + 1] = (double)cnt;  // exact: < 2^53
+  }
+}
+
+__global__ void k_ccl_final(const double* __restrict__ partial, int nblocks, double* __restrict__ out) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double mass = 0.0, cnt = 0.0;
+  for (int b = 0; b < nblocks; ++b) { mass += partial[2 * b]; cnt += partial[2 * b + 1]; }
+  out[0] = mass;
+  out[1] = cnt;
+}
+
+
 }  // namespace lbmk

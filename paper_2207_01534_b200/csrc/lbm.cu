@@ -782,58 +782,43 @@ int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, d
   if (c->bits == 64) launch_psi<double>(c, st); else launch_psi<float>(c, st);
   c->prof = was;
   CU(cudaPeekAtLastError());
-  const int nf = c->nf;
-  std::vector<double> rho;  // rho_comp per fluid node
-  std::vector<uint8_t> state;
-  try {
-    rho.resize(nf);
-    state.resize(nf);
-    if (c->bits == 64) {
-      std::vector<double> h((size_t)2 * nf);
-      CU(cudaMemcpyAsync(h.data(), c->psi, h.size() * 8, cudaMemcpyDeviceToHost, st));
-      CU(cudaStreamSynchronize(st));
-      for (int n = 0; n < nf; ++n) {
-        state[n] = ((h[2 * n] > h[2 * n + 1]) ? 0 : 1) == comp;
-        rho[n] = h[2 * n + comp];
-      }
-    } else {
-      std::vector<float> h((size_t)2 * nf);
-      CU(cudaMemcpyAsync(h.data(), c->psi, h.size() * 4, cudaMemcpyDeviceToHost, st));
-      CU(cudaStreamSynchronize(st));
-      for (int n = 0; n < nf; ++n) {
-        state[n] = ((h[2 * n] > h[2 * n + 1]) ? 0 : 1) == comp;
-        rho[n] = h[2 * n + comp];
-      }
-    }
-    // flood from both end planes through same-phase 6-neighbours (periodic x,y; not across z)
-    std::vector<int32_t> stack;
-    for (int z : {0, c->nz - 1})
-      for (int n = c->zstart[z]; n < c->zstart[z + 1]; ++n)
-        if (state[n] == 1) { state[n] = 2; stack.push_back(n); }
-    const int nx = c->nx, ny = c->ny, nz = c->nz;
-    const int d6[6][3] = {{1, 0, 0}, {-1, 0, 0}, {0, 1, 0}, {0, -1, 0}, {0, 0, 1}, {0, 0, -1}};
-    while (!stack.empty()) {
-      const int n = stack.back();
-      stack.pop_back();
-      const long long v = c->node_vox[n];
-      const int x = (int)(v % nx), y = (int)((v / nx) % ny), z = (int)(v / c->np);
-      for (int k = 0; k < 6; ++k) {
-        const int zn = z + d6[k][2];
-        if (zn < 0 || zn >= nz) continue;
-        const int xn = (x + d6[k][0] + nx) % nx, yn = (y + d6[k][1] + ny) % ny;
-        const int32_t m = c->vox2id[(long long)xn + (long long)nx * (yn + (long long)ny * zn)];
-        if (m >= 0 && m < nf && state[m] == 1) { state[m] = 2; stack.push_back(m); }
-      }
-    }
-  } catch (const std::bad_alloc&) {
-    return fail(LBM_ENOMEM, "host allocation failed");
+  const int nf = c->nf, nz = c->nz;
+  const int n0 = c->zstart[z0], n1 = c->zstart[z1];
+  // scratch: parent[nf], flag[nf] (int32), per-block partials and the two results (double)
+  const int chunk = std::max(kCclBlock, (int)(((long long)(n1 - n0) + 1183) / 1184));
+  const int nb = n1 > n0 ? blocks(n1 - n0, chunk) : 0;
+  const size_t ints = ((size_t)2 * nf + 1) & ~(size_t)1;
+  DevBuf tmp(ints * sizeof(int) + ((size_t)2 * nb + 2) * sizeof(double));
+  if (!tmp.p) return fail(LBM_ENOMEM, "device allocation failed");
+  int* parent = (int*)tmp.p;
+  int* flag = parent + nf;
+  double* partial = (double*)(parent + ints);
+  double* out = partial + (size_t)2 * nb;
+  const int g = blocks(nf, 256);
+  if (c->bits == 64)
+    k_ccl_init<double><<<g, 256, 0, st>>>((const Vec2<double>*)c->psi, nf, comp, parent, flag);
+  else
+    k_ccl_init<float><<<g, 256, 0, st>>>((const Vec2<float>*)c->psi, nf, comp, parent, flag);
+  k_ccl_unite<<<g, 256, 0, st>>>(c->nbr, nf, c->npad, parent);
+  k_ccl_flatten<<<g, 256, 0, st>>>(nf, parent);
+  const int a0 = c->zstart[0], a1 = c->zstart[1], b0 = c->zstart[nz - 1], b1 = c->zstart[nz];
+  if ((a1 - a0) + (b1 - b0) > 0)
+    k_ccl_mark<<<blocks((a1 - a0) + (b1 - b0), 256), 256, 0, st>>>(parent, a0, a1, b0, b1, flag);
+  if (nb > 0) {
+    if (c->bits == 64)
+      k_ccl_count<double><<<nb, kCclBlock, 0, st>>>((const Vec2<double>*)c->psi, parent, flag, n0,
+                                                    n1, comp, chunk, partial);
+    else
+      k_ccl_count<float><<<nb, kCclBlock, 0, st>>>((const Vec2<float>*)c->psi, parent, flag, n0, n1,
+                                                   comp, chunk, partial);
   }
-  long long cnt = 0;
-  double msum = 0.0;
-  for (int n = c->zstart[z0]; n < c->zstart[z1]; ++n)
-    if (state[n] == 1) { ++cnt; msum += rho[n]; }
-  *nodes = cnt;
-  *mass = msum;
+  k_ccl_final<<<1, 32, 0, st>>>(partial, nb, out);
+  CU(cudaPeekAtLastError());
+  double h[2] = {0.0, 0.0};
+  CU(cudaMemcpyAsync(h, out, sizeof h, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  *mass = h[0];
+  *nodes = (long long)h[1];
   return LBM_OK;
 }
 
