@@ -107,6 +107,12 @@ int lbm_saturation(lbm_ctx* c, int comp, int z0, int z1, double* S);
  * lbm_saturation.  Runs on the GPU (lock-free union-find over the compact ids, 8 B per fluid
  * node of temporary device memory); an empty z-range gives 0.  Synchronises. */
 int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, double* mass);
+/* Mean over the fluid nodes with z in [z0,z1) of the pressure of Eq. (12) (reading R13):
+ * P = (rho_A+rho_B)/3 + (G/3) rho_A rho_B.  The capillary pressure of the drainage protocol
+ * is P_c = mean over the inlet layer - mean over the outlet layer.  Computed on
+ * the GPU in the storage precision per node, accumulated in fp64 in a fixed order.
+ * LBM_ENOFLUID if the range holds no fluid node.  Synchronises. */
+int lbm_mean_pressure(lbm_ctx* c, int z0, int z1, double* P);
 
 long long lbm_num_fluid(lbm_ctx* c);       /* N_f, or -1 */
 long long lbm_num_wall_solid(lbm_ctx* c);  /* N_w: solid voxels with >= 1 fluid D3Q19 neighbour */

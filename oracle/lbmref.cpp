@@ -235,6 +235,13 @@ void lbmref_destroy(lbmref_ctx* c) { delete c; }
 
 long long lbmref_num_fluid(lbmref_ctx* c) { return c ? c->nfluid : -1; }
 
+int lbmref_set_boundary(lbmref_ctx* c, double inlet_value, double outlet_rho) {
+  if (!c || !c->p.z_open || !std::isfinite(inlet_value) || !std::isfinite(outlet_rho)) return -1;
+  if (c->p.inlet_kind == 1) c->p.inlet_rho = inlet_value; else c->p.inlet_uz = inlet_value;
+  c->p.outlet_rho = outlet_rho;
+  return 0;
+}
+
 int lbmref_set_density(lbmref_ctx* c, const double* rhoA, const double* rhoB) {
   if (!c || !rhoA || !rhoB) return -1;
   const double* r[2] = {rhoA, rhoB};

@@ -57,6 +57,10 @@ int lbmref_saturation(lbmref_ctx* c, int comp, int z0, int z1, double* S);
 int lbmref_trapped_volume(lbmref_ctx* c, int comp, int z0, int z1, long long* nodes,
                           double* mass);
 long long lbmref_num_fluid(lbmref_ctx* c);
+/* Change the imposed inlet value (rho for inlet_kind 1, u_z for inlet_kind 2) and the outlet
+ * density between steps: the pressure ramp of the drainage protocol, PAPER.md L223 ("the inlet
+ * density was gradually increased while the outlet density was kept constant").  A setter only. */
+int lbmref_set_boundary(lbmref_ctx* c, double inlet_value, double outlet_rho);
 /* the oracle's own lattice: w[19], e[19*3] (x,y,z), opp[19] */
 void lbmref_lattice(double* w, int* e, int* opp);
 int lbmref_threads(void);

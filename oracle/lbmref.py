@@ -38,6 +38,7 @@ def _load():
         lib.lbmref_saturation.argtypes = [P, I, I, I, D]
         lib.lbmref_trapped_volume.argtypes = [P, I, I, I, C.POINTER(C.c_longlong), D]
         lib.lbmref_num_fluid.argtypes = [P]
+        lib.lbmref_set_boundary.argtypes = [P, C.c_double, C.c_double]
         lib.lbmref_num_fluid.restype = C.c_longlong
         lib.lbmref_lattice.argtypes = [D, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         lib.lbmref_lattice.restype = None
@@ -115,6 +116,10 @@ class LbmRef:
 
     def step(self, n=1):
         _chk(_load().lbmref_step(self._h, int(n)), "step")
+
+    def set_boundary(self, inlet_value, outlet_rho):
+        _chk(_load().lbmref_set_boundary(self._h, float(inlet_value), float(outlet_rho)),
+             "set_boundary")
 
     def get_macroscopic(self):
         out = [np.empty(self.shape, np.float64) for _ in range(6)]

@@ -1147,7 +1147,7 @@ __global__ void __launch_bounds__(256) k_ccl_mark(const int* __restrict__ parent
 }
 
 // nodes and mass of the unmarked clusters in the id range [n0,n1); block b takes one contiguous
-// chunk and k_ccl_final adds the per-block results in block order (deterministic)
+// chunk and k_sum_pairs adds the per-block results in block order (deterministic)
 constexpr int kCclBlock = 256;
 template <typename T>
 __global__ void __launch_bounds__(kCclBlock) k_ccl_count(const Vec2<T>* __restrict__ psi,
@@ -1183,7 +1183,7 @@ __global__ void __launch_bounds__(kCclBlock) k_ccl_count(const Vec2<T>* __restri
   }
 }
 
-__global__ void k_ccl_final(const double* __restrict__ partial, int nblocks, double* __restrict__ out) {
+__global__ void k_sum_pairs(const double* __restrict__ partial, int nblocks, double* __restrict__ out) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   double mass = 0.0, cnt = 0.0;
   for (int b = 0; b < nblocks; ++b) { mass += partial[2 * b]; cnt += partial[2 * b + 1]; }
@@ -1191,5 +1191,32 @@ __global__ void k_ccl_final(const double* __restrict__ partial, int nblocks, dou
   out[1] = cnt;
 }
 
+
+// Mean pressure over an id range (capillary pressure P_c = P_in - P_out of PAPER.md L223 is the
+// difference of two such plane means): per-block sums of P = (rho_A+rho_B)/3 + (G/3) rho_A rho_B
+// (Eq. 12, reading R13), evaluated in T exactly as k_macroscopic does, accumulated in fp64;
+// k_sum_pairs adds the blocks in order.
+template <typename T>
+__global__ void __launch_bounds__(kCclBlock) k_pressure_sum(const Vec2<T>* __restrict__ psi, int n0,
+                                                            int n1, T G, int chunk,
+                                                            double* __restrict__ partial) {
+  __shared__ double ssum[kCclBlock / 32];
+  const int lo = n0 + blockIdx.x * chunk;
+  const int hi = min(n1, lo + chunk);
+  double sum = 0.0;
+  for (int n = lo + threadIdx.x; n < hi; n += kCclBlock) {
+    const Vec2<T> p = psi[n];
+    sum += (double)((p.a + p.b) / T(3) + (G / T(3)) * p.a * p.b);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+  if ((threadIdx.x & 31) == 0) ssum[threadIdx.x >> 5] = sum;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < kCclBlock / 32; ++w) sum += ssum[w];
+    partial[2 * blockIdx.x] = sum;
+    partial[2 * blockIdx.x + 1] = (double)(hi - lo);
+  }
+}
 
 }  // namespace lbmk

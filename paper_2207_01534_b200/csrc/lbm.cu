@@ -70,7 +70,7 @@ struct lbm_ctx {
   long long nvox = 0;
   int nf = 0, nw = 0;
   size_t npad = 0, nwpad = 0, esz = 4;
-  std::vector<int32_t> vox2id, node_vox, zstart;  // host copies used by queries
+  std::vector<int32_t> zstart;  // [nz+1] first fluid id of every z-plane (host copy, used by queries)
   void* f[2] = {nullptr, nullptr};                // two buffers of [19][npad][2 comps] T
   void* psi = nullptr;                            // [nf+nw] Vec2<T>
   int* nbr = nullptr;                             // [18][npad]
@@ -537,8 +537,6 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
     delete c;
     return fail(LBM_ECUDA, "upload failed: %s", cudaGetErrorString(e));
   }
-  c->vox2id.swap(g.vox2id);
-  c->node_vox.swap(g.node_vox);
   *out = c;
   return LBM_OK;
 }
@@ -812,13 +810,45 @@ int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, d
       k_ccl_count<float><<<nb, kCclBlock, 0, st>>>((const Vec2<float>*)c->psi, parent, flag, n0, n1,
                                                    comp, chunk, partial);
   }
-  k_ccl_final<<<1, 32, 0, st>>>(partial, nb, out);
+  k_sum_pairs<<<1, 32, 0, st>>>(partial, nb, out);
   CU(cudaPeekAtLastError());
   double h[2] = {0.0, 0.0};
   CU(cudaMemcpyAsync(h, out, sizeof h, cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));
   *mass = h[0];
   *nodes = (long long)h[1];
+  return LBM_OK;
+}
+
+int lbm_mean_pressure(lbm_ctx* c, int z0, int z1, double* P) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!P || z0 < 0 || z1 > c->nz || z0 >= z1) return fail(LBM_EINVAL, "bad argument");
+  const int n0 = c->zstart[z0], n1 = c->zstart[z1];
+  if (n1 <= n0) return fail(LBM_ENOFLUID, "no fluid node in the z-range");
+  cudaStream_t st = cur_stream();
+  const bool was = c->prof;
+  c->prof = false;
+  if (c->bits == 64) launch_psi<double>(c, st); else launch_psi<float>(c, st);
+  c->prof = was;
+  CU(cudaPeekAtLastError());
+  const int chunk = std::max(kCclBlock, (int)(((long long)(n1 - n0) + 1183) / 1184));
+  const int nb = blocks(n1 - n0, chunk);
+  DevBuf tmp(((size_t)2 * nb + 2) * sizeof(double));
+  if (!tmp.p) return fail(LBM_ENOMEM, "device allocation failed");
+  double* partial = (double*)tmp.p;
+  double* out = partial + (size_t)2 * nb;
+  if (c->bits == 64)
+    k_pressure_sum<double><<<nb, kCclBlock, 0, st>>>((const Vec2<double>*)c->psi, n0, n1, c->p.G,
+                                                     chunk, partial);
+  else
+    k_pressure_sum<float><<<nb, kCclBlock, 0, st>>>((const Vec2<float>*)c->psi, n0, n1,
+                                                    (float)c->p.G, chunk, partial);
+  k_sum_pairs<<<1, 32, 0, st>>>(partial, nb, out);
+  CU(cudaPeekAtLastError());
+  double h[2] = {0.0, 0.0};
+  CU(cudaMemcpyAsync(h, out, sizeof h, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  *P = h[0] / h[1];
   return LBM_OK;
 }
 

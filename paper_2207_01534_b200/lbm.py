@@ -20,7 +20,7 @@ LBM_OK, LBM_EINVAL, LBM_ENOFLUID, LBM_ESOLIDOPEN, LBM_ENOMEM, LBM_ECUDA, LBM_ENO
 SYMBOLS = [
     "lbm_create", "lbm_destroy", "lbm_set_density", "lbm_set_populations", "lbm_get_populations",
     "lbm_set_boundary", "lbm_step", "lbm_sync", "lbm_get_macroscopic", "lbm_diagnostics",
-    "lbm_saturation", "lbm_trapped_volume", "lbm_num_fluid", "lbm_num_wall_solid",
+    "lbm_saturation", "lbm_trapped_volume", "lbm_mean_pressure", "lbm_num_fluid", "lbm_num_wall_solid",
     "lbm_memory_bytes", "lbm_set_profiling", "lbm_last_step_profile", "lbm_last_error",
     "lbm_build_index", "lbm_build_schedule",
 ]
@@ -72,6 +72,7 @@ def load():
     lib.lbm_diagnostics.argtypes = [P, D, D]
     lib.lbm_saturation.argtypes = [P, I, I, I, D]
     lib.lbm_trapped_volume.argtypes = [P, I, I, I, C.POINTER(LL), D]
+    lib.lbm_mean_pressure.argtypes = [P, I, I, D]
     lib.lbm_num_fluid.argtypes = [P]
     lib.lbm_num_fluid.restype = LL
     lib.lbm_num_wall_solid.argtypes = [P]
@@ -85,7 +86,8 @@ def load():
     lib.lbm_build_schedule.argtypes = [V, I, I, I, I, I, I, V, LL, C.POINTER(LL)]
     for fn in ("lbm_create", "lbm_set_density", "lbm_set_populations", "lbm_get_populations",
                "lbm_set_boundary", "lbm_step", "lbm_sync", "lbm_get_macroscopic",
-               "lbm_diagnostics", "lbm_saturation", "lbm_trapped_volume", "lbm_memory_bytes",
+               "lbm_diagnostics", "lbm_saturation", "lbm_trapped_volume", "lbm_mean_pressure",
+               "lbm_memory_bytes",
                "lbm_set_profiling", "lbm_last_step_profile", "lbm_build_index",
                "lbm_build_schedule"):
         getattr(lib, fn).restype = I
@@ -241,6 +243,12 @@ class Lbm:
         _chk(load().lbm_trapped_volume(self._h, int(comp), int(z0), int(z1), C.byref(n),
                                        C.byref(m)), "lbm_trapped_volume")
         return n.value, m.value
+
+    def mean_pressure(self, z0=0, z1=None):
+        z1 = self.shape[0] if z1 is None else z1
+        v = C.c_double()
+        _chk(load().lbm_mean_pressure(self._h, int(z0), int(z1), C.byref(v)), "lbm_mean_pressure")
+        return v.value
 
     def memory_bytes(self):
         b = (C.c_longlong * 4)()
