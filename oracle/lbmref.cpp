@@ -8,6 +8,8 @@
  *   5. collision                        Eq. (1),(2),(9) PAPER.md L57-63, L94
  *   6. streaming + halfway bounce-back  Eq. (1) LHS; PAPER.md L191, L215 (R10)
  *   7. open planes                      PAPER.md L147-157, L107-113 (R12)  -- parity unpinned
+ *      (the NEEM variant, kinds 1-2; the Zou-He variant, kinds 3-4, reading R31, is pinned by its
+ *      defining properties and an exact fixed point, tests/test_oracle_zouhe.py)
  * No blocking, fusion or reordering: five plain loop nests over the dense box.
  */
 #include "lbmref.h"
@@ -183,8 +185,8 @@ int lbmref_create(lbmref_ctx** out, const uint8_t* solid, int nx, int ny, int nz
   if (!(p->tau[0] > 0.5) || !(p->tau[1] > 0.5)) return -1;
   if (p->z_open) {
     if (nz < 4) return -1;
-    if (p->inlet_kind != 1 && p->inlet_kind != 2) return -1;
-    if (p->outlet_kind != 1) return -1;
+    if (p->inlet_kind < 1 || p->inlet_kind > 4) return -1;
+    if (p->outlet_kind != 1 && p->outlet_kind != 3) return -1;
     if (p->inlet_comp < 0 || p->inlet_comp > 1 || p->outlet_comp < 0 || p->outlet_comp > 1)
       return -1;
   }
@@ -237,7 +239,8 @@ long long lbmref_num_fluid(lbmref_ctx* c) { return c ? c->nfluid : -1; }
 
 int lbmref_set_boundary(lbmref_ctx* c, double inlet_value, double outlet_rho) {
   if (!c || !c->p.z_open || !std::isfinite(inlet_value) || !std::isfinite(outlet_rho)) return -1;
-  if (c->p.inlet_kind == 1) c->p.inlet_rho = inlet_value; else c->p.inlet_uz = inlet_value;
+  if (c->p.inlet_kind == 1 || c->p.inlet_kind == 3) c->p.inlet_rho = inlet_value;
+  else c->p.inlet_uz = inlet_value;
   c->p.outlet_rho = outlet_rho;
   return 0;
 }
@@ -268,6 +271,46 @@ int lbmref_get_populations(lbmref_ctx* c, int comp, double* f) {
   if (!c || !f || comp < 0 || comp > 1) return -1;
   std::memcpy(f, c->f[comp].data(), sizeof(double) * 19 * c->nvox);
   return 0;
+}
+
+/* Zou-He condition ("Apply Zou-He (ZH) method [34] or ... NEEM"; ref. [34] is the
+ * D3Q19 form of Hecht & Harting) on the Dirichlet component's own populations at one node of an
+ * open plane, after streaming (reading R31).  sgn = +1 at the inlet (the 5 unknowns have
+ * e_z = +1), -1 at the outlet.  With K0 = sum of the populations with e_z = 0 and Km = sum of
+ * the known ones leaving the domain (e_z = -sgn), mass and z-momentum give
+ *     rho (1 - sgn u_z) = K0 + 2 Km ,
+ * which fixes u_z from the imposed rho (kind 3) or rho from the imposed u_z (kind 4); u_x = u_y
+ * = 0 are imposed.  The unknowns are the bounce-back of the non-equilibrium part,
+ *     f_i = f_opp(i) + 6 w_i rho (e_i . u)  -/+  the transverse corrections N_x, N_y
+ * chosen so that the x- and y-momentum of the node vanish:
+ *     N_a = 1/2 * sum over the in-plane populations of e_ia f_i      (a = x, y). */
+static void zou_he_plane_node(lbmref_ctx* c, int s, long v, int plane, int kind, double rho_given) {
+  const long nv = c->nvox;
+  const int sgn = plane == 0 ? 1 : -1;
+  double K0 = 0.0, Km = 0.0, Nx = 0.0, Ny = 0.0;
+  for (int i = 0; i < 19; ++i) {
+    const double fi = c->g[s][i * nv + v];
+    if (E[i][2] == 0) {
+      K0 += fi;
+      Nx += 0.5 * E[i][0] * fi;
+      Ny += 0.5 * E[i][1] * fi;
+    } else if (E[i][2] == -sgn) {
+      Km += fi;
+    }
+  }
+  double rho, uz;
+  if (kind == 3) {
+    rho = rho_given;
+    uz = sgn * (1.0 - (K0 + 2.0 * Km) / rho);
+  } else {
+    uz = c->p.inlet_uz;
+    rho = (K0 + 2.0 * Km) / (1.0 - sgn * uz);
+  }
+  for (int i = 0; i < 19; ++i) {
+    if (E[i][2] != sgn) continue;
+    c->g[s][i * nv + v] = c->g[s][OPP[i] * nv + v] + 6.0 * W[i] * rho * (E[i][2] * uz) -
+                          E[i][0] * Nx - E[i][1] * Ny;
+  }
 }
 
 int lbmref_step(lbmref_ctx* c, int nsteps) {
@@ -346,8 +389,13 @@ int lbmref_step(lbmref_ctx* c, int nsteps) {
             rho_b = rf[dc];
             ub[0] = 0.0; ub[1] = 0.0; ub[2] = c->p.inlet_uz;
           }
-          for (int i = 0; i < 19; ++i) /* NEEM */
-            c->g[dc][i * nv + vb] = feq(i, rho_b, ub) + (c->g[dc][i * nv + vf] - feq(i, rf[dc], uf));
+          if (kind <= 2) {
+            for (int i = 0; i < 19; ++i) /* NEEM */
+              c->g[dc][i * nv + vb] =
+                  feq(i, rho_b, ub) + (c->g[dc][i * nv + vf] - feq(i, rf[dc], uf));
+          } else {
+            zou_he_plane_node(c, dc, vb, plane, kind, rho_given);
+          }
           const int oc = 1 - dc; /* inward populations keep their initial values */
           for (int k = 0; k < 5; ++k)
             c->g[oc][INWARD[plane][k] * nv + vb] = c->frozen[plane][oc][k * np + q];

@@ -31,11 +31,12 @@ typedef struct {
   double xi;         /* chi1 = 1+xi, chi2 = 1-xi                       */
   double accel[3];   /* g; F^b_sigma = rho_sigma g (reading R8)            */
   int z_open;        /* 0 periodic in z; 1 inlet plane z=0, outlet plane z=nz-1           */
-  int inlet_kind;    /* 1 density (NEEM), 2 velocity (NEEM)          */
+  int inlet_kind;    /* 1 density (NEEM), 2 velocity (NEEM), 3 density (Zou-He), 4 velocity
+                        (Zou-He)                                     */
   int inlet_comp;    /* component (0/1) that gets the Dirichlet condition at the inlet    */
   double inlet_rho;
   double inlet_uz;
-  int outlet_kind;   /* 1 density (NEEM)                                                  */
+  int outlet_kind;   /* 1 density (NEEM), 3 density (Zou-He)                              */
   int outlet_comp;
   double outlet_rho;
   int storage_bits;  /* ignored by the oracle (always fp64)                               */
