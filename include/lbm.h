@@ -52,12 +52,13 @@ typedef struct {
   double xi;         /* wettability: chi_1 = 1+xi, chi_2 = 1-xi               */
   double accel[3];   /* g; body force F^b_sigma = rho_sigma g (reading R8)        */
   int z_open;        /* 0: periodic in z.  1: inlet plane z=0, outlet plane z=nz-1               */
-  int inlet_kind;    /* 1: density Dirichlet (NEEM), 2: velocity Dirichlet (NEEM); L149, L223    */
+  int inlet_kind;    /* 1: density (NEEM), 2: velocity (NEEM), 3: density (Zou-He), 4: velocity
+                        (Zou-He); PAPER.md L149 ("Zou-He (ZH) method [34] or ... NEEM"), L223   */
   int inlet_comp;    /* component (0 or 1) that receives the Dirichlet condition at the inlet;
                         the other keeps its inward populations frozen        */
-  double inlet_rho;  /* density imposed when inlet_kind == 1                                     */
-  double inlet_uz;   /* velocity imposed when inlet_kind == 2                                    */
-  int outlet_kind;   /* 1: density Dirichlet (NEEM)                                              */
+  double inlet_rho;  /* density imposed when inlet_kind is 1 or 3                                */
+  double inlet_uz;   /* velocity imposed when inlet_kind is 2 or 4                               */
+  int outlet_kind;   /* 1: density (NEEM), 3: density (Zou-He)                                   */
   int outlet_comp;
   double outlet_rho;
   int storage_bits;  /* 64: fp64 storage and arithmetic (validation build);

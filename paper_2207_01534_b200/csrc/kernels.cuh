@@ -795,13 +795,14 @@ __global__ void __launch_bounds__(TN, MINB)
 // a0  open-plane fix on the new buffer (reading R12 of PAPER.md L147-157, L223): planes z=0 and
 // z=nz-1 are all fluid, so their ids are q, nf-np+q and their interior neighbours np+q,
 // nf-2np+q.  Dirichlet component: all 19 populations <- feq(rho_b,u_b) + [f(x_f) - feq(rho(x_f),
-// u_f)] (non-equilibrium extrapolation); other component: its 5 inward populations <- frozen.
+// u_f)] (non-equilibrium extrapolation), or only its 5 inward populations by the Zou-He rule
+// (kinds 3, 4); other component: its 5 inward populations <- frozen.
 template <typename T>
 struct OpenPlane {
   int dc[2];       // Dirichlet component at inlet / outlet
-  int kind[2];     // 1 density, 2 velocity
-  T rho[2];        // imposed density (kind 1)
-  T uz[2];         // imposed velocity (kind 2)
+  int kind[2];     // 1 density (NEEM), 2 velocity (NEEM), 3 density (Zou-He), 4 velocity (Zou-He)
+  T rho[2];        // imposed density (kinds 1, 3)
+  T uz[2];         // imposed velocity (kinds 2, 4)
 };
 
 template <typename T>
@@ -822,38 +823,84 @@ __device__ __forceinline__ Vec2<T> open_plane_node(T* __restrict__ f, const T* _
                                                    const OpenPlane<T>& op, int plane, int q) {
   const int vb = plane == 0 ? q : nf - np + q;
   const int vf = plane == 0 ? np + q : nf - 2 * np + q;
-  T ff[2][Q];
-  T rf[2] = {T(0), T(0)}, j[3] = {T(0), T(0), T(0)};
+  const int dc = op.dc[plane];
+  T rd = T(0);  // new density of the Dirichlet component
+  if (op.kind[plane] <= 2) {
+    T ff[2][Q];
+    T rf[2] = {T(0), T(0)}, j[3] = {T(0), T(0), T(0)};
 #pragma unroll
-  for (int s = 0; s < 2; ++s)
+    for (int s = 0; s < 2; ++s)
+#pragma unroll
+      for (int i = 0; i < Q; ++i) {
+        const T v = f[pidx(s, i, vf, npad)];
+        ff[s][i] = v;
+        rf[s] += v;
+        if (ex(i)) j[0] += T(ex(i)) * v;
+        if (ey(i)) j[1] += T(ey(i)) * v;
+        if (ez(i)) j[2] += T(ez(i)) * v;
+      }
+    const T inv = T(1) / (rf[0] + rf[1]);
+    const T uf[3] = {j[0] * inv, j[1] * inv, j[2] * inv};  // R12 iii: bare mixture velocity
+    const T rfd = dc == 0 ? rf[0] : rf[1];
+    T rho_b, ub[3];
+    if (op.kind[plane] == 1) {
+      rho_b = op.rho[plane];
+      ub[0] = uf[0]; ub[1] = uf[1]; ub[2] = uf[2];
+    } else {
+      rho_b = rfd;
+      ub[0] = T(0); ub[1] = T(0); ub[2] = op.uz[plane];
+    }
 #pragma unroll
     for (int i = 0; i < Q; ++i) {
-      const T v = f[pidx(s, i, vf, npad)];
-      ff[s][i] = v;
-      rf[s] += v;
-      if (ex(i)) j[0] += T(ex(i)) * v;
-      if (ey(i)) j[1] += T(ey(i)) * v;
-      if (ez(i)) j[2] += T(ez(i)) * v;
+      const T fi = dc == 0 ? ff[0][i] : ff[1][i];
+      const T v = feq_of<T>(i, rho_b, ub) + (fi - feq_of<T>(i, rfd, uf));
+      f[pidx(dc, i, vb, npad)] = v;
+      rd = i == 0 ? v : rd + v;
     }
-  const T inv = T(1) / (rf[0] + rf[1]);
-  const T uf[3] = {j[0] * inv, j[1] * inv, j[2] * inv};  // R12 iii: bare mixture velocity
-  const int dc = op.dc[plane];
-  const T rfd = dc == 0 ? rf[0] : rf[1];
-  T rho_b, ub[3];
-  if (op.kind[plane] == 1) {
-    rho_b = op.rho[plane];
-    ub[0] = uf[0]; ub[1] = uf[1]; ub[2] = uf[2];
   } else {
-    rho_b = rfd;
-    ub[0] = T(0); ub[1] = T(0); ub[2] = op.uz[plane];
-  }
-  T rd = T(0);  // new density of the Dirichlet component
+    // Zou-He variant (ref. [34]; reading R31), kinds 3 (density) and 4 (velocity):
+    // purely local.  The 14 populations streaming delivered stay; the 5 that would come from
+    // beyond the plane are the bounce-back of the non-equilibrium part, with the transverse
+    // corrections N_x, N_y that make the node's x- and y-momentum vanish.  From mass and
+    // z-momentum, rho (1 - sgn u_z) = K0 + 2 Km (K0: in-plane sum, Km: outgoing sum).
+    const int sgn = plane == 0 ? 1 : -1;
+    T fb[Q];
+    T K0 = T(0), Km = T(0), Nx = T(0), Ny = T(0);
 #pragma unroll
-  for (int i = 0; i < Q; ++i) {
-    const T fi = dc == 0 ? ff[0][i] : ff[1][i];
-    const T v = feq_of<T>(i, rho_b, ub) + (fi - feq_of<T>(i, rfd, uf));
-    f[pidx(dc, i, vb, npad)] = v;
-    rd = i == 0 ? v : rd + v;
+    for (int i = 0; i < Q; ++i) {
+      if (ez(i) == 0) {
+        const T v = f[pidx(dc, i, vb, npad)];
+        fb[i] = v;
+        K0 += v;
+        if (ex(i)) Nx += T(0.5) * T(ex(i)) * v;
+        if (ey(i)) Ny += T(0.5) * T(ey(i)) * v;
+      } else if (ez(i) == -sgn) {
+        const T v = f[pidx(dc, i, vb, npad)];
+        fb[i] = v;
+        Km += v;
+      } else {
+        fb[i] = T(0);  // unknown: whatever the slot holds is stale
+      }
+    }
+    T rho, uz;
+    if (op.kind[plane] == 3) {
+      rho = op.rho[plane];
+      uz = T(sgn) * (T(1) - (K0 + T(2) * Km) / rho);
+    } else {
+      uz = op.uz[plane];
+      rho = (K0 + T(2) * Km) / (T(1) - T(sgn) * uz);
+    }
+#pragma unroll
+    for (int i = 1; i < Q; ++i) {
+      if (ez(i) == 0 || ez(i) != sgn) continue;
+      T v = fb[opp(i)] + T(6) * wgt<T>(i) * rho * (T(ez(i)) * uz);
+      if (ex(i)) v -= T(ex(i)) * Nx;
+      if (ey(i)) v -= T(ey(i)) * Ny;
+      fb[i] = v;
+      f[pidx(dc, i, vb, npad)] = v;
+    }
+#pragma unroll
+    for (int i = 0; i < Q; ++i) rd = i == 0 ? fb[i] : rd + fb[i];
   }
   const int oc = 1 - dc;
   T ro = T(0);  // new density of the other component: 14 streamed + 5 frozen populations

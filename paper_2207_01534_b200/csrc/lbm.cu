@@ -346,9 +346,10 @@ int validate_params(const lbm_params* p, int nz) {
     return fail(LBM_EINVAL, "storage_bits must be 32 or 64");
   if (p->z_open) {
     if (nz < 4) return fail(LBM_EINVAL, "z_open needs nz >= 4");
-    if (p->inlet_kind != 1 && p->inlet_kind != 2)
-      return fail(LBM_EINVAL, "inlet_kind must be 1 (density) or 2 (velocity)");
-    if (p->outlet_kind != 1) return fail(LBM_EINVAL, "outlet_kind must be 1 (density)");
+    if (p->inlet_kind < 1 || p->inlet_kind > 4)
+      return fail(LBM_EINVAL, "inlet_kind must be 1, 2 (NEEM density, velocity) or 3, 4 (Zou-He)");
+    if (p->outlet_kind != 1 && p->outlet_kind != 3)
+      return fail(LBM_EINVAL, "outlet_kind must be 1 (NEEM density) or 3 (Zou-He density)");
     if (p->inlet_comp < 0 || p->inlet_comp > 1 || p->outlet_comp < 0 || p->outlet_comp > 1)
       return fail(LBM_EINVAL, "inlet_comp / outlet_comp must be 0 or 1");
   }
@@ -564,7 +565,8 @@ int lbm_set_boundary(lbm_ctx* c, double inlet_value, double outlet_rho) {
     return fail(LBM_EINVAL, "boundary values must be finite");
   if (int rc = check_ctx(c)) return rc;
   apply_pending(c, cur_stream());  // the last step's fix uses the values it was run with
-  if (c->p.inlet_kind == 1) c->p.inlet_rho = inlet_value; else c->p.inlet_uz = inlet_value;
+  if (c->p.inlet_kind == 1 || c->p.inlet_kind == 3) c->p.inlet_rho = inlet_value;
+  else c->p.inlet_uz = inlet_value;
   c->p.outlet_rho = outlet_rho;
   return LBM_OK;
 }
