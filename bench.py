@@ -80,7 +80,7 @@ def cpu_sample(cfg, edge=128):
     return mask, rA, rB, f"leading {e}^3 corner of the {m.shape[0]}^3 mask"
 
 
-def time_oracle(cfg, steps, warmup, budget_s=25.0):
+def time_oracle(cfg, steps, warmup, budget_s=15.0):
     from oracle import LbmRef, threads
     mask, rA, rB, what = cpu_sample(cfg)
     p = dict(cfg["params"])
@@ -89,7 +89,7 @@ def time_oracle(cfg, steps, warmup, budget_s=25.0):
     t0 = time.perf_counter()
     o.step(max(1, warmup))
     per = (time.perf_counter() - t0) / max(1, warmup)
-    n = steps if steps is not None else max(1, min(20, int(budget_s / max(per, 1e-3))))
+    n = steps if steps is not None else max(1, min(200, int(budget_s / max(per, 1e-3))))
     t0 = time.perf_counter()
     o.step(n)
     dt = time.perf_counter() - t0
