@@ -131,6 +131,7 @@ int lbm_memory_bytes(lbm_ctx* c, long long bytes[4]);
  *   LBM_B200_COLLIDE=bulk|simple   bulk-async staged fused pass (default) | register kernel
  *   LBM_B200_IDX=16|32             16-bit tile-relative neighbour index (default) | int32 rows
  *   LBM_B200_REVERSE=1|0           fused pass walks tiles backwards (default) | forwards
+ *   LBM_B200_PDL=1|0               programmatic dependent launch of the three passes (default) | off
  *   LBM_B200_TILE, LBM_B200_LEAD   CTA shape of the fused pass; producer lead of the fused step */
 int lbm_set_profiling(lbm_ctx* c, int on);
 int lbm_last_step_profile(lbm_ctx* c, double ms[4], long long* launches);

@@ -11,6 +11,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "geometry.hpp"
@@ -101,6 +102,7 @@ struct lbm_ctx {
   int* fused_flags = nullptr;        // [ntf+32 | ntw+32] per-rank completion epochs
   int fused_epoch = 0;
   int fused_parity = 0;
+  int pdl = 1;              // programmatic dependent launch of the three passes; env LBM_B200_PDL=0
   int tile = 1286;          // fp32 bulk kernel variant: tile nodes * 10 + min CTAs/SM; env LBM_B200_TILE
   long long bytes[4] = {0, 0, 0, 0};
   bool prof = false;
@@ -160,28 +162,47 @@ struct Timed {  // brackets one launch with events when profiling is on
   }
 };
 
+// Launch with the programmatic-stream-serialization attribute: the kernel's blocks may become
+// resident while the previous kernel of the stream drains, and run up to their pdl_wait().
+template <typename... KArgs, typename... Args>
+void launch_k(bool pdl, void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem,
+              cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(block);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
+
 // a1 + a2 on the current buffer
 template <typename T>
 void launch_psi(lbm_ctx* c, cudaStream_t st) {
   T* fin = (T*)c->f[c->cur];
+  const bool pdl = c->pdl && !c->prof;  // events between the launches would serialise them anyway
   {
     Timed t(c, st, 0);
     if (c->open_pending) {  // a0 of the previous step rides along (k_density_open)
       const unsigned nbp = blocks(2LL * c->np, 256);
-      k_density_open<T><<<nbp + blocks(c->nf, 256), 256, 0, st>>>(
-          fin, (Vec2<T>*)c->psi, (const T*)c->frozen, c->nf, c->np, c->npad, (int)nbp,
-          make_open<T>(c->p));
+      launch_k(pdl, k_density_open<T>, nbp + blocks(c->nf, 256), 256, 0, st, fin,
+               (Vec2<T>*)c->psi, (const T*)c->frozen, c->nf, c->np, c->npad, (int)nbp,
+               make_open<T>(c->p));
       c->open_pending = false;
     } else {
-      k_density<T><<<blocks(c->nf, 256), 256, 0, st>>>(fin, (Vec2<T>*)c->psi, c->nf, c->npad);
+      launch_k(pdl, k_density<T>, blocks(c->nf, 256), 256, 0, st, (const T*)fin,
+               (Vec2<T>*)c->psi, c->nf, c->npad);
     }
   }
   if (c->nw > 0) {
     Timed t(c, st, 1);
-    k_wallpsi<T><<<blocks(c->nw, 256), 256, 0, st>>>((Vec2<T>*)c->psi, c->wall_nbr,
-                                                     (const T*)c->wall_inv_den, c->npad, c->nw,
-                                                     c->nwpad, (T)(1.0 + c->p.xi),
-                                                     (T)(1.0 - c->p.xi));
+    launch_k(pdl, k_wallpsi<T>, blocks(c->nw, 256), 256, 0, st, (Vec2<T>*)c->psi,
+             (const int*)c->wall_nbr, (const T*)c->wall_inv_den, c->npad, c->nw, c->nwpad,
+             (T)(1.0 + c->p.xi), (T)(1.0 - c->p.xi));
   }
 }
 
@@ -216,8 +237,11 @@ void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
   ix.meta = c->nbr16_meta;
   ix.np = c->p.z_open ? c->np : 0;
   ix.reverse = c->reverse;
-  k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX16><<<blocks(c->nf, TN), TN, smem, st>>>(
-      fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->npad, k, ix);
+  // Overlap only behind the wall pass: its blocks trigger after their own wait, i.e. once the
+  // density pass (which may have rewritten the open planes of fin) is complete and visible.
+  launch_k(c->pdl && !c->prof && c->nw > 0, k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX16>,
+           blocks(c->nf, TN), TN, smem, st, fin, fout, (const Vec2<T>*)c->psi,
+           (const int*)c->nbr, c->nf, c->npad, k, ix);
 }
 
 template <typename T>
@@ -423,6 +447,7 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   if (const char* e = std::getenv("LBM_B200_COLLIDE")) c->collide_variant = !std::strcmp(e, "simple") ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_TILE")) c->tile = std::atoi(e);
   if (const char* e = std::getenv("LBM_B200_REVERSE")) c->reverse = std::atoi(e) != 0;
+  if (const char* e = std::getenv("LBM_B200_PDL")) c->pdl = std::atoi(e) != 0;
   if (const char* e = std::getenv("LBM_B200_IDX")) c->idx16 = std::atoi(e) == 32 ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_STEP")) c->step_variant = !std::strcmp(e, "split") ? 0 : 1;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
