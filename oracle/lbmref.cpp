@@ -7,9 +7,13 @@
  *   4. rho, tau_s, u_eq                 Eq. (5)-(8) PAPER.md L73-87 (R2, R3, R4)
  *   5. collision                        Eq. (1),(2),(9) PAPER.md L57-63, L94
  *   6. streaming + halfway bounce-back  Eq. (1) LHS; PAPER.md L191, L215 (R10)
- *   7. open planes                      PAPER.md L147-157, L107-113 (R12)  -- parity unpinned
- *      (the NEEM variant, kinds 1-2; the Zou-He variant, kinds 3-4, reading R31, is pinned by its
- *      defining properties and an exact fixed point, tests/test_oracle_zouhe.py)
+ *   7. open planes                      PAPER.md L147-157, L107-113 (R12)
+ *      NEEM variant (kinds 1-2): pinned to the textbook identity of ref. [6], its exact
+ *      consequences, the frozen rule and a moving fixed point (tests/test_oracle_neem.py);
+ *      Zou-He variant (kinds 3-4, R31): pinned by its defining properties and a fixed point
+ *      (tests/test_oracle_zouhe.py).  What stays a READING of a garbled passage -- parity
+ *      unpinned -- is R12 iii/iv: which velocity NEEM extrapolates (the bare mixture velocity)
+ *      and the mirrored psi neighbours beyond a plane; the paper prints no number for either.
  * No blocking, fusion or reordering: five plain loop nests over the dense box.
  */
 #include "lbmref.h"
