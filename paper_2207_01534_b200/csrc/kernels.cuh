@@ -57,9 +57,33 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 // Lets the next kernel's blocks become resident (and run up to their pdl_wait) already now.
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
 
+// L2 eviction priority of a store: lines written with evict_last outlive the streaming traffic
+// around them.  psi (8 B per node, written by the density and wall passes, gathered 19 times by
+// the fused pass, rewritten every step) then never leaves L2 when it fits; `frac` is the share of
+// the lines that gets the priority (chosen by address, the same lines every step), 0 = plain store.
+__device__ __forceinline__ uint64_t l2_keep_policy(float frac) {
+  uint64_t pol = 0;
+  if (frac > 0.f)
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, %1;" : "=l"(pol) : "f"(frac));
+  return pol;
+}
+
 template <typename T> struct Vec2;
 template <> struct __align__(8) Vec2<float> { float a, b; };
 template <> struct __align__(16) Vec2<double> { double a, b; };
+// pol == 0: plain store
+__device__ __forceinline__ void store_vec2(Vec2<float>* p, Vec2<float> v, uint64_t pol) {
+  if (pol == 0) { *p = v; return; }
+  asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(v.a), "f"(v.b),
+               "l"(pol)
+               : "memory");
+}
+__device__ __forceinline__ void store_vec2(Vec2<double>* p, Vec2<double> v, uint64_t pol) {
+  if (pol == 0) { *p = v; return; }
+  asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.a), "d"(v.b),
+               "l"(pol)
+               : "memory");
+}
 
 template <typename T>
 struct Consts {
@@ -75,7 +99,7 @@ struct Consts {
 // One thread per fluid node; every load is a fully coalesced row read.
 template <typename T>
 __global__ void __launch_bounds__(256) k_density(const T* __restrict__ f, Vec2<T>* __restrict__ psi,
-                                                 int nf, size_t npad) {
+                                                 int nf, size_t npad, float keep_psi) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
   pdl_wait();  // f was written by the previous step's fused pass
   if (n >= nf) return;
@@ -87,7 +111,7 @@ __global__ void __launch_bounds__(256) k_density(const T* __restrict__ f, Vec2<T
 #pragma unroll
   for (int i = 1; i < Q; ++i) { ra += v[i].a; rb += v[i].b; }
   Vec2<T> o; o.a = ra; o.b = rb;
-  psi[n] = o;
+  store_vec2(psi + n, o, l2_keep_policy(keep_psi));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -99,7 +123,7 @@ __global__ void __launch_bounds__(256) k_wallpsi(Vec2<T>* __restrict__ psi,
                                                  const int* __restrict__ wall_nbr,
                                                  const T* __restrict__ inv_den,
                                                  size_t wall_base, int nw, size_t nwpad, T chiA,
-                                                 T chiB) {
+                                                 T chiB, float keep_psi) {
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
   const bool live = w < nw;
   int id[Q];
@@ -123,7 +147,8 @@ __global__ void __launch_bounds__(256) k_wallpsi(Vec2<T>* __restrict__ psi,
     }
   }
   Vec2<T> o; o.a = chiA * na * s; o.b = chiB * nb * s;
-  psi[wall_base + w] = o;  // wall ids are stored at wall_base = npad (tile-aligned)
+  // wall ids are stored at wall_base = npad (tile-aligned)
+  store_vec2(psi + wall_base + w, o, l2_keep_policy(keep_psi));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -965,8 +990,9 @@ __global__ void __launch_bounds__(128) k_open_planes(T* __restrict__ f,
 template <typename T>
 __global__ void __launch_bounds__(256, 4)
     k_density_open(T* __restrict__ f, Vec2<T>* __restrict__ psi, const T* __restrict__ frozen,
-                   int nf, int np, size_t npad, int nb_planes, OpenPlane<T> op) {
+                   int nf, int np, size_t npad, int nb_planes, OpenPlane<T> op, float keep_psi) {
   pdl_wait();  // f was written by the previous step's fused pass
+  const uint64_t pol = l2_keep_policy(keep_psi);
   if ((int)blockIdx.x >= nb_planes) {
     const int n = ((int)blockIdx.x - nb_planes) * blockDim.x + threadIdx.x;
     if (n >= nf || n < np || n >= nf - np) return;
@@ -978,12 +1004,13 @@ __global__ void __launch_bounds__(256, 4)
 #pragma unroll
     for (int i = 1; i < Q; ++i) { ra += v[i].a; rb += v[i].b; }
     Vec2<T> o; o.a = ra; o.b = rb;
-    psi[n] = o;
+    store_vec2(psi + n, o, pol);
   } else {  // the plane blocks come first so that their dependent chain overlaps the streaming
     const int t = (int)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= 2 * np) return;
     const int plane = t / np, q = t - plane * np;
-    psi[plane == 0 ? q : nf - np + q] = open_plane_node<T>(f, frozen, nf, np, npad, op, plane, q);
+    store_vec2(psi + (plane == 0 ? q : nf - np + q),
+               open_plane_node<T>(f, frozen, nf, np, npad, op, plane, q), pol);
   }
 }
 

@@ -4,6 +4,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -102,6 +103,8 @@ struct lbm_ctx {
   int* fused_flags = nullptr;        // [ntf+32 | ntw+32] per-rank completion epochs
   int fused_epoch = 0;
   int fused_parity = 0;
+  float keep_psi = 0.f;     // share of the psi lines stored with L2 evict_last priority, from
+  int keep_psi_mb = 48;     // this budget: min(1, MB / psi bytes); env LBM_B200_KEEP_PSI_MB (0: off)
   int pdl = 1;              // programmatic dependent launch of the three passes; env LBM_B200_PDL=0
   int tile = 1286;          // fp32 bulk kernel variant: tile nodes * 10 + min CTAs/SM; env LBM_B200_TILE
   long long bytes[4] = {0, 0, 0, 0};
@@ -191,18 +194,18 @@ void launch_psi(lbm_ctx* c, cudaStream_t st) {
       const unsigned nbp = blocks(2LL * c->np, 256);
       launch_k(pdl, k_density_open<T>, nbp + blocks(c->nf, 256), 256, 0, st, fin,
                (Vec2<T>*)c->psi, (const T*)c->frozen, c->nf, c->np, c->npad, (int)nbp,
-               make_open<T>(c->p));
+               make_open<T>(c->p), c->keep_psi);
       c->open_pending = false;
     } else {
       launch_k(pdl, k_density<T>, blocks(c->nf, 256), 256, 0, st, (const T*)fin,
-               (Vec2<T>*)c->psi, c->nf, c->npad);
+               (Vec2<T>*)c->psi, c->nf, c->npad, c->keep_psi);
     }
   }
   if (c->nw > 0) {
     Timed t(c, st, 1);
     launch_k(pdl, k_wallpsi<T>, blocks(c->nw, 256), 256, 0, st, (Vec2<T>*)c->psi,
              (const int*)c->wall_nbr, (const T*)c->wall_inv_den, c->npad, c->nw, c->nwpad,
-             (T)(1.0 + c->p.xi), (T)(1.0 - c->p.xi));
+             (T)(1.0 + c->p.xi), (T)(1.0 - c->p.xi), c->keep_psi);
   }
 }
 
@@ -448,6 +451,7 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   if (const char* e = std::getenv("LBM_B200_TILE")) c->tile = std::atoi(e);
   if (const char* e = std::getenv("LBM_B200_REVERSE")) c->reverse = std::atoi(e) != 0;
   if (const char* e = std::getenv("LBM_B200_PDL")) c->pdl = std::atoi(e) != 0;
+  if (const char* e = std::getenv("LBM_B200_KEEP_PSI_MB")) c->keep_psi_mb = std::atoi(e);
   if (const char* e = std::getenv("LBM_B200_IDX")) c->idx16 = std::atoi(e) == 32 ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_STEP")) c->step_variant = !std::strcmp(e, "split") ? 0 : 1;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
@@ -484,6 +488,9 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   }
   c->bytes[0] = 2 * (long long)fbytes;
   c->bytes[1] = (long long)psibytes;
+  c->keep_psi = c->keep_psi_mb > 0
+                    ? (float)std::min(1.0, (double)c->keep_psi_mb * 1048576.0 / (double)psibytes)
+                    : 0.f;
   c->bytes[2] = (long long)(nbrbytes + wnbrbytes + g.nw * c->esz + g.nf * sizeof(int));
   c->bytes[3] = (long long)(frozenbytes + c->diag_blocks * kDiagVals * 8 + 64);
   cudaError_t e = cudaSuccess;

@@ -350,8 +350,9 @@ def test_register_kernel_and_int32_index_paths_agree_with_production(monkeypatch
     sims = {}
     for name, env in (("prod", {}), ("simple", {"LBM_B200_COLLIDE": "simple"}),
                       ("idx32", {"LBM_B200_IDX": "32"}), ("fwd", {"LBM_B200_REVERSE": "0"}),
-                      ("nopdl", {"LBM_B200_PDL": "0"})):
-        for k in ("LBM_B200_COLLIDE", "LBM_B200_IDX", "LBM_B200_REVERSE", "LBM_B200_PDL"):
+                      ("nopdl", {"LBM_B200_PDL": "0"}), ("nokeep", {"LBM_B200_KEEP_PSI_MB": "0"})):
+        for k in ("LBM_B200_COLLIDE", "LBM_B200_IDX", "LBM_B200_REVERSE", "LBM_B200_PDL",
+                  "LBM_B200_KEEP_PSI_MB"):
             monkeypatch.delenv(k, raising=False)
         for k, v in env.items():
             monkeypatch.setenv(k, v)
@@ -365,6 +366,7 @@ def test_register_kernel_and_int32_index_paths_agree_with_production(monkeypatch
         assert np.array_equal(sims["prod"][s], sims["idx32"][s])      # same arithmetic, other index
         assert np.array_equal(sims["prod"][s], sims["fwd"][s])        # tile order is irrelevant
         assert np.array_equal(sims["prod"][s], sims["nopdl"][s])      # launch overlap is irrelevant
+        assert np.array_equal(sims["prod"][s], sims["nokeep"][s])     # so is the L2 priority of psi
         a, b = sims["simple"][s][:, fl], sims["prod"][s][:, fl]
         assert (np.abs(a - b) / np.abs(b)).max() < 1e-11              # different operation order
     o = LbmRef(c["mask"], c["params"])
