@@ -156,6 +156,54 @@ int lbm_build_index(const uint8_t* solid, int nx, int ny, int nz, int z_open, in
 int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open, int tile,
                        int lead, int32_t* records, long long cap_items, long long* n_items);
 
+/* ---- z-slab sharding across GPUs --------
+ * The step has two grid-wide dependencies (Eq. 11/13: every node's force needs its
+ * neighbours' rho(t); Eq. 15: every wall solid's rho~(t) needs its fluid neighbours' rho(t)) and
+ * one transport across a cut (Eq. 1 LHS: 5 populations per component cross a z-plane).  A box that
+ * is periodic in z is cut into contiguous z-slabs, one lbm_ctx per slab (one per GPU).  The slab's
+ * mask is the owned planes plus LBM_SLAB_GHOST = 2 halo planes at each z end (copies of the
+ * neighbour slabs' planes; periodic wrap of the global box): nz_local = owned + 4, owned >= 2.
+ * One time step of a slab is
+ *     lbm_slab_density                          a1 on the owned nodes
+ *     psi exchange (caller)                     buffers 0,1 (send) -> the neighbours' 2,3 (receive)
+ *     lbm_slab_collide                          a2 (all wall solids of the local box), a3-a6 on the
+ *                                               owned nodes, pack of the populations that crossed a cut
+ *     population exchange (caller)              buffers 4,5 (send) -> the neighbours' 6,7 (receive)
+ *     lbm_slab_unpack                           received populations -> rows of the owned boundary planes
+ * and the result on the owned nodes is bit-identical to the unsharded lbm_step (same kernels, same
+ * summation order).  The exchanges move DEVICE buffers and are the caller's (NCCL send/recv
+ * through torch.distributed in paper_2207_01534_b200/slab.py; device copies when several slabs
+ * live on one GPU).  All calls are asynchronous on torch's current stream.
+ * lbm_set_density / lbm_set_populations / lbm_get_* take dense arrays of the LOCAL box
+ * (nx*ny*nz_local); halo voxels are ignored on input and written as 0 by lbm_get_macroscopic,
+ * which in slab mode requires lbm_slab_density + the psi exchange to have been done on the current
+ * state.  lbm_diagnostics sums over the owned nodes.  lbm_step, lbm_saturation,
+ * lbm_trapped_volume and lbm_mean_pressure return LBM_EINVAL on a slab context; z_open must be 0. */
+#define LBM_SLAB_GHOST 2
+int lbm_create_slab(lbm_ctx** out, const uint8_t* solid_local, int nx, int ny, int nz_local,
+                    const lbm_params* p);
+int lbm_slab_density(lbm_ctx* c);
+int lbm_slab_collide(lbm_ctx* c);   /* LBM_EINVAL unless it follows lbm_slab_density */
+int lbm_slab_unpack(lbm_ctx* c);    /* LBM_EINVAL unless it follows lbm_slab_collide */
+/* Exchange buffers (DEVICE pointers into the context's memory, valid until lbm_destroy; psi
+ * buffers are (rho_A, rho_B) pairs of the storage type, population buffers (f_A, f_B) pairs).
+ * which = 2*kind + face, face 0 = low z, 1 = high z:
+ *   kind 0: psi of my two owned planes at that face (send)   kind 1: psi of my two halo planes (receive)
+ *   kind 2: packed populations that left through that face   kind 3: populations arriving through it
+ * A slab's send buffer of face 1 has the byte count of its upper neighbour's receive buffer of
+ * face 0, and vice versa (both are derived from the same mask planes). */
+int lbm_slab_buffer(lbm_ctx* c, int which, void** dev, long long* bytes);
+long long lbm_num_owned(lbm_ctx* c);   /* fluid nodes of the owned planes, or -1 */
+/* Host-only helper (no GPU needed): the halo lists lbm_create_slab builds, decoded for inspection.
+ * pack_dir_vox / unpack_dir_vox: caller-allocated, 2*cap int32 each; entry k is (direction i,
+ * local voxel index of the node whose row slot is read / written), low face first then high face;
+ * n_pack / n_unpack: entries per face; psi_send / psi_recv: fluid nodes per face of the psi
+ * exchange; *n_owned: fluid nodes of the owned planes. */
+int lbm_build_slab_halo(const uint8_t* solid_local, int nx, int ny, int nz_local,
+                        int32_t* pack_dir_vox, int32_t* unpack_dir_vox, long long cap,
+                        long long n_pack[2], long long n_unpack[2], long long psi_send[2],
+                        long long psi_recv[2], long long* n_owned);
+
 #ifdef __cplusplus
 }
 #endif

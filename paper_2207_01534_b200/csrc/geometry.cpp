@@ -35,8 +35,9 @@ struct Box {
 }  // namespace
 
 int build(Geometry& g, const uint8_t* solid, int nx, int ny, int nz, int z_open,
-          bool with_tables) {
+          bool with_tables, int ghost) {
   if (!solid || nx < 1 || ny < 1 || nz < 1) return -1;
+  if (ghost < 0 || (ghost > 0 && (z_open || nz < 2 * ghost + 2))) return -1;
   const long long nvox = (long long)nx * ny * nz;
   if (nvox >= (1LL << 31)) return -1;
   if (z_open && nz < 4) return -1;
@@ -48,13 +49,21 @@ int build(Geometry& g, const uint8_t* solid, int nx, int ny, int nz, int z_open,
         if (solid[(long long)zs[k] * np + q]) return -3;
   }
   g.nx = nx; g.ny = ny; g.nz = nz; g.z_open = z_open ? 1 : 0; g.nvox = nvox;
+  g.ghost = ghost;
   const Box box{nx, ny, nz, g.z_open};
   try {
     g.vox2id.assign(nvox, -1);
     long long nf = 0;
-    for (long long v = 0; v < nvox; ++v)
+    // owned planes first, then the low halo planes, then the high ones (ghost = 0: plain raster)
+    const long long v_lo = (long long)ghost * np, v_hi = nvox - (long long)ghost * np;
+    for (long long v = v_lo; v < v_hi; ++v)
       if (!solid[v]) g.vox2id[v] = (int32_t)nf++;
+    g.nact = nf;
     if (nf == 0) return -2;
+    for (long long v = 0; v < v_lo; ++v)
+      if (!solid[v]) g.vox2id[v] = (int32_t)nf++;
+    for (long long v = v_hi; v < nvox; ++v)
+      if (!solid[v]) g.vox2id[v] = (int32_t)nf++;
     g.nf = nf;
     g.node_vox.resize(nf);
     for (long long v = 0; v < nvox; ++v)
@@ -296,6 +305,62 @@ int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Ind
       wide += is_wide ? 1 : 0;
     }
     out.wide_tiles = wide;
+  } catch (const std::bad_alloc&) {
+    return -4;
+  }
+  return 0;
+}
+
+int build_halo(const Geometry& g, const uint8_t* solid, size_t npad, Halo& h) {
+  if (g.ghost != kSlabGhost || !solid) return -1;
+  const int nx = g.nx, ny = g.ny, nz = g.nz, G = g.ghost;
+  const long long np = (long long)nx * ny;
+  // directions that cross the low cut (e_z = -1) and the high cut (e_z = +1)
+  static const int kCross[2][5] = {{6, 13, 14, 17, 18}, {5, 11, 12, 15, 16}};
+  try {
+    for (int face = 0; face < 2; ++face) {
+      h.pack[face].clear();
+      h.unpack[face].clear();
+      // pack: what my owned boundary plane pushed into the inner halo plane of this face
+      const int z_halo = face == 0 ? G - 1 : nz - G;       // inner halo plane
+      const int z_own = face == 0 ? G : nz - G - 1;        // owned boundary plane
+      for (int k = 0; k < 5; ++k) {
+        const int i = kCross[face][k];       // travels from z_own to z_halo
+        const int j = kCross[1 - face][k];   // arrives at z_own from z_halo (neighbour's push)
+        for (int y = 0; y < ny; ++y)
+          for (int x = 0; x < nx; ++x) {
+            {  // destination x in the halo plane, source x - e_i in my owned plane
+              const long long vd = x + nx * (y + (long long)ny * z_halo);
+              const int xs = (x - kE[i][0] + nx) % nx, ys = (y - kE[i][1] + ny) % ny;
+              const long long vs = xs + nx * (ys + (long long)ny * z_own);
+              if (!solid[vd] && !solid[vs])
+                h.pack[face].push_back((int32_t)((size_t)i * npad + (size_t)g.vox2id[vd]));
+            }
+            {  // destination x in my owned plane, source x - e_j in the halo plane
+              const long long vd = x + nx * (y + (long long)ny * z_own);
+              const int xs = (x - kE[j][0] + nx) % nx, ys = (y - kE[j][1] + ny) % ny;
+              const long long vs = xs + nx * (ys + (long long)ny * z_halo);
+              if (!solid[vd] && !solid[vs])
+                h.unpack[face].push_back((int32_t)((size_t)j * npad + (size_t)g.vox2id[vd]));
+            }
+          }
+      }
+    }
+    // psi: fluid ids of whole planes are contiguous (raster order inside each id block)
+    auto count = [&](int z0, int z1) {
+      long long c = 0;
+      for (long long v = z0 * np; v < z1 * np; ++v) c += solid[v] ? 0 : 1;
+      return c;
+    };
+    const long long n_lo = count(0, G), n_hi = count(nz - G, nz);
+    h.psi_send[0][0] = 0;
+    h.psi_send[0][1] = count(G, 2 * G);
+    h.psi_send[1][1] = count(nz - 2 * G, nz - G);
+    h.psi_send[1][0] = g.nact - h.psi_send[1][1];
+    h.psi_recv[0][0] = g.nact;
+    h.psi_recv[0][1] = n_lo;
+    h.psi_recv[1][0] = g.nact + n_lo;
+    h.psi_recv[1][1] = n_hi;
   } catch (const std::bad_alloc&) {
     return -4;
   }

@@ -18,6 +18,12 @@ extern const int kOpp[kQ];
 struct Geometry {
   int nx = 0, ny = 0, nz = 0, z_open = 0;
   long long nvox = 0, nf = 0, nw = 0;
+  // Slab mode (multi-GPU z-slabs): the box carries `ghost` halo planes
+  // at each z end.  Fluid nodes of the owned planes get ids [0, nact) in raster order, the halo
+  // nodes ids [nact, nf): low halo planes first, then the high ones, each in raster order.
+  // ghost = 0: nact = nf and the ids are plain raster order.
+  int ghost = 0;
+  long long nact = 0;
   std::vector<int32_t> vox2id;    // [nvox]  fluid id | nf + wall id | -1
   std::vector<int32_t> node_vox;  // [nf]    voxel index of fluid node n
   std::vector<int32_t> wall_vox;  // [nw]    voxel index of wall solid w
@@ -69,6 +75,24 @@ int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Ind
 // Returns 0, or -1 bad arguments, -2 no fluid voxel, -3 solid on an open plane or its interior
 // neighbour plane (z in {0,1,nz-2,nz-1}), -4 out of memory.  `with_tables` = also fill nbr,
 // wall_nbr, wall_inv_den.
-int build(Geometry& g, const uint8_t* solid, int nx, int ny, int nz, int z_open, bool with_tables);
+int build(Geometry& g, const uint8_t* solid, int nx, int ny, int nz, int z_open, bool with_tables,
+          int ghost = 0);
+
+// Halo lists of a slab (ghost = kSlabGhost planes per side; z local: [0,ghost) low halo,
+// [ghost, nz-ghost) owned, [nz-ghost, nz) high halo).  After the fused pass the populations an
+// owned boundary-plane node pushed across the cut sit in the rows of the inner halo plane's
+// nodes; they are packed into one message per face and, on the neighbour slab, unpacked into the
+// same rows of its owned boundary plane.  An entry exists for (direction i crossing the cut,
+// node x of the destination plane) iff x - e_i is fluid (else halfway bounce-back filled the slot
+// locally).  Order: direction-major in the order of kCross, raster order of x within; both slabs
+// derive the same list from the same two mask planes.  Entries are pair-slot indices i*npad + id.
+constexpr int kSlabGhost = 2;
+struct Halo {
+  std::vector<int32_t> pack[2];    // [face 0 = low, 1 = high]: source slots (inner halo plane rows)
+  std::vector<int32_t> unpack[2];  // [face]: destination slots (owned boundary plane rows)
+  long long psi_send[2][2];        // [face]{first id, count}: owned nodes of the 2 planes at that face
+  long long psi_recv[2][2];        // [face]{first id, count}: halo nodes at that face
+};
+int build_halo(const Geometry& g, const uint8_t* solid, size_t npad, Halo& h);
 
 }  // namespace lbmgeo

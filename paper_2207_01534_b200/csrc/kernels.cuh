@@ -274,9 +274,9 @@ __global__ void __launch_bounds__(256) k_collide_stream(const T* __restrict__ fi
                                                         T* __restrict__ fout,
                                                         const Vec2<T>* __restrict__ psi,
                                                         const int* __restrict__ nbr, int nf,
-                                                        size_t npad, Consts<T> c) {
+                                                        int nact, size_t npad, Consts<T> c) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
-  if (n >= nf) return;
+  if (n >= nact) return;  // nact < nf in slab mode: halo nodes only receive pushes
   int id[Q];
   id[0] = n;
 #pragma unroll
@@ -585,6 +585,8 @@ struct Idx16 {
   const int* meta;        // [tiles][kIdxMeta]
   int np;                 // nodes per open plane (nx*ny) when z is open, else 0
   int reverse;            // 1: CTA b takes tile gridDim-1-b
+  int nact;               // nodes this pass updates: ids [0,nact).  = nf, except in slab mode, where
+                          // the halo nodes [nact,nf) only receive pushes
 };
 
 template <typename T, int TN>
@@ -667,7 +669,7 @@ __global__ void __launch_bounds__(TN, MINB)
       }
     }
   }
-  collide_tile_thread<T, TN, REMAINDER>(sf, sid, tid, n, n < nf, fout, psi, nf, npad, c);
+  collide_tile_thread<T, TN, REMAINDER>(sf, sid, tid, n, n < ix.nact, fout, psi, nf, npad, c);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1012,6 +1014,29 @@ __global__ void __launch_bounds__(256, 4)
     store_vec2(psi + (plane == 0 ? q : nf - np + q),
                open_plane_node<T>(f, frozen, nf, np, npad, op, plane, q), pol);
   }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Slab halo (multi-GPU z-slabs): the 5 populations per component that crossed a
+// cut sit, after the fused pass, in the rows of the inner halo plane's nodes.  k_halo_pack gathers
+// them (both faces in one launch) into the send buffer through a precomputed slot list;
+// k_halo_unpack scatters what the neighbour slabs sent into the rows of the owned boundary
+// planes.  One (A, B) pair per entry; geometry.hpp Halo.
+template <typename T>
+__global__ void __launch_bounds__(256) k_halo_pack(const T* __restrict__ f,
+                                                   const int* __restrict__ slots,
+                                                   T* __restrict__ buf, int n) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  reinterpret_cast<Vec2<T>*>(buf)[k] = reinterpret_cast<const Vec2<T>*>(f)[slots[k]];
+}
+template <typename T>
+__global__ void __launch_bounds__(256) k_halo_unpack(T* __restrict__ f,
+                                                     const int* __restrict__ slots,
+                                                     const T* __restrict__ buf, int n) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  reinterpret_cast<Vec2<T>*>(f)[slots[k]] = reinterpret_cast<const Vec2<T>*>(buf)[k];
 }
 
 // frozen[plane][comp][k][q] <- f[comp][inward(plane,k)][plane node q]   (reading R27)

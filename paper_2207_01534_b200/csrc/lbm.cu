@@ -71,6 +71,14 @@ struct lbm_ctx {
   int nx = 0, ny = 0, nz = 0, np = 0, bits = 32, device = 0;
   long long nvox = 0;
   int nf = 0, nw = 0;
+  int nact = 0;             // ids [0,nact) are updated by this context; = nf unless slab mode
+  int slab = 0;             // 1: z-slab of a larger box with kSlabGhost halo planes per side
+  int* halo_slots = nullptr;         // [pack low | pack high | unpack low | unpack high] pair slots
+  void* halo_send = nullptr;         // [pack low | pack high] (A,B) pairs
+  void* halo_recv = nullptr;         // [unpack low | unpack high] (A,B) pairs
+  int n_pack[2] = {0, 0}, n_unpack[2] = {0, 0};
+  long long psi_send[2][2] = {{0, 0}, {0, 0}}, psi_recv[2][2] = {{0, 0}, {0, 0}};
+  int slab_phase = 0;       // 0: expects lbm_slab_density, 1: lbm_slab_collide, 2: lbm_slab_unpack
   size_t npad = 0, nwpad = 0, esz = 4;
   std::vector<int32_t> zstart;  // [nz+1] first fluid id of every z-plane (host copy, used by queries)
   void* f[2] = {nullptr, nullptr};                // two buffers of [19][npad][2 comps] T
@@ -121,6 +129,7 @@ struct lbm_ctx {
     lbm_shim_free(sched_items); lbm_shim_free(fused_ctr); lbm_shim_free(nbr16);
     lbm_shim_free(nbr16_meta);
     lbm_shim_free(fused_flags);
+    lbm_shim_free(halo_slots); lbm_shim_free(halo_send); lbm_shim_free(halo_recv);
   }
 };
 
@@ -183,30 +192,41 @@ void launch_k(bool pdl, void (*kern)(KArgs...), unsigned grid, unsigned block, s
   cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
 }
 
-// a1 + a2 on the current buffer
+// a1 (+ the deferred a0 of the previous step) on the current buffer, ids [0, nact)
 template <typename T>
-void launch_psi(lbm_ctx* c, cudaStream_t st) {
+void launch_density(lbm_ctx* c, cudaStream_t st) {
   T* fin = (T*)c->f[c->cur];
   const bool pdl = c->pdl && !c->prof;  // events between the launches would serialise them anyway
-  {
-    Timed t(c, st, 0);
-    if (c->open_pending) {  // a0 of the previous step rides along (k_density_open)
-      const unsigned nbp = blocks(2LL * c->np, 256);
-      launch_k(pdl, k_density_open<T>, nbp + blocks(c->nf, 256), 256, 0, st, fin,
-               (Vec2<T>*)c->psi, (const T*)c->frozen, c->nf, c->np, c->npad, (int)nbp,
-               make_open<T>(c->p), c->keep_psi);
-      c->open_pending = false;
-    } else {
-      launch_k(pdl, k_density<T>, blocks(c->nf, 256), 256, 0, st, (const T*)fin,
-               (Vec2<T>*)c->psi, c->nf, c->npad, c->keep_psi);
-    }
+  Timed t(c, st, 0);
+  if (c->open_pending) {  // a0 of the previous step rides along (k_density_open)
+    const unsigned nbp = blocks(2LL * c->np, 256);
+    launch_k(pdl, k_density_open<T>, nbp + blocks(c->nf, 256), 256, 0, st, fin,
+             (Vec2<T>*)c->psi, (const T*)c->frozen, c->nf, c->np, c->npad, (int)nbp,
+             make_open<T>(c->p), c->keep_psi);
+    c->open_pending = false;
+  } else {
+    launch_k(pdl, k_density<T>, blocks(c->nact, 256), 256, 0, st, (const T*)fin,
+             (Vec2<T>*)c->psi, c->nact, c->npad, c->keep_psi);
   }
-  if (c->nw > 0) {
-    Timed t(c, st, 1);
-    launch_k(pdl, k_wallpsi<T>, blocks(c->nw, 256), 256, 0, st, (Vec2<T>*)c->psi,
-             (const int*)c->wall_nbr, (const T*)c->wall_inv_den, c->npad, c->nw, c->nwpad,
-             (T)(1.0 + c->p.xi), (T)(1.0 - c->p.xi), c->keep_psi);
-  }
+}
+
+// a2 on every wall solid of the box
+template <typename T>
+void launch_wall(lbm_ctx* c, cudaStream_t st) {
+  if (c->nw <= 0) return;
+  const bool pdl = c->pdl && !c->prof;
+  Timed t(c, st, 1);
+  launch_k(pdl, k_wallpsi<T>, blocks(c->nw, 256), 256, 0, st, (Vec2<T>*)c->psi,
+           (const int*)c->wall_nbr, (const T*)c->wall_inv_den, c->npad, c->nw, c->nwpad,
+           (T)(1.0 + c->p.xi), (T)(1.0 - c->p.xi), c->keep_psi);
+}
+
+// a1 + a2.  Slab mode: the density pass (lbm_slab_density) and the psi halo exchange are the
+// caller's; only the wall pass runs here.
+template <typename T>
+void launch_psi(lbm_ctx* c, cudaStream_t st) {
+  if (!c->slab) launch_density<T>(c, st);
+  launch_wall<T>(c, st);
 }
 
 
@@ -240,10 +260,11 @@ void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
   ix.meta = c->nbr16_meta;
   ix.np = c->p.z_open ? c->np : 0;
   ix.reverse = c->reverse;
+  ix.nact = c->nact;
   // Overlap only behind the wall pass: its blocks trigger after their own wait, i.e. once the
   // density pass (which may have rewritten the open planes of fin) is complete and visible.
   launch_k(c->pdl && !c->prof && c->nw > 0, k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX16>,
-           blocks(c->nf, TN), TN, smem, st, fin, fout, (const Vec2<T>*)c->psi,
+           blocks(c->nact, TN), TN, smem, st, fin, fout, (const Vec2<T>*)c->psi,
            (const int*)c->nbr, c->nf, c->npad, k, ix);
 }
 
@@ -251,8 +272,8 @@ template <typename T>
 void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
   constexpr bool kRemainder = sizeof(T) == 4;
   if (c->collide_variant == 0) {
-    k_collide_stream<T, kRemainder><<<blocks(c->nf, 256), 256, 0, st>>>(
-        fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->npad, k);
+    k_collide_stream<T, kRemainder><<<blocks(c->nact, 256), 256, 0, st>>>(
+        fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->nact, c->npad, k);
     return;
   }
   if constexpr (sizeof(T) == 4) {
@@ -420,13 +441,17 @@ int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open,
   return LBM_OK;
 }
 
-int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, const lbm_params* p) {
+static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz,
+                       const lbm_params* p, int ghost) {
   if (!out || !solid || !p) return fail(LBM_EINVAL, "NULL argument");
   if (nx < 1 || ny < 1 || nz < 1) return fail(LBM_EINVAL, "box dimensions must be positive");
   if (int rc = validate_params(p, nz)) return rc;
+  if (ghost && p->z_open) return fail(LBM_EINVAL, "slab mode needs z_open = 0");
+  if (ghost && nz < 2 * ghost + 2)
+    return fail(LBM_EINVAL, "a slab needs >= 2 owned planes plus %d halo planes per side", ghost);
   lbmgeo::Geometry g;
   {
-    const int rc = lbmgeo::build(g, solid, nx, ny, nz, p->z_open, true);
+    const int rc = lbmgeo::build(g, solid, nx, ny, nz, p->z_open, true, ghost);
     if (rc == -2) return fail(LBM_ENOFLUID, "the mask has no fluid voxel");
     if (rc == -3) return fail(LBM_ESOLIDOPEN, "solid voxel on an open plane or its neighbour plane");
     if (rc == -4) return fail(LBM_ENOMEM, "host allocation failed");
@@ -446,6 +471,7 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   c->p = *p;
   c->nx = nx; c->ny = ny; c->nz = nz; c->np = nx * ny; c->nvox = g.nvox;
   c->nf = (int)g.nf; c->nw = (int)g.nw;
+  c->nact = (int)g.nact; c->slab = ghost > 0 ? 1 : 0;
   c->bits = p->storage_bits; c->esz = p->storage_bits / 8;
   if (const char* e = std::getenv("LBM_B200_COLLIDE")) c->collide_variant = !std::strcmp(e, "simple") ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_TILE")) c->tile = std::atoi(e);
@@ -454,6 +480,7 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
   if (const char* e = std::getenv("LBM_B200_KEEP_PSI_MB")) c->keep_psi_mb = std::atoi(e);
   if (const char* e = std::getenv("LBM_B200_IDX")) c->idx16 = std::atoi(e) == 32 ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_STEP")) c->step_variant = !std::strcmp(e, "split") ? 0 : 1;
+  if (c->slab) c->step_variant = 0;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
   // pair-slot indices i * npad + k and psi indices npad + w are 32-bit
   if ((size_t)19 * c->npad >= ((size_t)1 << 31) || c->npad + c->nwpad >= ((size_t)1 << 31)) {
@@ -461,7 +488,7 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
     return fail(LBM_EINVAL, "too many fluid nodes for 32-bit slot indices");
   }
   c->zstart.assign(nz + 1, 0);
-  for (long long n = 0; n < g.nf; ++n) ++c->zstart[g.node_vox[n] / c->np + 1];
+  for (long long n = 0; n < g.nact; ++n) ++c->zstart[g.node_vox[n] / c->np + 1];
   for (int z = 0; z < nz; ++z) c->zstart[z + 1] += c->zstart[z];
   cudaStream_t st = cur_stream();
   const size_t fbytes = (size_t)2 * 19 * c->npad * c->esz;
@@ -565,12 +592,178 @@ int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, cons
     if (e == cudaSuccess) e = cudaMemsetAsync(c->fused_flags, 0, nflags * sizeof(int), st);
     c->bytes[2] += (long long)(sch.records.size() * 4 + nflags * 4);
   }
+  lbmgeo::Halo halo;  // declared here: its lists are upload sources until the sync below
+  if (c->slab) {
+    if (lbmgeo::build_halo(g, solid, c->npad, halo) != 0) {
+      delete c;
+      return fail(LBM_ENOMEM, "halo list build failed");
+    }
+    size_t nslots = 0;
+    for (int fc = 0; fc < 2; ++fc) {
+      c->n_pack[fc] = (int)halo.pack[fc].size();
+      c->n_unpack[fc] = (int)halo.unpack[fc].size();
+      nslots += halo.pack[fc].size() + halo.unpack[fc].size();
+      for (int k = 0; k < 2; ++k) {
+        c->psi_send[fc][k] = halo.psi_send[fc][k];
+        c->psi_recv[fc][k] = halo.psi_recv[fc][k];
+      }
+    }
+    const size_t sendb = (size_t)(c->n_pack[0] + c->n_pack[1]) * 2 * c->esz;
+    const size_t recvb = (size_t)(c->n_unpack[0] + c->n_unpack[1]) * 2 * c->esz;
+    c->halo_slots = (int*)lbm_shim_alloc(nslots * sizeof(int) + 16);
+    c->halo_send = lbm_shim_alloc(sendb + 16);
+    c->halo_recv = lbm_shim_alloc(recvb + 16);
+    if (!c->halo_slots || !c->halo_send || !c->halo_recv) {
+      delete c;
+      return fail(LBM_ENOMEM, "device allocation failed (halo)");
+    }
+    int* d = c->halo_slots;
+    for (int fc = 0; fc < 2; ++fc) { up(d, halo.pack[fc].data(), halo.pack[fc].size() * 4); d += halo.pack[fc].size(); }
+    for (int fc = 0; fc < 2; ++fc) { up(d, halo.unpack[fc].data(), halo.unpack[fc].size() * 4); d += halo.unpack[fc].size(); }
+    c->bytes[2] += (long long)(nslots * sizeof(int));
+    c->bytes[3] += (long long)(sendb + recvb);
+  }
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);  // host sources die with this scope
   if (e != cudaSuccess) {
     delete c;
     return fail(LBM_ECUDA, "upload failed: %s", cudaGetErrorString(e));
   }
   *out = c;
+  return LBM_OK;
+}
+
+int lbm_build_slab_halo(const uint8_t* solid_local, int nx, int ny, int nz_local,
+                        int32_t* pack_dir_vox, int32_t* unpack_dir_vox, long long cap,
+                        long long n_pack[2], long long n_unpack[2], long long psi_send[2],
+                        long long psi_recv[2], long long* n_owned) {
+  if (!solid_local || !pack_dir_vox || !unpack_dir_vox || !n_pack || !n_unpack || !psi_send ||
+      !psi_recv || !n_owned)
+    return fail(LBM_EINVAL, "NULL argument");
+  lbmgeo::Geometry g;
+  const int rc = lbmgeo::build(g, solid_local, nx, ny, nz_local, 0, false, lbmgeo::kSlabGhost);
+  if (rc) return fail(rc == -2 ? LBM_ENOFLUID : LBM_EINVAL, "geometry build failed (%d)", rc);
+  const size_t npad = pad256(g.nf);
+  lbmgeo::Halo h;
+  if (lbmgeo::build_halo(g, solid_local, npad, h) != 0) return fail(LBM_ENOMEM, "halo build failed");
+  if ((long long)(h.pack[0].size() + h.pack[1].size()) > cap ||
+      (long long)(h.unpack[0].size() + h.unpack[1].size()) > cap)
+    return fail(LBM_EINVAL, "list capacity too small");
+  for (int pass = 0; pass < 2; ++pass) {
+    int32_t* o = pass ? unpack_dir_vox : pack_dir_vox;
+    for (int fc = 0; fc < 2; ++fc) {
+      const std::vector<int32_t>& l = pass ? h.unpack[fc] : h.pack[fc];
+      for (int32_t slot : l) {
+        *o++ = (int32_t)((size_t)slot / npad);
+        *o++ = g.node_vox[(size_t)slot % npad];
+      }
+      (pass ? n_unpack : n_pack)[fc] = (long long)l.size();
+    }
+  }
+  for (int fc = 0; fc < 2; ++fc) { psi_send[fc] = h.psi_send[fc][1]; psi_recv[fc] = h.psi_recv[fc][1]; }
+  *n_owned = g.nact;
+  return LBM_OK;
+}
+
+int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, const lbm_params* p) {
+  return create_impl(out, solid, nx, ny, nz, p, 0);
+}
+
+int lbm_create_slab(lbm_ctx** out, const uint8_t* solid_local, int nx, int ny, int nz_local,
+                    const lbm_params* p) {
+  return create_impl(out, solid_local, nx, ny, nz_local, p, lbmgeo::kSlabGhost);
+}
+
+long long lbm_num_owned(lbm_ctx* c) { return c ? c->nact : -1; }
+
+int lbm_slab_density(lbm_ctx* c) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
+  if (c->slab_phase == 2)
+    return fail(LBM_EINVAL, "lbm_slab_unpack of the previous step is still missing");
+  cudaStream_t st = cur_stream();
+  if (c->bits == 64) launch_density<double>(c, st); else launch_density<float>(c, st);
+  CU(cudaPeekAtLastError());
+  c->slab_phase = 1;
+  return LBM_OK;
+}
+
+int lbm_slab_collide(lbm_ctx* c) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
+  if (c->slab_phase != 1)
+    return fail(LBM_EINVAL, "lbm_slab_collide must follow lbm_slab_density and the psi exchange");
+  cudaStream_t st = cur_stream();
+  const int np = c->n_pack[0] + c->n_pack[1];
+  if (c->bits == 64) {
+    launch_wall<double>(c, st);
+    { Timed t(c, st, 2);
+      launch_collide<double>(c, (const double*)c->f[c->cur], (double*)c->f[c->cur ^ 1],
+                             make_consts<double>(c->p), st); }
+    c->cur ^= 1;
+    if (np) { Timed t(c, st, 3);
+      k_halo_pack<double><<<blocks(np, 256), 256, 0, st>>>((const double*)c->f[c->cur], c->halo_slots,
+                                                           (double*)c->halo_send, np); }
+  } else {
+    launch_wall<float>(c, st);
+    { Timed t(c, st, 2);
+      launch_collide<float>(c, (const float*)c->f[c->cur], (float*)c->f[c->cur ^ 1],
+                            make_consts<float>(c->p), st); }
+    c->cur ^= 1;
+    if (np) { Timed t(c, st, 3);
+      k_halo_pack<float><<<blocks(np, 256), 256, 0, st>>>((const float*)c->f[c->cur], c->halo_slots,
+                                                          (float*)c->halo_send, np); }
+  }
+  CU(cudaPeekAtLastError());
+  c->slab_phase = 2;
+  return LBM_OK;
+}
+
+int lbm_slab_unpack(lbm_ctx* c) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
+  if (c->slab_phase != 2)
+    return fail(LBM_EINVAL, "lbm_slab_unpack must follow lbm_slab_collide and the population exchange");
+  cudaStream_t st = cur_stream();
+  const int nu = c->n_unpack[0] + c->n_unpack[1];
+  const int* slots = c->halo_slots + c->n_pack[0] + c->n_pack[1];
+  if (nu) {
+    Timed t(c, st, 3);
+    if (c->bits == 64)
+      k_halo_unpack<double><<<blocks(nu, 256), 256, 0, st>>>((double*)c->f[c->cur], slots,
+                                                             (const double*)c->halo_recv, nu);
+    else
+      k_halo_unpack<float><<<blocks(nu, 256), 256, 0, st>>>((float*)c->f[c->cur], slots,
+                                                            (const float*)c->halo_recv, nu);
+  }
+  CU(cudaPeekAtLastError());
+  c->slab_phase = 0;
+  return LBM_OK;
+}
+
+int lbm_slab_buffer(lbm_ctx* c, int which, void** dev, long long* bytes) {
+  if (!c || !dev || !bytes) return fail(LBM_EINVAL, "NULL argument");
+  if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
+  if (which < 0 || which > 7) return fail(LBM_EINVAL, "which must be 0..7");
+  const size_t pair = 2 * c->esz;
+  const int face = which & 1;
+  switch (which >> 1) {
+    case 0:  // psi of my two owned planes at that face
+      *dev = (char*)c->psi + (size_t)c->psi_send[face][0] * pair;
+      *bytes = c->psi_send[face][1] * (long long)pair;
+      break;
+    case 1:  // psi of my halo planes at that face
+      *dev = (char*)c->psi + (size_t)c->psi_recv[face][0] * pair;
+      *bytes = c->psi_recv[face][1] * (long long)pair;
+      break;
+    case 2:  // packed populations leaving through that face
+      *dev = (char*)c->halo_send + (face ? (size_t)c->n_pack[0] * pair : 0);
+      *bytes = c->n_pack[face] * (long long)pair;
+      break;
+    default:  // populations arriving through that face
+      *dev = (char*)c->halo_recv + (face ? (size_t)c->n_unpack[0] * pair : 0);
+      *bytes = c->n_unpack[face] * (long long)pair;
+      break;
+  }
   return LBM_OK;
 }
 
@@ -612,6 +805,9 @@ int lbm_sync(lbm_ctx* c) {
 int lbm_step(lbm_ctx* c, int n) {
   if (int rc = check_ctx(c)) return rc;
   if (n < 0) return fail(LBM_EINVAL, "n must be >= 0");
+  if (c->slab)
+    return fail(LBM_EINVAL, "slab context: a step is lbm_slab_density, psi exchange, "
+                            "lbm_slab_collide, population exchange, lbm_slab_unpack");
   cudaStream_t st = cur_stream();
   if (c->prof) {
     for (auto& e : c->prof_events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
@@ -624,6 +820,9 @@ int lbm_step(lbm_ctx* c, int n) {
 int lbm_set_profiling(lbm_ctx* c, int on) {
   if (!c) return fail(LBM_EINVAL, "NULL context");
   c->prof = on != 0;
+  for (auto& e : c->prof_events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  c->prof_events.clear();  // slab phases accumulate from here on; lbm_step restarts per call
+  c->prof_launches = 0;
   return LBM_OK;
 }
 
@@ -721,19 +920,20 @@ int lbm_get_macroscopic(lbm_ctx* c, double* rhoA, double* rhoB, double* ux, doub
   cudaStream_t st = cur_stream();
   const bool was = c->prof;
   c->prof = false;
-  DevBuf m((size_t)6 * c->nf * sizeof(double));
+  const int na = c->nact;  // owned nodes (all fluid nodes unless slab mode)
+  DevBuf m((size_t)6 * na * sizeof(double));
   const size_t bytes = (size_t)c->nvox * sizeof(double);
   DevBuf d(bytes);
   if (!m.p || !d.p) { c->prof = was; return fail(LBM_ENOMEM, "device staging allocation failed"); }
   if (c->bits == 64) {
     launch_psi<double>(c, st);
-    k_macroscopic<double><<<blocks(c->nf, 256), 256, 0, st>>>(
-        (const double*)c->f[c->cur], (const Vec2<double>*)c->psi, c->nbr, (double*)m.p, c->nf,
+    k_macroscopic<double><<<blocks(na, 256), 256, 0, st>>>(
+        (const double*)c->f[c->cur], (const Vec2<double>*)c->psi, c->nbr, (double*)m.p, na,
         c->npad, make_consts<double>(c->p));
   } else {
     launch_psi<float>(c, st);
-    k_macroscopic<float><<<blocks(c->nf, 256), 256, 0, st>>>(
-        (const float*)c->f[c->cur], (const Vec2<float>*)c->psi, c->nbr, (double*)m.p, c->nf,
+    k_macroscopic<float><<<blocks(na, 256), 256, 0, st>>>(
+        (const float*)c->f[c->cur], (const Vec2<float>*)c->psi, c->nbr, (double*)m.p, na,
         c->npad, make_consts<float>(c->p));
   }
   c->prof = was;
@@ -742,8 +942,8 @@ int lbm_get_macroscopic(lbm_ctx* c, double* rhoA, double* rhoB, double* ux, doub
   for (int q = 0; q < 6; ++q) {
     if (!outs[q]) continue;
     CU(cudaMemsetAsync(d.p, 0, bytes, st));
-    k_compact_to_dense<double><<<blocks(c->nf, 256), 256, 0, st>>>(
-        (const double*)m.p + (size_t)q * c->nf, c->node_vox_d, (double*)d.p, c->nf, 1);
+    k_compact_to_dense<double><<<blocks(na, 256), 256, 0, st>>>(
+        (const double*)m.p + (size_t)q * na, c->node_vox_d, (double*)d.p, na, 1);
     CU(cudaMemcpyAsync(outs[q], d.p, bytes, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
   }
@@ -759,9 +959,9 @@ int lbm_diagnostics(lbm_ctx* c, double mass[2], double momentum[3]) {
   const int nb = c->diag_blocks;
   if (c->bits == 64)
     k_diag_partial<double><<<nb, kDiagBlock, 0, st>>>((const double*)c->f[c->cur], c->partial,
-                                                      c->nf, c->npad);
+                                                      c->nact, c->npad);
   else
-    k_diag_partial<float><<<nb, kDiagBlock, 0, st>>>((const float*)c->f[c->cur], c->partial, c->nf,
+    k_diag_partial<float><<<nb, kDiagBlock, 0, st>>>((const float*)c->f[c->cur], c->partial, c->nact,
                                                      c->npad);
   k_diag_final<<<1, 32, 0, st>>>(c->partial, c->diag_out, nb);
   CU(cudaPeekAtLastError());
@@ -777,6 +977,7 @@ int lbm_diagnostics(lbm_ctx* c, double mass[2], double momentum[3]) {
 
 int lbm_saturation(lbm_ctx* c, int comp, int z0, int z1, double* S) {
   if (int rc = check_ctx(c)) return rc;
+  if (c->slab) return fail(LBM_EINVAL, "lbm_saturation is not available on a slab context");
   if (!S || comp < 0 || comp > 1 || z0 < 0 || z1 > c->nz || z0 >= z1)
     return fail(LBM_EINVAL, "bad argument");
   const int n0 = c->zstart[z0], n1 = c->zstart[z1];
@@ -806,6 +1007,7 @@ int lbm_saturation(lbm_ctx* c, int comp, int z0, int z1, double* S) {
 
 int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, double* mass) {
   if (int rc = check_ctx(c)) return rc;
+  if (c->slab) return fail(LBM_EINVAL, "lbm_trapped_volume is not available on a slab context");
   if (!nodes || !mass || comp < 0 || comp > 1 || z0 < 0 || z1 > c->nz || z0 >= z1)
     return fail(LBM_EINVAL, "bad argument");
   cudaStream_t st = cur_stream();
@@ -856,6 +1058,7 @@ int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, d
 
 int lbm_mean_pressure(lbm_ctx* c, int z0, int z1, double* P) {
   if (int rc = check_ctx(c)) return rc;
+  if (c->slab) return fail(LBM_EINVAL, "lbm_mean_pressure is not available on a slab context");
   if (!P || z0 < 0 || z1 > c->nz || z0 >= z1) return fail(LBM_EINVAL, "bad argument");
   const int n0 = c->zstart[z0], n1 = c->zstart[z1];
   if (n1 <= n0) return fail(LBM_ENOFLUID, "no fluid node in the z-range");

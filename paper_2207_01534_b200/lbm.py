@@ -23,6 +23,8 @@ SYMBOLS = [
     "lbm_saturation", "lbm_trapped_volume", "lbm_mean_pressure", "lbm_num_fluid", "lbm_num_wall_solid",
     "lbm_memory_bytes", "lbm_set_profiling", "lbm_last_step_profile", "lbm_last_error",
     "lbm_build_index", "lbm_build_schedule",
+    "lbm_create_slab", "lbm_slab_density", "lbm_slab_collide", "lbm_slab_unpack", "lbm_slab_buffer",
+    "lbm_num_owned", "lbm_build_slab_halo",
 ]
 
 
@@ -84,6 +86,17 @@ def load():
     lib.lbm_last_error.restype = C.c_char_p
     lib.lbm_build_index.argtypes = [V, I, I, I, I, V, V, LL, C.POINTER(LL), C.POINTER(LL)]
     lib.lbm_build_schedule.argtypes = [V, I, I, I, I, I, I, V, LL, C.POINTER(LL)]
+    lib.lbm_create_slab.argtypes = [C.POINTER(P), V, I, I, I, C.POINTER(lbm_params)]
+    lib.lbm_slab_density.argtypes = [P]
+    lib.lbm_slab_collide.argtypes = [P]
+    lib.lbm_slab_unpack.argtypes = [P]
+    lib.lbm_slab_buffer.argtypes = [P, I, C.POINTER(C.c_void_p), C.POINTER(LL)]
+    lib.lbm_num_owned.argtypes = [P]
+    lib.lbm_num_owned.restype = LL
+    lib.lbm_build_slab_halo.argtypes = [V, I, I, I, V, V, LL] + [C.POINTER(LL)] * 5
+    for fn in ("lbm_create_slab", "lbm_slab_density", "lbm_slab_collide", "lbm_slab_unpack",
+               "lbm_slab_buffer", "lbm_build_slab_halo"):
+        getattr(lib, fn).restype = I
     for fn in ("lbm_create", "lbm_set_density", "lbm_set_populations", "lbm_get_populations",
                "lbm_set_boundary", "lbm_step", "lbm_sync", "lbm_get_macroscopic",
                "lbm_diagnostics", "lbm_saturation", "lbm_trapped_volume", "lbm_mean_pressure",
@@ -146,10 +159,33 @@ def lbm_build_schedule(mask, z_open=0, tile=128, lead=256):
     return rec[:n.value]
 
 
-class Lbm:
-    """One simulation on the current CUDA device. Methods mirror the C ABI one to one."""
+def lbm_build_slab_halo(mask_local):
+    """Host-only: the halo lists lbm_create_slab builds for a local mask [owned + 4, y, x].
+    Returns a dict: pack / unpack = per face (low, high) an int32 array [n, 2] of (direction,
+    local voxel index); psi_send / psi_recv = fluid nodes per face; n_owned."""
+    lib = load()
+    mask_local = np.ascontiguousarray(mask_local, np.uint8)
+    nz, ny, nx = mask_local.shape
+    cap = 2 * 5 * nx * ny
+    pk = np.zeros((cap, 2), np.int32)
+    up = np.zeros((cap, 2), np.int32)
+    arr = lambda: (C.c_longlong * 2)()
+    n_pack, n_unpack, ps, pr = arr(), arr(), arr(), arr()
+    n_owned = C.c_longlong()
+    _chk(lib.lbm_build_slab_halo(mask_local.ctypes.data, nx, ny, nz, pk.ctypes.data,
+                                 up.ctypes.data, cap, n_pack, n_unpack, ps, pr,
+                                 C.byref(n_owned)), "lbm_build_slab_halo")
+    return {"pack": (pk[:n_pack[0]].copy(), pk[n_pack[0]:n_pack[0] + n_pack[1]].copy()),
+            "unpack": (up[:n_unpack[0]].copy(), up[n_unpack[0]:n_unpack[0] + n_unpack[1]].copy()),
+            "psi_send": (int(ps[0]), int(ps[1])), "psi_recv": (int(pr[0]), int(pr[1])),
+            "n_owned": int(n_owned.value)}
 
-    def __init__(self, mask, params):
+
+class Lbm:
+    """One simulation on the current CUDA device. Methods mirror the C ABI one to one.
+    slab=True: a z-slab context (lbm_create_slab; mask = owned planes + 2 halo planes per end)."""
+
+    def __init__(self, mask, params, slab=False):
         lib = load()
         import torch
         if torch.cuda.is_available():
@@ -163,8 +199,14 @@ class Lbm:
         self.params = dict(params)
         self._h = C.c_void_p()
         ps = make_params(params)
-        _chk(lib.lbm_create(C.byref(self._h), mask.ctypes.data, nx, ny, nz, C.byref(ps)),
-             "lbm_create")
+        self.slab = bool(slab)
+        if slab:
+            _chk(lib.lbm_create_slab(C.byref(self._h), mask.ctypes.data, nx, ny, nz,
+                                     C.byref(ps)), "lbm_create_slab")
+        else:
+            _chk(lib.lbm_create(C.byref(self._h), mask.ctypes.data, nx, ny, nz, C.byref(ps)),
+                 "lbm_create")
+        self.num_owned = int(lib.lbm_num_owned(self._h))
         self.num_fluid = int(lib.lbm_num_fluid(self._h))
         self.num_wall_solid = int(lib.lbm_num_wall_solid(self._h))
 
@@ -206,6 +248,23 @@ class Lbm:
 
     def step(self, n=1):
         _chk(load().lbm_step(self._h, int(n)), "lbm_step")
+
+    def slab_density(self):
+        _chk(load().lbm_slab_density(self._h), "lbm_slab_density")
+
+    def slab_collide(self):
+        _chk(load().lbm_slab_collide(self._h), "lbm_slab_collide")
+
+    def slab_unpack(self):
+        _chk(load().lbm_slab_unpack(self._h), "lbm_slab_unpack")
+
+    def slab_buffer(self, which):
+        """(device pointer, bytes) of exchange buffer `which` (include/lbm.h lbm_slab_buffer)."""
+        ptr = C.c_void_p()
+        n = C.c_longlong()
+        _chk(load().lbm_slab_buffer(self._h, int(which), C.byref(ptr), C.byref(n)),
+             "lbm_slab_buffer")
+        return int(ptr.value or 0), int(n.value)
 
     def sync(self):
         _chk(load().lbm_sync(self._h), "lbm_sync")

@@ -1,0 +1,215 @@
+"""z-slab sharding of the two-component D3Q19 step across GPUs (C ABI:
+include/lbm.h "z-slab sharding").
+
+The paper is single-GPU; its step has two grid-wide dependencies per time step
+(Eq. 11/13: forces need the neighbours' rho(t); Eq. 15: a wall solid's rho~(t) needs its fluid
+neighbours' rho(t)) and one transport across a cut (Eq. 1 LHS).  A box that is periodic in z is cut
+into contiguous z-slabs balanced by fluid-node count; every slab is one `Lbm(slab=True)` context
+with two halo planes per end, and a step is
+
+    slab_density -> psi exchange -> slab_collide -> population exchange -> slab_unpack
+
+All arithmetic runs in the library's kernels; this module only partitions the mask, slices the
+initial state and moves the DEVICE exchange buffers between neighbours:
+
+  * `RingTransport`   one slab per process / GPU; `torch.distributed.batch_isend_irecv` on the
+                      buffers (NCCL send/recv over NVLink on GPUs; gloo in the CPU tests of the
+                      choreography);
+  * in-process copies when all slabs live on one GPU (`SlabLbm(..., world=None)`): the slabs run one
+                      after another on one stream -- the single-GPU check that the sharded step
+                      is bit-identical to the unsharded one, not a performance mode.
+"""
+import numpy as np
+
+from .lbm import Lbm
+
+GHOST = 2  # LBM_SLAB_GHOST
+
+
+def partition(mask, parts):
+    """Cut [0, nz) into `parts` contiguous z-ranges with nearly equal fluid-node counts, each at
+    least GHOST planes thick.  Returns [(z0, z1), ...]."""
+    nz = mask.shape[0]
+    if parts < 1 or nz < GHOST * parts:
+        raise ValueError(f"cannot cut {nz} planes into {parts} slabs of >= {GHOST} planes")
+    per_plane = (np.asarray(mask).reshape(nz, -1) == 0).sum(axis=1).astype(np.int64)
+    cum = np.concatenate([[0], np.cumsum(per_plane)])
+    total = int(cum[-1])
+    cuts = [0]
+    for k in range(1, parts):
+        z = int(np.searchsorted(cum, total * k / parts, side="left"))
+        z = max(z, cuts[-1] + GHOST)                 # minimum thickness of the slab below
+        z = min(z, nz - GHOST * (parts - k))         # leave room for the slabs above
+        cuts.append(z)
+    cuts.append(nz)
+    return [(cuts[k], cuts[k + 1]) for k in range(parts)]
+
+
+def local_planes(nz, z0, z1):
+    """Global z index of every plane of the slab's local box (halo planes wrap periodically)."""
+    return np.arange(z0 - GHOST, z1 + GHOST) % nz
+
+
+def local_box(a, z0, z1):
+    """Slice a global [z, y, x] (or [q, z, y, x]) array to the slab's local box."""
+    a = np.asarray(a)
+    ax = a.ndim - 3
+    return np.ascontiguousarray(np.take(a, local_planes(a.shape[ax], z0, z1), axis=ax))
+
+
+class _DeviceBytes:
+    """A span of device memory owned by an lbm_ctx, exposed through __cuda_array_interface__ so
+    that torch can alias it (no copy)."""
+
+    def __init__(self, ptr, nbytes, keepalive):
+        self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1",
+                                         "data": (ptr, False), "version": 2}
+        self._keepalive = keepalive
+
+
+def buffer_tensor(sim, which):
+    """uint8 torch tensor aliasing exchange buffer `which` of a slab context (None if empty)."""
+    import torch
+    ptr, nbytes = sim.slab_buffer(which)
+    if nbytes == 0:
+        return None
+    return torch.as_tensor(_DeviceBytes(ptr, nbytes, sim),
+                           device=torch.device("cuda", torch.cuda.current_device()))
+
+
+class RingTransport:
+    """Neighbour exchange on the periodic ring of slabs, one slab per rank.  `exchange(send_lo,
+    send_hi, recv_lo, recv_hi)`: my low-face message goes to rank-1 and lands in its high-face
+    receive buffer, my high-face message goes to rank+1 and lands in its low-face buffer.  Posting
+    order (send up, send down, receive from below, receive from above) keeps the two messages
+    between the same pair of ranks (world size 2) matched.  A None tensor is an empty message; both
+    ends see it empty (the sizes derive from the same mask planes)."""
+
+    def __init__(self, rank, world, group=None):
+        self.rank, self.world, self.group = rank, world, group
+
+    def exchange(self, send_lo, send_hi, recv_lo, recv_hi):
+        if self.world == 1:
+            if recv_lo is not None:
+                recv_lo.copy_(send_hi)
+            if recv_hi is not None:
+                recv_hi.copy_(send_lo)
+            return
+        import torch.distributed as dist
+        up, down = (self.rank + 1) % self.world, (self.rank - 1) % self.world
+        ops = []
+        if send_hi is not None:
+            ops.append(dist.P2POp(dist.isend, send_hi, up, self.group))
+        if send_lo is not None:
+            ops.append(dist.P2POp(dist.isend, send_lo, down, self.group))
+        if recv_lo is not None:
+            ops.append(dist.P2POp(dist.irecv, recv_lo, down, self.group))
+        if recv_hi is not None:
+            ops.append(dist.P2POp(dist.irecv, recv_hi, up, self.group))
+        if ops:
+            for w in dist.batch_isend_irecv(ops):
+                w.wait()   # stream-ordered on CUDA tensors: no host block
+
+
+class SlabLbm:
+    """A z-periodic simulation cut into z-slabs.
+
+    world=None: all `parts` slabs are created in this process on the current GPU and stepped one
+    after another (validation of the sharded path on one GPU).
+    world=N, rank=r: this process owns slab r of N (one process per GPU); exchanges go through
+    torch.distributed's default (or the given) process group.
+
+    Global arrays are [z, y, x]; `get_macroscopic` returns the owned planes of this process
+    (all planes when world is None)."""
+
+    def __init__(self, mask, params, parts=None, rank=None, world=None, group=None):
+        mask = np.ascontiguousarray(mask, np.uint8)
+        if int(params["z_open"]) != 0:
+            raise ValueError("slab sharding needs a z-periodic box (z_open = 0)")
+        self.shape = mask.shape
+        self.world = world
+        nparts = world if world is not None else (parts or 1)
+        self.ranges = partition(mask, nparts)
+        self.mine = [rank] if world is not None else list(range(nparts))
+        self.sims = [Lbm(local_box(mask, *self.ranges[r]), params, slab=True) for r in self.mine]
+        self.num_fluid = sum(s.num_owned for s in self.sims)
+        self._ring = RingTransport(rank, world, group) if world is not None else None
+        self._buf = [[buffer_tensor(s, w) for w in range(8)] for s in self.sims]
+        self._psi_current = False
+
+    def close(self):
+        self._buf = []
+        for s in self.sims:
+            s.close()
+        self.sims = []
+
+    # -- exchanges: kind 0 = psi (buffers 0,1 -> 2,3), kind 1 = populations (4,5 -> 6,7)
+    def _exchange(self, kind):
+        b = 4 * kind
+        if self._ring is not None:
+            buf = self._buf[0]
+            self._ring.exchange(buf[b], buf[b + 1], buf[b + 2], buf[b + 3])
+            return
+        n = len(self.sims)
+        for r in range(n):
+            lo, hi = self._buf[(r - 1) % n], self._buf[(r + 1) % n]
+            if self._buf[r][b + 2] is not None:
+                self._buf[r][b + 2].copy_(lo[b + 1])   # my low halo <- lower slab's high face
+            if self._buf[r][b + 3] is not None:
+                self._buf[r][b + 3].copy_(hi[b])       # my high halo <- upper slab's low face
+
+    def _density_and_psi_halo(self):
+        for s in self.sims:
+            s.slab_density()
+        self._exchange(0)
+
+    def step(self, n=1):
+        for _ in range(int(n)):
+            self._density_and_psi_halo()
+            for s in self.sims:
+                s.slab_collide()
+            self._exchange(1)
+            for s in self.sims:
+                s.slab_unpack()
+
+    def sync(self):
+        for s in self.sims:
+            s.sync()
+
+    def set_density(self, rhoA, rhoB):
+        for s, r in zip(self.sims, self.mine):
+            z0, z1 = self.ranges[r]
+            s.set_density(local_box(rhoA, z0, z1), local_box(rhoB, z0, z1))
+
+    def set_populations(self, comp, f):
+        for s, r in zip(self.sims, self.mine):
+            s.set_populations(comp, local_box(f, *self.ranges[r]))
+
+    def _owned(self, a):
+        return a[..., GHOST:a.shape[-3] - GHOST, :, :]
+
+    def get_populations(self, comp):
+        return np.concatenate([self._owned(s.get_populations(comp)) for s in self.sims], axis=1)
+
+    def get_macroscopic(self, fields=("rhoA", "rhoB", "ux", "uy", "uz", "P")):
+        self._density_and_psi_halo()   # the library's slab getter needs psi of the current state
+        parts = [s.get_macroscopic(fields) for s in self.sims]
+        return {k: np.concatenate([self._owned(p[k]) for p in parts], axis=0) for k in parts[0]}
+
+    def diagnostics(self):
+        """(mass[2], momentum[3]) over the owned nodes of this process; summed over all ranks when
+        distributed (one all_reduce of 5 doubles)."""
+        m, j = np.zeros(2), np.zeros(3)
+        for s in self.sims:
+            a, b = s.diagnostics()
+            m += a
+            j += b
+        if self.world is not None and self.world > 1:
+            import torch
+            import torch.distributed as dist
+            dev = "cuda" if dist.get_backend(self._ring.group) == "nccl" else "cpu"
+            t = torch.tensor(np.concatenate([m, j]), dtype=torch.float64, device=dev)
+            dist.all_reduce(t, group=self._ring.group)
+            t = t.cpu().numpy()
+            m, j = t[:2], t[2:]
+        return m, j

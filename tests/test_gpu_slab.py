@@ -1,0 +1,185 @@
+"""GPU tests of the z-slab sharded step (include/lbm.h "z-slab sharding").
+All slabs of a box live on the one GPU of the test box and are stepped one after another, the
+exchanges being device copies of the very buffers NCCL would move (paper_2207_01534_b200/slab.py).
+
+What is checked: the sharded step is BIT-IDENTICAL to the unsharded CUDA path on every population
+(same kernels, same summation order, for any number of slabs, fp64 and fp32), and matches the CPU
+oracle to the north-star tolerances (fp64: every population 1e-10 relative)."""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+from oracle import LbmRef
+from paper_2207_01534_b200 import Lbm, LbmError, load, make_params
+from paper_2207_01534_b200 import lbm as binding
+from paper_2207_01534_b200.slab import SlabLbm, local_box
+from workloads import default_params, make_config, sphere_pack_mask
+
+pytestmark = pytest.mark.gpu
+
+
+def _rock_case(n=40, bits=64, seed=21):
+    """config 5 recipe at a small edge (periodic sphere pack, body force) plus wetting and a
+    viscosity ratio, so that every term of the step is switched on"""
+    c = make_config(5, size=n, seed=seed, storage_bits=bits, xi=-0.2, tau=(1.2, 0.7),
+                    accel=(1e-6, -2e-6, 3e-6))
+    rng = np.random.Generator(np.random.PCG64(seed))
+    fl = c["mask"] == 0
+    for k in ("rhoA", "rhoB"):
+        c[k] = np.where(fl, c[k] * (1.0 + rng.uniform(-1e-3, 1e-3, c[k].shape)), 0.0)
+    return c
+
+
+def _identical_pops(a, b, mask):
+    fl = mask == 0
+    for s in (0, 1):
+        fa, fb = a.get_populations(s)[:, fl], b.get_populations(s)[:, fl]
+        assert np.array_equal(fa, fb), (s, np.abs(fa - fb).max())
+
+
+@pytest.mark.parametrize("parts", [1, 2, 3])
+def test_slab_fp64_bit_identical_to_unsharded_and_matches_oracle(parts):
+    c = _rock_case(40, 64)
+    g = Lbm(c["mask"], c["params"])
+    s = SlabLbm(c["mask"], c["params"], parts=parts)
+    assert s.num_fluid == g.num_fluid
+    g.set_density(c["rhoA"], c["rhoB"])
+    s.set_density(c["rhoA"], c["rhoB"])
+    g.step(60)
+    s.step(60)
+    _identical_pops(s, g, c["mask"])
+    if parts == 3:
+        o = LbmRef(c["mask"], c["params"])
+        o.set_density(c["rhoA"], c["rhoB"])
+        o.step(60)
+        fl = c["mask"] == 0
+        for comp in (0, 1):
+            a, b = s.get_populations(comp)[:, fl], o.get_populations(comp)[:, fl]
+            assert (np.abs(a - b) / np.abs(b)).max() <= 1e-10
+    # macroscopic fields and sums over slabs
+    mg, ms = g.get_macroscopic(), s.get_macroscopic()
+    for k in mg:
+        assert np.array_equal(mg[k], ms[k]), k
+    m_g, j_g = g.diagnostics()
+    m_s, j_s = s.diagnostics()
+    assert np.max(np.abs(m_s - m_g) / m_g) < 1e-13 and np.max(np.abs(j_s - j_g)) < 1e-10
+    # stepping continues correctly after the getters
+    g.step(5)
+    s.step(5)
+    _identical_pops(s, g, c["mask"])
+    s.close()
+    g.close()
+
+
+@pytest.mark.parametrize("parts", [2, 4])
+def test_slab_fp32_bit_identical_to_unsharded(parts):
+    c = _rock_case(48, 32, seed=22)
+    g = Lbm(c["mask"], c["params"])
+    s = SlabLbm(c["mask"], c["params"], parts=parts)
+    g.set_density(c["rhoA"], c["rhoB"])
+    s.set_density(c["rhoA"], c["rhoB"])
+    g.step(100)
+    s.step(100)
+    _identical_pops(s, g, c["mask"])
+    mg, ms = g.get_macroscopic(("rhoA", "rhoB", "uz")), s.get_macroscopic(("rhoA", "rhoB", "uz"))
+    for k in mg:
+        assert np.array_equal(mg[k], ms[k]), k
+    s.close()
+    g.close()
+
+
+def test_slab_no_solids_and_thinnest_slabs():
+    """config 1 (no solids: empty wall pass, full planes) cut into slabs of exactly 2 planes: every
+    owned plane is a boundary plane and both halo planes of a face come from different slabs'
+    planes."""
+    c = make_config(1, size=16)
+    g = Lbm(c["mask"], c["params"])
+    s = SlabLbm(c["mask"], c["params"], parts=8)
+    assert all(z1 - z0 == 2 for z0, z1 in s.ranges)
+    g.set_density(c["rhoA"], c["rhoB"])
+    s.set_density(c["rhoA"], c["rhoB"])
+    g.step(40)
+    s.step(40)
+    _identical_pops(s, g, c["mask"])
+    s.close()
+    g.close()
+
+
+def test_slab_index_variants_agree(monkeypatch):
+    """The int32-index fused pass and the register kernel give the same sharded result as the
+    default 16-bit index path (boundary tiles fall back to the wide rows there)."""
+    c = _rock_case(32, 32, seed=23)
+    ref = None
+    for env in ({}, {"LBM_B200_IDX": "32"}, {"LBM_B200_COLLIDE": "simple"}, {"LBM_B200_PDL": "0"}):
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        s = SlabLbm(c["mask"], c["params"], parts=2)
+        s.set_density(c["rhoA"], c["rhoB"])
+        s.step(30)
+        f = [s.get_populations(k) for k in (0, 1)]
+        s.close()
+        for k in env:
+            monkeypatch.delenv(k)
+        if ref is None:
+            ref = f
+        elif env.get("LBM_B200_COLLIDE") == "simple":
+            fl = c["mask"] == 0   # different arithmetic order: fp32 agreement, not identity
+            for a, b in zip(f, ref):
+                assert np.abs(a[:, fl] - b[:, fl]).max() < 1e-5 * np.abs(b[:, fl]).max()
+        else:
+            for a, b in zip(f, ref):
+                assert np.array_equal(a, b), env
+
+
+def test_slab_checkpoint_roundtrip():
+    c = _rock_case(32, 64, seed=24)
+    a = SlabLbm(c["mask"], c["params"], parts=2)
+    a.set_density(c["rhoA"], c["rhoB"])
+    a.step(10)
+    f = [a.get_populations(k) for k in (0, 1)]
+    b = SlabLbm(c["mask"], c["params"], parts=3)     # restore onto a different cut
+    for k in (0, 1):
+        b.set_populations(k, f[k])
+    a.step(10)
+    b.step(10)
+    _identical_pops(a, b, c["mask"])
+    a.close()
+    b.close()
+
+
+def test_slab_error_paths():
+    lib = load()
+    m = sphere_pack_mask(16, 5, 3.0, 4.0)[0]
+    ml = local_box(m, 0, 8)
+    p = default_params()
+    s = Lbm(ml, p, slab=True)
+    with pytest.raises(LbmError) as e:
+        s.step(1)                                   # lbm_step is not the slab step
+    assert e.value.code == binding.LBM_EINVAL
+    with pytest.raises(LbmError):
+        s.slab_collide()                            # density pass + psi exchange come first
+    with pytest.raises(LbmError):
+        s.slab_unpack()
+    with pytest.raises(LbmError):
+        s.saturation(0)
+    s.slab_density()
+    s.slab_collide()
+    with pytest.raises(LbmError):
+        s.slab_density()                            # unpack of the running step is missing
+    s.slab_unpack()
+    with pytest.raises(LbmError):
+        s.slab_buffer(8)
+    sizes = [s.slab_buffer(w)[1] for w in range(8)]
+    assert all(b % 8 == 0 for b in sizes) and sizes[0] > 0
+    s.close()
+    g = Lbm(m, p)
+    with pytest.raises(LbmError):
+        g.slab_density()                            # not a slab context
+    g.close()
+    h = C.c_void_p()
+    ps = make_params(default_params(z_open=1, inlet_kind=1, outlet_kind=1))
+    assert lib.lbm_create_slab(C.byref(h), ml.ctypes.data, 16, 16, 12, C.byref(ps)) == binding.LBM_EINVAL
+    ps = make_params(p)
+    thin = np.zeros((5, 4, 4), np.uint8)
+    assert lib.lbm_create_slab(C.byref(h), thin.ctypes.data, 4, 4, 5, C.byref(ps)) == binding.LBM_EINVAL
