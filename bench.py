@@ -2,15 +2,18 @@
 """bench.py -- two-component D3Q19 MLUPS on B200 (BASELINE.json metric), one JSON line on stdout.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+                    [--shard replicas|slab]
 
 A "step" is one pass of the whole hot path (SURVEY.md §8a rows a0-a7 except on-demand
 diagnostics) over all fluid nodes of the workload.  Default workload: BASELINE.json config 4, the
 256^3 sandstone-like mask the north_star quotes its roofline target on.  Inputs are seeded and
 synthetic (workloads/generators.py); they stand in for the paper's Bentheimer image.
 
-N > 1: the path is single-GPU by the north_star ("no sharding"): ranks run independent replicas
-(DESIGN.md "Multi-GPU: replicas only"), no data-path collective; value = all ranks' updates / max
-time over ranks.
+N > 1: the headline metric is single-GPU by the north_star ("no sharding"), so by default ranks
+run independent replicas (no data-path collective; value = all ranks' updates / max time over
+ranks, "scaling": "weak").  --shard slab instead cuts ONE z-periodic box (default config 5) into
+N z-slabs, one per rank, with the psi-plane and 5-population halo exchanges of SURVEY.md §8e over
+NCCL send/recv ("scaling": "strong").
 
 --impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the
 same workload on the host cores; it is a deliberately slow program, reported as a baseline.
@@ -42,6 +45,7 @@ def parse_args():
     ap.add_argument("--size", type=int, default=None, help="override the box edge (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "slab"])
     return ap.parse_args()
 
 
@@ -288,9 +292,111 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_slab(args):
+    """--shard slab: one z-periodic box cut into WORLD_SIZE z-slabs (strong scaling)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2207_01534_b200.slab import SlabLbm
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    K = args.steps if args.steps is not None else 200
+    W = args.warmup if args.warmup is not None else 20
+    cfg = workload(args)
+    if cfg["params"]["z_open"]:
+        raise SystemExit("bench.py --shard slab needs a z-periodic config (1, 2 or 5)")
+    sim = SlabLbm(cfg["mask"], cfg["params"], rank=rank, world=world)
+    sim.set_density(cfg["rhoA"], cfg["rhoB"])
+    one = sim.sims[0]
+    total_nf = int((cfg["mask"] == 0).sum())
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sim.step(W)
+    barrier()
+    one.set_profiling(False)             # restarts the launch counter
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    sim.step(K)
+    e1.record()
+    barrier()
+    sampler.stop_flag = True
+    sampler.join()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    value = total_nf * K / (ms_total * 1e-3) / 1e6
+    _, launches = one.last_step_profile()
+    mass, _ = sim.diagnostics()
+    one.set_profiling(True)
+    sim.step(K)
+    kms, _ = one.last_step_profile()
+    one.set_profiling(False)
+    peak, peak_src = measured_peaks()
+    t_col = kms["collide_stream"] / K * 1e-3
+    achieved = BYTES_PER_UPDATE_COLLIDE * one.num_owned / t_col / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_collide_stream", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": BYTES_PER_UPDATE_COLLIDE * one.num_owned,
+                "kernel_ms_per_launch": {("halo_pack_unpack" if k == "open_planes" else k): v / K
+                                         for k, v in kms.items()},
+                "note": "rank 0's slab"}
+    e2e = None
+    if not args.no_e2e:
+        barrier()
+        t0 = time.perf_counter()
+        sim.set_density(cfg["rhoA"], cfg["rhoB"])
+        sim.step(K)
+        out = sim.get_macroscopic(("rhoA", "rhoB"))
+        torch.cuda.synchronize()
+        dt = torch.tensor([time.perf_counter() - t0], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        z0, z1 = sim.ranges[rank]
+        up = 2 * (z1 - z0 + 4) * cfg["mask"][0].size * 8
+        down = sum(v.nbytes for v in out.values())
+        e2e = {"value": total_nf * K / float(dt.item()) / 1e6, "unit": "MLUPS",
+               "h2d_bytes_per_step": up / K, "d2h_bytes_per_step": down / K,
+               "job": f"per rank: lbm_set_density of the local box (host f64) + {K} sharded steps + "
+                      "lbm_get_macroscopic(rhoA,rhoB) of the owned planes"}
+    if rank == 0:
+        line = {"metric": "two_component_d3q19_mlups", "value": value, "unit": "MLUPS",
+                "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_total / K,
+                "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                "dtype": "f32" if cfg["params"]["storage_bits"] == 32 else "f64",
+                "data": "synthetic",
+                "config": {"workload": cfg["name"], "box": list(cfg["mask"].shape[::-1]),
+                           "fluid_nodes": total_nf, "porosity": cfg["porosity"],
+                           "parallelism": f"z-slabs x{world}", "slab_z_ranges": sim.ranges,
+                           "l2": "populations exceed the 126 MB L2 at the default size; no flush"},
+                "clocks": sampler.result(), "e2e": e2e, "gpu_launches": launches,
+                "roofline": roofline, "cpu_baseline": None,
+                "mass_check": [float(mass[0]), float(mass[1])]}
+        print(json.dumps(line), flush=True)
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 if __name__ == "__main__":
     a = parse_args()
     if a.impl == "reference":
         run_reference(a)
+    elif a.shard == "slab":
+        if a.config == 4 and "--config" not in " ".join(sys.argv):
+            a.config = 5
+        run_slab(a)
     else:
         run_ours(a)
