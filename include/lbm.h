@@ -163,28 +163,34 @@ int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open,
  * is periodic in z is cut into contiguous z-slabs, one lbm_ctx per slab (one per GPU).  The slab's
  * mask is the owned planes plus LBM_SLAB_GHOST = 2 halo planes at each z end (copies of the
  * neighbour slabs' planes; periodic wrap of the global box): nz_local = owned + 4, owned >= 2.
- * One time step of a slab is
- *     lbm_slab_density                          a1 on the owned nodes
- *     psi exchange (caller)                     buffers 0,1 (send) -> the neighbours' 2,3 (receive)
- *     lbm_slab_collide                          a2 (all wall solids of the local box), a3-a6 on the
- *                                               owned nodes, pack of the populations that crossed a cut
- *     population exchange (caller)              buffers 4,5 (send) -> the neighbours' 6,7 (receive)
- *     lbm_slab_unpack                           received populations -> rows of the owned boundary planes
+ * One time step of a slab is, in this order (anything else returns LBM_EINVAL),
+ *     lbm_slab_density(c, 0)     a1 on the two owned planes at each face (the psi the neighbours need)
+ *     psi exchange START         buffers 0,1 (send) -> the neighbours' 2,3 (receive)
+ *     lbm_slab_density(c, 1)     a1 on the interior: overlaps the exchange
+ *     psi exchange COMPLETE
+ *     lbm_slab_collide(c, 0)     a2 on all wall solids of the local box; a3-a6 on the tiles of the
+ *                                outermost owned plane of each face; pack of what crossed a cut
+ *     population exchange START  buffers 4,5 (send) -> the neighbours' 6,7 (receive)
+ *     lbm_slab_collide(c, 1)     a3-a6 on the interior tiles: overlaps the exchange
+ *     population exchange COMPLETE
+ *     lbm_slab_unpack(c)         received populations -> rows of the owned boundary planes
+ * (a getter may follow lbm_slab_density(c, 1) + the completed psi exchange; the next step then
+ * starts again with lbm_slab_density(c, 0)),
  * and the result on the owned nodes is bit-identical to the unsharded lbm_step (same kernels, same
  * summation order).  The exchanges move DEVICE buffers and are the caller's (NCCL send/recv
  * through torch.distributed in paper_2207_01534_b200/slab.py; device copies when several slabs
  * live on one GPU).  All calls are asynchronous on torch's current stream.
  * lbm_set_density / lbm_set_populations / lbm_get_* take dense arrays of the LOCAL box
  * (nx*ny*nz_local); halo voxels are ignored on input and written as 0 by lbm_get_macroscopic,
- * which in slab mode requires lbm_slab_density + the psi exchange to have been done on the current
- * state.  lbm_diagnostics sums over the owned nodes.  lbm_step, lbm_saturation,
+ * which in slab mode requires both lbm_slab_density parts + the psi exchange to have been done on
+ * the current state.  lbm_diagnostics sums over the owned nodes.  lbm_step, lbm_saturation,
  * lbm_trapped_volume and lbm_mean_pressure return LBM_EINVAL on a slab context; z_open must be 0. */
 #define LBM_SLAB_GHOST 2
 int lbm_create_slab(lbm_ctx** out, const uint8_t* solid_local, int nx, int ny, int nz_local,
                     const lbm_params* p);
-int lbm_slab_density(lbm_ctx* c);
-int lbm_slab_collide(lbm_ctx* c);   /* LBM_EINVAL unless it follows lbm_slab_density */
-int lbm_slab_unpack(lbm_ctx* c);    /* LBM_EINVAL unless it follows lbm_slab_collide */
+int lbm_slab_density(lbm_ctx* c, int part);
+int lbm_slab_collide(lbm_ctx* c, int part);
+int lbm_slab_unpack(lbm_ctx* c);
 /* Exchange buffers (DEVICE pointers into the context's memory, valid until lbm_destroy; psi
  * buffers are (rho_A, rho_B) pairs of the storage type, population buffers (f_A, f_B) pairs).
  * which = 2*kind + face, face 0 = low z, 1 = high z:

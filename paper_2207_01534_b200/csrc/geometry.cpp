@@ -361,6 +361,8 @@ int build_halo(const Geometry& g, const uint8_t* solid, size_t npad, Halo& h) {
     h.psi_recv[0][1] = n_lo;
     h.psi_recv[1][0] = g.nact + n_lo;
     h.psi_recv[1][1] = n_hi;
+    h.edge_plane[0] = count(G, G + 1);
+    h.edge_plane[1] = count(nz - G - 1, nz - G);
   } catch (const std::bad_alloc&) {
     return -4;
   }

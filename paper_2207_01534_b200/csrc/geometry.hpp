@@ -92,6 +92,8 @@ struct Halo {
   std::vector<int32_t> unpack[2];  // [face]: destination slots (owned boundary plane rows)
   long long psi_send[2][2];        // [face]{first id, count}: owned nodes of the 2 planes at that face
   long long psi_recv[2][2];        // [face]{first id, count}: halo nodes at that face
+  long long edge_plane[2];         // fluid nodes of the outermost owned plane at that face (the only
+                                   // nodes whose pushes cross the cut)
 };
 int build_halo(const Geometry& g, const uint8_t* solid, size_t npad, Halo& h);
 

@@ -97,12 +97,22 @@ struct Consts {
 // ---------------------------------------------------------------------------------------------
 // a1  density / psi pass: rho_sigma = sum_i f_i^sigma (Eq. 3); psi = rho (L105).
 // One thread per fluid node; every load is a fully coalesced row read.
+// Node range of a launch: blocks [0, split) take ids from a0 on, the remaining blocks from a1 on
+// (whole pass: a0 = 0, split = grid; slab mode launches the two boundary id ranges first and the
+// interior separately, so that the psi halo exchange overlaps the interior; a0, a1 are multiples
+// of the block size, which keeps every warp's loads line-aligned).
+struct NodeRange {
+  int a0, split, a1;
+  int nend;   // ids >= nend are not processed
+};
 template <typename T>
 __global__ void __launch_bounds__(256) k_density(const T* __restrict__ f, Vec2<T>* __restrict__ psi,
-                                                 int nf, size_t npad, float keep_psi) {
-  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+                                                 NodeRange r, size_t npad, float keep_psi) {
+  const int b = (int)blockIdx.x;
+  const int n = (b < r.split ? r.a0 + b * (int)blockDim.x : r.a1 + (b - r.split) * (int)blockDim.x) +
+                (int)threadIdx.x;
   pdl_wait();  // f was written by the previous step's fused pass
-  if (n >= nf) return;
+  if (n >= r.nend) return;
   const Vec2<T>* f2 = reinterpret_cast<const Vec2<T>*>(f);
   Vec2<T> v[Q];
 #pragma unroll
@@ -587,6 +597,9 @@ struct Idx16 {
   int reverse;            // 1: CTA b takes tile gridDim-1-b
   int nact;               // nodes this pass updates: ids [0,nact).  = nf, except in slab mode, where
                           // the halo nodes [nact,nf) only receive pushes
+  int tile0, split, tile1;  // tiles of this launch: position b < split -> tile0 + b, else
+                            // tile1 + (b - split)  (whole pass: 0, grid, 0; slab mode: the boundary
+                            // tiles of both faces in one launch, the interior in another)
 };
 
 template <typename T, int TN>
@@ -610,7 +623,8 @@ __global__ void __launch_bounds__(TN, MINB)
   // Tiles are taken from the END of the id range first: the density pass that ran just before
   // walked the range forwards, so the last ~100 MB of populations it read are still in L2, and
   // this kernel's last writes (the head of the range) are what the next density pass reads first.
-  const unsigned tile = ix.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
+  const int pos = ix.reverse ? (int)(gridDim.x - 1u - blockIdx.x) : (int)blockIdx.x;
+  const unsigned tile = (unsigned)(pos < ix.split ? ix.tile0 + pos : ix.tile1 + (pos - ix.split));
   const size_t t0 = (size_t)tile * TN;
   if (tid == 0) mbar_init(&bar, 1);
   __syncthreads();

@@ -78,7 +78,11 @@ struct lbm_ctx {
   void* halo_recv = nullptr;         // [unpack low | unpack high] (A,B) pairs
   int n_pack[2] = {0, 0}, n_unpack[2] = {0, 0};
   long long psi_send[2][2] = {{0, 0}, {0, 0}}, psi_recv[2][2] = {{0, 0}, {0, 0}};
-  int slab_phase = 0;       // 0: expects lbm_slab_density, 1: lbm_slab_collide, 2: lbm_slab_unpack
+  int slab_phase = 0;       // next slab call: 0 density(0), 1 density(1), 2 collide(0), 3 collide(1),
+                            // 4 unpack
+  // slab mode: id ranges [0, bnd_lo1) and [bnd_hi0, nact) hold the two owned planes at each face
+  // (rounded to 256 ids), tiles [0, tile_lo1) and [tile_hi0, tiles) the outermost owned plane
+  int bnd_lo1 = 0, bnd_hi0 = 0, tile_lo1 = 0, tile_hi0 = 0;
   size_t npad = 0, nwpad = 0, esz = 4;
   std::vector<int32_t> zstart;  // [nz+1] first fluid id of every z-plane (host copy, used by queries)
   void* f[2] = {nullptr, nullptr};                // two buffers of [19][npad][2 comps] T
@@ -192,9 +196,10 @@ void launch_k(bool pdl, void (*kern)(KArgs...), unsigned grid, unsigned block, s
   cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
 }
 
-// a1 (+ the deferred a0 of the previous step) on the current buffer, ids [0, nact)
+// a1 (+ the deferred a0 of the previous step) on the current buffer, ids [0, nact).
+// part: -1 whole range; slab mode: 0 = the boundary id ranges of both faces, 1 = the interior.
 template <typename T>
-void launch_density(lbm_ctx* c, cudaStream_t st) {
+void launch_density(lbm_ctx* c, cudaStream_t st, int part = -1) {
   T* fin = (T*)c->f[c->cur];
   const bool pdl = c->pdl && !c->prof;  // events between the launches would serialise them anyway
   Timed t(c, st, 0);
@@ -205,8 +210,21 @@ void launch_density(lbm_ctx* c, cudaStream_t st) {
              make_open<T>(c->p), c->keep_psi);
     c->open_pending = false;
   } else {
-    launch_k(pdl, k_density<T>, blocks(c->nact, 256), 256, 0, st, (const T*)fin,
-             (Vec2<T>*)c->psi, c->nact, c->npad, c->keep_psi);
+    NodeRange r{0, (int)blocks(c->nact, 256), 0, c->nact};
+    unsigned grid = blocks(c->nact, 256);
+    if (part == 0) {
+      r.split = c->bnd_lo1 / 256;
+      r.a1 = c->bnd_hi0;
+      grid = (unsigned)r.split + blocks(c->nact - c->bnd_hi0, 256);
+    } else if (part == 1) {
+      r.a0 = c->bnd_lo1;
+      r.nend = c->bnd_hi0;
+      grid = (unsigned)((c->bnd_hi0 - c->bnd_lo1) / 256);
+      r.split = (int)grid;
+    }
+    if (grid > 0)
+      launch_k(pdl, k_density<T>, grid, 256, 0, st, (const T*)fin, (Vec2<T>*)c->psi, r, c->npad,
+               c->keep_psi);
   }
 }
 
@@ -246,7 +264,7 @@ void apply_pending(lbm_ctx* c, cudaStream_t st) {
 }
 
 template <typename T, int TN, int MINB, bool IDX16>
-void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
+void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st, int part) {
   constexpr bool kRemainder = sizeof(T) == 4;
   constexpr size_t smem = IDX16 ? collide16_smem_bytes<T, TN>() : collide_smem_bytes<T, TN>();
   static bool configured[64] = {};  // function attributes are per device
@@ -261,35 +279,52 @@ void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
   ix.np = c->p.z_open ? c->np : 0;
   ix.reverse = c->reverse;
   ix.nact = c->nact;
+  static_assert(TN == 128 || TN == 256, "tile ranges below are in units of 128 ids");
+  const int per = TN / 128;                      // slab tile ranges are kept in 128-id tiles
+  unsigned grid = blocks(c->nact, TN);
+  ix.tile0 = 0; ix.split = (int)grid; ix.tile1 = 0;
+  if (part == 0) {                               // boundary tiles of both faces
+    const int lo1 = (c->tile_lo1 + per - 1) / per, hi0 = std::max(lo1, c->tile_hi0 / per);
+    ix.split = lo1; ix.tile1 = hi0;
+    grid = (unsigned)lo1 + (blocks(c->nact, TN) - (unsigned)hi0);
+  } else if (part == 1) {                        // interior tiles
+    const int lo1 = (c->tile_lo1 + per - 1) / per, hi0 = std::max(lo1, c->tile_hi0 / per);
+    ix.tile0 = lo1;
+    grid = (unsigned)(hi0 - lo1);
+    ix.split = (int)grid;
+  }
+  if (grid == 0) return;
   // Overlap only behind the wall pass: its blocks trigger after their own wait, i.e. once the
   // density pass (which may have rewritten the open planes of fin) is complete and visible.
   launch_k(c->pdl && !c->prof && c->nw > 0, k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX16>,
-           blocks(c->nact, TN), TN, smem, st, fin, fout, (const Vec2<T>*)c->psi,
+           grid, TN, smem, st, fin, fout, (const Vec2<T>*)c->psi,
            (const int*)c->nbr, c->nf, c->npad, k, ix);
 }
 
 template <typename T>
-void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
+void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st,
+                    int part = -1) {
   constexpr bool kRemainder = sizeof(T) == 4;
-  if (c->collide_variant == 0) {
-    k_collide_stream<T, kRemainder><<<blocks(c->nact, 256), 256, 0, st>>>(
-        fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->nact, c->npad, k);
+  if (c->collide_variant == 0) {  // A/B register kernel: no split, everything in part 0 (or -1)
+    if (part != 1)
+      k_collide_stream<T, kRemainder><<<blocks(c->nact, 256), 256, 0, st>>>(
+          fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->nact, c->npad, k);
     return;
   }
   if constexpr (sizeof(T) == 4) {
     if (c->idx16) {
-      if (c->tile == 1285) launch_bulk<T, 128, 5, true>(c, fin, fout, k, st);
-      else launch_bulk<T, 128, 6, true>(c, fin, fout, k, st);
+      if (c->tile == 1285) launch_bulk<T, 128, 5, true>(c, fin, fout, k, st, part);
+      else launch_bulk<T, 128, 6, true>(c, fin, fout, k, st, part);
       return;
     }
     switch (c->tile) {
-      case 1285: launch_bulk<T, 128, 5, false>(c, fin, fout, k, st); break;
-      case 2563: launch_bulk<T, 256, 3, false>(c, fin, fout, k, st); break;
-      default: launch_bulk<T, 128, 6, false>(c, fin, fout, k, st); break;
+      case 1285: launch_bulk<T, 128, 5, false>(c, fin, fout, k, st, part); break;
+      case 2563: launch_bulk<T, 256, 3, false>(c, fin, fout, k, st, part); break;
+      default: launch_bulk<T, 128, 6, false>(c, fin, fout, k, st, part); break;
     }
   } else {
-    if (c->idx16) launch_bulk<T, 128, 2, true>(c, fin, fout, k, st);
-    else launch_bulk<T, 128, 2, false>(c, fin, fout, k, st);
+    if (c->idx16) launch_bulk<T, 128, 2, true>(c, fin, fout, k, st, part);
+    else launch_bulk<T, 128, 2, false>(c, fin, fout, k, st, part);
   }
 }
 
@@ -608,6 +643,14 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
         c->psi_recv[fc][k] = halo.psi_recv[fc][k];
       }
     }
+    {  // boundary-first launch ranges (ids in units of 256, tiles of 128)
+      const long long na = g.nact;
+      long long hi0 = std::max(0LL, na - halo.psi_send[1][1]) / 256 * 256;
+      long long lo1 = std::min((long long)pad256(halo.psi_send[0][1]), hi0);
+      c->bnd_lo1 = (int)lo1; c->bnd_hi0 = (int)hi0;
+      c->tile_lo1 = (int)((halo.edge_plane[0] + 127) / 128);
+      c->tile_hi0 = (int)(std::max(0LL, na - halo.edge_plane[1]) / 128);
+    }
     const size_t sendb = (size_t)(c->n_pack[0] + c->n_pack[1]) * 2 * c->esz;
     const size_t recvb = (size_t)(c->n_unpack[0] + c->n_unpack[1]) * 2 * c->esz;
     c->halo_slots = (int*)lbm_shim_alloc(nslots * sizeof(int) + 16);
@@ -675,54 +718,60 @@ int lbm_create_slab(lbm_ctx** out, const uint8_t* solid_local, int nx, int ny, i
 
 long long lbm_num_owned(lbm_ctx* c) { return c ? c->nact : -1; }
 
-int lbm_slab_density(lbm_ctx* c) {
+int lbm_slab_density(lbm_ctx* c, int part) {
   if (int rc = check_ctx(c)) return rc;
   if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
-  if (c->slab_phase == 2)
-    return fail(LBM_EINVAL, "lbm_slab_unpack of the previous step is still missing");
+  if (part != 0 && part != 1) return fail(LBM_EINVAL, "part must be 0 or 1");
+  // part 0 may restart a step that stopped after its density pass (getters do that)
+  if (part == 0 ? c->slab_phase > 2 : c->slab_phase != 1)
+    return fail(LBM_EINVAL, "slab calls out of order (expected phase %d)", c->slab_phase);
   cudaStream_t st = cur_stream();
-  if (c->bits == 64) launch_density<double>(c, st); else launch_density<float>(c, st);
+  if (c->bits == 64) launch_density<double>(c, st, part); else launch_density<float>(c, st, part);
   CU(cudaPeekAtLastError());
-  c->slab_phase = 1;
+  c->slab_phase = part + 1;
   return LBM_OK;
 }
 
-int lbm_slab_collide(lbm_ctx* c) {
+extern "C++" {
+template <typename T>
+static int slab_collide_T(lbm_ctx* c, int part, cudaStream_t st) {
+  const T* fin = (const T*)c->f[c->cur];
+  T* fout = (T*)c->f[c->cur ^ 1];
+  if (part == 0) launch_wall<T>(c, st);
+  {
+    Timed t(c, st, 2);
+    launch_collide<T>(c, fin, fout, make_consts<T>(c->p), st, part);
+  }
+  const int np = c->n_pack[0] + c->n_pack[1];
+  if (part == 0 && np) {  // the boundary tiles are the only ones that push across a cut
+    Timed t(c, st, 3);
+    k_halo_pack<T><<<blocks(np, 256), 256, 0, st>>>((const T*)fout, c->halo_slots,
+                                                    (T*)c->halo_send, np);
+  }
+  if (part == 1) c->cur ^= 1;
+  CU(cudaPeekAtLastError());
+  return LBM_OK;
+}
+}  // extern "C++"
+
+int lbm_slab_collide(lbm_ctx* c, int part) {
   if (int rc = check_ctx(c)) return rc;
   if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
-  if (c->slab_phase != 1)
-    return fail(LBM_EINVAL, "lbm_slab_collide must follow lbm_slab_density and the psi exchange");
+  if (part != 0 && part != 1) return fail(LBM_EINVAL, "part must be 0 or 1");
+  if (c->slab_phase != 2 + part)
+    return fail(LBM_EINVAL, "slab calls out of order (expected phase %d)", c->slab_phase);
   cudaStream_t st = cur_stream();
-  const int np = c->n_pack[0] + c->n_pack[1];
-  if (c->bits == 64) {
-    launch_wall<double>(c, st);
-    { Timed t(c, st, 2);
-      launch_collide<double>(c, (const double*)c->f[c->cur], (double*)c->f[c->cur ^ 1],
-                             make_consts<double>(c->p), st); }
-    c->cur ^= 1;
-    if (np) { Timed t(c, st, 3);
-      k_halo_pack<double><<<blocks(np, 256), 256, 0, st>>>((const double*)c->f[c->cur], c->halo_slots,
-                                                           (double*)c->halo_send, np); }
-  } else {
-    launch_wall<float>(c, st);
-    { Timed t(c, st, 2);
-      launch_collide<float>(c, (const float*)c->f[c->cur], (float*)c->f[c->cur ^ 1],
-                            make_consts<float>(c->p), st); }
-    c->cur ^= 1;
-    if (np) { Timed t(c, st, 3);
-      k_halo_pack<float><<<blocks(np, 256), 256, 0, st>>>((const float*)c->f[c->cur], c->halo_slots,
-                                                          (float*)c->halo_send, np); }
-  }
-  CU(cudaPeekAtLastError());
-  c->slab_phase = 2;
+  if (int rc = c->bits == 64 ? slab_collide_T<double>(c, part, st) : slab_collide_T<float>(c, part, st))
+    return rc;
+  c->slab_phase = 3 + part;
   return LBM_OK;
 }
 
 int lbm_slab_unpack(lbm_ctx* c) {
   if (int rc = check_ctx(c)) return rc;
   if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
-  if (c->slab_phase != 2)
-    return fail(LBM_EINVAL, "lbm_slab_unpack must follow lbm_slab_collide and the population exchange");
+  if (c->slab_phase != 4)
+    return fail(LBM_EINVAL, "slab calls out of order (expected phase %d)", c->slab_phase);
   cudaStream_t st = cur_stream();
   const int nu = c->n_unpack[0] + c->n_unpack[1];
   const int* slots = c->halo_slots + c->n_pack[0] + c->n_pack[1];
@@ -917,6 +966,9 @@ int lbm_get_populations(lbm_ctx* c, int comp, double* f) {
 int lbm_get_macroscopic(lbm_ctx* c, double* rhoA, double* rhoB, double* ux, double* uy,
                         double* uz, double* P) {
   if (int rc = check_ctx(c)) return rc;
+  if (c->slab && c->slab_phase != 2)
+    return fail(LBM_EINVAL, "slab context: lbm_get_macroscopic needs both lbm_slab_density parts "
+                            "and the psi exchange on the current state");
   cudaStream_t st = cur_stream();
   const bool was = c->prof;
   c->prof = false;

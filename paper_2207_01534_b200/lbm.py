@@ -87,8 +87,8 @@ def load():
     lib.lbm_build_index.argtypes = [V, I, I, I, I, V, V, LL, C.POINTER(LL), C.POINTER(LL)]
     lib.lbm_build_schedule.argtypes = [V, I, I, I, I, I, I, V, LL, C.POINTER(LL)]
     lib.lbm_create_slab.argtypes = [C.POINTER(P), V, I, I, I, C.POINTER(lbm_params)]
-    lib.lbm_slab_density.argtypes = [P]
-    lib.lbm_slab_collide.argtypes = [P]
+    lib.lbm_slab_density.argtypes = [P, I]
+    lib.lbm_slab_collide.argtypes = [P, I]
     lib.lbm_slab_unpack.argtypes = [P]
     lib.lbm_slab_buffer.argtypes = [P, I, C.POINTER(C.c_void_p), C.POINTER(LL)]
     lib.lbm_num_owned.argtypes = [P]
@@ -249,11 +249,11 @@ class Lbm:
     def step(self, n=1):
         _chk(load().lbm_step(self._h, int(n)), "lbm_step")
 
-    def slab_density(self):
-        _chk(load().lbm_slab_density(self._h), "lbm_slab_density")
+    def slab_density(self, part):
+        _chk(load().lbm_slab_density(self._h, int(part)), "lbm_slab_density")
 
-    def slab_collide(self):
-        _chk(load().lbm_slab_collide(self._h), "lbm_slab_collide")
+    def slab_collide(self, part):
+        _chk(load().lbm_slab_collide(self._h, int(part)), "lbm_slab_collide")
 
     def slab_unpack(self):
         _chk(load().lbm_slab_unpack(self._h), "lbm_slab_unpack")

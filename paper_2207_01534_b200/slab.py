@@ -7,7 +7,13 @@ neighbours' rho(t)) and one transport across a cut (Eq. 1 LHS).  A box that is p
 into contiguous z-slabs balanced by fluid-node count; every slab is one `Lbm(slab=True)` context
 with two halo planes per end, and a step is
 
-    slab_density -> psi exchange -> slab_collide -> population exchange -> slab_unpack
+    slab_density(0)  [boundary planes]   -> psi exchange starts
+    slab_density(1)  [interior]          -> psi exchange completes
+    slab_collide(0)  [wall pass, boundary tiles, pack] -> population exchange starts
+    slab_collide(1)  [interior tiles]    -> population exchange completes
+    slab_unpack
+
+so that both exchanges run beside the interior work of the same pass.
 
 All arithmetic runs in the library's kernels; this module only partitions the mask, slices the
 initial state and moves the DEVICE exchange buffers between neighbours:
@@ -89,12 +95,23 @@ class RingTransport:
         self.rank, self.world, self.group = rank, world, group
 
     def exchange(self, send_lo, send_hi, recv_lo, recv_hi):
+        self.finish(self.start(send_lo, send_hi, recv_lo, recv_hi))
+
+    @staticmethod
+    def finish(works):
+        for w in works:
+            w.wait()   # stream-ordered on CUDA tensors: no host block
+
+    def start(self, send_lo, send_hi, recv_lo, recv_hi):
+        """Post the four messages; returns the handles `finish` waits on.  On CUDA tensors the
+        transfers run on NCCL's stream, after everything enqueued so far on the current stream and
+        beside whatever is enqueued next."""
         if self.world == 1:
             if recv_lo is not None:
                 recv_lo.copy_(send_hi)
             if recv_hi is not None:
                 recv_hi.copy_(send_lo)
-            return
+            return []
         import torch.distributed as dist
         up, down = (self.rank + 1) % self.world, (self.rank - 1) % self.world
         ops = []
@@ -106,9 +123,7 @@ class RingTransport:
             ops.append(dist.P2POp(dist.irecv, recv_lo, down, self.group))
         if recv_hi is not None:
             ops.append(dist.P2POp(dist.irecv, recv_hi, up, self.group))
-        if ops:
-            for w in dist.batch_isend_irecv(ops):
-                w.wait()   # stream-ordered on CUDA tensors: no host block
+        return dist.batch_isend_irecv(ops) if ops else []
 
 
 class SlabLbm:
@@ -144,12 +159,11 @@ class SlabLbm:
         self.sims = []
 
     # -- exchanges: kind 0 = psi (buffers 0,1 -> 2,3), kind 1 = populations (4,5 -> 6,7)
-    def _exchange(self, kind):
+    def _exchange_start(self, kind):
         b = 4 * kind
         if self._ring is not None:
             buf = self._buf[0]
-            self._ring.exchange(buf[b], buf[b + 1], buf[b + 2], buf[b + 3])
-            return
+            return self._ring.start(buf[b], buf[b + 1], buf[b + 2], buf[b + 3])
         n = len(self.sims)
         for r in range(n):
             lo, hi = self._buf[(r - 1) % n], self._buf[(r + 1) % n]
@@ -157,18 +171,25 @@ class SlabLbm:
                 self._buf[r][b + 2].copy_(lo[b + 1])   # my low halo <- lower slab's high face
             if self._buf[r][b + 3] is not None:
                 self._buf[r][b + 3].copy_(hi[b])       # my high halo <- upper slab's low face
+        return []
 
     def _density_and_psi_halo(self):
         for s in self.sims:
-            s.slab_density()
-        self._exchange(0)
+            s.slab_density(0)
+        works = self._exchange_start(0)
+        for s in self.sims:
+            s.slab_density(1)
+        RingTransport.finish(works)
 
     def step(self, n=1):
         for _ in range(int(n)):
             self._density_and_psi_halo()
             for s in self.sims:
-                s.slab_collide()
-            self._exchange(1)
+                s.slab_collide(0)
+            works = self._exchange_start(1)
+            for s in self.sims:
+                s.slab_collide(1)
+            RingTransport.finish(works)
             for s in self.sims:
                 s.slab_unpack()
 

@@ -158,15 +158,27 @@ def test_slab_error_paths():
         s.step(1)                                   # lbm_step is not the slab step
     assert e.value.code == binding.LBM_EINVAL
     with pytest.raises(LbmError):
-        s.slab_collide()                            # density pass + psi exchange come first
+        s.slab_collide(0)                           # density pass + psi exchange come first
     with pytest.raises(LbmError):
         s.slab_unpack()
     with pytest.raises(LbmError):
         s.saturation(0)
-    s.slab_density()
-    s.slab_collide()
     with pytest.raises(LbmError):
-        s.slab_density()                            # unpack of the running step is missing
+        s.get_macroscopic()                         # psi of the current state is missing
+    with pytest.raises(LbmError):
+        s.slab_density(1)                           # boundary part first
+    s.slab_density(0)
+    with pytest.raises(LbmError):
+        s.slab_collide(0)
+    s.slab_density(1)
+    s.slab_density(0)                               # a step may restart after its density pass
+    s.slab_density(1)
+    with pytest.raises(LbmError):
+        s.slab_collide(1)
+    s.slab_collide(0)
+    s.slab_collide(1)
+    with pytest.raises(LbmError):
+        s.slab_density(0)                           # unpack of the running step is missing
     s.slab_unpack()
     with pytest.raises(LbmError):
         s.slab_buffer(8)
@@ -175,7 +187,7 @@ def test_slab_error_paths():
     s.close()
     g = Lbm(m, p)
     with pytest.raises(LbmError):
-        g.slab_density()                            # not a slab context
+        g.slab_density(0)                           # not a slab context
     g.close()
     h = C.c_void_p()
     ps = make_params(default_params(z_open=1, inlet_kind=1, outlet_kind=1))
