@@ -159,10 +159,13 @@ int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open,
 /* ---- z-slab sharding across GPUs --------
  * The step has two grid-wide dependencies (Eq. 11/13: every node's force needs its
  * neighbours' rho(t); Eq. 15: every wall solid's rho~(t) needs its fluid neighbours' rho(t)) and
- * one transport across a cut (Eq. 1 LHS: 5 populations per component cross a z-plane).  A box that
- * is periodic in z is cut into contiguous z-slabs, one lbm_ctx per slab (one per GPU).  The slab's
- * mask is the owned planes plus LBM_SLAB_GHOST = 2 halo planes at each z end (copies of the
- * neighbour slabs' planes; periodic wrap of the global box): nz_local = owned + 4, owned >= 2.
+ * one transport across a cut (Eq. 1 LHS: 5 populations per component cross a z-plane).  The box
+ * is cut into contiguous z-slabs, one lbm_ctx per slab (one per GPU).  An end of a slab is either a
+ * CUT (halo_lo / halo_hi = 1: the mask carries LBM_SLAB_GHOST = 2 halo planes there, copies of the
+ * neighbour slab's planes) or the global box's own end (0: no halo planes; allowed only when
+ * z_open = 1, and the slab then owns the inlet plane z = 0 / the outlet plane z = nz-1 with the
+ * open-plane treatment of PAPER.md L147-157).  A z-periodic box has cuts at both ends of every
+ * slab (the halo planes wrap around).  nz_local = owned + 2*(halo_lo + halo_hi), owned >= 2.
  * One time step of a slab is, in this order (anything else returns LBM_EINVAL),
  *     lbm_slab_density(c, 0)     a1 on the two owned planes at each face (the psi the neighbours need)
  *     psi exchange START         buffers 0,1 (send) -> the neighbours' 2,3 (receive)
@@ -183,11 +186,12 @@ int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open,
  * lbm_set_density / lbm_set_populations / lbm_get_* take dense arrays of the LOCAL box
  * (nx*ny*nz_local); halo voxels are ignored on input and written as 0 by lbm_get_macroscopic,
  * which in slab mode requires both lbm_slab_density parts + the psi exchange to have been done on
- * the current state.  lbm_diagnostics sums over the owned nodes.  lbm_step, lbm_saturation,
- * lbm_trapped_volume and lbm_mean_pressure return LBM_EINVAL on a slab context; z_open must be 0. */
+ * the current state; so do lbm_saturation and lbm_mean_pressure, whose z-range is in LOCAL planes
+ * and which cover the owned nodes only (halo planes are empty ranges).  lbm_diagnostics sums over
+ * the owned nodes.  lbm_step and lbm_trapped_volume return LBM_EINVAL on a slab context. */
 #define LBM_SLAB_GHOST 2
 int lbm_create_slab(lbm_ctx** out, const uint8_t* solid_local, int nx, int ny, int nz_local,
-                    const lbm_params* p);
+                    const lbm_params* p, int halo_lo, int halo_hi);
 int lbm_slab_density(lbm_ctx* c, int part);
 int lbm_slab_collide(lbm_ctx* c, int part);
 int lbm_slab_unpack(lbm_ctx* c);
@@ -205,8 +209,8 @@ long long lbm_num_owned(lbm_ctx* c);   /* fluid nodes of the owned planes, or -1
  * local voxel index of the node whose row slot is read / written), low face first then high face;
  * n_pack / n_unpack: entries per face; psi_send / psi_recv: fluid nodes per face of the psi
  * exchange; *n_owned: fluid nodes of the owned planes. */
-int lbm_build_slab_halo(const uint8_t* solid_local, int nx, int ny, int nz_local,
-                        int32_t* pack_dir_vox, int32_t* unpack_dir_vox, long long cap,
+int lbm_build_slab_halo(const uint8_t* solid_local, int nx, int ny, int nz_local, int z_open,
+                        int halo_lo, int halo_hi, int32_t* pack_dir_vox, int32_t* unpack_dir_vox, long long cap,
                         long long n_pack[2], long long n_unpack[2], long long psi_send[2],
                         long long psi_recv[2], long long* n_owned);
 

@@ -16,7 +16,7 @@ const int kOpp[kQ] = {0, 2, 1, 4, 3, 6, 5, 10, 9, 8, 7, 14, 13, 12, 11, 18, 17, 
 namespace {
 
 struct Box {
-  int nx, ny, nz, z_open;
+  int nx, ny, nz, open_lo, open_hi;
   // voxel index of (x,y,z)+e_i; *beyond = the true neighbour lies past an open plane and the
   // returned voxel is its mirror image across that plane.
   inline long long nb(int x, int y, int z, int i, bool* beyond) const {
@@ -25,8 +25,8 @@ struct Box {
     if (yn < 0) yn += ny; else if (yn >= ny) yn -= ny;
     *beyond = false;
     if (zn < 0 || zn >= nz) {
-      if (z_open) { *beyond = true; zn = z - kE[i][2]; }
-      else zn = zn < 0 ? zn + nz : zn - nz;
+      if (zn < 0 ? open_lo : open_hi) { *beyond = true; zn = z - kE[i][2]; }
+      else zn = zn < 0 ? zn + nz : zn - nz;  // periodic; across a halo end: never read
     }
     return (long long)xn + (long long)nx * ((long long)yn + (long long)ny * (long long)zn);
   }
@@ -35,27 +35,31 @@ struct Box {
 }  // namespace
 
 int build(Geometry& g, const uint8_t* solid, int nx, int ny, int nz, int z_open,
-          bool with_tables, int ghost) {
+          bool with_tables, int ghost_lo, int ghost_hi) {
   if (!solid || nx < 1 || ny < 1 || nz < 1) return -1;
-  if (ghost < 0 || (ghost > 0 && (z_open || nz < 2 * ghost + 2))) return -1;
+  if ((ghost_lo != 0 && ghost_lo != kSlabGhost) || (ghost_hi != 0 && ghost_hi != kSlabGhost)) return -1;
+  if (!z_open && ghost_lo != ghost_hi) return -1;
+  if ((ghost_lo || ghost_hi) && nz < ghost_lo + ghost_hi + 2) return -1;
+  const int open_lo = z_open && !ghost_lo, open_hi = z_open && !ghost_hi;
   const long long nvox = (long long)nx * ny * nz;
   if (nvox >= (1LL << 31)) return -1;
   if (z_open && nz < 4) return -1;
   const long long np = (long long)nx * ny;
-  if (z_open) {
+  {
     const int zs[4] = {0, 1, nz - 2, nz - 1};
     for (int k = 0; k < 4; ++k)
-      for (long long q = 0; q < np; ++q)
-        if (solid[(long long)zs[k] * np + q]) return -3;
+      if (k < 2 ? open_lo : open_hi)
+        for (long long q = 0; q < np; ++q)
+          if (solid[(long long)zs[k] * np + q]) return -3;
   }
   g.nx = nx; g.ny = ny; g.nz = nz; g.z_open = z_open ? 1 : 0; g.nvox = nvox;
-  g.ghost = ghost;
-  const Box box{nx, ny, nz, g.z_open};
+  g.ghost_lo = ghost_lo; g.ghost_hi = ghost_hi; g.open_lo = open_lo; g.open_hi = open_hi;
+  const Box box{nx, ny, nz, open_lo, open_hi};
   try {
     g.vox2id.assign(nvox, -1);
     long long nf = 0;
     // owned planes first, then the low halo planes, then the high ones (ghost = 0: plain raster)
-    const long long v_lo = (long long)ghost * np, v_hi = nvox - (long long)ghost * np;
+    const long long v_lo = (long long)ghost_lo * np, v_hi = nvox - (long long)ghost_hi * np;
     for (long long v = v_lo; v < v_hi; ++v)
       if (!solid[v]) g.vox2id[v] = (int32_t)nf++;
     g.nact = nf;
@@ -312,8 +316,9 @@ int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Ind
 }
 
 int build_halo(const Geometry& g, const uint8_t* solid, size_t npad, Halo& h) {
-  if (g.ghost != kSlabGhost || !solid) return -1;
-  const int nx = g.nx, ny = g.ny, nz = g.nz, G = g.ghost;
+  if (!solid) return -1;
+  const int nx = g.nx, ny = g.ny, nz = g.nz, G = kSlabGhost;
+  const int gl = g.ghost_lo, gh = g.ghost_hi;
   const long long np = (long long)nx * ny;
   // directions that cross the low cut (e_z = -1) and the high cut (e_z = +1)
   static const int kCross[2][5] = {{6, 13, 14, 17, 18}, {5, 11, 12, 15, 16}};
@@ -321,9 +326,10 @@ int build_halo(const Geometry& g, const uint8_t* solid, size_t npad, Halo& h) {
     for (int face = 0; face < 2; ++face) {
       h.pack[face].clear();
       h.unpack[face].clear();
+      if ((face == 0 ? gl : gh) == 0) continue;            // the global box's end: nothing crosses
       // pack: what my owned boundary plane pushed into the inner halo plane of this face
-      const int z_halo = face == 0 ? G - 1 : nz - G;       // inner halo plane
-      const int z_own = face == 0 ? G : nz - G - 1;        // owned boundary plane
+      const int z_halo = face == 0 ? gl - 1 : nz - gh;     // inner halo plane
+      const int z_own = face == 0 ? gl : nz - gh - 1;      // owned boundary plane
       for (int k = 0; k < 5; ++k) {
         const int i = kCross[face][k];       // travels from z_own to z_halo
         const int j = kCross[1 - face][k];   // arrives at z_own from z_halo (neighbour's push)
@@ -352,17 +358,17 @@ int build_halo(const Geometry& g, const uint8_t* solid, size_t npad, Halo& h) {
       for (long long v = z0 * np; v < z1 * np; ++v) c += solid[v] ? 0 : 1;
       return c;
     };
-    const long long n_lo = count(0, G), n_hi = count(nz - G, nz);
+    const long long n_lo = count(0, gl), n_hi = count(nz - gh, nz);
     h.psi_send[0][0] = 0;
-    h.psi_send[0][1] = count(G, 2 * G);
-    h.psi_send[1][1] = count(nz - 2 * G, nz - G);
+    h.psi_send[0][1] = gl ? count(gl, gl + G) : 0;
+    h.psi_send[1][1] = gh ? count(nz - gh - G, nz - gh) : 0;
     h.psi_send[1][0] = g.nact - h.psi_send[1][1];
     h.psi_recv[0][0] = g.nact;
     h.psi_recv[0][1] = n_lo;
     h.psi_recv[1][0] = g.nact + n_lo;
     h.psi_recv[1][1] = n_hi;
-    h.edge_plane[0] = count(G, G + 1);
-    h.edge_plane[1] = count(nz - G - 1, nz - G);
+    h.edge_plane[0] = count(gl, gl + 1);
+    h.edge_plane[1] = count(nz - gh - 1, nz - gh);
   } catch (const std::bad_alloc&) {
     return -4;
   }

@@ -21,8 +21,11 @@ struct Geometry {
   // Slab mode (multi-GPU z-slabs): the box carries `ghost` halo planes
   // at each z end.  Fluid nodes of the owned planes get ids [0, nact) in raster order, the halo
   // nodes ids [nact, nf): low halo planes first, then the high ones, each in raster order.
-  // ghost = 0: nact = nf and the ids are plain raster order.
-  int ghost = 0;
+  // No halo: nact = nf and the ids are plain raster order.  An end of the box with halo planes is
+  // a cut; an end without is the global box's end: an open plane there if z_open (open_lo /
+  // open_hi), else periodic (then both ends have halo planes or neither has).
+  int ghost_lo = 0, ghost_hi = 0;
+  int open_lo = 0, open_hi = 0;
   long long nact = 0;
   std::vector<int32_t> vox2id;    // [nvox]  fluid id | nf + wall id | -1
   std::vector<int32_t> node_vox;  // [nf]    voxel index of fluid node n
@@ -76,10 +79,11 @@ int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Ind
 // neighbour plane (z in {0,1,nz-2,nz-1}), -4 out of memory.  `with_tables` = also fill nbr,
 // wall_nbr, wall_inv_den.
 int build(Geometry& g, const uint8_t* solid, int nx, int ny, int nz, int z_open, bool with_tables,
-          int ghost = 0);
+          int ghost_lo = 0, int ghost_hi = 0);
 
-// Halo lists of a slab (ghost = kSlabGhost planes per side; z local: [0,ghost) low halo,
-// [ghost, nz-ghost) owned, [nz-ghost, nz) high halo).  After the fused pass the populations an
+// Halo lists of a slab (ghost_lo, ghost_hi in {0, kSlabGhost}; z local: [0,ghost_lo) low halo,
+// [ghost_lo, nz-ghost_hi) owned, [nz-ghost_hi, nz) high halo; a face without halo planes has
+// empty lists).  After the fused pass the populations an
 // owned boundary-plane node pushed across the cut sit in the rows of the inner halo plane's
 // nodes; they are packed into one message per face and, on the neighbour slab, unpacked into the
 // same rows of its owned boundary plane.  An entry exists for (direction i crossing the cut,

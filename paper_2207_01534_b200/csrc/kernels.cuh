@@ -593,7 +593,8 @@ constexpr int kIdxMeta = 40;
 struct Idx16 {
   const uint16_t* nbr16;  // [18][npad]
   const int* meta;        // [tiles][kIdxMeta]
-  int np;                 // nodes per open plane (nx*ny) when z is open, else 0
+  int np_lo, np_hi;       // nodes per open plane (nx*ny) at the low / high z end, 0 if that end is
+                          // not an open plane (periodic, or a slab cut)
   int reverse;            // 1: CTA b takes tile gridDim-1-b
   int nact;               // nodes this pass updates: ids [0,nact).  = nf, except in slab mode, where
                           // the halo nodes [nact,nf) only receive pushes
@@ -672,7 +673,7 @@ __global__ void __launch_bounds__(TN, MINB)
     } else {
       // decode this thread's column into the int32 form the tile function reads; a neighbour
       // beyond an open plane (reading R12 iv) is recognised from the node's plane and e_z
-      const bool lo_plane = n < ix.np, hi_plane = n >= nf - ix.np;
+      const bool lo_plane = n < ix.np_lo, hi_plane = n >= ix.nact - ix.np_hi;
 #pragma unroll
       for (int i = 1; i < Q; ++i) {
         const int e = s16[(i - 1) * TN + tid];
@@ -863,7 +864,8 @@ __global__ void __launch_bounds__(TN, MINB)
 template <typename T>
 struct OpenPlane {
   int dc[2];       // Dirichlet component at inlet / outlet
-  int kind[2];     // 1 density (NEEM), 2 velocity (NEEM), 3 density (Zou-He), 4 velocity (Zou-He)
+  int kind[2];     // 1 density (NEEM), 2 velocity (NEEM), 3 density (Zou-He), 4 velocity (Zou-He);
+                   // 0: that end of this box is not an open plane (a slab cut)
   T rho[2];        // imposed density (kinds 1, 3)
   T uz[2];         // imposed velocity (kinds 2, 4)
 };
@@ -995,6 +997,7 @@ __global__ void __launch_bounds__(128) k_open_planes(T* __restrict__ f,
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= 2 * np) return;
   const int plane = t / np;
+  if (op.kind[plane] == 0) return;
   open_plane_node<T>(f, frozen, nf, np, npad, op, plane, t - plane * np);
 }
 
@@ -1006,12 +1009,16 @@ __global__ void __launch_bounds__(128) k_open_planes(T* __restrict__ f,
 template <typename T>
 __global__ void __launch_bounds__(256, 4)
     k_density_open(T* __restrict__ f, Vec2<T>* __restrict__ psi, const T* __restrict__ frozen,
-                   int nf, int np, size_t npad, int nb_planes, OpenPlane<T> op, float keep_psi) {
+                   int nf, int np, size_t npad, int nb_planes, OpenPlane<T> op, float keep_psi,
+                   NodeRange r) {
+  // nf = number of nodes this context updates (all fluid nodes; the owned ones in slab mode)
   pdl_wait();  // f was written by the previous step's fused pass
   const uint64_t pol = l2_keep_policy(keep_psi);
   if ((int)blockIdx.x >= nb_planes) {
-    const int n = ((int)blockIdx.x - nb_planes) * blockDim.x + threadIdx.x;
-    if (n >= nf || n < np || n >= nf - np) return;
+    const int b = (int)blockIdx.x - nb_planes;
+    const int n = (b < r.split ? r.a0 + b * (int)blockDim.x : r.a1 + (b - r.split) * (int)blockDim.x) +
+                  (int)threadIdx.x;
+    if (n >= r.nend || (op.kind[0] && n < np) || (op.kind[1] && n >= nf - np)) return;
     const Vec2<T>* f2 = reinterpret_cast<const Vec2<T>*>(f);
     Vec2<T> v[Q];
 #pragma unroll
@@ -1025,6 +1032,7 @@ __global__ void __launch_bounds__(256, 4)
     const int t = (int)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= 2 * np) return;
     const int plane = t / np, q = t - plane * np;
+    if (op.kind[plane] == 0) return;
     store_vec2(psi + (plane == 0 ? q : nf - np + q),
                open_plane_node<T>(f, frozen, nf, np, npad, op, plane, q), pol);
   }
@@ -1056,10 +1064,11 @@ __global__ void __launch_bounds__(256) k_halo_unpack(T* __restrict__ f,
 // frozen[plane][comp][k][q] <- f[comp][inward(plane,k)][plane node q]   (reading R27)
 template <typename T>
 __global__ void k_record_frozen(const T* __restrict__ f, T* __restrict__ frozen, int comp, int nf,
-                                int np, size_t npad) {
+                                int np, size_t npad, int planes /* bit p: plane p is open */) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= 2 * np) return;
   const int plane = t / np, q = t - plane * np;
+  if (!((planes >> plane) & 1)) return;
   const int vb = plane == 0 ? q : nf - np + q;
 #pragma unroll
   for (int k = 0; k < 5; ++k) {

@@ -72,7 +72,8 @@ struct lbm_ctx {
   long long nvox = 0;
   int nf = 0, nw = 0;
   int nact = 0;             // ids [0,nact) are updated by this context; = nf unless slab mode
-  int slab = 0;             // 1: z-slab of a larger box with kSlabGhost halo planes per side
+  int slab = 0;             // 1: z-slab of a larger box (halo planes at the ends that are cuts)
+  int open_end[2] = {0, 0}; // this box's low / high z end is an open plane (inlet / outlet)
   int* halo_slots = nullptr;         // [pack low | pack high | unpack low | unpack high] pair slots
   void* halo_send = nullptr;         // [pack low | pack high] (A,B) pairs
   void* halo_recv = nullptr;         // [unpack low | unpack high] (A,B) pairs
@@ -152,10 +153,10 @@ Consts<T> make_consts(const lbm_params& p) {
 }
 
 template <typename T>
-OpenPlane<T> make_open(const lbm_params& p) {
+OpenPlane<T> make_open(const lbm_params& p, const int (&open_end)[2]) {
   OpenPlane<T> o;
   o.dc[0] = p.inlet_comp; o.dc[1] = p.outlet_comp;
-  o.kind[0] = p.inlet_kind; o.kind[1] = p.outlet_kind;
+  o.kind[0] = open_end[0] ? p.inlet_kind : 0; o.kind[1] = open_end[1] ? p.outlet_kind : 0;
   o.rho[0] = (T)p.inlet_rho; o.rho[1] = (T)p.outlet_rho;
   o.uz[0] = (T)p.inlet_uz; o.uz[1] = (T)0;
   return o;
@@ -203,15 +204,21 @@ void launch_density(lbm_ctx* c, cudaStream_t st, int part = -1) {
   T* fin = (T*)c->f[c->cur];
   const bool pdl = c->pdl && !c->prof;  // events between the launches would serialise them anyway
   Timed t(c, st, 0);
-  if (c->open_pending) {  // a0 of the previous step rides along (k_density_open)
+  NodeRange r{0, (int)blocks(c->nact, 256), 0, c->nact};
+  unsigned grid = blocks(c->nact, 256);
+  if (c->open_pending && part != 1) {  // a0 of the previous step rides along (k_density_open);
+    // in slab mode with the boundary launch: the open planes lie inside the boundary id ranges
     const unsigned nbp = blocks(2LL * c->np, 256);
-    launch_k(pdl, k_density_open<T>, nbp + blocks(c->nf, 256), 256, 0, st, fin,
-             (Vec2<T>*)c->psi, (const T*)c->frozen, c->nf, c->np, c->npad, (int)nbp,
-             make_open<T>(c->p), c->keep_psi);
+    if (part == 0) {
+      r.split = c->bnd_lo1 / 256;
+      r.a1 = c->bnd_hi0;
+      grid = (unsigned)r.split + blocks(c->nact - c->bnd_hi0, 256);
+    }
+    launch_k(pdl, k_density_open<T>, nbp + grid, 256, 0, st, fin,
+             (Vec2<T>*)c->psi, (const T*)c->frozen, c->nact, c->np, c->npad, (int)nbp,
+             make_open<T>(c->p, c->open_end), c->keep_psi, r);
     c->open_pending = false;
   } else {
-    NodeRange r{0, (int)blocks(c->nact, 256), 0, c->nact};
-    unsigned grid = blocks(c->nact, 256);
     if (part == 0) {
       r.split = c->bnd_lo1 / 256;
       r.a1 = c->bnd_hi0;
@@ -255,8 +262,8 @@ template <typename T>
 void apply_pending_T(lbm_ctx* c, cudaStream_t st) {
   if (!c->open_pending) return;
   k_open_planes<T><<<blocks(2LL * c->np, 128), 128, 0, st>>>((T*)c->f[c->cur], (const T*)c->frozen,
-                                                             c->nf, c->np, c->npad,
-                                                             make_open<T>(c->p));
+                                                             c->nact, c->np, c->npad,
+                                                             make_open<T>(c->p, c->open_end));
   c->open_pending = false;
 }
 void apply_pending(lbm_ctx* c, cudaStream_t st) {
@@ -276,7 +283,8 @@ void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
   Idx16 ix;
   ix.nbr16 = c->nbr16;
   ix.meta = c->nbr16_meta;
-  ix.np = c->p.z_open ? c->np : 0;
+  ix.np_lo = c->open_end[0] ? c->np : 0;
+  ix.np_hi = c->open_end[1] ? c->np : 0;
   ix.reverse = c->reverse;
   ix.nact = c->nact;
   static_assert(TN == 128 || TN == 256, "tile ranges below are in units of 128 ids");
@@ -371,7 +379,7 @@ int launch_fused(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
 template <typename T>
 int step_T(lbm_ctx* c, int n, cudaStream_t st) {
   const Consts<T> k = make_consts<T>(c->p);
-  const OpenPlane<T> op = make_open<T>(c->p);
+  const OpenPlane<T> op = make_open<T>(c->p, c->open_end);
   for (int it = 0; it < n; ++it) {
     const T* fin = (const T*)c->f[c->cur];
     T* fout = (T*)c->f[c->cur ^ 1];
@@ -404,10 +412,10 @@ int step_T(lbm_ctx* c, int n, cudaStream_t st) {
 
 template <typename T>
 int record_frozen_T(lbm_ctx* c, int comp, cudaStream_t st) {
-  if (!c->p.z_open) return LBM_OK;
-  k_record_frozen<T><<<blocks(2LL * c->np, 128), 128, 0, st>>>((const T*)c->f[c->cur],
-                                                               (T*)c->frozen, comp, c->nf, c->np,
-                                                               c->npad);
+  if (!c->open_end[0] && !c->open_end[1]) return LBM_OK;
+  k_record_frozen<T><<<blocks(2LL * c->np, 128), 128, 0, st>>>(
+      (const T*)c->f[c->cur], (T*)c->frozen, comp, c->nact, c->np, c->npad,
+      c->open_end[0] | (c->open_end[1] << 1));
   CU(cudaPeekAtLastError());
   return LBM_OK;
 }
@@ -477,16 +485,22 @@ int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open,
 }
 
 static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz,
-                       const lbm_params* p, int ghost) {
+                       const lbm_params* p, bool slab, int halo_lo, int halo_hi) {
   if (!out || !solid || !p) return fail(LBM_EINVAL, "NULL argument");
   if (nx < 1 || ny < 1 || nz < 1) return fail(LBM_EINVAL, "box dimensions must be positive");
   if (int rc = validate_params(p, nz)) return rc;
-  if (ghost && p->z_open) return fail(LBM_EINVAL, "slab mode needs z_open = 0");
-  if (ghost && nz < 2 * ghost + 2)
-    return fail(LBM_EINVAL, "a slab needs >= 2 owned planes plus %d halo planes per side", ghost);
+  if (slab && ((halo_lo != 0 && halo_lo != 1) || (halo_hi != 0 && halo_hi != 1)))
+    return fail(LBM_EINVAL, "halo_lo / halo_hi must be 0 or 1");
+  if (slab && !p->z_open && !(halo_lo && halo_hi))
+    return fail(LBM_EINVAL, "a slab of a z-periodic box is a cut at both ends (halo_lo = halo_hi = 1)");
+  const int ghost_lo = slab && halo_lo ? lbmgeo::kSlabGhost : 0;
+  const int ghost_hi = slab && halo_hi ? lbmgeo::kSlabGhost : 0;
+  if (slab && nz < ghost_lo + ghost_hi + 2)
+    return fail(LBM_EINVAL, "a slab needs >= 2 owned planes plus %d halo planes per cut end",
+                lbmgeo::kSlabGhost);
   lbmgeo::Geometry g;
   {
-    const int rc = lbmgeo::build(g, solid, nx, ny, nz, p->z_open, true, ghost);
+    const int rc = lbmgeo::build(g, solid, nx, ny, nz, p->z_open, true, ghost_lo, ghost_hi);
     if (rc == -2) return fail(LBM_ENOFLUID, "the mask has no fluid voxel");
     if (rc == -3) return fail(LBM_ESOLIDOPEN, "solid voxel on an open plane or its neighbour plane");
     if (rc == -4) return fail(LBM_ENOMEM, "host allocation failed");
@@ -506,7 +520,8 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   c->p = *p;
   c->nx = nx; c->ny = ny; c->nz = nz; c->np = nx * ny; c->nvox = g.nvox;
   c->nf = (int)g.nf; c->nw = (int)g.nw;
-  c->nact = (int)g.nact; c->slab = ghost > 0 ? 1 : 0;
+  c->nact = (int)g.nact; c->slab = slab ? 1 : 0;
+  c->open_end[0] = g.open_lo; c->open_end[1] = g.open_hi;
   c->bits = p->storage_bits; c->esz = p->storage_bits / 8;
   if (const char* e = std::getenv("LBM_B200_COLLIDE")) c->collide_variant = !std::strcmp(e, "simple") ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_TILE")) c->tile = std::atoi(e);
@@ -645,8 +660,11 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
     }
     {  // boundary-first launch ranges (ids in units of 256, tiles of 128)
       const long long na = g.nact;
-      long long hi0 = std::max(0LL, na - halo.psi_send[1][1]) / 256 * 256;
-      long long lo1 = std::min((long long)pad256(halo.psi_send[0][1]), hi0);
+      // an open end's plane rides in the boundary launch too (its deferred fix needs it there)
+      const long long n_hi = g.open_hi ? c->np : halo.psi_send[1][1];
+      const long long n_lo = g.open_lo ? c->np : halo.psi_send[0][1];
+      long long hi0 = std::max(0LL, na - n_hi) / 256 * 256;
+      long long lo1 = std::min((long long)pad256(n_lo), hi0);
       c->bnd_lo1 = (int)lo1; c->bnd_hi0 = (int)hi0;
       c->tile_lo1 = (int)((halo.edge_plane[0] + 127) / 128);
       c->tile_hi0 = (int)(std::max(0LL, na - halo.edge_plane[1]) / 128);
@@ -675,15 +693,16 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   return LBM_OK;
 }
 
-int lbm_build_slab_halo(const uint8_t* solid_local, int nx, int ny, int nz_local,
-                        int32_t* pack_dir_vox, int32_t* unpack_dir_vox, long long cap,
+int lbm_build_slab_halo(const uint8_t* solid_local, int nx, int ny, int nz_local, int z_open,
+                        int halo_lo, int halo_hi, int32_t* pack_dir_vox, int32_t* unpack_dir_vox, long long cap,
                         long long n_pack[2], long long n_unpack[2], long long psi_send[2],
                         long long psi_recv[2], long long* n_owned) {
   if (!solid_local || !pack_dir_vox || !unpack_dir_vox || !n_pack || !n_unpack || !psi_send ||
       !psi_recv || !n_owned)
     return fail(LBM_EINVAL, "NULL argument");
   lbmgeo::Geometry g;
-  const int rc = lbmgeo::build(g, solid_local, nx, ny, nz_local, 0, false, lbmgeo::kSlabGhost);
+  const int rc = lbmgeo::build(g, solid_local, nx, ny, nz_local, z_open, false,
+                               halo_lo ? lbmgeo::kSlabGhost : 0, halo_hi ? lbmgeo::kSlabGhost : 0);
   if (rc) return fail(rc == -2 ? LBM_ENOFLUID : LBM_EINVAL, "geometry build failed (%d)", rc);
   const size_t npad = pad256(g.nf);
   lbmgeo::Halo h;
@@ -708,12 +727,12 @@ int lbm_build_slab_halo(const uint8_t* solid_local, int nx, int ny, int nz_local
 }
 
 int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, const lbm_params* p) {
-  return create_impl(out, solid, nx, ny, nz, p, 0);
+  return create_impl(out, solid, nx, ny, nz, p, false, 0, 0);
 }
 
 int lbm_create_slab(lbm_ctx** out, const uint8_t* solid_local, int nx, int ny, int nz_local,
-                    const lbm_params* p) {
-  return create_impl(out, solid_local, nx, ny, nz_local, p, lbmgeo::kSlabGhost);
+                    const lbm_params* p, int halo_lo, int halo_hi) {
+  return create_impl(out, solid_local, nx, ny, nz_local, p, true, halo_lo, halo_hi);
 }
 
 long long lbm_num_owned(lbm_ctx* c) { return c ? c->nact : -1; }
@@ -748,7 +767,10 @@ static int slab_collide_T(lbm_ctx* c, int part, cudaStream_t st) {
     k_halo_pack<T><<<blocks(np, 256), 256, 0, st>>>((const T*)fout, c->halo_slots,
                                                     (T*)c->halo_send, np);
   }
-  if (part == 1) c->cur ^= 1;
+  if (part == 1) {
+    c->cur ^= 1;
+    if (c->open_end[0] || c->open_end[1]) c->open_pending = true;  // a0 rides in the next density(0)
+  }
   CU(cudaPeekAtLastError());
   return LBM_OK;
 }
@@ -835,6 +857,8 @@ int lbm_memory_bytes(lbm_ctx* c, long long bytes[4]) {
 int lbm_set_boundary(lbm_ctx* c, double inlet_value, double outlet_rho) {
   if (!c) return fail(LBM_EINVAL, "NULL context");
   if (!c->p.z_open) return fail(LBM_EINVAL, "z is periodic: no boundary values to set");
+  if (c->slab && c->slab_phase > 2)
+    return fail(LBM_EINVAL, "slab context: lbm_set_boundary is not allowed inside a step");
   if (!std::isfinite(inlet_value) || !std::isfinite(outlet_rho))
     return fail(LBM_EINVAL, "boundary values must be finite");
   if (int rc = check_ctx(c)) return rc;
@@ -1029,7 +1053,9 @@ int lbm_diagnostics(lbm_ctx* c, double mass[2], double momentum[3]) {
 
 int lbm_saturation(lbm_ctx* c, int comp, int z0, int z1, double* S) {
   if (int rc = check_ctx(c)) return rc;
-  if (c->slab) return fail(LBM_EINVAL, "lbm_saturation is not available on a slab context");
+  if (c->slab && c->slab_phase != 2)
+    return fail(LBM_EINVAL, "slab context: lbm_saturation needs both lbm_slab_density parts and the psi "
+                            "exchange on the current state");
   if (!S || comp < 0 || comp > 1 || z0 < 0 || z1 > c->nz || z0 >= z1)
     return fail(LBM_EINVAL, "bad argument");
   const int n0 = c->zstart[z0], n1 = c->zstart[z1];
@@ -1110,7 +1136,9 @@ int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, d
 
 int lbm_mean_pressure(lbm_ctx* c, int z0, int z1, double* P) {
   if (int rc = check_ctx(c)) return rc;
-  if (c->slab) return fail(LBM_EINVAL, "lbm_mean_pressure is not available on a slab context");
+  if (c->slab && c->slab_phase != 2)
+    return fail(LBM_EINVAL, "slab context: lbm_mean_pressure needs both lbm_slab_density parts and the psi "
+                            "exchange on the current state");
   if (!P || z0 < 0 || z1 > c->nz || z0 >= z1) return fail(LBM_EINVAL, "bad argument");
   const int n0 = c->zstart[z0], n1 = c->zstart[z1];
   if (n1 <= n0) return fail(LBM_ENOFLUID, "no fluid node in the z-range");

@@ -86,14 +86,14 @@ def load():
     lib.lbm_last_error.restype = C.c_char_p
     lib.lbm_build_index.argtypes = [V, I, I, I, I, V, V, LL, C.POINTER(LL), C.POINTER(LL)]
     lib.lbm_build_schedule.argtypes = [V, I, I, I, I, I, I, V, LL, C.POINTER(LL)]
-    lib.lbm_create_slab.argtypes = [C.POINTER(P), V, I, I, I, C.POINTER(lbm_params)]
+    lib.lbm_create_slab.argtypes = [C.POINTER(P), V, I, I, I, C.POINTER(lbm_params), I, I]
     lib.lbm_slab_density.argtypes = [P, I]
     lib.lbm_slab_collide.argtypes = [P, I]
     lib.lbm_slab_unpack.argtypes = [P]
     lib.lbm_slab_buffer.argtypes = [P, I, C.POINTER(C.c_void_p), C.POINTER(LL)]
     lib.lbm_num_owned.argtypes = [P]
     lib.lbm_num_owned.restype = LL
-    lib.lbm_build_slab_halo.argtypes = [V, I, I, I, V, V, LL] + [C.POINTER(LL)] * 5
+    lib.lbm_build_slab_halo.argtypes = [V, I, I, I, I, I, I, V, V, LL] + [C.POINTER(LL)] * 5
     for fn in ("lbm_create_slab", "lbm_slab_density", "lbm_slab_collide", "lbm_slab_unpack",
                "lbm_slab_buffer", "lbm_build_slab_halo"):
         getattr(lib, fn).restype = I
@@ -159,8 +159,9 @@ def lbm_build_schedule(mask, z_open=0, tile=128, lead=256):
     return rec[:n.value]
 
 
-def lbm_build_slab_halo(mask_local):
-    """Host-only: the halo lists lbm_create_slab builds for a local mask [owned + 4, y, x].
+def lbm_build_slab_halo(mask_local, z_open=0, halo=(1, 1)):
+    """Host-only: the halo lists lbm_create_slab builds for a local mask [owned + halo planes, y, x];
+    halo = (low, high): 1 = that end is a cut with 2 halo planes, 0 = the open box's own end.
     Returns a dict: pack / unpack = per face (low, high) an int32 array [n, 2] of (direction,
     local voxel index); psi_send / psi_recv = fluid nodes per face; n_owned."""
     lib = load()
@@ -172,7 +173,8 @@ def lbm_build_slab_halo(mask_local):
     arr = lambda: (C.c_longlong * 2)()
     n_pack, n_unpack, ps, pr = arr(), arr(), arr(), arr()
     n_owned = C.c_longlong()
-    _chk(lib.lbm_build_slab_halo(mask_local.ctypes.data, nx, ny, nz, pk.ctypes.data,
+    _chk(lib.lbm_build_slab_halo(mask_local.ctypes.data, nx, ny, nz, int(z_open), int(halo[0]),
+                                 int(halo[1]), pk.ctypes.data,
                                  up.ctypes.data, cap, n_pack, n_unpack, ps, pr,
                                  C.byref(n_owned)), "lbm_build_slab_halo")
     return {"pack": (pk[:n_pack[0]].copy(), pk[n_pack[0]:n_pack[0] + n_pack[1]].copy()),
@@ -183,9 +185,10 @@ def lbm_build_slab_halo(mask_local):
 
 class Lbm:
     """One simulation on the current CUDA device. Methods mirror the C ABI one to one.
-    slab=True: a z-slab context (lbm_create_slab; mask = owned planes + 2 halo planes per end)."""
+    slab=True: a z-slab context (lbm_create_slab; mask = owned planes + 2 halo planes per cut
+    end; halo = (low, high) flags, 0 only at the ends of a z-open box)."""
 
-    def __init__(self, mask, params, slab=False):
+    def __init__(self, mask, params, slab=False, halo=(1, 1)):
         lib = load()
         import torch
         if torch.cuda.is_available():
@@ -202,7 +205,7 @@ class Lbm:
         self.slab = bool(slab)
         if slab:
             _chk(lib.lbm_create_slab(C.byref(self._h), mask.ctypes.data, nx, ny, nz,
-                                     C.byref(ps)), "lbm_create_slab")
+                                     C.byref(ps), int(halo[0]), int(halo[1])), "lbm_create_slab")
         else:
             _chk(lib.lbm_create(C.byref(self._h), mask.ctypes.data, nx, ny, nz, C.byref(ps)),
                  "lbm_create")

@@ -51,16 +51,22 @@ def partition(mask, parts):
     return [(cuts[k], cuts[k + 1]) for k in range(parts)]
 
 
-def local_planes(nz, z0, z1):
-    """Global z index of every plane of the slab's local box (halo planes wrap periodically)."""
-    return np.arange(z0 - GHOST, z1 + GHOST) % nz
+def local_planes(nz, z0, z1, halo=(1, 1)):
+    """Global z index of every plane of the slab's local box: the owned planes [z0, z1) plus GHOST
+    halo planes at each end that is a cut (they wrap periodically)."""
+    return np.arange(z0 - GHOST * halo[0], z1 + GHOST * halo[1]) % nz
 
 
-def local_box(a, z0, z1):
+def local_box(a, z0, z1, halo=(1, 1)):
     """Slice a global [z, y, x] (or [q, z, y, x]) array to the slab's local box."""
     a = np.asarray(a)
     ax = a.ndim - 3
-    return np.ascontiguousarray(np.take(a, local_planes(a.shape[ax], z0, z1), axis=ax))
+    return np.ascontiguousarray(np.take(a, local_planes(a.shape[ax], z0, z1, halo), axis=ax))
+
+
+def halo_flags(r, parts, z_open):
+    """(low, high): 1 = that end of slab r is a cut; 0 = the end of a z-open box."""
+    return (0 if (z_open and r == 0) else 1, 0 if (z_open and r == parts - 1) else 1)
 
 
 class _DeviceBytes:
@@ -127,7 +133,8 @@ class RingTransport:
 
 
 class SlabLbm:
-    """A z-periodic simulation cut into z-slabs.
+    """A simulation cut into z-slabs (z periodic, or z open with the inlet plane on the first and
+    the outlet plane on the last slab).
 
     world=None: all `parts` slabs are created in this process on the current GPU and stepped one
     after another (validation of the sharded path on one GPU).
@@ -139,14 +146,17 @@ class SlabLbm:
 
     def __init__(self, mask, params, parts=None, rank=None, world=None, group=None):
         mask = np.ascontiguousarray(mask, np.uint8)
-        if int(params["z_open"]) != 0:
-            raise ValueError("slab sharding needs a z-periodic box (z_open = 0)")
         self.shape = mask.shape
         self.world = world
+        self.z_open = int(params["z_open"]) != 0
         nparts = world if world is not None else (parts or 1)
         self.ranges = partition(mask, nparts)
         self.mine = [rank] if world is not None else list(range(nparts))
-        self.sims = [Lbm(local_box(mask, *self.ranges[r]), params, slab=True) for r in self.mine]
+        self.halo = [halo_flags(r, nparts, self.z_open) for r in range(nparts)]
+        self.sims = [Lbm(local_box(mask, *self.ranges[r], self.halo[r]), params, slab=True,
+                         halo=self.halo[r]) for r in self.mine]
+        # fluid nodes per global plane (host copy of the mask statistics the queries weight with)
+        self._plane_fluid = (mask.reshape(mask.shape[0], -1) == 0).sum(axis=1).astype(np.int64)
         self.num_fluid = sum(s.num_owned for s in self.sims)
         self._ring = RingTransport(rank, world, group) if world is not None else None
         self._buf = [[buffer_tensor(s, w) for w in range(8)] for s in self.sims]
@@ -200,22 +210,62 @@ class SlabLbm:
     def set_density(self, rhoA, rhoB):
         for s, r in zip(self.sims, self.mine):
             z0, z1 = self.ranges[r]
-            s.set_density(local_box(rhoA, z0, z1), local_box(rhoB, z0, z1))
+            s.set_density(local_box(rhoA, z0, z1, self.halo[r]),
+                          local_box(rhoB, z0, z1, self.halo[r]))
 
     def set_populations(self, comp, f):
         for s, r in zip(self.sims, self.mine):
-            s.set_populations(comp, local_box(f, *self.ranges[r]))
+            s.set_populations(comp, local_box(f, *self.ranges[r], self.halo[r]))
 
-    def _owned(self, a):
-        return a[..., GHOST:a.shape[-3] - GHOST, :, :]
+    def set_boundary(self, inlet_value, outlet_rho):
+        for s in self.sims:
+            s.set_boundary(inlet_value, outlet_rho)
+
+    def _owned(self, a, r):
+        lo, hi = self.halo[r]
+        return a[..., GHOST * lo:a.shape[-3] - GHOST * hi, :, :]
 
     def get_populations(self, comp):
-        return np.concatenate([self._owned(s.get_populations(comp)) for s in self.sims], axis=1)
+        return np.concatenate([self._owned(s.get_populations(comp), r)
+                               for s, r in zip(self.sims, self.mine)], axis=1)
+
+    def _weighted_mean(self, call, z0, z1):
+        """sum over slabs of (plane-range mean x fluid nodes in it) / nodes: how a query over the
+        global planes [z0, z1) is put together from the per-slab library queries (local planes)."""
+        self._density_and_psi_halo()
+        num, den = 0.0, 0
+        for s, r in zip(self.sims, self.mine):
+            a, b = max(z0, self.ranges[r][0]), min(z1, self.ranges[r][1])
+            n = int(self._plane_fluid[a:b].sum()) if b > a else 0
+            if n == 0:
+                continue
+            off = GHOST * self.halo[r][0] - self.ranges[r][0]
+            num += call(s, a + off, b + off) * n
+            den += n
+        if self.world is not None and self.world > 1:
+            import torch
+            import torch.distributed as dist
+            dev = "cuda" if dist.get_backend(self._ring.group) == "nccl" else "cpu"
+            t = torch.tensor([num, float(den)], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, group=self._ring.group)
+            num, den = float(t[0]), int(round(float(t[1])))
+        if den == 0:
+            raise ValueError("no fluid node in the z-range")
+        return num / den
+
+    def saturation(self, comp, z0=0, z1=None):
+        z1 = self.shape[0] if z1 is None else z1
+        return self._weighted_mean(lambda s, a, b: s.saturation(comp, a, b), z0, z1)
+
+    def mean_pressure(self, z0=0, z1=None):
+        z1 = self.shape[0] if z1 is None else z1
+        return self._weighted_mean(lambda s, a, b: s.mean_pressure(a, b), z0, z1)
 
     def get_macroscopic(self, fields=("rhoA", "rhoB", "ux", "uy", "uz", "P")):
         self._density_and_psi_halo()   # the library's slab getter needs psi of the current state
         parts = [s.get_macroscopic(fields) for s in self.sims]
-        return {k: np.concatenate([self._owned(p[k]) for p in parts], axis=0) for k in parts[0]}
+        return {k: np.concatenate([self._owned(p[k], r) for p, r in zip(parts, self.mine)], axis=0)
+                for k in parts[0]}
 
     def diagnostics(self):
         """(mass[2], momentum[3]) over the owned nodes of this process; summed over all ranks when

@@ -190,8 +190,89 @@ def test_slab_error_paths():
         g.slab_density(0)                           # not a slab context
     g.close()
     h = C.c_void_p()
-    ps = make_params(default_params(z_open=1, inlet_kind=1, outlet_kind=1))
-    assert lib.lbm_create_slab(C.byref(h), ml.ctypes.data, 16, 16, 12, C.byref(ps)) == binding.LBM_EINVAL
     ps = make_params(p)
+    # a z-periodic box has no end of its own: both ends of every slab are cuts
+    assert lib.lbm_create_slab(C.byref(h), ml.ctypes.data, 16, 16, 12, C.byref(ps), 0, 1) == binding.LBM_EINVAL
+    assert lib.lbm_create_slab(C.byref(h), ml.ctypes.data, 16, 16, 12, C.byref(ps), 1, 2) == binding.LBM_EINVAL
     thin = np.zeros((5, 4, 4), np.uint8)
-    assert lib.lbm_create_slab(C.byref(h), thin.ctypes.data, 4, 4, 5, C.byref(ps)) == binding.LBM_EINVAL
+    assert lib.lbm_create_slab(C.byref(h), thin.ctypes.data, 4, 4, 5, C.byref(ps), 1, 1) == binding.LBM_EINVAL
+    # the open end of a slab must be solid-free like the open planes of lbm_create (reading R12)
+    po = make_params(default_params(z_open=1, inlet_kind=1, outlet_kind=1))
+    mo = np.zeros((8, 4, 4), np.uint8)
+    mo[1, 2, 2] = 1
+    assert lib.lbm_create_slab(C.byref(h), mo.ctypes.data, 4, 4, 8, C.byref(po), 0, 1) == binding.LBM_ESOLIDOPEN
+    assert lib.lbm_create_slab(C.byref(h), mo.ctypes.data, 4, 4, 8, C.byref(po), 1, 1) == binding.LBM_OK
+    lib.lbm_destroy(h)
+
+
+# ------------------------------------------------------------------ z-open boxes (configs 3, 4)
+
+def _open_case(k, n, bits, **kw):
+    c = make_config(k, size=n, storage_bits=bits, **kw)
+    rng = np.random.Generator(np.random.PCG64(100 + k))
+    fl = c["mask"] == 0
+    for key in ("rhoA", "rhoB"):
+        c[key] = np.where(fl, c[key] * (1.0 + rng.uniform(-1e-3, 1e-3, c[key].shape)), 0.0)
+    return c
+
+
+@pytest.mark.parametrize("k,parts,kinds", [(3, 2, None), (3, 3, (4, 3)), (4, 2, None), (4, 4, (3, 3))])
+def test_open_box_slabs_fp64_bit_identical_and_oracle(k, parts, kinds):
+    """configs 3 (velocity inlet) and 4 (pressure inlet, viscosity ratio 10) at 40^3: the inlet
+    plane lives on the first slab, the outlet plane on the last, middle slabs have none; NEEM
+    (kinds 1, 2) and Zou-He (kinds 3, 4) planes; boundary ramp between the steps."""
+    kw = {} if kinds is None else {"inlet_kind": kinds[0], "outlet_kind": kinds[1]}
+    c = _open_case(k, 40, 64, **kw)
+    g = Lbm(c["mask"], c["params"])
+    s = SlabLbm(c["mask"], c["params"], parts=parts)
+    assert s.halo[0] == (0, 1) and s.halo[-1] == (1, 0)
+    g.set_density(c["rhoA"], c["rhoB"])
+    s.set_density(c["rhoA"], c["rhoB"])
+    g.step(30)
+    s.step(30)
+    _identical_pops(s, g, c["mask"])
+    iv = 1.03 if c["params"]["inlet_kind"] in (1, 3) else 2e-4
+    g.set_boundary(iv, 0.99)
+    s.set_boundary(iv, 0.99)
+    g.step(30)
+    s.step(30)
+    _identical_pops(s, g, c["mask"])
+    mg, ms = g.get_macroscopic(), s.get_macroscopic()
+    for key in mg:
+        assert np.array_equal(mg[key], ms[key]), key
+    nz = c["mask"].shape[0]
+    for z0, z1 in ((0, nz), (8, nz - 8), (0, 1), (nz - 1, nz), (5, 23)):
+        assert abs(s.saturation(1, z0, z1) - g.saturation(1, z0, z1)) < 1e-12
+        assert abs(s.mean_pressure(z0, z1) - g.mean_pressure(z0, z1)) < 1e-12
+    g.step(3)
+    s.step(3)
+    _identical_pops(s, g, c["mask"])
+    if parts == 2:
+        o = LbmRef(c["mask"], c["params"])
+        o.set_density(c["rhoA"], c["rhoB"])
+        o.step(30)
+        o.set_boundary(iv, 0.99)
+        o.step(33)
+        fl = c["mask"] == 0
+        for comp in (0, 1):
+            a, b = s.get_populations(comp)[:, fl], o.get_populations(comp)[:, fl]
+            assert (np.abs(a - b) / np.abs(b)).max() <= 1e-10
+    s.close()
+    g.close()
+
+
+@pytest.mark.parametrize("k,parts", [(3, 3), (4, 2)])
+def test_open_box_slabs_fp32_bit_identical(k, parts):
+    c = _open_case(k, 48, 32)
+    g = Lbm(c["mask"], c["params"])
+    s = SlabLbm(c["mask"], c["params"], parts=parts)
+    g.set_density(c["rhoA"], c["rhoB"])
+    s.set_density(c["rhoA"], c["rhoB"])
+    g.step(100)
+    s.step(100)
+    _identical_pops(s, g, c["mask"])
+    m_g, _ = g.diagnostics()
+    m_s, _ = s.diagnostics()
+    assert np.max(np.abs(m_s - m_g) / m_g) < 1e-12
+    s.close()
+    g.close()

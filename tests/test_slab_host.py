@@ -125,6 +125,33 @@ def test_neighbouring_slabs_agree_on_every_message():
         assert sum(h["n_owned"] for h in hs) == int((m == 0).sum())
 
 
+def test_open_box_slabs_agree_and_have_no_message_at_the_box_ends():
+    from workloads import make_config
+    m = make_config(3, size=32)["mask"]
+    nz, ny, nx = m.shape
+    for parts in (2, 3):
+        ranges = slab.partition(m, parts)
+        flags = [slab.halo_flags(r, parts, True) for r in range(parts)]
+        assert flags[0] == (0, 1) and flags[-1] == (1, 0)
+        hs = [lbm_build_slab_halo(slab.local_box(m, *ranges[r], flags[r]), 1, flags[r])
+              for r in range(parts)]
+        pl = [slab.local_planes(nz, *ranges[r], flags[r]) for r in range(parts)]
+        assert len(hs[0]["pack"][0]) == len(hs[0]["unpack"][0]) == 0
+        assert len(hs[-1]["pack"][1]) == len(hs[-1]["unpack"][1]) == 0
+        assert hs[0]["psi_send"][0] == hs[0]["psi_recv"][0] == 0
+        assert hs[-1]["psi_send"][1] == hs[-1]["psi_recv"][1] == 0
+        for r in range(parts - 1):
+            a = _to_global(hs[r]["pack"][1], pl[r], nx, ny)
+            b = _to_global(hs[r + 1]["unpack"][0], pl[r + 1], nx, ny)
+            assert len(a) > 0 and np.array_equal(a, b)
+            a = _to_global(hs[r + 1]["pack"][0], pl[r + 1], nx, ny)
+            b = _to_global(hs[r]["unpack"][1], pl[r], nx, ny)
+            assert np.array_equal(a, b)
+            assert hs[r]["psi_send"][1] == hs[r + 1]["psi_recv"][0]
+            assert hs[r + 1]["psi_send"][0] == hs[r]["psi_recv"][1]
+        assert sum(h["n_owned"] for h in hs) == int((m == 0).sum())
+
+
 def test_slab_rejects_too_thin_box():
     from paper_2207_01534_b200.lbm import LbmError
     with pytest.raises(LbmError):
