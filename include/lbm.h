@@ -132,6 +132,9 @@ int lbm_memory_bytes(lbm_ctx* c, long long bytes[4]);
  *   LBM_B200_IDX=16|32             16-bit tile-relative neighbour index (default) | int32 rows
  *   LBM_B200_REVERSE=1|0           fused pass walks tiles backwards (default) | forwards
  *   LBM_B200_PDL=1|0               programmatic dependent launch of the three passes (default) | off
+ *   LBM_B200_GRAPH=1|0             lbm_step replays a captured CUDA graph of 16 steps | launches every
+ *                                  kernel from the host (default: graph for boxes of <= 600 000 fluid
+ *                                  nodes, where a step is shorter than its three host launches)
  *   LBM_B200_KEEP_PSI_MB=48        L2 budget (MB) for psi stored with evict_last priority; 0: plain stores
  *   LBM_B200_TILE, LBM_B200_LEAD   CTA shape of the fused pass; producer lead of the fused step */
 int lbm_set_profiling(lbm_ctx* c, int on);

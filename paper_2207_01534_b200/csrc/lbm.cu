@@ -120,13 +120,30 @@ struct lbm_ctx {
   int keep_psi_mb = 48;     // this budget: min(1, MB / psi bytes); env LBM_B200_KEEP_PSI_MB (0: off)
   int pdl = 1;              // programmatic dependent launch of the three passes; env LBM_B200_PDL=0
   int tile = 1286;          // fp32 bulk kernel variant: tile nodes * 10 + min CTAs/SM; env LBM_B200_TILE
+  // Launch-bound boxes (a step of config 1 or 2 is three kernels of 3-8 us each): lbm_step replays
+  // a captured CUDA graph of kGraphSteps steps (programmatic-dependent-launch edges included)
+  // instead of launching every kernel from the host.  One graph per starting buffer parity;
+  // dropped when a kernel argument changes (lbm_set_boundary).  env LBM_B200_GRAPH=0|1 (default:
+  // on for boxes of up to kGraphAutoNodes fluid nodes, where the host launch rate is the limit).
+  int graph_mode = -1;      // -1 auto, 0 off, 1 on
+  cudaGraphExec_t graph_exec[2] = {nullptr, nullptr};
+  cudaStream_t cap_stream = nullptr;   // capture happens here (torch's current stream may be the
+                                       // legacy default stream, which cannot be captured); the
+                                       // graphs are launched on the caller's stream
+  long long graph_launches = 0;   // kernel launches inside one graph
+  long long steps_done = 0;
   long long bytes[4] = {0, 0, 0, 0};
   bool prof = false;
   std::vector<ProfEvent> prof_events;
   double prof_ms[4] = {0, 0, 0, 0};
   long long prof_launches = 0;
 
+  void drop_graphs() {
+    for (auto& g : graph_exec) { if (g) cudaGraphExecDestroy(g); g = nullptr; }
+  }
   ~lbm_ctx() {
+    drop_graphs();
+    if (cap_stream) cudaStreamDestroy(cap_stream);
     for (auto& e : prof_events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     lbm_shim_free(f[0]); lbm_shim_free(f[1]); lbm_shim_free(psi); lbm_shim_free(nbr);
     lbm_shim_free(wall_nbr); lbm_shim_free(wall_inv_den); lbm_shim_free(node_vox_d);
@@ -410,6 +427,58 @@ int step_T(lbm_ctx* c, int n, cudaStream_t st) {
   return LBM_OK;
 }
 
+constexpr int kGraphSteps = 16;            // even: the buffer parity returns to its start
+constexpr int kGraphAutoNodes = 600000;    // above this a step is long enough to hide the launches
+
+// n steps, through graph replays where that pays (see lbm_ctx::graph_mode)
+template <typename T>
+int step_graphed_T(lbm_ctx* c, int n, cudaStream_t st) {
+  const bool want = c->graph_mode == 1 || (c->graph_mode < 0 && c->nf <= kGraphAutoNodes);
+  const bool open = c->open_end[0] || c->open_end[1];
+  // the first steps run directly: they configure the kernels' attributes and bring the deferred
+  // open-plane fix into its steady state (pending at the start of every step)
+  if (!want || c->prof || c->step_variant != 0 || c->slab) return step_T<T>(c, n, st);
+  if (c->steps_done == 0 || (open && !c->open_pending)) {
+    if (n == 0) return LBM_OK;
+    if (int rc = step_T<T>(c, 1, st)) return rc;
+    ++c->steps_done;
+    --n;
+  }
+  while (n >= kGraphSteps) {
+    cudaGraphExec_t& exec = c->graph_exec[c->cur];
+    if (!exec) {
+      const long long before = c->prof_launches;
+      cudaGraph_t graph = nullptr;
+      if (!c->cap_stream) CU(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+      CU(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+      const int rc = step_T<T>(c, kGraphSteps, c->cap_stream);   // captured, not executed
+      const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
+      c->graph_launches = c->prof_launches - before;
+      c->prof_launches = before;
+      if (rc || e != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        c->graph_mode = 0;   // capture is not available here: plain launches from now on
+        return rc ? rc : step_T<T>(c, n, st);
+      }
+      const cudaError_t ei = cudaGraphInstantiate(&exec, graph, 0);
+      cudaGraphDestroy(graph);
+      if (ei != cudaSuccess) {
+        exec = nullptr;
+        cudaGetLastError();
+        c->graph_mode = 0;
+        return step_T<T>(c, n, st);
+      }
+    }
+    CU(cudaGraphLaunch(exec, st));
+    c->prof_launches += c->graph_launches;
+    c->steps_done += kGraphSteps;
+    n -= kGraphSteps;
+  }
+  c->steps_done += n;
+  return step_T<T>(c, n, st);
+}
+
 template <typename T>
 int record_frozen_T(lbm_ctx* c, int comp, cudaStream_t st) {
   if (!c->open_end[0] && !c->open_end[1]) return LBM_OK;
@@ -527,6 +596,7 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   if (const char* e = std::getenv("LBM_B200_TILE")) c->tile = std::atoi(e);
   if (const char* e = std::getenv("LBM_B200_REVERSE")) c->reverse = std::atoi(e) != 0;
   if (const char* e = std::getenv("LBM_B200_PDL")) c->pdl = std::atoi(e) != 0;
+  if (const char* e = std::getenv("LBM_B200_GRAPH")) c->graph_mode = std::atoi(e) != 0;
   if (const char* e = std::getenv("LBM_B200_KEEP_PSI_MB")) c->keep_psi_mb = std::atoi(e);
   if (const char* e = std::getenv("LBM_B200_IDX")) c->idx16 = std::atoi(e) == 32 ? 0 : 1;
   if (const char* e = std::getenv("LBM_B200_STEP")) c->step_variant = !std::strcmp(e, "split") ? 0 : 1;
@@ -863,6 +933,7 @@ int lbm_set_boundary(lbm_ctx* c, double inlet_value, double outlet_rho) {
     return fail(LBM_EINVAL, "boundary values must be finite");
   if (int rc = check_ctx(c)) return rc;
   apply_pending(c, cur_stream());  // the last step's fix uses the values it was run with
+  c->drop_graphs();                // the boundary values are kernel arguments
   if (c->p.inlet_kind == 1 || c->p.inlet_kind == 3) c->p.inlet_rho = inlet_value;
   else c->p.inlet_uz = inlet_value;
   c->p.outlet_rho = outlet_rho;
@@ -887,7 +958,7 @@ int lbm_step(lbm_ctx* c, int n) {
     c->prof_events.clear();
   }
   c->prof_launches = 0;
-  return c->bits == 64 ? step_T<double>(c, n, st) : step_T<float>(c, n, st);
+  return c->bits == 64 ? step_graphed_T<double>(c, n, st) : step_graphed_T<float>(c, n, st);
 }
 
 int lbm_set_profiling(lbm_ctx* c, int on) {
