@@ -160,7 +160,6 @@ class SlabLbm:
         self.num_fluid = sum(s.num_owned for s in self.sims)
         self._ring = RingTransport(rank, world, group) if world is not None else None
         self._buf = [[buffer_tensor(s, w) for w in range(8)] for s in self.sims]
-        self._psi_current = False
 
     def close(self):
         self._buf = []
@@ -266,6 +265,11 @@ class SlabLbm:
         parts = [s.get_macroscopic(fields) for s in self.sims]
         return {k: np.concatenate([self._owned(p[k], r) for p, r in zip(parts, self.mine)], axis=0)
                 for k in parts[0]}
+
+    def trapped_volume(self, comp, z0=0, z1=None):
+        raise NotImplementedError(
+            "trapped volume on slabs needs a cross-slab union of the per-slab connected components "
+            "(DESIGN.md section 9); use an unsharded Lbm for this query")
 
     def diagnostics(self):
         """(mass[2], momentum[3]) over the owned nodes of this process; summed over all ranks when
