@@ -97,8 +97,24 @@ class RingTransport:
     between the same pair of ranks (world size 2) matched.  A None tensor is an empty message; both
     ends see it empty (the sizes derive from the same mask planes)."""
 
-    def __init__(self, rank, world, group=None):
+    def __init__(self, rank, world, group=None, stage_host=None):
         self.rank, self.world, self.group = rank, world, group
+        # NCCL moves device buffers directly.  Any other backend (gloo) gets the messages staged
+        # through pinned host buffers: slower, but the same choreography -- it is what the
+        # two-process test on one GPU runs, where NCCL refuses two ranks on one device.
+        if stage_host is None and world > 1:
+            import torch.distributed as dist
+            stage_host = dist.get_backend(group) != "nccl"
+        self.stage_host = bool(stage_host)
+        self._pinned = {}
+
+    def _host(self, t, key):
+        import torch
+        h = self._pinned.get(key)
+        if h is None or h.shape != t.shape or h.dtype != t.dtype:
+            h = torch.empty(t.shape, dtype=t.dtype, pin_memory=t.is_cuda)
+            self._pinned[key] = h
+        return h
 
     def exchange(self, send_lo, send_hi, recv_lo, recv_hi):
         self.finish(self.start(send_lo, send_hi, recv_lo, recv_hi))
@@ -106,7 +122,11 @@ class RingTransport:
     @staticmethod
     def finish(works):
         for w in works:
-            w.wait()   # stream-ordered on CUDA tensors: no host block
+            if isinstance(w, tuple):      # staged receive: (work, host buffer, device buffer)
+                w[0].wait()
+                w[2].copy_(w[1], non_blocking=True)
+            else:
+                w.wait()   # NCCL: stream-ordered on CUDA tensors, no host block
 
     def start(self, send_lo, send_hi, recv_lo, recv_hi):
         """Post the four messages; returns the handles `finish` waits on.  On CUDA tensors the
@@ -120,6 +140,8 @@ class RingTransport:
             return []
         import torch.distributed as dist
         up, down = (self.rank + 1) % self.world, (self.rank - 1) % self.world
+        if self.stage_host:
+            return self._start_staged(send_lo, send_hi, recv_lo, recv_hi, up, down)
         ops = []
         if send_hi is not None:
             ops.append(dist.P2POp(dist.isend, send_hi, up, self.group))
@@ -130,6 +152,31 @@ class RingTransport:
         if recv_hi is not None:
             ops.append(dist.P2POp(dist.irecv, recv_hi, up, self.group))
         return dist.batch_isend_irecv(ops) if ops else []
+
+    def _start_staged(self, send_lo, send_hi, recv_lo, recv_hi, up, down):
+        import torch
+        import torch.distributed as dist
+        works = []
+        hs_hi = hs_lo = None
+        if send_hi is not None:
+            hs_hi = self._host(send_hi, "s_hi")
+            hs_hi.copy_(send_hi, non_blocking=True)
+        if send_lo is not None:
+            hs_lo = self._host(send_lo, "s_lo")
+            hs_lo.copy_(send_lo, non_blocking=True)
+        if (send_hi is not None and send_hi.is_cuda) or (send_lo is not None and send_lo.is_cuda):
+            torch.cuda.current_stream().synchronize()   # the host copies must be complete
+        if hs_hi is not None:
+            works.append(dist.isend(hs_hi, up, group=self.group))
+        if hs_lo is not None:
+            works.append(dist.isend(hs_lo, down, group=self.group))
+        if recv_lo is not None:
+            h = self._host(recv_lo, "r_lo")
+            works.append((dist.irecv(h, down, group=self.group), h, recv_lo))
+        if recv_hi is not None:
+            h = self._host(recv_hi, "r_hi")
+            works.append((dist.irecv(h, up, group=self.group), h, recv_hi))
+        return works
 
 
 class SlabLbm:

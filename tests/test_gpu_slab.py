@@ -276,3 +276,81 @@ def test_open_box_slabs_fp32_bit_identical(k, parts):
     assert np.max(np.abs(m_s - m_g) / m_g) < 1e-12
     s.close()
     g.close()
+
+
+# ------------------------------------------------------------------ two processes, one GPU
+
+def _rank_worker(rank, world, port, out):
+    """One rank of the distributed driver: owns slab `rank`, exchanges through torch.distributed
+    (gloo, messages staged through pinned host memory -- NCCL refuses two ranks on one device; no
+    kernel ever waits on another rank, the waits are on the host), and compares its owned planes
+    with an unsharded run of the same box that it makes itself."""
+    import os
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path.insert(0, root)
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    import torch
+    import torch.distributed as dist
+    torch.cuda.set_device(0)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ok, msg = True, ""
+    try:
+        for k, bits in ((5, 64), (4, 32)):
+            c = make_config(k, size=32, storage_bits=bits)
+            s = SlabLbm(c["mask"], c["params"], rank=rank, world=world)
+            g = Lbm(c["mask"], c["params"])
+            s.set_density(c["rhoA"], c["rhoB"])
+            g.set_density(c["rhoA"], c["rhoB"])
+            s.step(25)
+            g.step(25)
+            z0, z1 = s.ranges[rank]
+            fl = c["mask"][z0:z1] == 0
+            for comp in (0, 1):
+                a = s.get_populations(comp)[:, fl]
+                b = g.get_populations(comp)[:, z0:z1][:, fl]
+                if not np.array_equal(a, b):
+                    ok, msg = False, f"cfg {k} comp {comp}: populations differ"
+            ms = s.get_macroscopic(("rhoA", "uz"))
+            mg = g.get_macroscopic(("rhoA", "uz"))
+            for key in ms:
+                if not np.array_equal(ms[key], mg[key][z0:z1]):
+                    ok, msg = False, f"cfg {k}: {key} differs"
+            m_s, j_s = s.diagnostics()          # all_reduce over ranks
+            m_g, j_g = g.diagnostics()
+            if np.max(np.abs(m_s - m_g) / m_g) > 1e-12:
+                ok, msg = False, f"cfg {k}: mass {m_s} vs {m_g}"
+            nz = c["mask"].shape[0]
+            if abs(s.saturation(1, 3, nz - 3) - g.saturation(1, 3, nz - 3)) > 1e-12:
+                ok, msg = False, f"cfg {k}: saturation"
+            s.step(3)
+            g.step(3)
+            a = s.get_populations(0)[:, fl]
+            b = g.get_populations(0)[:, z0:z1][:, fl]
+            if not np.array_equal(a, b):
+                ok, msg = False, f"cfg {k}: populations differ after the getters"
+            s.close()
+            g.close()
+        dist.barrier()
+    except Exception as e:  # noqa: BLE001 -- reported to the parent
+        ok, msg = False, repr(e)
+    out.put((rank, ok, msg))
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_distributed_driver_ranks_share_one_gpu(world):
+    import os
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = 32500 + os.getpid() % 2000 + world
+    procs = [ctx.Process(target=_rank_worker, args=(r, world, port, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(out.get(timeout=600) for _ in procs)
+    for p in procs:
+        p.join(120)
+        assert p.exitcode == 0
+    assert all(ok for _, ok, _ in res), res
