@@ -191,7 +191,8 @@ int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open,
  * which in slab mode requires both lbm_slab_density parts + the psi exchange to have been done on
  * the current state; so do lbm_saturation and lbm_mean_pressure, whose z-range is in LOCAL planes
  * and which cover the owned nodes only (halo planes are empty ranges).  lbm_diagnostics sums over
- * the owned nodes.  lbm_step and lbm_trapped_volume return LBM_EINVAL on a slab context. */
+ * the owned nodes.  lbm_step and lbm_trapped_volume return LBM_EINVAL on a slab context (the
+ * trapped volume of a cut box is the lbm_slab_ccl_* sequence below). */
 #define LBM_SLAB_GHOST 2
 int lbm_create_slab(lbm_ctx** out, const uint8_t* solid_local, int nx, int ny, int nz_local,
                     const lbm_params* p, int halo_lo, int halo_hi);
@@ -203,10 +204,27 @@ int lbm_slab_unpack(lbm_ctx* c);
  * which = 2*kind + face, face 0 = low z, 1 = high z:
  *   kind 0: psi of my two owned planes at that face (send)   kind 1: psi of my two halo planes (receive)
  *   kind 2: packed populations that left through that face   kind 3: populations arriving through it
+ *   kind 4 (which 8, 9): cluster flags of my boundary planes  kind 5 (which 10, 11): the neighbours' (ints)
  * A slab's send buffer of face 1 has the byte count of its upper neighbour's receive buffer of
  * face 0, and vice versa (both are derived from the same mask planes). */
 int lbm_slab_buffer(lbm_ctx* c, int which, void** dev, long long* bytes);
 long long lbm_num_owned(lbm_ctx* c);   /* fluid nodes of the owned planes, or -1 */
+/* Trapped volume (reading R15) of a box cut into slabs.  Every slab labels the connected
+ * components of the phase-comp nodes it owns (lbm_slab_ccl_begin; needs psi of the current state
+ * like the other slab queries; mark_lo / mark_hi = this slab owns the global plane z = 0 /
+ * z = nz-1, whose clusters are "connected to an end").  Then, until no slab reports a change:
+ * lbm_slab_ccl_export fills buffers 8 (low face) and 9 (high face) of lbm_slab_buffer with one
+ * int per (x,y) of the outermost owned plane -- the end-connected flag of the phase cluster
+ * there, -1 where there is none --, the caller moves them into the neighbours' buffers 11 and 10,
+ * and lbm_slab_ccl_import raises the flags of the clusters of its own boundary-plane nodes whose
+ * neighbour across the cut is end-connected (use_lo / use_hi = 0 ignores a face: the box's own
+ * end, or the periodic wrap, across which R15 does not connect); *changed = clusters newly
+ * flagged.  lbm_slab_ccl_finish counts the nodes, and adds rho_comp, of the unflagged clusters in
+ * the LOCAL planes [z0,z1) and ends the session.  import and finish synchronise. */
+int lbm_slab_ccl_begin(lbm_ctx* c, int comp, int mark_lo, int mark_hi);
+int lbm_slab_ccl_export(lbm_ctx* c);
+int lbm_slab_ccl_import(lbm_ctx* c, int use_lo, int use_hi, int* changed);
+int lbm_slab_ccl_finish(lbm_ctx* c, int z0, int z1, long long* nodes, double* mass);
 /* Host-only helper (no GPU needed): the halo lists lbm_create_slab builds, decoded for inspection.
  * pack_dir_vox / unpack_dir_vox: caller-allocated, 2*cap int32 each; entry k is (direction i,
  * local voxel index of the node whose row slot is read / written), low face first then high face;

@@ -1291,6 +1291,33 @@ __global__ void __launch_bounds__(256) k_ccl_mark(const int* __restrict__ parent
   if (r >= 0) flag[r] = 1;
 }
 
+// Trapped volume across slab cuts.  Each slab labels its owned nodes on its own (the kernels
+// above; edges into halo nodes are skipped because their ids are >= the owned count), marks the
+// clusters that touch a global end plane it owns, and then the "connected to an end plane" flag is
+// propagated across the cuts until nothing changes: k_ccl_export writes, for every (x,y) of an
+// owned boundary plane, the flag of the phase cluster there (-1: solid or other phase) into a
+// dense nx*ny plane; the neighbour slab's k_ccl_import reads the plane at the (x,y) of its own
+// boundary-plane nodes (the 6-neighbour across the cut) and raises the flag of their clusters.
+__global__ void __launch_bounds__(256) k_ccl_export(const int* __restrict__ parent,
+                                                    const int* __restrict__ flag,
+                                                    const int* __restrict__ node_vox, int n0, int n1,
+                                                    int np, int* __restrict__ out) {
+  const int n = n0 + blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= n1) return;
+  const int r = parent[n];
+  out[node_vox[n] % np] = r >= 0 ? flag[r] : -1;
+}
+__global__ void __launch_bounds__(256) k_ccl_import(const int* __restrict__ parent, int* flag,
+                                                    const int* __restrict__ node_vox, int n0, int n1,
+                                                    int np, const int* __restrict__ in,
+                                                    int* __restrict__ changed) {
+  const int n = n0 + blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= n1) return;
+  const int r = parent[n];
+  if (r < 0 || in[node_vox[n] % np] != 1) return;
+  if (atomicExch(flag + r, 1) == 0) atomicAdd(changed, 1);
+}
+
 // nodes and mass of the unmarked clusters in the id range [n0,n1); block b takes one contiguous
 // chunk and k_sum_pairs adds the per-block results in block order (deterministic)
 constexpr int kCclBlock = 256;

@@ -79,6 +79,10 @@ struct lbm_ctx {
   void* halo_recv = nullptr;         // [unpack low | unpack high] (A,B) pairs
   int n_pack[2] = {0, 0}, n_unpack[2] = {0, 0};
   long long psi_send[2][2] = {{0, 0}, {0, 0}}, psi_recv[2][2] = {{0, 0}, {0, 0}};
+  int edge_plane[2] = {0, 0};        // fluid nodes of the outermost owned plane at each end
+  int* ccl = nullptr;                // slab trapped volume: parent[nact] | flag[nact] | 4 planes of
+                                     // np ints (send low, send high, receive low, receive high) | counter
+  int ccl_comp = -1;                 // component of the running ccl session, -1: none
   int slab_phase = 0;       // next slab call: 0 density(0), 1 density(1), 2 collide(0), 3 collide(1),
                             // 4 unpack
   // slab mode: id ranges [0, bnd_lo1) and [bnd_hi0, nact) hold the two owned planes at each face
@@ -152,6 +156,7 @@ struct lbm_ctx {
     lbm_shim_free(nbr16_meta);
     lbm_shim_free(fused_flags);
     lbm_shim_free(halo_slots); lbm_shim_free(halo_send); lbm_shim_free(halo_recv);
+    lbm_shim_free(ccl);
   }
 };
 
@@ -736,6 +741,7 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
       long long hi0 = std::max(0LL, na - n_hi) / 256 * 256;
       long long lo1 = std::min((long long)pad256(n_lo), hi0);
       c->bnd_lo1 = (int)lo1; c->bnd_hi0 = (int)hi0;
+      c->edge_plane[0] = (int)halo.edge_plane[0]; c->edge_plane[1] = (int)halo.edge_plane[1];
       c->tile_lo1 = (int)((halo.edge_plane[0] + 127) / 128);
       c->tile_hi0 = (int)(std::max(0LL, na - halo.edge_plane[1]) / 128);
     }
@@ -753,6 +759,13 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
     for (int fc = 0; fc < 2; ++fc) { up(d, halo.unpack[fc].data(), halo.unpack[fc].size() * 4); d += halo.unpack[fc].size(); }
     c->bytes[2] += (long long)(nslots * sizeof(int));
     c->bytes[3] += (long long)(sendb + recvb);
+    const size_t cclb = ((size_t)2 * c->nact + (size_t)4 * c->np + 4) * sizeof(int);
+    c->ccl = (int*)lbm_shim_alloc(cclb);
+    if (!c->ccl) {
+      delete c;
+      return fail(LBM_ENOMEM, "device allocation failed (slab ccl)");
+    }
+    c->bytes[3] += (long long)cclb;
   }
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);  // host sources die with this scope
   if (e != cudaSuccess) {
@@ -881,10 +894,120 @@ int lbm_slab_unpack(lbm_ctx* c) {
   return LBM_OK;
 }
 
+int lbm_slab_ccl_begin(lbm_ctx* c, int comp, int mark_lo, int mark_hi) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
+  if (comp < 0 || comp > 1) return fail(LBM_EINVAL, "bad argument");
+  if (c->slab_phase != 2)
+    return fail(LBM_EINVAL, "slab context: lbm_slab_ccl_begin needs both lbm_slab_density parts and "
+                            "the psi exchange on the current state");
+  cudaStream_t st = cur_stream();
+  const int na = c->nact;
+  int* parent = c->ccl;
+  int* flag = parent + na;
+  const int g = blocks(na, 256);
+  if (c->bits == 64)
+    k_ccl_init<double><<<g, 256, 0, st>>>((const Vec2<double>*)c->psi, na, comp, parent, flag);
+  else
+    k_ccl_init<float><<<g, 256, 0, st>>>((const Vec2<float>*)c->psi, na, comp, parent, flag);
+  k_ccl_unite<<<g, 256, 0, st>>>(c->nbr, na, c->npad, parent);   // ids >= na (halo) are skipped
+  k_ccl_flatten<<<g, 256, 0, st>>>(na, parent);
+  const int a1 = mark_lo ? c->edge_plane[0] : 0, b0 = mark_hi ? na - c->edge_plane[1] : na;
+  if (a1 + (na - b0) > 0)
+    k_ccl_mark<<<blocks(a1 + (na - b0), 256), 256, 0, st>>>(parent, 0, a1, b0, na, flag);
+  CU(cudaPeekAtLastError());
+  c->ccl_comp = comp;
+  return LBM_OK;
+}
+
+int lbm_slab_ccl_export(lbm_ctx* c) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!c->slab || c->ccl_comp < 0) return fail(LBM_EINVAL, "no lbm_slab_ccl_begin on this context");
+  cudaStream_t st = cur_stream();
+  const int na = c->nact;
+  int* parent = c->ccl;
+  int* flag = parent + na;
+  int* planes = parent + (size_t)2 * na;
+  CU(cudaMemsetAsync(planes, 0xff, (size_t)2 * c->np * sizeof(int), st));  // -1: nothing there
+  if (c->edge_plane[0] > 0)
+    k_ccl_export<<<blocks(c->edge_plane[0], 256), 256, 0, st>>>(parent, flag, c->node_vox_d, 0,
+                                                                c->edge_plane[0], c->np, planes);
+  if (c->edge_plane[1] > 0)
+    k_ccl_export<<<blocks(c->edge_plane[1], 256), 256, 0, st>>>(
+        parent, flag, c->node_vox_d, na - c->edge_plane[1], na, c->np, planes + c->np);
+  CU(cudaPeekAtLastError());
+  return LBM_OK;
+}
+
+int lbm_slab_ccl_import(lbm_ctx* c, int use_lo, int use_hi, int* changed) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!changed) return fail(LBM_EINVAL, "NULL argument");
+  if (!c->slab || c->ccl_comp < 0) return fail(LBM_EINVAL, "no lbm_slab_ccl_begin on this context");
+  cudaStream_t st = cur_stream();
+  const int na = c->nact;
+  int* parent = c->ccl;
+  int* flag = parent + na;
+  int* planes = parent + (size_t)2 * na;
+  int* counter = planes + (size_t)4 * c->np;
+  CU(cudaMemsetAsync(counter, 0, sizeof(int), st));
+  if (use_lo && c->edge_plane[0] > 0)
+    k_ccl_import<<<blocks(c->edge_plane[0], 256), 256, 0, st>>>(
+        parent, flag, c->node_vox_d, 0, c->edge_plane[0], c->np, planes + (size_t)2 * c->np, counter);
+  if (use_hi && c->edge_plane[1] > 0)
+    k_ccl_import<<<blocks(c->edge_plane[1], 256), 256, 0, st>>>(
+        parent, flag, c->node_vox_d, na - c->edge_plane[1], na, c->np, planes + (size_t)3 * c->np,
+        counter);
+  CU(cudaPeekAtLastError());
+  int h = 0;
+  CU(cudaMemcpyAsync(&h, counter, sizeof h, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  *changed = h;
+  return LBM_OK;
+}
+
+int lbm_slab_ccl_finish(lbm_ctx* c, int z0, int z1, long long* nodes, double* mass) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!nodes || !mass || z0 < 0 || z1 > c->nz || z0 > z1) return fail(LBM_EINVAL, "bad argument");
+  if (!c->slab || c->ccl_comp < 0) return fail(LBM_EINVAL, "no lbm_slab_ccl_begin on this context");
+  cudaStream_t st = cur_stream();
+  const int na = c->nact, comp = c->ccl_comp;
+  int* parent = c->ccl;
+  int* flag = parent + na;
+  const int n0 = c->zstart[z0], n1 = c->zstart[z1];
+  const int chunk = std::max(kCclBlock, (int)(((long long)(n1 - n0) + 1183) / 1184));
+  const int nb = n1 > n0 ? blocks(n1 - n0, chunk) : 0;
+  DevBuf tmp(((size_t)2 * nb + 2) * sizeof(double));
+  if (!tmp.p) return fail(LBM_ENOMEM, "device allocation failed");
+  double* partial = (double*)tmp.p;
+  double* out = partial + (size_t)2 * nb;
+  if (nb > 0) {
+    if (c->bits == 64)
+      k_ccl_count<double><<<nb, kCclBlock, 0, st>>>((const Vec2<double>*)c->psi, parent, flag, n0,
+                                                    n1, comp, chunk, partial);
+    else
+      k_ccl_count<float><<<nb, kCclBlock, 0, st>>>((const Vec2<float>*)c->psi, parent, flag, n0, n1,
+                                                   comp, chunk, partial);
+  }
+  k_sum_pairs<<<1, 32, 0, st>>>(partial, nb, out);
+  CU(cudaPeekAtLastError());
+  double h[2] = {0.0, 0.0};
+  CU(cudaMemcpyAsync(h, out, sizeof h, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  *mass = h[0];
+  *nodes = (long long)h[1];
+  c->ccl_comp = -1;
+  return LBM_OK;
+}
+
 int lbm_slab_buffer(lbm_ctx* c, int which, void** dev, long long* bytes) {
   if (!c || !dev || !bytes) return fail(LBM_EINVAL, "NULL argument");
   if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
-  if (which < 0 || which > 7) return fail(LBM_EINVAL, "which must be 0..7");
+  if (which < 0 || which > 11) return fail(LBM_EINVAL, "which must be 0..11");
+  if (which >= 8) {  // cluster-flag planes of the trapped-volume query: send low/high, receive low/high
+    *dev = c->ccl + (size_t)2 * c->nact + (size_t)(which - 8) * c->np;
+    *bytes = (long long)c->np * (long long)sizeof(int);
+    return LBM_OK;
+  }
   const size_t pair = 2 * c->esz;
   const int face = which & 1;
   switch (which >> 1) {

@@ -25,6 +25,7 @@ SYMBOLS = [
     "lbm_build_index", "lbm_build_schedule",
     "lbm_create_slab", "lbm_slab_density", "lbm_slab_collide", "lbm_slab_unpack", "lbm_slab_buffer",
     "lbm_num_owned", "lbm_build_slab_halo",
+    "lbm_slab_ccl_begin", "lbm_slab_ccl_export", "lbm_slab_ccl_import", "lbm_slab_ccl_finish",
 ]
 
 
@@ -94,6 +95,13 @@ def load():
     lib.lbm_num_owned.argtypes = [P]
     lib.lbm_num_owned.restype = LL
     lib.lbm_build_slab_halo.argtypes = [V, I, I, I, I, I, I, V, V, LL] + [C.POINTER(LL)] * 5
+    lib.lbm_slab_ccl_begin.argtypes = [P, I, I, I]
+    lib.lbm_slab_ccl_export.argtypes = [P]
+    lib.lbm_slab_ccl_import.argtypes = [P, I, I, C.POINTER(I)]
+    lib.lbm_slab_ccl_finish.argtypes = [P, I, I, C.POINTER(LL), D]
+    for fn in ("lbm_slab_ccl_begin", "lbm_slab_ccl_export", "lbm_slab_ccl_import",
+               "lbm_slab_ccl_finish"):
+        getattr(lib, fn).restype = I
     for fn in ("lbm_create_slab", "lbm_slab_density", "lbm_slab_collide", "lbm_slab_unpack",
                "lbm_slab_buffer", "lbm_build_slab_halo"):
         getattr(lib, fn).restype = I
@@ -260,6 +268,26 @@ class Lbm:
 
     def slab_unpack(self):
         _chk(load().lbm_slab_unpack(self._h), "lbm_slab_unpack")
+
+    def slab_ccl_begin(self, comp, mark_lo, mark_hi):
+        _chk(load().lbm_slab_ccl_begin(self._h, int(comp), int(bool(mark_lo)), int(bool(mark_hi))),
+             "lbm_slab_ccl_begin")
+
+    def slab_ccl_export(self):
+        _chk(load().lbm_slab_ccl_export(self._h), "lbm_slab_ccl_export")
+
+    def slab_ccl_import(self, use_lo, use_hi):
+        n = C.c_int()
+        _chk(load().lbm_slab_ccl_import(self._h, int(bool(use_lo)), int(bool(use_hi)), C.byref(n)),
+             "lbm_slab_ccl_import")
+        return int(n.value)
+
+    def slab_ccl_finish(self, z0, z1):
+        n = C.c_longlong()
+        m = C.c_double()
+        _chk(load().lbm_slab_ccl_finish(self._h, int(z0), int(z1), C.byref(n), C.byref(m)),
+             "lbm_slab_ccl_finish")
+        return n.value, m.value
 
     def slab_buffer(self, which):
         """(device pointer, bytes) of exchange buffer `which` (include/lbm.h lbm_slab_buffer)."""

@@ -206,7 +206,7 @@ class SlabLbm:
         self._plane_fluid = (mask.reshape(mask.shape[0], -1) == 0).sum(axis=1).astype(np.int64)
         self.num_fluid = sum(s.num_owned for s in self.sims)
         self._ring = RingTransport(rank, world, group) if world is not None else None
-        self._buf = [[buffer_tensor(s, w) for w in range(8)] for s in self.sims]
+        self._buf = [[buffer_tensor(s, w) for w in range(12)] for s in self.sims]
 
     def close(self):
         self._buf = []
@@ -214,7 +214,8 @@ class SlabLbm:
             s.close()
         self.sims = []
 
-    # -- exchanges: kind 0 = psi (buffers 0,1 -> 2,3), kind 1 = populations (4,5 -> 6,7)
+    # -- exchanges: kind 0 = psi (buffers 0,1 -> 2,3), kind 1 = populations (4,5 -> 6,7),
+    #    kind 2 = cluster flags of the trapped-volume query (8,9 -> 10,11)
     def _exchange_start(self, kind):
         b = 4 * kind
         if self._ring is not None:
@@ -313,10 +314,45 @@ class SlabLbm:
         return {k: np.concatenate([self._owned(p[k], r) for p, r in zip(parts, self.mine)], axis=0)
                 for k in parts[0]}
 
+    def _sum_over_ranks(self, values):
+        if self.world is None or self.world == 1:
+            return values
+        import torch
+        import torch.distributed as dist
+        dev = "cuda" if dist.get_backend(self._ring.group) == "nccl" else "cpu"
+        t = torch.tensor(values, dtype=torch.float64, device=dev)
+        dist.all_reduce(t, group=self._ring.group)
+        return [float(v) for v in t.cpu()]
+
     def trapped_volume(self, comp, z0=0, z1=None):
-        raise NotImplementedError(
-            "trapped volume on slabs needs a cross-slab union of the per-slab connected components "
-            "(DESIGN.md section 9); use an unsharded Lbm for this query")
+        """(nodes, mass) of the phase-`comp` clusters in the global planes [z0, z1) that reach
+        neither z = 0 nor z = nz-1 (reading R15): per-slab connected components, then the
+        end-connected flag is passed across the cuts until no slab changes (include/lbm.h
+        lbm_slab_ccl_*).  Nothing connects across the periodic wrap."""
+        nz = self.shape[0]
+        z1 = nz if z1 is None else z1
+        last = len(self.ranges) - 1
+        self._density_and_psi_halo()
+        for s, r in zip(self.sims, self.mine):
+            s.slab_ccl_begin(comp, r == 0, r == last)
+        while True:
+            for s in self.sims:
+                s.slab_ccl_export()
+            RingTransport.finish(self._exchange_start(2))
+            changed = sum(s.slab_ccl_import(r > 0, r < last) for s, r in zip(self.sims, self.mine))
+            if self._sum_over_ranks([float(changed)])[0] == 0:
+                break
+        nodes, mass = 0, 0.0
+        for s, r in zip(self.sims, self.mine):
+            a, b = max(z0, self.ranges[r][0]), min(z1, self.ranges[r][1])
+            if b <= a:
+                a = b = self.ranges[r][0]          # empty range: the session still has to end
+            off = GHOST * self.halo[r][0] - self.ranges[r][0]
+            n, m = s.slab_ccl_finish(a + off, b + off)
+            nodes += n
+            mass += m
+        nodes, mass = self._sum_over_ranks([float(nodes), mass])
+        return int(round(nodes)), mass
 
     def diagnostics(self):
         """(mass[2], momentum[3]) over the owned nodes of this process; summed over all ranks when

@@ -86,3 +86,26 @@ def test_staged_drainage_protocol_matches_oracle():
     # the ramp does something: the inlet pressure follows the imposed density
     assert curve[2].P_in > curve[1].P_in > curve[0].P_in
     assert curve[2].P_c > 0.0
+
+
+def test_staged_drainage_protocol_on_slabs_matches_unsharded():
+    """The same protocol driven on the box cut into 3 z-slabs (SlabLbm has the calls
+    `primary_drainage` makes): stage lengths, S_w and trapped node counts identical to the
+    unsharded run, pressures and trapped mass to rounding of the per-slab sums."""
+    from paper_2207_01534_b200.slab import SlabLbm
+    c = make_config(4, size=40, storage_bits=64)
+    mask, p = c["mask"], c["params"]
+    kw = dict(defending_comp=p["outlet_comp"], layers=8, check_every=60, plateau_tol=2e-4,
+              max_steps_per_stage=240)
+    stages = [1.0, 1.04, 1.08]
+    curves = []
+    for make in (lambda: Lbm(mask, p), lambda: SlabLbm(mask, p, parts=3)):
+        sim = make()
+        sim.set_density(c["rhoA"], c["rhoB"])
+        curves.append(primary_drainage(sim, stages, 1.0, **kw))
+        sim.close()
+    for a, b in zip(*curves):
+        assert (a.steps, a.settled, a.trapped_nodes) == (b.steps, b.settled, b.trapped_nodes)
+        assert abs(a.S_w - b.S_w) < 1e-12
+        assert abs(a.P_in - b.P_in) < 1e-12 and abs(a.P_out - b.P_out) < 1e-12
+        assert abs(a.trapped_mass - b.trapped_mass) <= 1e-10 * max(1.0, a.trapped_mass)

@@ -181,9 +181,13 @@ def test_slab_error_paths():
         s.slab_density(0)                           # unpack of the running step is missing
     s.slab_unpack()
     with pytest.raises(LbmError):
-        s.slab_buffer(8)
-    sizes = [s.slab_buffer(w)[1] for w in range(8)]
-    assert all(b % 8 == 0 for b in sizes) and sizes[0] > 0
+        s.slab_buffer(12)
+    sizes = [s.slab_buffer(w)[1] for w in range(12)]
+    assert all(b % 8 == 0 for b in sizes) and sizes[0] > 0 and sizes[8:] == [16 * 16 * 4] * 4
+    with pytest.raises(LbmError):
+        s.slab_ccl_export()                         # no lbm_slab_ccl_begin
+    with pytest.raises(LbmError):
+        s.slab_ccl_begin(0, 1, 1)                   # psi of the current state is missing
     s.close()
     g = Lbm(m, p)
     with pytest.raises(LbmError):
@@ -354,3 +358,89 @@ def test_distributed_driver_ranks_share_one_gpu(world):
         p.join(120)
         assert p.exitcode == 0
     assert all(ok for _, ok, _ in res), res
+
+
+# ------------------------------------------------------------------ trapped volume across cuts
+
+def _blob_state(shape, seed, solid, z_open):
+    """Smooth random two-phase field on a random solid mask: many clusters of both phases, some
+    touching the ends, many cut by slab boundaries."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    mask = (rng.uniform(size=shape) < solid).astype(np.uint8)
+    if z_open:
+        mask[:2] = 0
+        mask[-2:] = 0
+    f = rng.standard_normal(shape)
+    k = [np.fft.fftfreq(n) for n in shape]
+    kk = k[0][:, None, None] ** 2 + k[1][None, :, None] ** 2 + k[2][None, None, :] ** 2
+    f = np.real(np.fft.ifftn(np.fft.fftn(f) * np.exp(-2 * (np.pi * 2.5) ** 2 * kk)))
+    f /= f.std()
+    rA = np.where(f > 0.3, 0.9, 0.1) + 0.01 * rng.uniform(size=shape)
+    return mask, rA, 1.0 - rA
+
+
+@pytest.mark.parametrize("shape,solid,z_open,parts", [((40, 36, 44), 0.25, 0, 2),
+                                                      ((40, 36, 44), 0.15, 0, 5),
+                                                      ((48, 32, 32), 0.2, 1, 3),
+                                                      ((64, 24, 24), 0.3, 1, 8)])
+def test_slab_trapped_volume_matches_unsharded(shape, solid, z_open, parts):
+    mask, rA, rB = _blob_state(shape, 41, solid, z_open)
+    kw = dict(storage_bits=64)
+    if z_open:
+        kw.update(z_open=1, inlet_kind=1, inlet_comp=1, inlet_rho=1.0, outlet_kind=1, outlet_comp=0,
+                  outlet_rho=1.0)
+    p = default_params(**kw)
+    g = Lbm(mask, p)
+    s = SlabLbm(mask, p, parts=parts)
+    g.set_density(rA, rB)
+    s.set_density(rA, rB)
+    nz = shape[0]
+    seen = 0
+    for comp in (0, 1):
+        for z0, z1 in ((0, nz), (nz // 4, 3 * nz // 4), (nz - 1, nz), (0, 1), (5, 6)):
+            ng, mg = g.trapped_volume(comp, z0, z1)
+            ns, ms = s.trapped_volume(comp, z0, z1)
+            assert ns == ng, (comp, z0, z1, ns, ng)
+            assert abs(ms - mg) <= 1e-12 * max(1.0, mg)
+            seen += ng
+    assert seen > 0
+    g.step(3)
+    s.step(3)
+    assert s.trapped_volume(0) == pytest.approx(g.trapped_volume(0), rel=1e-12)
+    s.step(2)                                      # stepping goes on after the query
+    g.step(2)
+    _identical_pops(s, g, mask)
+    s.close()
+    g.close()
+
+
+def test_slab_trapped_volume_serpentine_crosses_every_cut_many_times():
+    """A single phase-A channel that winds up and down through the whole box: its end-connected
+    flag has to travel across every cut several times before the iteration settles.  A second,
+    closed loop of the same shape but detached from the end planes is trapped."""
+    nz, ny, nx = 32, 12, 40
+    mask = np.zeros((nz, ny, nx), np.uint8)
+    A = np.zeros((nz, ny, nx), bool)
+    for k, x in enumerate(range(2, 38, 4)):        # vertical legs, joined alternately at top/bottom
+        A[3:29, 2, x] = True
+        if x + 4 < 38:
+            A[28 if k % 2 == 0 else 3, 2, x:x + 5] = True
+    A[0:4, 2, 2] = True                            # the first leg reaches z = 0
+    B = np.zeros_like(A)
+    for k, x in enumerate(range(2, 38, 4)):        # same serpentine at y = 8, not reaching an end
+        B[3:29, 8, x] = True
+        if x + 4 < 38:
+            B[28 if k % 2 == 0 else 3, 8, x:x + 5] = True
+    rA = np.where(A | B, 0.9, 0.1)
+    p = default_params(storage_bits=64)
+    g = Lbm(mask, p)
+    g.set_density(rA, 1.0 - rA)
+    want = g.trapped_volume(0)
+    assert want[0] == int(B.sum())
+    for parts in (2, 4, 8):
+        s = SlabLbm(mask, p, parts=parts)
+        s.set_density(rA, 1.0 - rA)
+        got = s.trapped_volume(0)
+        assert got[0] == want[0] and abs(got[1] - want[1]) < 1e-9
+        s.close()
+    g.close()
