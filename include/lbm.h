@@ -129,7 +129,9 @@ int lbm_memory_bytes(lbm_ctx* c, long long bytes[4]);
  * Tuning / A-B knobs read from the environment by lbm_create (defaults are the production path):
  *   LBM_B200_STEP=split|fused      one kernel per pass (default) | experimental single-kernel step
  *   LBM_B200_COLLIDE=bulk|simple   bulk-async staged fused pass (default) | register kernel
- *   LBM_B200_IDX=16|32             16-bit tile-relative neighbour index (default) | int32 rows
+ *   LBM_B200_IDX=16|32|bits        16-bit tile-relative neighbour index (default) | int32 rows |
+ *                                  geometric index: ids from per-row bitmasks and prefix ids (0.5 B per
+ *                                  voxel + 4 B per node instead of 36 B per node; measured 2.5 % slower)
  *   LBM_B200_REVERSE=1|0           fused pass walks tiles backwards (default) | forwards
  *   LBM_B200_PDL=1|0               programmatic dependent launch of the three passes (default) | off
  *   LBM_B200_GRAPH=1|0             lbm_step replays a captured CUDA graph of 16 steps | launches every

@@ -315,6 +315,43 @@ int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Ind
   return 0;
 }
 
+int build_bitindex(const Geometry& g, long long psi_wall_base, BitIndex& out) {
+  if (g.nf <= 0 || g.vox2id.empty()) return -1;
+  if (g.nx > 1024 || g.ny > 1024 || g.nz > 1024) return -1;
+  const int nx = g.nx, W = (nx + 31) / 32;
+  const long long rows = (long long)g.ny * g.nz, nf = g.nf;
+  try {
+    out.words = W;
+    out.rec.assign((size_t)rows * W * 4, 0);
+    out.coord.assign((size_t)nf, 0);
+#pragma omp parallel for schedule(static)
+    for (long long r = 0; r < rows; ++r) {
+      const int32_t* id = &g.vox2id[(size_t)r * nx];
+      uint32_t* rec = &out.rec[(size_t)r * W * 4];
+      // first fluid id / wall psi index at or after each word: walk the row backwards
+      long long next_f = 0, next_w = 0;
+      for (int w = W - 1; w >= 0; --w) {
+        uint32_t fm = 0, wm = 0;
+        for (int b = std::min(31, nx - 1 - 32 * w); b >= 0; --b) {
+          const int32_t v = id[32 * w + b];
+          if (v < 0) continue;
+          if (v < nf) { fm |= 1u << b; next_f = v; }
+          else { wm |= 1u << b; next_w = psi_wall_base + (v - nf); }
+        }
+        rec[4 * w] = fm; rec[4 * w + 1] = wm;
+        rec[4 * w + 2] = (uint32_t)next_f; rec[4 * w + 3] = (uint32_t)next_w;
+      }
+      const int y = (int)(r % g.ny), z = (int)(r / g.ny);
+      for (int x = 0; x < nx; ++x)
+        if (id[x] >= 0 && id[x] < nf)
+          out.coord[id[x]] = (uint32_t)x | ((uint32_t)y << 10) | ((uint32_t)z << 20);
+    }
+  } catch (const std::bad_alloc&) {
+    return -4;
+  }
+  return 0;
+}
+
 int build_halo(const Geometry& g, const uint8_t* solid, size_t npad, Halo& h) {
   if (!solid) return -1;
   const int nx = g.nx, ny = g.ny, nz = g.nz, G = kSlabGhost;

@@ -598,6 +598,10 @@ struct Idx16 {
   int reverse;            // 1: CTA b takes tile gridDim-1-b
   int nact;               // nodes this pass updates: ids [0,nact).  = nf, except in slab mode, where
                           // the halo nodes [nact,nf) only receive pushes
+  // IDX = 2 (geometric index, geometry.hpp BitIndex): per-row-word records and packed coordinates
+  const uint4* bits;        // [nz*ny][words] {fluid mask, wall mask, first fluid id, first wall psi index}
+  const uint32_t* coord;    // [npad] x | y << 10 | z << 20
+  int nx, ny, nz, words;
   int tile0, split, tile1;  // tiles of this launch: position b < split -> tile0 + b, else
                             // tile1 + (b - split)  (whole pass: 0, grid, 0; slab mode: the boundary
                             // tiles of both faces in one launch, the interior in another)
@@ -608,7 +612,8 @@ constexpr size_t collide16_smem_bytes() {
   return collide_smem_bytes<T, TN>() + (size_t)18 * TN * sizeof(uint16_t) + kIdxMeta * sizeof(int);
 }
 
-template <typename T, int TN, int MINB, bool REMAINDER, bool IDX16>
+// IDX: 0 = int32 neighbour rows, 1 = 16-bit tile-relative rows, 2 = geometric (bitmask) index
+template <typename T, int TN, int MINB, bool REMAINDER, int IDX>
 __global__ void __launch_bounds__(TN, MINB)
     k_collide_stream_bulk(const T* __restrict__ fin, T* __restrict__ fout,
                           const Vec2<T>* __restrict__ psi, const int* __restrict__ nbr, int nf,
@@ -631,8 +636,61 @@ __global__ void __launch_bounds__(TN, MINB)
   __syncthreads();
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // compiler-visible warp-uniform value
   const int n = (int)t0 + tid;
-  if constexpr (!IDX16) {
+  if constexpr (IDX == 0) {
     if (warp == 0) load_tile<T, TN>(sf, sid, fin, nbr, npad, t0, &bar);
+    pdl_wait();
+    mbar_wait(&bar, 0);
+  } else if constexpr (IDX == 2) {
+    if (warp == 0) {
+      if (elect_one()) {
+        mbar_expect_tx(&bar, (uint32_t)((size_t)2 * Q * TN * sizeof(T)));
+#pragma unroll
+        for (int r = 0; r < Q; ++r)  // one row of TN (A, B) pairs per direction
+          bulk_g2s(sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2, 2 * TN * sizeof(T),
+                   &bar);
+      }
+      __syncwarp();
+    }
+    // Neighbour ids from the geometry while the populations arrive: nothing below depends on the
+    // previous kernels (static tables), so it runs before the dependency wait.
+    {
+      const uint32_t cw = ix.coord[n];  // coord is npad long, zero beyond nf
+      const int x = (int)(cw & 1023u), y = (int)((cw >> 10) & 1023u), z = (int)(cw >> 20);
+      int word[3];
+      uint32_t below[3], bit[3];
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {  // ex = d - 1, periodic in x
+        int xx = x + d - 1;
+        xx = xx < 0 ? ix.nx - 1 : (xx == ix.nx ? 0 : xx);
+        word[d] = xx >> 5;
+        bit[d] = (uint32_t)xx & 31u;
+        below[d] = (1u << bit[d]) - 1u;
+      }
+      int yy[3], zz[3];
+      bool beyond[3];
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        int v = y + d - 1;
+        yy[d] = v < 0 ? ix.ny - 1 : (v == ix.ny ? 0 : v);
+        int w = z + d - 1;
+        beyond[d] = false;
+        if (w < 0) {
+          if (ix.np_lo) { beyond[d] = true; w = z + 1; } else w = ix.nz - 1;  // mirror (R12 iv) | wrap
+        } else if (w == ix.nz) {
+          if (ix.np_hi) { beyond[d] = true; w = z - 1; } else w = 0;
+        }
+        zz[d] = w;
+      }
+#pragma unroll
+      for (int i = 1; i < Q; ++i) {
+        const int dx = ex(i) + 1, dy = ey(i) + 1, dz = ez(i) + 1;
+        const uint4 q = __ldg(ix.bits + ((size_t)(zz[dz] * ix.ny + yy[dy]) * ix.words + word[dx]));
+        const bool fl = (q.x >> bit[dx]) & 1u;
+        int k = fl ? (int)(q.z + __popc(q.x & below[dx])) : (int)(q.w + __popc(q.y & below[dx]));
+        if (ez(i) != 0 && beyond[dz]) k = -k - 1;
+        sid[(i - 1) * TN + tid] = k;
+      }
+    }
     pdl_wait();
     mbar_wait(&bar, 0);
   } else {

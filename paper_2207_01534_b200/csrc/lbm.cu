@@ -106,7 +106,12 @@ struct lbm_ctx {
   int collide_variant = 1;  // 0: register kernel (A/B reference), 1: bulk-async staged tiles
                             // (production); env LBM_B200_COLLIDE=simple|bulk
   int num_sms = 148;
-  int idx16 = 1;            // fused pass reads the 16-bit tile-relative index (env LBM_B200_IDX=32: int32)
+  int idx16 = 1;            // index the fused pass reads: 1 = 16-bit tile-relative rows (default),
+                            // 0 = int32 rows (env LBM_B200_IDX=32), 2 = geometric bitmask index
+                            // (env LBM_B200_IDX=bits; geometry.hpp BitIndex)
+  uint32_t* bit_rec = nullptr;       // [nz*ny][bit_words][4]
+  uint32_t* bit_coord = nullptr;     // [npad]
+  int bit_words = 0;
   uint16_t* nbr16 = nullptr;         // [18][npad]
   int* nbr16_meta = nullptr;         // [tiles][kIdxMeta]
   long long wide_tiles = 0;
@@ -157,6 +162,7 @@ struct lbm_ctx {
     lbm_shim_free(fused_flags);
     lbm_shim_free(halo_slots); lbm_shim_free(halo_send); lbm_shim_free(halo_recv);
     lbm_shim_free(ccl);
+    lbm_shim_free(bit_rec); lbm_shim_free(bit_coord);
   }
 };
 
@@ -292,13 +298,13 @@ void apply_pending(lbm_ctx* c, cudaStream_t st) {
   if (c->bits == 64) apply_pending_T<double>(c, st); else apply_pending_T<float>(c, st);
 }
 
-template <typename T, int TN, int MINB, bool IDX16>
+template <typename T, int TN, int MINB, int IDX>
 void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st, int part) {
   constexpr bool kRemainder = sizeof(T) == 4;
-  constexpr size_t smem = IDX16 ? collide16_smem_bytes<T, TN>() : collide_smem_bytes<T, TN>();
+  constexpr size_t smem = IDX == 1 ? collide16_smem_bytes<T, TN>() : collide_smem_bytes<T, TN>();
   static bool configured[64] = {};  // function attributes are per device
   if (!configured[c->device & 63]) {
-    cudaFuncSetAttribute(k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX16>,
+    cudaFuncSetAttribute(k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX>,
                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured[c->device & 63] = true;
   }
@@ -309,6 +315,9 @@ void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
   ix.np_hi = c->open_end[1] ? c->np : 0;
   ix.reverse = c->reverse;
   ix.nact = c->nact;
+  ix.bits = (const uint4*)c->bit_rec;
+  ix.coord = c->bit_coord;
+  ix.nx = c->nx; ix.ny = c->ny; ix.nz = c->nz; ix.words = c->bit_words;
   static_assert(TN == 128 || TN == 256, "tile ranges below are in units of 128 ids");
   const int per = TN / 128;                      // slab tile ranges are kept in 128-id tiles
   unsigned grid = blocks(c->nact, TN);
@@ -326,7 +335,7 @@ void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
   if (grid == 0) return;
   // Overlap only behind the wall pass: its blocks trigger after their own wait, i.e. once the
   // density pass (which may have rewritten the open planes of fin) is complete and visible.
-  launch_k(c->pdl && !c->prof && c->nw > 0, k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX16>,
+  launch_k(c->pdl && !c->prof && c->nw > 0, k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX>,
            grid, TN, smem, st, fin, fout, (const Vec2<T>*)c->psi,
            (const int*)c->nbr, c->nf, c->npad, k, ix);
 }
@@ -342,19 +351,25 @@ void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaS
     return;
   }
   if constexpr (sizeof(T) == 4) {
+    if (c->idx16 == 2) {
+      if (c->tile == 1287) launch_bulk<T, 128, 7, 2>(c, fin, fout, k, st, part);
+      else launch_bulk<T, 128, 6, 2>(c, fin, fout, k, st, part);
+      return;
+    }
     if (c->idx16) {
-      if (c->tile == 1285) launch_bulk<T, 128, 5, true>(c, fin, fout, k, st, part);
-      else launch_bulk<T, 128, 6, true>(c, fin, fout, k, st, part);
+      if (c->tile == 1285) launch_bulk<T, 128, 5, 1>(c, fin, fout, k, st, part);
+      else launch_bulk<T, 128, 6, 1>(c, fin, fout, k, st, part);
       return;
     }
     switch (c->tile) {
-      case 1285: launch_bulk<T, 128, 5, false>(c, fin, fout, k, st, part); break;
-      case 2563: launch_bulk<T, 256, 3, false>(c, fin, fout, k, st, part); break;
-      default: launch_bulk<T, 128, 6, false>(c, fin, fout, k, st, part); break;
+      case 1285: launch_bulk<T, 128, 5, 0>(c, fin, fout, k, st, part); break;
+      case 2563: launch_bulk<T, 256, 3, 0>(c, fin, fout, k, st, part); break;
+      default: launch_bulk<T, 128, 6, 0>(c, fin, fout, k, st, part); break;
     }
   } else {
-    if (c->idx16) launch_bulk<T, 128, 2, true>(c, fin, fout, k, st, part);
-    else launch_bulk<T, 128, 2, false>(c, fin, fout, k, st, part);
+    if (c->idx16 == 2) launch_bulk<T, 128, 2, 2>(c, fin, fout, k, st, part);
+    else if (c->idx16) launch_bulk<T, 128, 2, 1>(c, fin, fout, k, st, part);
+    else launch_bulk<T, 128, 2, 0>(c, fin, fout, k, st, part);
   }
 }
 
@@ -603,7 +618,8 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   if (const char* e = std::getenv("LBM_B200_PDL")) c->pdl = std::atoi(e) != 0;
   if (const char* e = std::getenv("LBM_B200_GRAPH")) c->graph_mode = std::atoi(e) != 0;
   if (const char* e = std::getenv("LBM_B200_KEEP_PSI_MB")) c->keep_psi_mb = std::atoi(e);
-  if (const char* e = std::getenv("LBM_B200_IDX")) c->idx16 = std::atoi(e) == 32 ? 0 : 1;
+  if (const char* e = std::getenv("LBM_B200_IDX"))
+    c->idx16 = !std::strcmp(e, "bits") ? 2 : (std::atoi(e) == 32 ? 0 : 1);
   if (const char* e = std::getenv("LBM_B200_STEP")) c->step_variant = !std::strcmp(e, "split") ? 0 : 1;
   if (c->slab) c->step_variant = 0;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
@@ -716,6 +732,24 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
     if (e == cudaSuccess) e = cudaMemsetAsync(c->fused_ctr, 0, 8 * sizeof(int), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->fused_flags, 0, nflags * sizeof(int), st);
     c->bytes[2] += (long long)(sch.records.size() * 4 + nflags * 4);
+  }
+  lbmgeo::BitIndex bix;  // upload source until the sync below
+  if (c->idx16 == 2) {
+    if (lbmgeo::build_bitindex(g, (long long)c->npad, bix) != 0) {
+      c->idx16 = 1;   // a box edge above 1024: the packed coordinates do not fit
+    } else {
+      c->bit_words = bix.words;
+      c->bit_rec = (uint32_t*)lbm_shim_alloc(bix.rec.size() * sizeof(uint32_t));
+      c->bit_coord = (uint32_t*)lbm_shim_alloc(c->npad * sizeof(uint32_t));
+      if (!c->bit_rec || !c->bit_coord) {
+        delete c;
+        return fail(LBM_ENOMEM, "device allocation failed (bit index)");
+      }
+      if (e == cudaSuccess) e = cudaMemsetAsync(c->bit_coord, 0, c->npad * sizeof(uint32_t), st);
+      up(c->bit_rec, bix.rec.data(), bix.rec.size() * sizeof(uint32_t));
+      up(c->bit_coord, bix.coord.data(), bix.coord.size() * sizeof(uint32_t));
+      c->bytes[2] += (long long)(bix.rec.size() * 4 + c->npad * 4);
+    }
   }
   lbmgeo::Halo halo;  // declared here: its lists are upload sources until the sync below
   if (c->slab) {

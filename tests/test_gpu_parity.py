@@ -349,7 +349,8 @@ def test_register_kernel_and_int32_index_paths_agree_with_production(monkeypatch
     c = make_config(3, size=32, storage_bits=64)
     sims = {}
     for name, env in (("prod", {}), ("simple", {"LBM_B200_COLLIDE": "simple"}),
-                      ("idx32", {"LBM_B200_IDX": "32"}), ("fwd", {"LBM_B200_REVERSE": "0"}),
+                      ("idx32", {"LBM_B200_IDX": "32"}), ("bits", {"LBM_B200_IDX": "bits"}),
+                      ("fwd", {"LBM_B200_REVERSE": "0"}),
                       ("nopdl", {"LBM_B200_PDL": "0"}), ("nokeep", {"LBM_B200_KEEP_PSI_MB": "0"})):
         for k in ("LBM_B200_COLLIDE", "LBM_B200_IDX", "LBM_B200_REVERSE", "LBM_B200_PDL",
                   "LBM_B200_KEEP_PSI_MB"):
@@ -364,6 +365,7 @@ def test_register_kernel_and_int32_index_paths_agree_with_production(monkeypatch
     fl = c["mask"] == 0
     for s in (0, 1):
         assert np.array_equal(sims["prod"][s], sims["idx32"][s])      # same arithmetic, other index
+        assert np.array_equal(sims["prod"][s], sims["bits"][s])       # ... ids from the bitmask tables
         assert np.array_equal(sims["prod"][s], sims["fwd"][s])        # tile order is irrelevant
         assert np.array_equal(sims["prod"][s], sims["nopdl"][s])      # launch overlap is irrelevant
         assert np.array_equal(sims["prod"][s], sims["nokeep"][s])     # so is the L2 priority of psi

@@ -111,7 +111,8 @@ def test_slab_index_variants_agree(monkeypatch):
     default 16-bit index path (boundary tiles fall back to the wide rows there)."""
     c = _rock_case(32, 32, seed=23)
     ref = None
-    for env in ({}, {"LBM_B200_IDX": "32"}, {"LBM_B200_COLLIDE": "simple"}, {"LBM_B200_PDL": "0"}):
+    for env in ({}, {"LBM_B200_IDX": "32"}, {"LBM_B200_IDX": "bits"}, {"LBM_B200_COLLIDE": "simple"},
+                {"LBM_B200_PDL": "0"}):
         for k, v in env.items():
             monkeypatch.setenv(k, v)
         s = SlabLbm(c["mask"], c["params"], parts=2)

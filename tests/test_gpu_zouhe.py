@@ -109,7 +109,7 @@ def test_zou_he_all_step_paths_agree(monkeypatch):
         return [g.get_populations(s) for s in (0, 1)]
 
     base = run()
-    for env in (dict(LBM_B200_COLLIDE="simple"), dict(LBM_B200_IDX="32"),
+    for env in (dict(LBM_B200_COLLIDE="simple"), dict(LBM_B200_IDX="32"), dict(LBM_B200_IDX="bits"),
                 dict(LBM_B200_STEP="fused", LBM_B200_LEAD="8")):
         for k, v in env.items():
             monkeypatch.setenv(k, v)
