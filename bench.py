@@ -156,8 +156,8 @@ def aggregate_over_ranks(local_ms, units_per_rank, world, device):
 
 
 # DRAM bytes per launch of the fused pass from the committed `ncu --set full` capture
-# (profiles/r1_v9_step.md): dram__bytes_read.sum + dram__bytes_write.sum on config 4.
-NCU_TRAFFIC_CFG4_COLLIDE = 1.478e9
+# (profiles/r1_v10_step.md): dram__bytes_read.sum + dram__bytes_write.sum on config 4.
+NCU_TRAFFIC_CFG4_COLLIDE = 1.480e9
 
 
 def run_reference(args):

@@ -128,7 +128,9 @@ struct lbm_ctx {
   float keep_psi = 0.f;     // share of the psi lines stored with L2 evict_last priority, from
   int keep_psi_mb = 48;     // this budget: min(1, MB / psi bytes); env LBM_B200_KEEP_PSI_MB (0: off)
   int pdl = 1;              // programmatic dependent launch of the three passes; env LBM_B200_PDL=0
-  int tile = 1286;          // fp32 bulk kernel variant: tile nodes * 10 + min CTAs/SM; env LBM_B200_TILE
+  int tile = 1287;          // fp32 bulk kernel variant: tile nodes * 10 + min CTAs/SM; env LBM_B200_TILE
+                            // (1287: 7 CTAs per SM at 72 registers, the 16-bit rows staged inside the
+                            // id array; 1286: 6 CTAs at 80 registers, the previous default)
   // Launch-bound boxes (a step of config 1 or 2 is three kernels of 3-8 us each): lbm_step replays
   // a captured CUDA graph of kGraphSteps steps (programmatic-dependent-launch edges included)
   // instead of launching every kernel from the host.  One graph per starting buffer parity;
@@ -301,7 +303,8 @@ void apply_pending(lbm_ctx* c, cudaStream_t st) {
 template <typename T, int TN, int MINB, int IDX>
 void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st, int part) {
   constexpr bool kRemainder = sizeof(T) == 4;
-  constexpr size_t smem = IDX == 1 ? collide16_smem_bytes<T, TN>() : collide_smem_bytes<T, TN>();
+  constexpr size_t smem = IDX == 1 ? collide16_smem_bytes<T, TN, (MINB >= 7)>()
+                                   : collide_smem_bytes<T, TN>();
   static bool configured[64] = {};  // function attributes are per device
   if (!configured[c->device & 63]) {
     cudaFuncSetAttribute(k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX>,
@@ -358,6 +361,7 @@ void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaS
     }
     if (c->idx16) {
       if (c->tile == 1285) launch_bulk<T, 128, 5, 1>(c, fin, fout, k, st, part);
+      else if (c->tile == 1287) launch_bulk<T, 128, 7, 1>(c, fin, fout, k, st, part);
       else launch_bulk<T, 128, 6, 1>(c, fin, fout, k, st, part);
       return;
     }

@@ -350,10 +350,10 @@ def test_register_kernel_and_int32_index_paths_agree_with_production(monkeypatch
     sims = {}
     for name, env in (("prod", {}), ("simple", {"LBM_B200_COLLIDE": "simple"}),
                       ("idx32", {"LBM_B200_IDX": "32"}), ("bits", {"LBM_B200_IDX": "bits"}),
-                      ("fwd", {"LBM_B200_REVERSE": "0"}),
+                      ("cta6", {"LBM_B200_TILE": "1286"}), ("fwd", {"LBM_B200_REVERSE": "0"}),
                       ("nopdl", {"LBM_B200_PDL": "0"}), ("nokeep", {"LBM_B200_KEEP_PSI_MB": "0"})):
         for k in ("LBM_B200_COLLIDE", "LBM_B200_IDX", "LBM_B200_REVERSE", "LBM_B200_PDL",
-                  "LBM_B200_KEEP_PSI_MB"):
+                  "LBM_B200_KEEP_PSI_MB", "LBM_B200_TILE"):
             monkeypatch.delenv(k, raising=False)
         for k, v in env.items():
             monkeypatch.setenv(k, v)
@@ -367,6 +367,7 @@ def test_register_kernel_and_int32_index_paths_agree_with_production(monkeypatch
         assert np.array_equal(sims["prod"][s], sims["idx32"][s])      # same arithmetic, other index
         assert np.array_equal(sims["prod"][s], sims["bits"][s])       # ... ids from the bitmask tables
         assert np.array_equal(sims["prod"][s], sims["fwd"][s])        # tile order is irrelevant
+        assert np.array_equal(sims["prod"][s], sims["cta6"][s])       # so is the CTA residency
         assert np.array_equal(sims["prod"][s], sims["nopdl"][s])      # launch overlap is irrelevant
         assert np.array_equal(sims["prod"][s], sims["nokeep"][s])     # so is the L2 priority of psi
         a, b = sims["simple"][s][:, fl], sims["prod"][s][:, fl]
