@@ -138,7 +138,8 @@ int lbm_memory_bytes(lbm_ctx* c, long long bytes[4]);
  *                                  kernel from the host (default: graph for boxes of <= 600 000 fluid
  *                                  nodes, where a step is shorter than its three host launches)
  *   LBM_B200_KEEP_PSI_MB=48        L2 budget (MB) for psi stored with evict_last priority; 0: plain stores
- *   LBM_B200_TILE=1287|1286|1285   fused pass (fp32): 128-node CTAs, 7 (default) | 6 | 5 resident per SM
+ *   LBM_B200_TILE=1287|1286|1285|1288  fused pass (fp32): 128-node CTAs, 7 (default) | 6 | 5 | 8 resident
+ *                                  per SM (8: 64 registers, rest population from a register; slower)
  *   LBM_B200_LEAD                  producer lead of the experimental fused step */
 int lbm_set_profiling(lbm_ctx* c, int on);
 int lbm_last_step_profile(lbm_ctx* c, double ms[4], long long* launches);

@@ -454,13 +454,16 @@ __device__ __forceinline__ Pr<T> edot2(int i, Pr<T> x, Pr<T> y, Pr<T> z) {
 // neighbour ids in shared memory; tid = column of this thread in the tile; n = its node id.
 // Threads of the ragged last tile (valid = false) compute on the zero padding and only their
 // stores are predicated off, so control flow stays warp-uniform.
-template <typename T, int TN, bool REMAINDER>
+// ROW0: the rest population of this thread's node comes in `r0` (a register pair loaded straight
+// from global memory) instead of row 0 of the staged tile, which is then not staged at all.
+template <typename T, int TN, bool REMAINDER, bool ROW0 = false>
 __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
                                                     const int* __restrict__ sid, const int tid,
                                                     const int n, const bool valid,
                                                     T* __restrict__ fout,
                                                     const Vec2<T>* __restrict__ psi, const int nf,
-                                                    const size_t npad, const Consts<T>& c) {
+                                                    const size_t npad, const Consts<T>& c,
+                                                    const Pr<T> r0 = Pr<T>{T(0), T(0)}) {
   using P = Pr<T>;
   // staged populations: [19][TN] pairs (A, B); column tid
   const P* sfp = reinterpret_cast<const P*>(sf) + tid;
@@ -488,7 +491,7 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
       S[d] = pfma(pbc(wgt<T>(1)), a1[d], pmul(pbc(wgt<T>(7)), a2[d]));
   }
   // a1 (recomputed locally): R = (rho_A, rho_B); J[d] = per-component bare momentum
-  P R = sfp[0];
+  P R = ROW0 ? r0 : sfp[0];
   P J[3] = {{T(0), T(0)}, {T(0), T(0)}, {T(0), T(0)}};
 #pragma unroll
   for (int i = 1; i < Q; ++i) {
@@ -563,7 +566,7 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
     v0 = psub(R, acc);
   } else {
     const T w0 = wgt<T>(0);
-    const P f0 = sfp[0];
+    const P f0 = ROW0 ? r0 : sfp[0];
     v0 = pfma(pbc(c1), f0, pfma(pbc(om * w0 * k0), R, pmul(pbc(cS * w0), M3UF)));
   }
   if (valid) fo[n] = v0;
@@ -622,7 +625,12 @@ __global__ void __launch_bounds__(TN, MINB)
     k_collide_stream_bulk(const T* __restrict__ fin, T* __restrict__ fout,
                           const Vec2<T>* __restrict__ psi, const int* __restrict__ nbr, int nf,
                           size_t npad, Consts<T> c, Idx16 ix) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_dyn[];
+  // 8 CTAs per SM: row 0 (the rest populations) is not staged -- each thread loads its own pair
+  // from global memory -- which takes the CTA's last 1 KB off the shared-memory budget.  The
+  // layout below is kept by letting the (never touched) row 0 lie in front of the buffer.
+  constexpr bool kRow0 = IDX == 1 && MINB >= 8;
+  unsigned char* smem_raw = smem_dyn - (kRow0 ? (size_t)2 * TN * sizeof(T) : 0);
   T* sf = reinterpret_cast<T*>(smem_raw);                                        // [38][TN]
   int* sid = reinterpret_cast<int*>(smem_raw + (size_t)2 * Q * TN * sizeof(T));  // [18][TN]
   constexpr bool kAlias = IDX == 1 && MINB >= 7;
@@ -703,10 +711,10 @@ __global__ void __launch_bounds__(TN, MINB)
   } else {
     if (warp == 0) {
       if (elect_one()) {
-        mbar_expect_tx(&bar, (uint32_t)((size_t)2 * Q * TN * sizeof(T) +
+        mbar_expect_tx(&bar, (uint32_t)((size_t)2 * (kRow0 ? Q - 1 : Q) * TN * sizeof(T) +
                                         (size_t)18 * TN * sizeof(uint16_t) + kIdxMeta * sizeof(int)));
 #pragma unroll
-        for (int r = 0; r < Q; ++r)  // one row of TN (A, B) pairs per direction
+        for (int r = kRow0 ? 1 : 0; r < Q; ++r)  // one row of TN (A, B) pairs per direction
           bulk_g2s(sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2, 2 * TN * sizeof(T),
                    &bar);
 #pragma unroll
@@ -755,7 +763,13 @@ __global__ void __launch_bounds__(TN, MINB)
       }
     }
   }
-  collide_tile_thread<T, TN, REMAINDER>(sf, sid, tid, n, n < ix.nact, fout, psi, nf, npad, c);
+  if constexpr (kRow0) {
+    const Vec2<T> v = reinterpret_cast<const Vec2<T>*>(fin)[n];  // n < npad; complete like the tile
+    collide_tile_thread<T, TN, REMAINDER, true>(sf, sid, tid, n, n < ix.nact, fout, psi, nf, npad,
+                                                c, Pr<T>{v.a, v.b});
+  } else {
+    collide_tile_thread<T, TN, REMAINDER>(sf, sid, tid, n, n < ix.nact, fout, psi, nf, npad, c);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------

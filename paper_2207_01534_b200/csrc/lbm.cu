@@ -303,7 +303,8 @@ void apply_pending(lbm_ctx* c, cudaStream_t st) {
 template <typename T, int TN, int MINB, int IDX>
 void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st, int part) {
   constexpr bool kRemainder = sizeof(T) == 4;
-  constexpr size_t smem = IDX == 1 ? collide16_smem_bytes<T, TN, (MINB >= 7)>()
+  constexpr size_t smem = IDX == 1 ? collide16_smem_bytes<T, TN, (MINB >= 7)>() -
+                                         (MINB >= 8 ? (size_t)2 * TN * sizeof(T) : 0)
                                    : collide_smem_bytes<T, TN>();
   static bool configured[64] = {};  // function attributes are per device
   if (!configured[c->device & 63]) {
@@ -362,6 +363,7 @@ void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaS
     if (c->idx16) {
       if (c->tile == 1285) launch_bulk<T, 128, 5, 1>(c, fin, fout, k, st, part);
       else if (c->tile == 1287) launch_bulk<T, 128, 7, 1>(c, fin, fout, k, st, part);
+      else if (c->tile == 1288) launch_bulk<T, 128, 8, 1>(c, fin, fout, k, st, part);
       else launch_bulk<T, 128, 6, 1>(c, fin, fout, k, st, part);
       return;
     }

@@ -350,7 +350,8 @@ def test_register_kernel_and_int32_index_paths_agree_with_production(monkeypatch
     sims = {}
     for name, env in (("prod", {}), ("simple", {"LBM_B200_COLLIDE": "simple"}),
                       ("idx32", {"LBM_B200_IDX": "32"}), ("bits", {"LBM_B200_IDX": "bits"}),
-                      ("cta6", {"LBM_B200_TILE": "1286"}), ("fwd", {"LBM_B200_REVERSE": "0"}),
+                      ("cta6", {"LBM_B200_TILE": "1286"}), ("cta8", {"LBM_B200_TILE": "1288"}),
+                      ("fwd", {"LBM_B200_REVERSE": "0"}),
                       ("nopdl", {"LBM_B200_PDL": "0"}), ("nokeep", {"LBM_B200_KEEP_PSI_MB": "0"})):
         for k in ("LBM_B200_COLLIDE", "LBM_B200_IDX", "LBM_B200_REVERSE", "LBM_B200_PDL",
                   "LBM_B200_KEEP_PSI_MB", "LBM_B200_TILE"):
@@ -368,6 +369,7 @@ def test_register_kernel_and_int32_index_paths_agree_with_production(monkeypatch
         assert np.array_equal(sims["prod"][s], sims["bits"][s])       # ... ids from the bitmask tables
         assert np.array_equal(sims["prod"][s], sims["fwd"][s])        # tile order is irrelevant
         assert np.array_equal(sims["prod"][s], sims["cta6"][s])       # so is the CTA residency
+        assert np.array_equal(sims["prod"][s], sims["cta8"][s])       # (fp64 build: same kernel)
         assert np.array_equal(sims["prod"][s], sims["nopdl"][s])      # launch overlap is irrelevant
         assert np.array_equal(sims["prod"][s], sims["nokeep"][s])     # so is the L2 priority of psi
         a, b = sims["simple"][s][:, fl], sims["prod"][s][:, fl]
@@ -409,3 +411,22 @@ def test_graph_replay_is_bit_identical_to_host_launches(k, bits, monkeypatch):
         g.close()
     for a, b in zip(res[0], res[1]):
         assert np.array_equal(a, b)
+
+
+def test_fp32_cta_residency_variants_are_bit_identical(monkeypatch):
+    """LBM_B200_TILE selects how many CTAs of the fused pass share an SM (5, 6, 7 = default, 8) and
+    with it the shared-memory layout (7: 16-bit index rows staged inside the id array; 8: rest
+    populations from a register instead of a staged row).  Same arithmetic: identical populations."""
+    c = make_config(4, size=40, storage_bits=32)
+    res = {}
+    for tile in ("1287", "1285", "1286", "1288"):
+        monkeypatch.setenv("LBM_B200_TILE", tile)
+        g = Lbm(c["mask"], c["params"])
+        g.set_density(c["rhoA"], c["rhoB"])
+        g.step(40)
+        res[tile] = [g.get_populations(s) for s in (0, 1)]
+        g.close()
+    monkeypatch.delenv("LBM_B200_TILE")
+    for tile in ("1285", "1286", "1288"):
+        for a, b in zip(res["1287"], res[tile]):
+            assert np.array_equal(a, b), tile
