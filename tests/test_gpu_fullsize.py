@@ -90,6 +90,8 @@ def _elementwise_fp32(cfg, steps):
     assert np.abs(ug - uo).max() <= 1e-4 * np.abs(uo).max()
     m_o, _ = o.diagnostics()
     m_g, _ = g.diagnostics()
+    o.close()
+    g.close()
     assert np.max(np.abs(m_g - m_o) / m_o) <= 1e-6
 
 
@@ -105,4 +107,25 @@ def test_config3_full_size_elementwise_100_steps():
     outlet on B), fp32, every fluid node, 100 steps."""
     cfg = make_config(3)
     assert cfg["mask"].shape == (128, 128, 128)
+    _elementwise_fp32(cfg, 100)
+
+
+def test_config4_full_size_elementwise_100_steps():
+    """BASELINE.json config 4 -- the headline workload of bench.py -- at its full 256^3 size
+    (Gaussian-random-field rock, 4.3 M fluid nodes, pressure inlet on wetting B, pressure outlet
+    on A, tau = (1.5, 0.6)), fp32 production build, EVERY fluid node including both open planes,
+    100 steps, against the oracle at the north-star tolerances (1e-4 densities and velocities,
+    1e-6 mass per component).  The oracle needs ~10 GB of host memory and 2-3 minutes."""
+    cfg = make_config(4)
+    assert cfg["mask"].shape == (256, 256, 256) and cfg["params"]["storage_bits"] == 32
+    assert cfg["params"]["z_open"] == 1
+    _elementwise_fp32(cfg, 100)
+
+
+def test_config5_at_256_elementwise_100_steps():
+    """BASELINE.json config 5's recipe (periodic sphere pack, body force 1e-6 along z) at edge
+    256 -- the largest box the dense fp64 oracle holds comfortably (6.4 M fluid nodes; the 512^3
+    original would need 82 GB): fp32, every fluid node, 100 steps."""
+    cfg = make_config(5, size=256)
+    assert cfg["mask"].shape == (256, 256, 256)
     _elementwise_fp32(cfg, 100)

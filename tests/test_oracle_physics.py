@@ -129,17 +129,54 @@ def _laplace_2d(n, r0, tau, steps, half_force=1):
 
 def test_laplace_surface_tension_matches_paper():
     """2-D slab (cylinder) Laplace law dP = gamma/R with P from Eq. (12): the paper's regression
-    gives gamma = 0.071 at G=3.5 for every viscosity ratio. Reduced size
-    (96^2, R=12 and 20, vs the paper's 128^3, R=30) costs a few per cent: tolerance 6 %."""
-    g = []
-    for r0, steps in ((12, 4000), (20, 5000)):
+    gives gamma = 0.071 at G=3.5 for every viscosity ratio.  SURVEY.md 8(c):
+    three radii within 5 % of 0.071 each, the regression slope of dP against 1/R within 5 %, and
+    equality across M = 1 and M = 25 within 2 % at every radius (measured: +2.7..+3.1 % at M = 1,
+    +1.6..+2.5 % at M = 25; reduced size 96^2, R = 12..24, against the paper's 128^3, R = 30)."""
+    cases = ((12, 4000), (16, 4500), (24, 6000))
+    g1, invR, dPs = [], [], []
+    for r0, steps in cases:
         R, dP = _laplace_2d(96, r0, (1.0, 1.0), steps)
         assert abs(R - r0) < 1.0 and dP > 0
-        g.append(dP * R)
-    assert all(abs(v / PAPER["gamma"][0] - 1.0) < 0.06 for v in g), g
+        g1.append(dP * R)
+        invR.append(1.0 / R)
+        dPs.append(dP)
+    assert all(abs(v / PAPER["gamma"][0] - 1.0) < 0.05 for v in g1), g1
+    slope, icpt = np.polyfit(invR, dPs, 1)                           # Laplace law is linear (L165, L183)
+    assert abs(slope / PAPER["gamma"][0] - 1.0) < 0.05, slope
+    assert abs(icpt) < 0.02 * dPs[-1], icpt
     # independent of the viscosity ratio: M = 25 <=> tau = (3.5, 0.62) (PAPER.md L175)
-    R, dP = _laplace_2d(96, 12, tuple(PAPER["tau_M25"]), 4000)
-    assert abs(dP * R / g[0] - 1.0) < 0.03
+    for (r0, steps), ref in zip(cases, g1):
+        R, dP = _laplace_2d(96, r0, tuple(PAPER["tau_M25"]), steps)
+        assert abs(dP * R / PAPER["gamma"][0] - 1.0) < 0.05
+        assert abs(dP * R / ref - 1.0) < 0.02, (r0, dP * R, ref)
+    # M = 1/25 is M = 25 with the components' relaxation times exchanged (PAPER.md L175, L183)
+    R, dP = _laplace_2d(96, 16, tuple(PAPER["tau_M25"])[::-1], 4500)
+    assert abs(dP * R / g1[1] - 1.0) < 0.02
+
+
+@pytest.mark.skipif(not os.environ.get("LBM_ORACLE_SLOW"),
+                    reason="6 minutes of oracle time: set LBM_ORACLE_SLOW=1 (result recorded in DESIGN.md section 3)")
+def test_laplace_3d_point():
+    """one 3-D point at R >= 15 within 10 % of gamma = 0.071 (dP = 2 gamma / R,
+    PAPER.md L165, L181).  64^3, r0 = 20, 4000 steps."""
+    n, r0 = 64, 20
+    shape = (n, n, n)
+    c = (n - 1) / 2.0
+    rA = tanh_profile(shape, (c, c, c), r0)
+    o = LbmRef(np.zeros(shape, np.uint8), default_params(G=3.5, tau=(1.0, 1.0)))
+    o.set_density(rA, 1.027 - rA)
+    o.step(4000)
+    m = o.get_macroscopic()
+    d = (m["rhoA"] - m["rhoB"])
+    row = 0.25 * (d[n // 2 - 1, n // 2 - 1] + d[n // 2, n // 2] + d[n // 2 - 1, n // 2] + d[n // 2, n // 2 - 1])
+    i = np.nonzero((row[:-1] > 0) & (row[1:] <= 0))[0][0]
+    R = i + row[i] / (row[i] - row[i + 1]) - c
+    P = m["P"]
+    Pin = P[n // 2 - 1:n // 2 + 1, n // 2 - 1:n // 2 + 1, n // 2 - 1:n // 2 + 1].mean()
+    gamma = (Pin - P[0, 0, 0]) * R / 2.0
+    print("3-D Laplace point: R = %.3f, gamma = %.5f" % (R, gamma))
+    assert R >= 15 and abs(gamma / PAPER["gamma"][0] - 1.0) < 0.10, (R, gamma)
 
 
 def test_laplace_negative_control_literal_eq4():
