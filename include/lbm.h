@@ -66,12 +66,54 @@ typedef struct {
   int half_force;    /* 1: u_eq carries F/2 (reading R3); 0: literal Eq. (4) (negative control)  */
 } lbm_params;
 
+/* Execution options (plain data, copied by lbm_create_opt; every combination computes the same
+ * numbers bit for bit -- tests/test_gpu_parity.py -- they select how the step is scheduled).
+ * lbm_options_default fills in the defaults; lbm_create uses them. */
+enum { LBM_STEP_AUTO = 0, LBM_STEP_SPLIT = 1, LBM_STEP_WINDOW = 2 };
+enum { LBM_INDEX_16 = 0, LBM_INDEX_BITS = 1 };
+typedef struct {
+  int step;         /* LBM_STEP_SPLIT: one kernel per pass (density, virtual solid, fused
+                       force+collide+stream), chained by programmatic dependent launch.
+                       LBM_STEP_WINDOW: the whole step (a0-a6) as ONE persistent kernel in which the
+                       density pass runs a fixed distance ahead of the fused pass, so that the fused
+                       pass finds the populations in L2.
+                       LBM_STEP_AUTO (default): WINDOW for boxes above 600 000 fluid nodes whose
+                       lead window fits the L2, SPLIT otherwise (small boxes replay a CUDA graph)   */
+  int index;        /* neighbour index of the fused pass: LBM_INDEX_16 (default) 16-bit tile-relative
+                       rows, 37 B per node; LBM_INDEX_BITS per-row bitmasks + prefix ids, 0.5 B per
+                       voxel + 4 B per node (low-memory option, split step only, ~2.5 % slower)     */
+  int graph;        /* split step: -1 (default) replay a captured CUDA graph of 16 steps on boxes of
+                       <= 600 000 fluid nodes, 0 never, 1 always                                    */
+  int pdl;          /* split step: 1 (default) programmatic dependent launch of the three passes    */
+  int reverse;      /* split step: 1 (default) the fused pass walks the tiles backwards (L2 reuse
+                       across the two passes)                                                       */
+  int keep_psi_mb;  /* split step: L2 budget in MB for psi stored with evict_last priority
+                       (default 48; 0: plain stores)                                                */
+  int window_slack; /* window step: how many fluid tiles (of 128 nodes) before its first consumer a
+                       producer item is issued; 0 (default) = 450.  The density items then lead the
+                       fused items by one z-plane of tiles + twice this                             */
+  int window_ctas;  /* window step, fp32: resident CTAs per SM the kernel is compiled for: 0 (default)
+                       = 7 (72 registers), 6 (80 registers)                                        */
+} lbm_options;
+void lbm_options_default(lbm_options* o);
+
 /* Build a simulation from a geometry mask (binary rock image).
  *  solid: nx*ny*nz bytes, nonzero = solid.  Classifies voxels, compacts the fluid nodes,
  *  builds the neighbour index, allocates and uploads.  Populations start at zero: call
  *  lbm_set_density or lbm_set_populations next.  *out is written only on success. */
 int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, const lbm_params* p);
-void lbm_destroy(lbm_ctx* c); /* NULL is allowed */
+/* The same with explicit execution options (opt == NULL: the defaults).  LBM_EINVAL on a value
+ * outside the documented ones. */
+int lbm_create_opt(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz,
+                   const lbm_params* p, const lbm_options* opt);
+/* Synchronises the device (kernels of the context may be in flight on any stream it was used
+ * from), then releases everything.  NULL is allowed. */
+void lbm_destroy(lbm_ctx* c);
+/* What lbm_create chose: info[0] step (LBM_STEP_SPLIT / LBM_STEP_WINDOW), [1] index form,
+ * [2] slack and [3] largest stencil reach of the window schedule (tiles), [4] unused, [5] its item count,
+ * [6] CTAs of the window kernel (0 before the first step), [7] tiles that fall back to int32
+ * index rows. */
+int lbm_step_info(lbm_ctx* c, int info[8]);
 
 /* f_i^sigma = w_i * rho_sigma (reading R11); dense double arrays of nx*ny*nz.  Also records the
  * frozen inlet/outlet populations (reading R27). */
@@ -86,7 +128,9 @@ int lbm_set_boundary(lbm_ctx* c, double inlet_value, double outlet_rho);
 /* Advance n time steps (SURVEY.md §8c steps 1-7 per step): density pass (Eq. 3), virtual solid
  * density (Eq. 14-15), forces (Eq. 10, 11, 13), tau_s and u_eq (Eq. 5-8), collision (Eq. 1, 2,
  * 9), streaming with halfway bounce-back, open-plane fix (L147-157).
- * Asynchronous; n >= 0.  The open-plane fix of the last step is deferred: it is applied by the
+ * Asynchronous on torch's current stream; n >= 0.  A context may be used from different streams
+ * in turn: a call on another stream than the previous call's first waits for the work enqueued
+ * there.  In the split step the open-plane fix of the last step is deferred: it is applied by the
  * next lbm_step (inside its density pass) or by the next getter, whichever comes first, with the
  * boundary values that were in force when the step ran; callers always observe a complete state. */
 int lbm_step(lbm_ctx* c, int n);
@@ -122,25 +166,9 @@ int lbm_memory_bytes(lbm_ctx* c, long long bytes[4]);
 /* Device time (ms) of the kernels of the last lbm_step call, by kind, measured with CUDA events
  * on the launching stream when profiling is enabled with lbm_set_profiling(c, 1):
  * ms[0] density pass (in the default path it carries the open-plane fix of the previous step),
- * [1] virtual-solid pass, [2] collide+stream (the whole step when LBM_B200_STEP=fused),
+ * [1] virtual-solid pass, [2] collide+stream (the whole step in the window step),
  * [3] open-plane fix when it is launched on its own; launches = number of kernel launches of that
- * call.  Synchronises.
- *
- * Tuning / A-B knobs read from the environment by lbm_create (defaults are the production path):
- *   LBM_B200_STEP=split|fused      one kernel per pass (default) | experimental single-kernel step
- *   LBM_B200_COLLIDE=bulk|simple   bulk-async staged fused pass (default) | register kernel
- *   LBM_B200_IDX=16|32|bits        16-bit tile-relative neighbour index (default) | int32 rows |
- *                                  geometric index: ids from per-row bitmasks and prefix ids (0.5 B per
- *                                  voxel + 4 B per node instead of 36 B per node; measured 2.5 % slower)
- *   LBM_B200_REVERSE=1|0           fused pass walks tiles backwards (default) | forwards
- *   LBM_B200_PDL=1|0               programmatic dependent launch of the three passes (default) | off
- *   LBM_B200_GRAPH=1|0             lbm_step replays a captured CUDA graph of 16 steps | launches every
- *                                  kernel from the host (default: graph for boxes of <= 600 000 fluid
- *                                  nodes, where a step is shorter than its three host launches)
- *   LBM_B200_KEEP_PSI_MB=48        L2 budget (MB) for psi stored with evict_last priority; 0: plain stores
- *   LBM_B200_TILE=1287|1286|1285|1288  fused pass (fp32): 128-node CTAs, 7 (default) | 6 | 5 | 8 resident
- *                                  per SM (8: 64 registers, rest population from a register; slower)
- *   LBM_B200_LEAD                  producer lead of the experimental fused step */
+ * call.  Synchronises. */
 int lbm_set_profiling(lbm_ctx* c, int on);
 int lbm_last_step_profile(lbm_ctx* c, double ms[4], long long* launches);
 const char* lbm_last_error(void);
@@ -154,14 +182,17 @@ const char* lbm_last_error(void);
 int lbm_build_index(const uint8_t* solid, int nx, int ny, int nz, int z_open, int32_t* vox2id,
                     int32_t* nbr, long long nbr_cap, long long* nf, long long* nw);
 
-/* Host-only helper (no GPU needed): the work schedule of the fused single-kernel step exactly as
- * lbm_create builds it.  records: caller-allocated, cap_items*16 int32;
- * item k is records[16k..16k+15] = {type<<30 | tile, 3 x (lo,cnt) D-tile dependency ranges,
- * 3 x (lo,cnt) W-tile dependency ranges, 0, 0, 0}, type 0 = density pass on a fluid tile, 1 =
- * virtual-solid pass on a wall tile, 2 = fused collide+stream pass on a fluid tile; tiles are
- * `tile` consecutive ids.  *n_items receives the item count (2*ceil(N_f/tile)+ceil(N_w/tile)). */
-int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open, int tile,
-                       int lead, int32_t* records, long long cap_items, long long* n_items);
+/* Host-only helper (no GPU needed): the work schedule of the window step exactly as lbm_create
+ * builds it.  records: caller-allocated, cap_items*16 int32; item k is
+ * records[16k..16k+15] = {type<<28 | tile, 3 x (lo,cnt) dependency ranges of a first kind,
+ * 3 x (lo,cnt) of a second kind, 0, 0, 0}: type 0 = D, density pass on a fluid tile (no
+ * dependencies); 1 = W, virtual-solid pass on a wall tile (first kind: D tiles); 2 = C, fused
+ * collide+stream pass on a fluid tile (first kind: D tiles, second kind: W tiles); 3 = P,
+ * open-plane fix on `tile` nodes of plane tile / ntp (first kind: C tiles).  Tiles are `tile`
+ * consecutive ids.  Every item follows the items it depends on.  *n_items receives the item
+ * count. */
+int lbm_build_window(const uint8_t* solid, int nx, int ny, int nz, int z_open, int tile,
+                     int lead, int32_t* records, long long cap_items, long long* n_items);
 
 /* ---- z-slab sharding across GPUs --------
  * The step has two grid-wide dependencies (Eq. 11/13: every node's force needs its
@@ -200,6 +231,8 @@ int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open,
 #define LBM_SLAB_GHOST 2
 int lbm_create_slab(lbm_ctx** out, const uint8_t* solid_local, int nx, int ny, int nz_local,
                     const lbm_params* p, int halo_lo, int halo_hi);
+int lbm_create_slab_opt(lbm_ctx** out, const uint8_t* solid_local, int nx, int ny, int nz_local,
+                        const lbm_params* p, const lbm_options* opt, int halo_lo, int halo_hi);
 int lbm_slab_density(lbm_ctx* c, int part);
 int lbm_slab_collide(lbm_ctx* c, int part);
 int lbm_slab_unpack(lbm_ctx* c);

@@ -160,16 +160,19 @@ void to_ranges(std::vector<int32_t>& ids, int32_t* out /* 2*kDepRanges */) {
 
 }  // namespace
 
-int build_schedule(const Geometry& g, int tile, int lead, Schedule& s) {
-  if (tile < 32 || g.nf <= 0 || g.nbr.empty()) return -1;
-  const long long nf = g.nf, nw = g.nw;
+int build_window(const Geometry& g, int tile, int lead, Window& s) {
+  if (tile < 32 || g.nf <= 0 || g.nbr.empty() || g.nact != g.nf) return -1;
+  const long long nf = g.nf, nw = g.nw, np = (long long)g.nx * g.ny;
   s.tile = tile;
   s.ntf = (int)((nf + tile - 1) / tile);
   s.ntw = (int)((nw + tile - 1) / tile);
-  const int ntf = s.ntf, ntw = s.ntw;
+  s.ntp = (g.open_lo || g.open_hi) ? (int)((np + tile - 1) / tile) : 0;
+  const int ntf = s.ntf, ntw = s.ntw, ntp = s.ntp;
   try {
-    // dependency ranges
+    // dependency ranges: C(t) -> D, W tiles of its psi stencil; W(j) -> D tiles of its fluid
+    // neighbours; P(k) -> C tiles that write into its plane nodes and their interior neighbours
     std::vector<int32_t> dep_c((size_t)ntf * 4 * kDepRanges), dep_w((size_t)ntw * 2 * kDepRanges);
+    std::vector<int32_t> dep_p((size_t)2 * ntp * 2 * kDepRanges, 0);
 #pragma omp parallel
     {
       std::vector<int32_t> ds, ws;
@@ -201,40 +204,26 @@ int build_schedule(const Geometry& g, int tile, int lead, Schedule& s) {
           }
         to_ranges(ds, &dep_w[(size_t)j * 2 * kDepRanges]);
       }
-    }
-    // one global order in which dependencies always come first
-    s.records.clear();
-    s.records.reserve(((size_t)2 * ntf + ntw) * kRecordInts);
-    std::vector<uint8_t> done_d(ntf, 0), done_w(ntw, 0);
-    auto push = [&](int type, int t, const int32_t* d, const int32_t* w) {
-      const size_t base = s.records.size();
-      s.records.resize(base + kRecordInts, 0);
-      s.records[base] = (int32_t)(((uint32_t)type << 30) | (uint32_t)t);
-      for (int k = 0; k < 2 * kDepRanges; ++k) {
-        s.records[base + 1 + k] = d ? d[k] : 0;
-        s.records[base + 1 + 2 * kDepRanges + k] = w ? w[k] : 0;
+#pragma omp for schedule(static)
+      for (int k = 0; k < 2 * ntp; ++k) {
+        const int plane = k / ntp;
+        if (!(plane == 0 ? g.open_lo : g.open_hi)) continue;
+        ds.clear();
+        const long long q0 = (long long)(k - plane * ntp) * tile, q1 = std::min(np, q0 + tile);
+        for (long long q = q0; q < q1; ++q) {
+          // open planes and their interior neighbours are solid-free: ids q, np+q / nf-np+q, nf-2np+q
+          const long long v2[2] = {plane == 0 ? q : nf - np + q, plane == 0 ? np + q : nf - 2 * np + q};
+          for (long long v : v2) {
+            ds.push_back((int32_t)(v / tile));
+            for (int i = 1; i < kQ; ++i) {  // population i of v is pushed by the node at v - e_i
+              const int32_t src = g.nbr[(size_t)(kOpp[i] - 1) * nf + v];
+              if (src >= 0 && src < nf) ds.push_back((int32_t)(src / tile));
+            }
+          }
+        }
+        to_ranges(ds, &dep_p[(size_t)k * 2 * kDepRanges]);
       }
-    };
-    auto emit_d = [&](int t) {
-      if (t < 0 || t >= ntf || done_d[t]) return;
-      done_d[t] = 1;
-      push(0, t, nullptr, nullptr);
-    };
-    auto emit_w = [&](int j) {
-      if (j < 0 || j >= ntw || done_w[j]) return;
-      done_w[j] = 1;
-      const int32_t* d = &dep_w[(size_t)j * 2 * kDepRanges];
-      for (int k = 0; k < kDepRanges; ++k)
-        for (int q = 0; q < d[2 * k + 1]; ++q) emit_d(d[2 * k] + q);
-      push(1, j, d, nullptr);
-    };
-    // Producers are issued ahead of need (lead D tiles, lead/4 W tiles beyond the furthest
-    // non-wrapping dependency), so that a consumer normally finds its flags set and never waits.
-    const int lead_w = lead / 4;
-    int cur_d = 0, cur_w = 0;
-    auto d_upto = [&](int x) {  // all D tiles <= x, in natural order
-      for (; cur_d <= std::min(ntf - 1, x); ++cur_d) emit_d(cur_d);
-    };
+    }
     // furthest tile of 3 ranges that is not a periodic wrap-around seen from `from` (-1 if none)
     auto far_of = [&](const int32_t* r, int from, int n) {
       int far = -1;
@@ -244,26 +233,102 @@ int build_schedule(const Geometry& g, int tile, int lead, Schedule& s) {
       }
       return far;
     };
-    int want_w = -1;  // furthest W tile any C tile so far depends on
-    for (int t = 0; t < ntf; ++t) {
+    // Issue time of every item, in units of fluid tiles: C(t) is issued at time t.  A producer
+    // is issued `slack` before its first consumer, so that it has normally completed (and its
+    // flag need not be waited for) when the consumer starts: W(j) at (first C tile that reads
+    // it) - slack, D(k) at min(first C tile that reads it, issue time of the first W tile that
+    // reads it) - slack.  D(k) thus leads C(k) by (local reach of the psi stencil, about one
+    // z-plane of tiles) + 2 * slack: the window of populations the L2 has to hold.
+    const int slack = std::max(0, lead);
+    const long long kNever = (long long)4 * ntf + 8;
+    std::vector<long long> time_d(ntf, kNever), time_w(ntw, kNever);
+    for (int t = ntf - 1; t >= 0; --t) {  // first consumer = smallest t: walk down, overwrite
       const int32_t* d = &dep_c[(size_t)t * 4 * kDepRanges];
       const int32_t* w = d + 2 * kDepRanges;
-      want_w = std::max(want_w, far_of(w, std::max(want_w, 0), ntw));
-      for (; want_w >= 0 && cur_w <= std::min(ntw - 1, want_w + lead_w); ++cur_w) {
-        // the D tiles a W item reads are issued `lead` tiles before it
-        const int fd = far_of(&dep_w[(size_t)cur_w * 2 * kDepRanges], t, ntf);
-        if (fd >= 0) d_upto(fd + lead);
-        emit_w(cur_w);
+      for (int k = 0; k < kDepRanges; ++k) {
+        for (int q = 0; q < d[2 * k + 1]; ++q) time_d[d[2 * k] + q] = t;
+        for (int q = 0; q < w[2 * k + 1]; ++q) time_w[w[2 * k] + q] = t;
       }
-      d_upto(far_of(d, t, ntf) + lead);
+    }
+    for (int j = 0; j < ntw; ++j) time_w[j] -= slack;   // a wall tile nobody reads goes last
+    for (int k = 0; k < ntf; ++k) time_d[k] -= slack;
+    for (int j = 0; j < ntw; ++j) {
+      const int32_t* d = &dep_w[(size_t)j * 2 * kDepRanges];
+      for (int k = 0; k < kDepRanges; ++k)
+        for (int q = 0; q < d[2 * k + 1]; ++q)
+          time_d[d[2 * k] + q] = std::min(time_d[d[2 * k] + q], time_w[j] - slack);
+    }
+    int reach = 0;
+    for (int t = 0; t < ntf; ++t)
+      reach = std::max(reach, far_of(&dep_c[(size_t)t * 4 * kDepRanges], t, ntf) - t);
+    s.reach = reach;
+    s.slack = slack;
+    struct Item { long long key; int type, idx; };
+    std::vector<Item> order;
+    order.reserve((size_t)2 * ntf + ntw + 2 * ntp);
+    for (int j = 0; j < ntf; ++j) order.push_back({time_d[j], 0, j});
+    for (int j = 0; j < ntw; ++j) order.push_back({time_w[j], 1, j});
+    for (int t = 0; t < ntf; ++t) order.push_back({(long long)t, 2, t});
+    for (int k = 0; k < 2 * ntp; ++k) {
+      const int plane = k / ntp;
+      if (!(plane == 0 ? g.open_lo : g.open_hi)) continue;
+      const int32_t* d = &dep_p[(size_t)k * 2 * kDepRanges];
+      int far = 0;
+      for (int q = 0; q < kDepRanges; ++q)
+        if (d[2 * q + 1] > 0) far = std::max(far, d[2 * q] + d[2 * q + 1] - 1);
+      order.push_back({(long long)far + std::max(slack, 1), 3, k});
+    }
+    std::stable_sort(order.begin(), order.end(),
+                     [](const Item& a, const Item& b) { return a.key < b.key; });
+    // emit in that order; an item whose dependency has not been emitted yet (periodic wrap, tiny
+    // boxes) pulls it in front of itself, so every item follows what it waits for
+    s.records.clear();
+    s.records.reserve(order.size() * kWinRecordInts);
+    std::vector<uint8_t> done_d(ntf, 0), done_w(ntw, 0), done_c(ntf, 0);
+    auto push = [&](int type, int t, const int32_t* a, const int32_t* b) {
+      const size_t base = s.records.size();
+      s.records.resize(base + kWinRecordInts, 0);
+      s.records[base] = (int32_t)(((uint32_t)type << 28) | (uint32_t)t);
+      for (int k = 0; k < 2 * kDepRanges; ++k) {
+        s.records[base + 1 + k] = a ? a[k] : 0;
+        s.records[base + 1 + 2 * kDepRanges + k] = b ? b[k] : 0;
+      }
+    };
+    auto emit_d = [&](int t) {
+      if (done_d[t]) return;
+      done_d[t] = 1;
+      push(0, t, nullptr, nullptr);
+    };
+    auto emit_w = [&](int j) {
+      if (done_w[j]) return;
+      done_w[j] = 1;
+      const int32_t* d = &dep_w[(size_t)j * 2 * kDepRanges];
+      for (int k = 0; k < kDepRanges; ++k)
+        for (int q = 0; q < d[2 * k + 1]; ++q) emit_d(d[2 * k] + q);
+      push(1, j, d, nullptr);
+    };
+    auto emit_c = [&](int t) {
+      if (done_c[t]) return;
+      done_c[t] = 1;
+      const int32_t* d = &dep_c[(size_t)t * 4 * kDepRanges];
+      const int32_t* w = d + 2 * kDepRanges;
       for (int k = 0; k < kDepRanges; ++k) {
         for (int q = 0; q < w[2 * k + 1]; ++q) emit_w(w[2 * k] + q);
         for (int q = 0; q < d[2 * k + 1]; ++q) emit_d(d[2 * k] + q);
       }
       push(2, t, d, w);
+    };
+    for (const Item& it : order) {
+      if (it.type == 0) emit_d(it.idx);
+      else if (it.type == 1) emit_w(it.idx);
+      else if (it.type == 2) emit_c(it.idx);
+      else {
+        const int32_t* d = &dep_p[(size_t)it.idx * 2 * kDepRanges];
+        for (int k = 0; k < kDepRanges; ++k)
+          for (int q = 0; q < d[2 * k + 1]; ++q) emit_c(d[2 * k] + q);
+        push(3, it.idx, d, nullptr);
+      }
     }
-    for (int j = 0; j < ntw; ++j) emit_w(j);
-    for (int t = 0; t < ntf; ++t) emit_d(t);
   } catch (const std::bad_alloc&) {
     return -4;
   }

@@ -85,6 +85,18 @@ __device__ __forceinline__ void store_vec2(Vec2<double>* p, Vec2<double> v, uint
                : "memory");
 }
 
+// Explicitly rounded scalar operations.  The same device function is inlined into several kernels
+// (the open-plane fix runs in k_open_planes, k_density_open and k_step_window; the virtual-solid
+// sum in k_wallpsi and k_step_window); left to the compiler, whether a*b+c becomes one FMA or a
+// multiply and an add depends on the surrounding code, and the kernels would differ in the last
+// bit.  Every product-sum of such shared code is therefore spelled out.
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ float fma_rn(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double fma_rn(double a, double b, double c) { return __fma_rn(a, b, c); }
+
 template <typename T>
 struct Consts {
   T G;            // G_coh, Eq. (11)/(13)
@@ -152,11 +164,11 @@ __global__ void __launch_bounds__(256) k_wallpsi(Vec2<T>* __restrict__ psi,
   for (int i = 1; i < Q; ++i) {
     if (id[i] >= 0) {
       const Vec2<T> p = psi[id[i]];
-      na += wgt<T>(i) * p.a;
-      nb += wgt<T>(i) * p.b;
+      na = fma_rn(wgt<T>(i), p.a, na);
+      nb = fma_rn(wgt<T>(i), p.b, nb);
     }
   }
-  Vec2<T> o; o.a = chiA * na * s; o.b = chiB * nb * s;
+  Vec2<T> o; o.a = mul_rn(mul_rn(chiA, na), s); o.b = mul_rn(mul_rn(chiB, nb), s);
   // wall ids are stored at wall_base = npad (tile-aligned)
   store_vec2(psi + wall_base + w, o, l2_keep_policy(keep_psi));
 }
@@ -243,68 +255,7 @@ __device__ __forceinline__ void node_state(const T (&fa)[Q], const T (&fb)[Q],
 // equals Eq. (1) for i=0 exactly in exact arithmetic (sum_i feq = rho, sum_i S_i = 0) and removes
 // the 1.5e-8-per-step mass drift that the fp32-rounded weights (sum = 1 + 1.49e-8) would inject
 // (DESIGN.md "fp32 build").
-template <typename T, bool REMAINDER>
-__device__ __forceinline__ void collide_component(const T (&f)[Q], T rho, const T (&F)[3],
-                                                  const T (&u)[3], T om, T (&out)[Q]) {
-  const T uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
-  const T uF = u[0] * F[0] + u[1] * F[1] + u[2] * F[2];
-  const T c1 = T(1) - om;
-  const T cS = T(1) - T(0.5) * om;
-  T acc = T(0);
-#pragma unroll
-  for (int i = Q - 1; i >= 0; --i) {
-    T eu = T(0), eF = T(0);
-    if (ex(i)) { eu += T(ex(i)) * u[0]; eF += T(ex(i)) * F[0]; }
-    if (ey(i)) { eu += T(ey(i)) * u[1]; eF += T(ey(i)) * F[1]; }
-    if (ez(i)) { eu += T(ez(i)) * u[2]; eF += T(ez(i)) * F[2]; }
-    const T feq = wgt<T>(i) * rho * (T(1) + T(3) * eu + T(4.5) * eu * eu - T(1.5) * uu);
-    const T S = wgt<T>(i) * (T(3) * (eF - uF) + T(9) * eu * eF);
-    T v = c1 * f[i] + om * feq + cS * S;
-    if (REMAINDER && i == 0) v = rho - acc;
-    if (i > 0) acc += v;
-    out[i] = v;
-  }
-}
-
-template <typename T>
-__device__ __forceinline__ void push_component(T* __restrict__ fo, int s, const T (&v)[Q],
-                                               const int (&id)[Q], int n, int nf, size_t npad) {
-  fo[pidx(s, 0, n, npad)] = v[0];
-#pragma unroll
-  for (int i = 1; i < Q; ++i) {
-    const int k = id[i];
-    if ((unsigned)k < (unsigned)nf) fo[pidx(s, i, k, npad)] = v[i];         // fluid neighbour
-    else if (k >= nf) fo[pidx(s, opp(i), n, npad)] = v[i];                   // halfway bounce-back
-    // k < 0: the population leaves through an open plane
-  }
-}
-
-template <typename T, bool REMAINDER>
-__global__ void __launch_bounds__(256) k_collide_stream(const T* __restrict__ fin,
-                                                        T* __restrict__ fout,
-                                                        const Vec2<T>* __restrict__ psi,
-                                                        const int* __restrict__ nbr, int nf,
-                                                        int nact, size_t npad, Consts<T> c) {
-  const int n = blockIdx.x * blockDim.x + threadIdx.x;
-  if (n >= nact) return;  // nact < nf in slab mode: halo nodes only receive pushes
-  int id[Q];
-  id[0] = n;
-#pragma unroll
-  for (int i = 1; i < Q; ++i) id[i] = nbr[(size_t)(i - 1) * npad + n];
-  T fa[Q], fb[Q];
-#pragma unroll
-  for (int i = 0; i < Q; ++i) {
-    fa[i] = fin[pidx(0, i, n, npad)];
-    fb[i] = fin[pidx(1, i, n, npad)];
-  }
-  NodeState<T> s;
-  node_state<T>(fa, fb, psi, id, c, s);
-  T v[Q];
-  collide_component<T, REMAINDER>(fa, s.rhoA, s.FA, s.u, s.om, v);
-  push_component<T>(fout, 0, v, id, n, nf, npad);
-  collide_component<T, REMAINDER>(fb, s.rhoB, s.FB, s.u, s.om, v);
-  push_component<T>(fout, 1, v, id, n, nf, npad);
-}
+// (the formulas above are implemented by collide_tile_thread below)
 
 // ---------------------------------------------------------------------------------------------
 // Bulk-async (TMA engine) staging for the fused pass.  One CTA owns a tile of TN consecutive
@@ -403,9 +354,11 @@ template <typename T> struct alignas(2 * sizeof(T)) Pr { T a, b; };
 
 __device__ __forceinline__ Pr<double> padd(Pr<double> x, Pr<double> y) { return {x.a + y.a, x.b + y.b}; }
 __device__ __forceinline__ Pr<double> psub(Pr<double> x, Pr<double> y) { return {x.a - y.a, x.b - y.b}; }
-__device__ __forceinline__ Pr<double> pmul(Pr<double> x, Pr<double> y) { return {x.a * y.a, x.b * y.b}; }
+__device__ __forceinline__ Pr<double> pmul(Pr<double> x, Pr<double> y) {
+  return {__dmul_rn(x.a, y.a), __dmul_rn(x.b, y.b)};
+}
 __device__ __forceinline__ Pr<double> pfma(Pr<double> x, Pr<double> y, Pr<double> z) {
-  return {x.a * y.a + z.a, x.b * y.b + z.b};
+  return {__fma_rn(x.a, y.a, z.a), __fma_rn(x.b, y.b, z.b)};
 }
 __device__ __forceinline__ Pr<float> padd(Pr<float> x, Pr<float> y) {
   Pr<float> d;
@@ -450,20 +403,67 @@ __device__ __forceinline__ Pr<T> edot2(int i, Pr<T> x, Pr<T> y, Pr<T> z) {
   return r;
 }
 
+// L2 eviction policies and hinted accesses of the single-kernel step (k_step_window).  evict_last
+// on the density items' loads keeps a tile's populations in L2 until the fused item of the same
+// tile reads them again a short while later; evict_first on that second read and streaming stores
+// let them leave first.
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ Vec2<float> load_vec2_keep(const Vec2<float>* p, uint64_t pol) {
+  Vec2<float> v;
+  asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;"
+               : "=f"(v.a), "=f"(v.b) : "l"(p), "l"(pol));
+  return v;
+}
+__device__ __forceinline__ Vec2<double> load_vec2_keep(const Vec2<double>* p, uint64_t pol) {
+  Vec2<double> v;
+  asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;"
+               : "=d"(v.a), "=d"(v.b) : "l"(p), "l"(pol));
+  return v;
+}
+__device__ __forceinline__ void bulk_g2s_hint(void* dst, const void* src, uint32_t bytes,
+                                              uint64_t* bar, uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
+      "[%0], [%1], %2, [%3], %4;" ::"r"(smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
+      : "memory");
+}
+// one (A, B) pair of a population; CS: streaming store
+template <bool CS>
+__device__ __forceinline__ void store_pair(Pr<float>* p, Pr<float> v) {
+  if constexpr (CS)
+    asm volatile("st.global.cs.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.a), "f"(v.b) : "memory");
+  else
+    *p = v;
+}
+template <bool CS>
+__device__ __forceinline__ void store_pair(Pr<double>* p, Pr<double> v) {
+  if constexpr (CS)
+    asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.a), "d"(v.b) : "memory");
+  else
+    *p = v;
+}
+
 // Per-thread work of the fused pass on a staged tile: sf = [38][TN] populations, sid = [18][TN]
 // neighbour ids in shared memory; tid = column of this thread in the tile; n = its node id.
 // Threads of the ragged last tile (valid = false) compute on the zero padding and only their
-// stores are predicated off, so control flow stays warp-uniform.
-// ROW0: the rest population of this thread's node comes in `r0` (a register pair loaded straight
-// from global memory) instead of row 0 of the staged tile, which is then not staged at all.
-template <typename T, int TN, bool REMAINDER, bool ROW0 = false>
+// stores are predicated off, so control flow stays warp-uniform.  CS: streaming push stores.
+template <typename T, int TN, bool REMAINDER, bool CS = false>
 __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
                                                     const int* __restrict__ sid, const int tid,
                                                     const int n, const bool valid,
                                                     T* __restrict__ fout,
                                                     const Vec2<T>* __restrict__ psi, const int nf,
-                                                    const size_t npad, const Consts<T>& c,
-                                                    const Pr<T> r0 = Pr<T>{T(0), T(0)}) {
+                                                    const size_t npad, const Consts<T>& c) {
   using P = Pr<T>;
   // staged populations: [19][TN] pairs (A, B); column tid
   const P* sfp = reinterpret_cast<const P*>(sf) + tid;
@@ -491,7 +491,7 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
       S[d] = pfma(pbc(wgt<T>(1)), a1[d], pmul(pbc(wgt<T>(7)), a2[d]));
   }
   // a1 (recomputed locally): R = (rho_A, rho_B); J[d] = per-component bare momentum
-  P R = ROW0 ? r0 : sfp[0];
+  P R = sfp[0];
   P J[3] = {{T(0), T(0)}, {T(0), T(0)}, {T(0), T(0)}};
 #pragma unroll
   for (int i = 1; i < Q; ++i) {
@@ -511,19 +511,19 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
   for (int d = 0; d < 3; ++d) {
     F[d] = pmul(R, pfma(pbc(-c.G), pswap(S[d]), pbc(g[d])));
     // a4: u_eq = (sum_sigma j_sigma + hf * sum_sigma F_sigma) / rho   (Eq. 8, R3)
-    u[d] = ((J[d].a + J[d].b) + c.hf * (F[d].a + F[d].b)) * inv;
+    u[d] = mul_rn(fma_rn(c.hf, add_rn(F[d].a, F[d].b), add_rn(J[d].a, J[d].b)), inv);
   }
-  const T om = rho / (R.a * c.tauA + R.b * c.tauB);  // 1/tau_s, Eq. (6)-(7)
+  const T om = rho / fma_rn(R.a, c.tauA, mul_rn(R.b, c.tauB));  // 1/tau_s, Eq. (6)-(7)
   // a5 in opposite-direction pairs (i, opp(i)): with A = 1 + 4.5 (e.u)^2 - 1.5 u.u and
   // B = 9 (e.u)(e.F) - 3 u.F, Eq. (1),(2),(9) give
   //   f*_i      = (1-om) f_i      + [om w rho A + cS w B] + 3 [om w rho (e.u) + cS w (e.F)]
   //   f*_opp(i) = (1-om) f_opp(i) + [om w rho A + cS w B] - 3 [om w rho (e.u) + cS w (e.F)]
   // with cS = 1 - om/2; both components at once as pairs.
-  const T k0 = T(1) - T(1.5) * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
-  const T c1 = T(1) - om, cS = T(1) - T(0.5) * om;
+  const T k0 = fma_rn(T(-1.5), fma_rn(u[2], u[2], fma_rn(u[1], u[1], mul_rn(u[0], u[0]))), T(1));
+  const T c1 = T(1) - om, cS = fma_rn(T(-0.5), om, T(1));
   const P M3UF = pmul(pbc(T(-3)), pfma(pbc(u[0]), F[0], pfma(pbc(u[1]), F[1], pmul(pbc(u[2]), F[2]))));
-  const P KA1 = pmul(pbc(om * wgt<T>(1)), R), KA2 = pmul(pbc(om * wgt<T>(7)), R);
-  const T kB1 = cS * wgt<T>(1), kB2 = cS * wgt<T>(7);
+  const P KA1 = pmul(pbc(mul_rn(om, wgt<T>(1))), R), KA2 = pmul(pbc(mul_rn(om, wgt<T>(7))), R);
+  const T kB1 = mul_rn(cS, wgt<T>(1)), kB2 = mul_rn(cS, wgt<T>(7));
   const unsigned np32 = (unsigned)npad;  // 19 * npad < 2^31: 32-bit pair-slot indices
   P* fo = reinterpret_cast<P*>(fout);  // pair (A, B) of population i at node k: fo[i * npad + k]
   P acc = {T(0), T(0)};
@@ -535,8 +535,8 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
     const T kB = ip < 7 ? kB1 : kB2;
     const T eu = edot<T>(ip, u[0], u[1], u[2]);
     const P EF = edot2<T>(ip, F[0], F[1], F[2]);
-    const T A = T(4.5) * eu * eu + k0;
-    const P B = pfma(pbc(T(9) * eu), EF, M3UF);
+    const T A = fma_rn(mul_rn(T(4.5), eu), eu, k0);
+    const P B = pfma(pbc(mul_rn(T(9), eu)), EF, M3UF);
     const P X = pfma(KA, pbc(A), pmul(pbc(kB), B));
     const P Y = pfma(KA, pbc(eu), pmul(pbc(kB), EF));
     const P fp = sfp[ip * TN];
@@ -551,13 +551,13 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
       const int k = sidc[(ip - 1) * TN];
       const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)ip * np32 + (unsigned)k
                                                        : (unsigned)im * np32 + (unsigned)n;
-      if (valid && k >= 0) fo[slot] = vp;
+      if (valid && k >= 0) store_pair<CS>(fo + slot, vp);
     }
     {
       const int k = sidc[(im - 1) * TN];
       const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)im * np32 + (unsigned)k
                                                        : (unsigned)ip * np32 + (unsigned)n;
-      if (valid && k >= 0) fo[slot] = vm;
+      if (valid && k >= 0) store_pair<CS>(fo + slot, vm);
     }
   }
   // rest population: Eq. (1) with e_0 = 0, or the remainder rho - sum_{i>=1} f*_i (fp32 build)
@@ -566,28 +566,10 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
     v0 = psub(R, acc);
   } else {
     const T w0 = wgt<T>(0);
-    const P f0 = ROW0 ? r0 : sfp[0];
-    v0 = pfma(pbc(c1), f0, pfma(pbc(om * w0 * k0), R, pmul(pbc(cS * w0), M3UF)));
+    const P f0 = sfp[0];
+    v0 = pfma(pbc(c1), f0, pfma(pbc(mul_rn(mul_rn(om, w0), k0)), R, pmul(pbc(mul_rn(cS, w0)), M3UF)));
   }
-  if (valid) fo[n] = v0;
-}
-
-// Stage one tile: 38 population rows + 18 neighbour-index rows of TN nodes -> shared memory,
-// completion on `bar`.  Call from one converged warp.
-template <typename T, int TN>
-__device__ __forceinline__ void load_tile(T* sf, int* sid, const T* __restrict__ fin,
-                                          const int* __restrict__ nbr, size_t npad, size_t t0,
-                                          uint64_t* bar) {
-  if (elect_one()) {
-    mbar_expect_tx(bar, (uint32_t)collide_smem_bytes<T, TN>());
-#pragma unroll
-    for (int r = 0; r < Q; ++r)  // one row of TN (A, B) pairs per direction
-      bulk_g2s(sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2, 2 * TN * sizeof(T), bar);
-#pragma unroll
-    for (int r = 0; r < 18; ++r)
-      bulk_g2s(sid + (size_t)r * TN, nbr + (size_t)r * npad + t0, TN * sizeof(int), bar);
-  }
-  __syncwarp();
+  if (valid) store_pair<CS>(fo + n, v0);
 }
 
 // 16-bit tile-relative neighbour index (geometry.hpp Index16): per tile 18 rows of TN uint16 plus
@@ -619,26 +601,110 @@ constexpr size_t collide16_smem_bytes() {
          kIdxMeta * sizeof(int);
 }
 
-// IDX: 0 = int32 neighbour rows, 1 = 16-bit tile-relative rows, 2 = geometric (bitmask) index
+// Shared-memory carve-up of one staged tile (16-bit index form)
+template <typename T, int TN, bool ALIAS>
+struct TileSmem {
+  T* sf;           // [38][TN] populations
+  int* sid;        // [18][TN] decoded neighbour ids
+  uint16_t* s16;   // [18][TN] staged 16-bit rows (inside the upper half of sid when ALIAS)
+  int* smeta;      // [kIdxMeta]
+  __device__ __forceinline__ explicit TileSmem(unsigned char* raw) {
+    sf = reinterpret_cast<T*>(raw);
+    sid = reinterpret_cast<int*>(raw + (size_t)2 * Q * TN * sizeof(T));
+    s16 = reinterpret_cast<uint16_t*>(raw + collide_smem_bytes<T, TN>() -
+                                      (ALIAS ? (size_t)18 * TN * sizeof(uint16_t) : 0));
+    smeta = reinterpret_cast<int*>(raw + collide16_smem_bytes<T, TN, ALIAS>() -
+                                   kIdxMeta * sizeof(int));
+  }
+};
+
+// Stage one tile: 19 population rows of TN (A, B) pairs, 18 rows of 16-bit index, the tile's
+// record of bases -> shared memory, completion on `bar`.  Call from one converged warp.
+// HINT: the population rows are read with the L2 policy `pol`.
+template <typename T, int TN, bool ALIAS, bool HINT>
+__device__ __forceinline__ void stage_tile16(const TileSmem<T, TN, ALIAS> sm,
+                                             const T* __restrict__ fin, const Idx16& ix,
+                                             size_t npad, unsigned tile, uint64_t* bar,
+                                             uint64_t pol) {
+  const size_t t0 = (size_t)tile * TN;
+  if (elect_one()) {
+    mbar_expect_tx(bar, (uint32_t)((size_t)2 * Q * TN * sizeof(T) +
+                                   (size_t)18 * TN * sizeof(uint16_t) + kIdxMeta * sizeof(int)));
+#pragma unroll
+    for (int r = 0; r < Q; ++r) {  // one row of TN (A, B) pairs per direction
+      if constexpr (HINT)
+        bulk_g2s_hint(sm.sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2,
+                      2 * TN * sizeof(T), bar, pol);
+      else
+        bulk_g2s(sm.sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2,
+                 2 * TN * sizeof(T), bar);
+    }
+#pragma unroll
+    for (int r = 0; r < 18; ++r)
+      bulk_g2s(sm.s16 + (size_t)r * TN, ix.nbr16 + (size_t)r * npad + t0, TN * sizeof(uint16_t),
+               bar);
+    bulk_g2s(sm.smeta, ix.meta + (size_t)tile * kIdxMeta, kIdxMeta * sizeof(int), bar);
+  }
+  __syncwarp();
+}
+
+// After the staged tile has arrived: decode this thread's column of the 16-bit rows into the
+// int32 form the tile function reads.  A neighbour beyond an open plane (reading R12 iv) is
+// recognised from the node's plane and e_z.  Rare "wide" tiles (an offset range does not fit 15
+// bits) take the int32 rows with a second round of bulk copies (one more phase of `bar`).
+// Called by every thread of the CTA.
+template <typename T, int TN, bool ALIAS, bool REREAD = false>
+__device__ __forceinline__ void decode_tile16(const TileSmem<T, TN, ALIAS> sm,
+                                              const int* __restrict__ nbr, const Idx16& ix,
+                                              size_t npad, size_t t0, int n, int tid, int warp,
+                                              uint64_t* bar, uint32_t& phase) {
+  const int wide = __shfl_sync(0xffffffffu, sm.smeta[36], 0);
+  if (wide) {
+    if (warp == 0) {
+      if (elect_one()) {
+        mbar_expect_tx(bar, (uint32_t)((size_t)18 * TN * sizeof(int)));
+#pragma unroll
+        for (int r = 0; r < 18; ++r)
+          bulk_g2s(sm.sid + (size_t)r * TN, nbr + (size_t)r * npad + t0, TN * sizeof(int), bar);
+      }
+      __syncwarp();
+    }
+    mbar_wait(bar, phase);
+    phase ^= 1u;
+  } else {
+    const bool lo_plane = n < ix.np_lo, hi_plane = n >= ix.nact - ix.np_hi;
+    int ev[Q];
+    if constexpr (ALIAS) {
+#pragma unroll
+      for (int i = 1; i < Q; ++i) ev[i] = sm.s16[(i - 1) * TN + tid];
+      __syncthreads();  // every column is in registers before the ids overwrite the rows
+    }
+#pragma unroll
+    for (int i = 1; i < Q; ++i) {
+      const int e = ALIAS ? ev[i] : (int)sm.s16[(i - 1) * TN + tid];
+      int k = sm.smeta[(e >> 15) * 18 + (i - 1)] + (e & 0x7fff);
+      if (ez(i) < 0) k = lo_plane ? -k - 1 : k;
+      if (ez(i) > 0) k = hi_plane ? -k - 1 : k;
+      sm.sid[(i - 1) * TN + tid] = k;
+    }
+  }
+  // REREAD: the tile function re-reads the ids from shared memory where it needs them; without
+  // this compiler barrier the 18 decoded ids are forwarded in registers across the psi gathers
+  // (fine in the one-tile kernel, more spills in the persistent one)
+  if constexpr (REREAD) asm volatile("" ::: "memory");
+}
+
+// The fused pass of the split step (one kernel per pass): one CTA per tile.
+// IDX: 1 = 16-bit tile-relative rows (default), 2 = geometric (bitmask) index (low-memory option)
 template <typename T, int TN, int MINB, bool REMAINDER, int IDX>
 __global__ void __launch_bounds__(TN, MINB)
     k_collide_stream_bulk(const T* __restrict__ fin, T* __restrict__ fout,
                           const Vec2<T>* __restrict__ psi, const int* __restrict__ nbr, int nf,
                           size_t npad, Consts<T> c, Idx16 ix) {
-  extern __shared__ __align__(128) unsigned char smem_dyn[];
-  // 8 CTAs per SM: row 0 (the rest populations) is not staged -- each thread loads its own pair
-  // from global memory -- which takes the CTA's last 1 KB off the shared-memory budget.  The
-  // layout below is kept by letting the (never touched) row 0 lie in front of the buffer.
-  constexpr bool kRow0 = IDX == 1 && MINB >= 8;
-  unsigned char* smem_raw = smem_dyn - (kRow0 ? (size_t)2 * TN * sizeof(T) : 0);
-  T* sf = reinterpret_cast<T*>(smem_raw);                                        // [38][TN]
-  int* sid = reinterpret_cast<int*>(smem_raw + (size_t)2 * Q * TN * sizeof(T));  // [18][TN]
+  static_assert(IDX == 1 || IDX == 2, "index form");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr bool kAlias = IDX == 1 && MINB >= 7;
-  uint16_t* s16 = reinterpret_cast<uint16_t*>(
-      smem_raw + collide_smem_bytes<T, TN>() -
-      (kAlias ? (size_t)18 * TN * sizeof(uint16_t) : 0));                        // [18][TN]
-  int* smeta = reinterpret_cast<int*>(smem_raw + collide16_smem_bytes<T, TN, kAlias>() -
-                                      kIdxMeta * sizeof(int));                   // [kIdxMeta]
+  const TileSmem<T, TN, kAlias> sm(smem_raw);
   __shared__ uint64_t bar;
   const int tid = threadIdx.x;
   // Tiles are taken from the END of the id range first: the density pass that ran just before
@@ -651,18 +717,15 @@ __global__ void __launch_bounds__(TN, MINB)
   __syncthreads();
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // compiler-visible warp-uniform value
   const int n = (int)t0 + tid;
-  if constexpr (IDX == 0) {
-    if (warp == 0) load_tile<T, TN>(sf, sid, fin, nbr, npad, t0, &bar);
-    pdl_wait();
-    mbar_wait(&bar, 0);
-  } else if constexpr (IDX == 2) {
+  uint32_t phase = 0;
+  if constexpr (IDX == 2) {
     if (warp == 0) {
       if (elect_one()) {
         mbar_expect_tx(&bar, (uint32_t)((size_t)2 * Q * TN * sizeof(T)));
 #pragma unroll
         for (int r = 0; r < Q; ++r)  // one row of TN (A, B) pairs per direction
-          bulk_g2s(sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2, 2 * TN * sizeof(T),
-                   &bar);
+          bulk_g2s(sm.sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2,
+                   2 * TN * sizeof(T), &bar);
       }
       __syncwarp();
     }
@@ -703,241 +766,23 @@ __global__ void __launch_bounds__(TN, MINB)
         const bool fl = (q.x >> bit[dx]) & 1u;
         int k = fl ? (int)(q.z + __popc(q.x & below[dx])) : (int)(q.w + __popc(q.y & below[dx]));
         if (ez(i) != 0 && beyond[dz]) k = -k - 1;
-        sid[(i - 1) * TN + tid] = k;
+        sm.sid[(i - 1) * TN + tid] = k;
       }
     }
     pdl_wait();
-    mbar_wait(&bar, 0);
+    mbar_wait(&bar, phase);
+    phase ^= 1u;
   } else {
-    if (warp == 0) {
-      if (elect_one()) {
-        mbar_expect_tx(&bar, (uint32_t)((size_t)2 * (kRow0 ? Q - 1 : Q) * TN * sizeof(T) +
-                                        (size_t)18 * TN * sizeof(uint16_t) + kIdxMeta * sizeof(int)));
-#pragma unroll
-        for (int r = kRow0 ? 1 : 0; r < Q; ++r)  // one row of TN (A, B) pairs per direction
-          bulk_g2s(sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2, 2 * TN * sizeof(T),
-                   &bar);
-#pragma unroll
-        for (int r = 0; r < 18; ++r)
-          bulk_g2s(s16 + (size_t)r * TN, ix.nbr16 + (size_t)r * npad + t0, TN * sizeof(uint16_t),
-                   &bar);
-        bulk_g2s(smeta, ix.meta + (size_t)tile * kIdxMeta, kIdxMeta * sizeof(int), &bar);
-      }
-      __syncwarp();
-    }
+    if (warp == 0) stage_tile16<T, TN, kAlias, false>(sm, fin, ix, npad, tile, &bar, 0);
     // the bulk copies above read the populations (complete since the previous step; the density
     // pass that fixed the open planes finished before the wall pass began) and the static index;
     // psi and the wall psi are this step's
     pdl_wait();
-    mbar_wait(&bar, 0);
-    const int wide = __shfl_sync(0xffffffffu, smeta[36], 0);
-    if (wide) {
-      // rare: an offset range of this tile does not fit 15 bits -> take the int32 rows
-      if (warp == 0) {
-        if (elect_one()) {
-          mbar_expect_tx(&bar, (uint32_t)((size_t)18 * TN * sizeof(int)));
-#pragma unroll
-          for (int r = 0; r < 18; ++r)
-            bulk_g2s(sid + (size_t)r * TN, nbr + (size_t)r * npad + t0, TN * sizeof(int), &bar);
-        }
-        __syncwarp();
-      }
-      mbar_wait(&bar, 1);
-    } else {
-      // decode this thread's column into the int32 form the tile function reads; a neighbour
-      // beyond an open plane (reading R12 iv) is recognised from the node's plane and e_z
-      const bool lo_plane = n < ix.np_lo, hi_plane = n >= ix.nact - ix.np_hi;
-      int ev[Q];
-      if constexpr (kAlias) {
-#pragma unroll
-        for (int i = 1; i < Q; ++i) ev[i] = s16[(i - 1) * TN + tid];
-        __syncthreads();  // every column is in registers before the ids overwrite the rows
-      }
-#pragma unroll
-      for (int i = 1; i < Q; ++i) {
-        const int e = kAlias ? ev[i] : (int)s16[(i - 1) * TN + tid];
-        int k = smeta[(e >> 15) * 18 + (i - 1)] + (e & 0x7fff);
-        if (ez(i) < 0) k = lo_plane ? -k - 1 : k;
-        if (ez(i) > 0) k = hi_plane ? -k - 1 : k;
-        sid[(i - 1) * TN + tid] = k;
-      }
-    }
+    mbar_wait(&bar, phase);
+    phase ^= 1u;
+    decode_tile16<T, TN, kAlias>(sm, nbr, ix, npad, t0, n, tid, warp, &bar, phase);
   }
-  if constexpr (kRow0) {
-    const Vec2<T> v = reinterpret_cast<const Vec2<T>*>(fin)[n];  // n < npad; complete like the tile
-    collide_tile_thread<T, TN, REMAINDER, true>(sf, sid, tid, n, n < ix.nact, fout, psi, nf, npad,
-                                                c, Pr<T>{v.a, v.b});
-  } else {
-    collide_tile_thread<T, TN, REMAINDER>(sf, sid, tid, n, n < ix.nact, fout, psi, nf, npad, c);
-  }
-}
-
-// ---------------------------------------------------------------------------------------------
-// Fused single-kernel step (EXPERIMENTAL, LBM_B200_STEP=fused; slower than the default one kernel
-// per pass on B200).  The two grid-wide dependencies of a step -- every
-// node's force needs its neighbours' rho(t), every wall solid's rho~(t) needs its fluid
-// neighbours' rho(t) -- are resolved INSIDE one persistent kernel instead of by kernel
-// boundaries, so that the density pass runs only a short distance ahead of the fused pass and the
-// populations it has just read are still in the 126 MB L2 when the fused pass reads them again
-// (saves the second 152 B/node DRAM read of the two-pass method).
-//
-// Work items (tiles of TN consecutive ids): D(t) density, W(j) virtual solid density, C(t) fused
-// force+collide+stream; host-built global order `sched` in which every item follows the items
-// whose psi it reads (geometry.hpp Schedule).  CTAs take items with an atomic ticket.  D and W
-// items publish a per-tile completion flag; a consumer polls exactly the ~10 tiles its psi stencil
-// touches (wait_ranges).  All CTAs are co-resident (cooperative launch), tickets are handed
-// out in schedule order and every wait is on an earlier item: the item with the smallest ticket
-// can always finish, so the scheme cannot deadlock.
-__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
-  int v;
-  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
-  int v;
-  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st_release_gpu(int* p, int v) {
-  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-// Completion tracking.  D(t) / W(j) publish flags[t] = epoch with a gpu-scope release store after
-// the CTA barrier that follows their psi stores (release is cumulative over the barrier).  A
-// consumer checks exactly the tiles it depends on, given as up to 3 (lo,cnt) ranges: one warp
-// polls 32 flags per round with relaxed gpu-scope loads (served by L2) until all carry this
-// step's epoch; the CTA barrier that follows orders every thread's psi loads after the poll.
-// No acquire fence is used: a gpu-scope acquire invalidates the SM's whole L1 (CCTL.IVALL), which
-// six co-resident CTAs pay for on every item, and it is not needed here -- a psi line can only
-// enter an L1 after its tile's flag was seen set (tiles are line-aligned), i.e. with final data,
-// and L1 does not survive a kernel boundary.  Call from all 32 lanes of one warp.
-__device__ __forceinline__ void wait_ranges(const int* __restrict__ flags, const int* rng,
-                                            int epoch) {
-  const int lane = threadIdx.x & 31;
-#pragma unroll
-  for (int r = 0; r < 3; ++r) {
-    const int lo = rng[2 * r], cnt = rng[2 * r + 1];
-    for (int b = 0; b < cnt; b += 32) {
-      const int k = b + lane;
-      while (true) {
-        const int ok = k >= cnt || ld_relaxed_gpu(flags + lo + k) == epoch;
-        if (__all_sync(0xffffffffu, ok)) break;
-        __nanosleep(64);
-      }
-    }
-  }
-}
-
-struct FusedSched {
-  int* flags_d;        // [ntf] epoch of the last step in which D(t) completed
-  int* flags_w;        // [ntw]
-  int epoch;           // this step's epoch (> 0, increases by one per step)
-  const int4* items;   // [nitems][4] = 16 ints per item (geometry.hpp kRecordInts):
-                       //   {type << 30 | tile, D deps 3 x (lo,cnt), W deps 3 x (lo,cnt), 0, 0, 0}
-  int nitems;
-};
-
-template <typename T, int TN, int MINB, bool REMAINDER>
-__global__ void __launch_bounds__(TN, MINB)
-    k_step_fused(const T* __restrict__ fin, T* __restrict__ fout, Vec2<T>* __restrict__ psi,
-                 const int* __restrict__ nbr, const int* __restrict__ wall_nbr,
-                 const T* __restrict__ inv_den, int nf, int nw, size_t npad, size_t nwpad,
-                 Consts<T> c, FusedSched sc, int* __restrict__ ctr, int* __restrict__ ctr_next) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  T* sf = reinterpret_cast<T*>(smem_raw);                                        // [38][TN]
-  int* sid = reinterpret_cast<int*>(smem_raw + (size_t)2 * Q * TN * sizeof(T));  // [18][TN]
-  __shared__ uint64_t bar;
-  const int tid = threadIdx.x;
-  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // compiler-visible warp-uniform value
-  if (tid == 0) {
-    mbar_init(&bar, 1);
-    if (blockIdx.x == 0) {  // the other watermark set is idle during this launch: reset it
-    }
-  }
-  __syncthreads();
-  uint32_t phase = 0;
-  // Items are handed out in schedule order by an atomic ticket (fast CTAs take more items, so no
-  // CTA falls behind the others).  A ticket holder waits only on items with smaller tickets,
-  // which are finished or running on co-resident CTAs: progress is guaranteed.  Thread 0 draws
-  // the NEXT ticket and fetches its record while the CTA works on the current item.
-  __shared__ __align__(16) int s_rec[2][16];  // double-buffered item record
-  if (tid < 4) {
-    int k = 0;
-    if (tid == 0) k = atomicAdd(&ctr[0], 1);
-    k = __shfl_sync(0xfu, k, 0);
-    reinterpret_cast<int4*>(s_rec[0])[tid] =
-        k < sc.nitems ? __ldg(sc.items + (size_t)4 * k + tid) : make_int4(-1, 0, 0, 0);
-    if (blockIdx.x == 0 && tid == 0) ctr_next[0] = 0;
-  }
-  __syncthreads();
-  int buf = 0;
-  while (true) {
-    const int* rec = s_rec[buf];
-    const int head = __shfl_sync(0xffffffffu, rec[0], 0);
-    if (head == -1) break;
-    // draw the next ticket and fetch its record into the other buffer (read next iteration)
-    if (tid < 4) {
-      int k = 0;
-      if (tid == 0) k = atomicAdd(&ctr[0], 1);
-      k = __shfl_sync(0xfu, k, 0);
-      reinterpret_cast<int4*>(s_rec[buf ^ 1])[tid] =
-          k < sc.nitems ? __ldg(sc.items + (size_t)4 * k + tid) : make_int4(-1, 0, 0, 0);
-    }
-    const int type = (int)((unsigned)head >> 30), t = head & 0x3fffffff;
-    if (type == 0) {
-      // ---- D(t): a1 on fluid tile t
-      const int n = t * TN + tid;
-      const Vec2<T>* f2 = reinterpret_cast<const Vec2<T>*>(fin);
-      Vec2<T> v0 = f2[n];
-      T ra = v0.a, rb = v0.b;
-#pragma unroll
-      for (int i = 1; i < Q; ++i) {
-        const Vec2<T> v = f2[(size_t)i * npad + n];
-        ra += v.a;
-        rb += v.b;
-      }
-      Vec2<T> o; o.a = ra; o.b = rb;
-      psi[n] = o;  // n < npad always; the padding holds zeros
-      __syncthreads();
-      if (tid == 0) st_release_gpu(sc.flags_d + t, sc.epoch);
-    } else if (type == 1) {
-      // ---- W(j): a2 on wall tile t
-      if (warp == 0) wait_ranges(sc.flags_d, rec + 1, sc.epoch);
-      __syncthreads();
-      const int w = t * TN + tid;
-      if (w < nw) {
-        T na = T(0), nb = T(0);
-#pragma unroll
-        for (int i = 1; i < Q; ++i) {
-          const int id = wall_nbr[(size_t)(i - 1) * nwpad + w];
-          if (id >= 0) {
-            const Vec2<T> p = psi[id];
-            na += wgt<T>(i) * p.a;
-            nb += wgt<T>(i) * p.b;
-          }
-        }
-        const T s = inv_den[w];
-        Vec2<T> o; o.a = c.chiA * na * s; o.b = c.chiB * nb * s;
-        psi[npad + w] = o;
-      }
-      __syncthreads();
-      if (tid == 0) st_release_gpu(sc.flags_w + t, sc.epoch);
-    } else {
-      // ---- C(t): a3-a6 on fluid tile t.  The tile's populations and ids do not depend on psi:
-      // their bulk copies are issued before the dependency wait.
-      if (warp == 0) {
-        load_tile<T, TN>(sf, sid, fin, nbr, npad, (size_t)t * TN, &bar);
-        wait_ranges(sc.flags_d, rec + 1, sc.epoch);
-        wait_ranges(sc.flags_w, rec + 7, sc.epoch);
-      }
-      __syncthreads();
-      mbar_wait(&bar, phase);
-      phase ^= 1u;
-      const int n = t * TN + tid;
-      collide_tile_thread<T, TN, REMAINDER>(sf, sid, tid, n, n < nf, fout, psi, nf, npad, c);
-    }
-    buf ^= 1;
-    __syncthreads();  // next record is in place; the stage is free for the next C item
-  }
+  collide_tile_thread<T, TN, REMAINDER>(sm.sf, sm.sid, tid, n, n < ix.nact, fout, psi, nf, npad, c);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -961,8 +806,11 @@ __device__ __forceinline__ T feq_of(int i, T rho, const T (&u)[3]) {
   if (ex(i)) eu += T(ex(i)) * u[0];
   if (ey(i)) eu += T(ey(i)) * u[1];
   if (ez(i)) eu += T(ez(i)) * u[2];
-  const T uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
-  return wgt<T>(i) * rho * (T(1) + T(3) * eu + T(4.5) * eu * eu - T(1.5) * uu);
+  const T uu = fma_rn(u[2], u[2], fma_rn(u[1], u[1], mul_rn(u[0], u[0])));
+  T t = fma_rn(T(3), eu, T(1));
+  t = fma_rn(mul_rn(T(4.5), eu), eu, t);
+  t = fma_rn(T(-1.5), uu, t);
+  return mul_rn(mul_rn(wgt<T>(i), rho), t);
 }
 
 // One node of an open plane: applies the fix in place and returns the node's new densities,
@@ -990,7 +838,7 @@ __device__ __forceinline__ Vec2<T> open_plane_node(T* __restrict__ f, const T* _
         if (ez(i)) j[2] += T(ez(i)) * v;
       }
     const T inv = T(1) / (rf[0] + rf[1]);
-    const T uf[3] = {j[0] * inv, j[1] * inv, j[2] * inv};  // R12 iii: bare mixture velocity
+    const T uf[3] = {mul_rn(j[0], inv), mul_rn(j[1], inv), mul_rn(j[2], inv)};  // R12 iii: bare mixture velocity
     const T rfd = dc == 0 ? rf[0] : rf[1];
     T rho_b, ub[3];
     if (op.kind[plane] == 1) {
@@ -1003,7 +851,7 @@ __device__ __forceinline__ Vec2<T> open_plane_node(T* __restrict__ f, const T* _
 #pragma unroll
     for (int i = 0; i < Q; ++i) {
       const T fi = dc == 0 ? ff[0][i] : ff[1][i];
-      const T v = feq_of<T>(i, rho_b, ub) + (fi - feq_of<T>(i, rfd, uf));
+      const T v = add_rn(feq_of<T>(i, rho_b, ub), add_rn(fi, -feq_of<T>(i, rfd, uf)));
       f[pidx(dc, i, vb, npad)] = v;
       rd = i == 0 ? v : rd + v;
     }
@@ -1022,8 +870,8 @@ __device__ __forceinline__ Vec2<T> open_plane_node(T* __restrict__ f, const T* _
         const T v = f[pidx(dc, i, vb, npad)];
         fb[i] = v;
         K0 += v;
-        if (ex(i)) Nx += T(0.5) * T(ex(i)) * v;
-        if (ey(i)) Ny += T(0.5) * T(ey(i)) * v;
+        if (ex(i)) Nx = fma_rn(T(0.5) * T(ex(i)), v, Nx);
+        if (ey(i)) Ny = fma_rn(T(0.5) * T(ey(i)), v, Ny);
       } else if (ez(i) == -sgn) {
         const T v = f[pidx(dc, i, vb, npad)];
         fb[i] = v;
@@ -1035,17 +883,17 @@ __device__ __forceinline__ Vec2<T> open_plane_node(T* __restrict__ f, const T* _
     T rho, uz;
     if (op.kind[plane] == 3) {
       rho = op.rho[plane];
-      uz = T(sgn) * (T(1) - (K0 + T(2) * Km) / rho);
+      uz = mul_rn(T(sgn), add_rn(T(1), -(fma_rn(T(2), Km, K0) / rho)));
     } else {
       uz = op.uz[plane];
-      rho = (K0 + T(2) * Km) / (T(1) - T(sgn) * uz);
+      rho = fma_rn(T(2), Km, K0) / add_rn(T(1), -mul_rn(T(sgn), uz));
     }
 #pragma unroll
     for (int i = 1; i < Q; ++i) {
       if (ez(i) == 0 || ez(i) != sgn) continue;
-      T v = fb[opp(i)] + T(6) * wgt<T>(i) * rho * (T(ez(i)) * uz);
-      if (ex(i)) v -= T(ex(i)) * Nx;
-      if (ey(i)) v -= T(ey(i)) * Ny;
+      T v = add_rn(fb[opp(i)], mul_rn(mul_rn(T(6) * wgt<T>(i), rho), mul_rn(T(ez(i)), uz)));
+      if (ex(i)) v = add_rn(v, -mul_rn(T(ex(i)), Nx));
+      if (ey(i)) v = add_rn(v, -mul_rn(T(ey(i)), Ny));
       fb[i] = v;
       f[pidx(dc, i, vb, npad)] = v;
     }
@@ -1120,6 +968,208 @@ __global__ void __launch_bounds__(256, 4)
     if (op.kind[plane] == 0) return;
     store_vec2(psi + (plane == 0 ? q : nf - np + q),
                open_plane_node<T>(f, frozen, nf, np, npad, op, plane, q), pol);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Single-kernel step ("window" step).  The two grid-wide dependencies of a step -- every node's
+// force needs its neighbours' rho(t) (Eq. 11/13), every wall solid's rho~(t) needs its fluid
+// neighbours' rho(t) (Eq. 15) -- are resolved INSIDE one persistent kernel instead of by kernel
+// boundaries, so that the density pass runs only a short, fixed distance (the "lead", ~20 MB of
+// populations) ahead of the fused pass: the populations it has just read are then still in the
+// 126 MB L2 when the fused pass reads them again, and the second 152 B/node DRAM read of the
+// two-pass method disappears (472 -> ~320 B/node of DRAM traffic).
+//
+// Work items over tiles of TN consecutive ids, in ONE host-built order (geometry.hpp Window) in
+// which every item follows the items it depends on:
+//   D(t)  a1 on fluid tile t             publishes flags_d[t]
+//   W(j)  a2 on wall tile j              needs D of its fluid neighbours; publishes flags_w[j]
+//   C(t)  a3-a6 on fluid tile t          needs D and W of its psi stencil; publishes flags_c[t]
+//   P(k)  a0 on TN nodes of an open plane (after streaming, as PAPER.md L147-157 has it)
+//                                        needs C of every tile that pushes into those nodes or
+//                                        into their interior neighbours
+// CTAs take items with an atomic ticket, in that order.  A ticket holder waits only on items with
+// smaller tickets, which are finished or held by running CTAs, so the scheme cannot deadlock and
+// needs no co-residency guarantee.  An item's dependencies are at most 6 (lo,cnt) ranges of flags
+// (a psi stencil touches ~10 D tiles in three id ranges, one per z-plane); one warp loads all of
+// them at once and spins until each carries this step's epoch.  Producers run far enough ahead
+// (lead) that the flags are normally already set.
+//
+// Visibility.  A producer's stores are followed by the CTA barrier at the end of the item and a
+// gpu-scope release store of the flag by thread 0 (release is cumulative over the barrier).  The
+// consumer's warp 0 polls with relaxed gpu-scope loads (served by L2), and the CTA barrier that
+// follows orders every thread's loads after the poll.  No acquire fence is used: a gpu-scope
+// acquire invalidates the SM's whole L1 (CCTL.IVALL), which seven co-resident CTAs would pay on
+// every item, and it is not needed -- within one launch every psi / fout line is written once,
+// a line can only enter an L1 after the flag of its (line-aligned) tile was seen set, i.e. with
+// final data, and L1 does not survive a kernel boundary.
+__device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
+  int v;
+  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_gpu(int* p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+constexpr int kWinRecordInts = 16;  // geometry.hpp kWinRecordInts
+// rec[1..12] = 6 x (lo,cnt): ranges 0-2 index fa, ranges 3-5 index fb.  Call from all 32 lanes of
+// one warp.
+__device__ __forceinline__ void wait_flags(const int* __restrict__ fa, const int* __restrict__ fb,
+                                           const int* rec, int epoch) {
+  const int lane = threadIdx.x & 31;
+  int total = 0;
+#pragma unroll
+  for (int r = 0; r < 6; ++r) total += rec[2 + 2 * r];
+  for (int base = 0; base < total; base += 32) {
+    const int k = base + lane;
+    const int* p = nullptr;
+    int c0 = 0;
+#pragma unroll
+    for (int r = 0; r < 6; ++r) {
+      const int cnt = rec[2 + 2 * r];
+      if (k >= c0 && k < c0 + cnt) p = (r < 3 ? fa : fb) + rec[1 + 2 * r] + (k - c0);
+      c0 += cnt;
+    }
+    while (true) {
+      const int ok = p == nullptr || ld_relaxed_gpu(p) == epoch;
+      if (__all_sync(0xffffffffu, ok)) break;
+      __nanosleep(32);
+    }
+  }
+}
+
+struct WinSched {
+  const int4* items;   // [nitems][4]: 16 ints per item = {type << 28 | tile, 6 x (lo,cnt), 0, 0, 0}
+  int nitems;
+  int* flags_d;        // [fluid tiles]  epoch of the last step in which D(t) completed
+  int* flags_w;        // [wall tiles]
+  int* flags_c;        // [fluid tiles]  (used by the P items: only in z-open boxes)
+  int epoch;           // this step's epoch (> 0, increases by one per step)
+  int np;              // nodes per z-plane; P item k covers plane k / ntp, nodes (k % ntp)*TN ...
+  int ntp;             // P items per open plane
+};
+
+template <typename T, int TN, int MINB, bool REMAINDER>
+__global__ void __launch_bounds__(TN, MINB)
+    k_step_window(const T* __restrict__ fin, T* __restrict__ fout, Vec2<T>* __restrict__ psi,
+                  const int* __restrict__ nbr, const int* __restrict__ wall_nbr,
+                  const T* __restrict__ inv_den, const T* __restrict__ frozen, int nf, int nw,
+                  size_t npad, size_t nwpad, Consts<T> c, Idx16 ix, OpenPlane<T> op, WinSched sc,
+                  int* __restrict__ ctr, int* __restrict__ ctr_next) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr bool kAlias = MINB >= 7;
+  const TileSmem<T, TN, kAlias> sm(smem_raw);
+  __shared__ uint64_t bar;
+  __shared__ __align__(16) int s_rec[2][kWinRecordInts];  // double-buffered item record
+  const int tid = threadIdx.x;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // compiler-visible warp-uniform value
+  if (tid == 0) mbar_init(&bar, 1);
+  // Thread 0 draws a ticket, threads 0-3 fetch its record; the NEXT ticket is drawn while the CTA
+  // works on the current item.
+  if (tid < 4) {
+    int k = 0;
+    if (tid == 0) k = atomicAdd(&ctr[0], 1);
+    k = __shfl_sync(0xfu, k, 0);
+    reinterpret_cast<int4*>(s_rec[0])[tid] =
+        k < sc.nitems ? __ldg(sc.items + (size_t)4 * k + tid) : make_int4(-1, 0, 0, 0);
+    if (blockIdx.x == 0 && tid == 0) ctr_next[0] = 0;  // the other step's counter is idle now
+  }
+  __syncthreads();
+  uint32_t phase = 0;
+  int buf = 0;
+  while (true) {
+    const int* rec = s_rec[buf];
+    const int head = __shfl_sync(0xffffffffu, rec[0], 0);
+    if (head == -1) break;
+    if (tid < 4) {
+      int k = 0;
+      if (tid == 0) k = atomicAdd(&ctr[0], 1);
+      k = __shfl_sync(0xfu, k, 0);
+      reinterpret_cast<int4*>(s_rec[buf ^ 1])[tid] =
+          k < sc.nitems ? __ldg(sc.items + (size_t)4 * k + tid) : make_int4(-1, 0, 0, 0);
+    }
+    const int type = (int)((unsigned)head >> 28), t = head & 0x0fffffff;
+    if (type == 0) {
+#ifndef WIN_NO_D
+      // ---- D(t): a1 on fluid tile t, summed in direction order exactly as k_density does
+      const int n = t * TN + tid;  // < npad; the padding holds zeros
+      const Vec2<T>* f2 = reinterpret_cast<const Vec2<T>*>(fin);
+      const uint64_t keep = l2_policy_evict_last();
+      Vec2<T> v[Q];
+#pragma unroll
+      for (int i = 0; i < Q; ++i) v[i] = load_vec2_keep(f2 + (size_t)i * npad + n, keep);
+      T ra = v[0].a, rb = v[0].b;
+#pragma unroll
+      for (int i = 1; i < Q; ++i) { ra += v[i].a; rb += v[i].b; }
+      Vec2<T> o; o.a = ra; o.b = rb;
+      psi[n] = o;
+#endif
+    } else if (type == 1) {
+#ifndef WIN_NO_W
+      // ---- W(j): a2 on wall tile t (Eq. 14-15), as k_wallpsi
+      const int w = t * TN + tid;
+      const bool live = w < nw;
+      int id[Q];
+#pragma unroll
+      for (int i = 1; i < Q; ++i) id[i] = live ? wall_nbr[(size_t)(i - 1) * nwpad + w] : -1;
+      const T s = live ? inv_den[w] : T(0);
+      if (warp == 0) wait_flags(sc.flags_d, sc.flags_d, rec, sc.epoch);
+      __syncthreads();
+      if (live) {
+        T na = T(0), nb = T(0);
+#pragma unroll
+        for (int i = 1; i < Q; ++i) {
+          if (id[i] >= 0) {
+            const Vec2<T> p = psi[id[i]];
+            na = fma_rn(wgt<T>(i), p.a, na);
+            nb = fma_rn(wgt<T>(i), p.b, nb);
+          }
+        }
+        Vec2<T> o; o.a = mul_rn(mul_rn(c.chiA, na), s); o.b = mul_rn(mul_rn(c.chiB, nb), s);
+        psi[npad + w] = o;
+      }
+#endif
+    } else if (type == 2) {
+      // ---- C(t): a3-a6 on fluid tile t.  The tile's populations and index do not depend on
+      // psi: their bulk copies are in flight while warp 0 checks the flags.
+      // (the row stride is laundered through an empty asm so that the compiler does not hoist the
+      // 37 row offsets out of the item loop and then spill them)
+      size_t np_it = npad;
+      asm volatile("" : "+l"(np_it));
+      if (warp == 0) {
+        stage_tile16<T, TN, kAlias, true>(sm, fin, ix, np_it, (unsigned)t, &bar,
+                                          l2_policy_evict_first());
+        wait_flags(sc.flags_d, sc.flags_w, rec, sc.epoch);
+      }
+      __syncthreads();
+      mbar_wait(&bar, phase);
+      phase ^= 1u;
+      const size_t t0 = (size_t)t * TN;
+      const int n = (int)t0 + tid;
+      decode_tile16<T, TN, kAlias, true>(sm, nbr, ix, np_it, t0, n, tid, warp, &bar, phase);
+      collide_tile_thread<T, TN, REMAINDER, true>(sm.sf, sm.sid, tid, n, n < nf, fout, psi, nf,
+                                                  np_it, c);
+      // the decoded ids were written through the generic proxy; the next item's bulk copies write
+      // the same shared memory through the async proxy
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    } else {
+      // ---- P(k): a0 on TN nodes of an open plane of the NEW buffer (reading R12)
+#ifndef WIN_NO_P
+      if (warp == 0) wait_flags(sc.flags_c, sc.flags_c, rec, sc.epoch);
+      __syncthreads();
+      const int plane = t / sc.ntp, q = (t - plane * sc.ntp) * TN + tid;
+      if (q < sc.np && op.kind[plane] != 0)
+        open_plane_node<T>(fout, frozen, nf, sc.np, npad, op, plane, q);
+#endif
+    }
+    __syncthreads();  // the item's stores are issued; the stage is free; the next record is in place
+    if (tid == 0) {
+      int* flag = type == 0 ? sc.flags_d + t : type == 1 ? sc.flags_w + t
+                  : (type == 2 && sc.flags_c) ? sc.flags_c + t : nullptr;
+      if (flag) st_release_gpu(flag, sc.epoch);
+    }
+    buf ^= 1;
   }
 }
 

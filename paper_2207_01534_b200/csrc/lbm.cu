@@ -103,38 +103,34 @@ struct lbm_ctx {
   int cur = 0;
   bool open_pending = false;  // the open-plane fix of the last step has not been applied yet (it
                               // is folded into the next density pass, or applied by a getter)
-  int collide_variant = 1;  // 0: register kernel (A/B reference), 1: bulk-async staged tiles
-                            // (production); env LBM_B200_COLLIDE=simple|bulk
   int num_sms = 148;
   int idx16 = 1;            // index the fused pass reads: 1 = 16-bit tile-relative rows (default),
-                            // 0 = int32 rows (env LBM_B200_IDX=32), 2 = geometric bitmask index
-                            // (env LBM_B200_IDX=bits; geometry.hpp BitIndex)
+                            // 2 = geometric bitmask index (lbm_options.index = LBM_INDEX_BITS;
+                            // geometry.hpp BitIndex)
   uint32_t* bit_rec = nullptr;       // [nz*ny][bit_words][4]
   uint32_t* bit_coord = nullptr;     // [npad]
   int bit_words = 0;
   uint16_t* nbr16 = nullptr;         // [18][npad]
   int* nbr16_meta = nullptr;         // [tiles][kIdxMeta]
   long long wide_tiles = 0;
-  int reverse = 1;          // fused pass walks the tiles backwards (L2 reuse across passes); env LBM_B200_REVERSE=0
-  int step_variant = 0;     // 0: one kernel per pass (split, default), 1: fused persistent step kernel
-                            // (experimental); env LBM_B200_STEP=split|fused
-  int fused_grid = 0;       // co-resident CTAs of the fused kernel
-  int4* sched_items = nullptr;       // fused-step schedule records (geometry.hpp Schedule)
-  int sched_nitems = 0, sched_ntf = 0, sched_ntw = 0;
-  int* fused_ctr = nullptr;          // [2][4] ticket / D watermark / W watermark, alternating per step
-  int* fused_flags = nullptr;        // [ntf+32 | ntw+32] per-rank completion epochs
-  int fused_epoch = 0;
-  int fused_parity = 0;
+  int reverse = 1;          // fused pass of the split step walks the tiles backwards (L2 reuse across passes)
+  int step_variant = 0;     // 0: one kernel per pass (split), 1: single-kernel window step
+  int win_grid = 0;         // CTAs of the window kernel (resident CTAs per SM x SMs)
+  int win_reach = 0, win_slack = 0;
+  int win_ctas = 7;         // resident CTAs per SM the fp32 window kernel is compiled for (6: 80 registers)
+  int4* win_items = nullptr;         // window-step schedule records (geometry.hpp Window)
+  int win_nitems = 0, win_ntf = 0, win_ntw = 0, win_ntp = 0;
+  int* win_ctr = nullptr;            // [2][4] ticket counters, alternating per step
+  int* win_flags = nullptr;          // [ntf | ntw | ntf] completion epochs of D, W, C items
+  int win_epoch = 0;
+  int win_parity = 0;
   float keep_psi = 0.f;     // share of the psi lines stored with L2 evict_last priority, from
-  int keep_psi_mb = 48;     // this budget: min(1, MB / psi bytes); env LBM_B200_KEEP_PSI_MB (0: off)
-  int pdl = 1;              // programmatic dependent launch of the three passes; env LBM_B200_PDL=0
-  int tile = 1287;          // fp32 bulk kernel variant: tile nodes * 10 + min CTAs/SM; env LBM_B200_TILE
-                            // (1287: 7 CTAs per SM at 72 registers, the 16-bit rows staged inside the
-                            // id array; 1286: 6 CTAs at 80 registers, the previous default)
+  int keep_psi_mb = 48;     // this budget: min(1, MB / psi bytes) (0: off)
+  int pdl = 1;              // programmatic dependent launch of the three passes of the split step
   // Launch-bound boxes (a step of config 1 or 2 is three kernels of 3-8 us each): lbm_step replays
   // a captured CUDA graph of kGraphSteps steps (programmatic-dependent-launch edges included)
   // instead of launching every kernel from the host.  One graph per starting buffer parity;
-  // dropped when a kernel argument changes (lbm_set_boundary).  env LBM_B200_GRAPH=0|1 (default:
+  // dropped when a kernel argument changes (lbm_set_boundary).  lbm_options.graph (default:
   // on for boxes of up to kGraphAutoNodes fluid nodes, where the host launch rate is the limit).
   int graph_mode = -1;      // -1 auto, 0 off, 1 on
   cudaGraphExec_t graph_exec[2] = {nullptr, nullptr};
@@ -143,6 +139,13 @@ struct lbm_ctx {
                                        // graphs are launched on the caller's stream
   long long graph_launches = 0;   // kernel launches inside one graph
   long long steps_done = 0;
+  // Streams: work is enqueued on torch's current stream at each call.  The context remembers the
+  // last stream it used; a call on a different stream first waits (event) for the work enqueued on
+  // the previous one, and lbm_destroy synchronises the device before the buffers go back to the
+  // caching allocator.
+  cudaStream_t last_stream = nullptr;
+  bool has_stream = false;
+  cudaEvent_t order_ev = nullptr;
   long long bytes[4] = {0, 0, 0, 0};
   bool prof = false;
   std::vector<ProfEvent> prof_events;
@@ -155,13 +158,14 @@ struct lbm_ctx {
   ~lbm_ctx() {
     drop_graphs();
     if (cap_stream) cudaStreamDestroy(cap_stream);
+    if (order_ev) cudaEventDestroy(order_ev);
     for (auto& e : prof_events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     lbm_shim_free(f[0]); lbm_shim_free(f[1]); lbm_shim_free(psi); lbm_shim_free(nbr);
     lbm_shim_free(wall_nbr); lbm_shim_free(wall_inv_den); lbm_shim_free(node_vox_d);
     lbm_shim_free(frozen); lbm_shim_free(partial); lbm_shim_free(diag_out);
-    lbm_shim_free(sched_items); lbm_shim_free(fused_ctr); lbm_shim_free(nbr16);
+    lbm_shim_free(win_items); lbm_shim_free(win_ctr); lbm_shim_free(nbr16);
     lbm_shim_free(nbr16_meta);
-    lbm_shim_free(fused_flags);
+    lbm_shim_free(win_flags);
     lbm_shim_free(halo_slots); lbm_shim_free(halo_send); lbm_shim_free(halo_recv);
     lbm_shim_free(ccl);
     lbm_shim_free(bit_rec); lbm_shim_free(bit_coord);
@@ -182,6 +186,16 @@ Consts<T> make_consts(const lbm_params& p) {
   return c;
 }
 
+constexpr int kGraphSteps = 16;            // even: the buffer parity returns to its start
+constexpr int kGraphAutoNodes = 600000;    // above this a step is long enough to hide the launches
+// Window step: a producer item is issued this many fluid tiles before its first consumer (about
+// the number of items in flight on 148 SMs x 7 CTAs, in tile units); LBM_STEP_AUTO takes the
+// window step only if the resulting lead is a window of populations the L2 holds beside the
+// step's write stream.
+constexpr int kWindowSlackTiles = 450;
+constexpr long long kWindowMaxBytes = 40LL << 20;
+constexpr bool kWindowAuto = true;
+
 template <typename T>
 OpenPlane<T> make_open(const lbm_params& p, const int (&open_end)[2]) {
   OpenPlane<T> o;
@@ -193,6 +207,29 @@ OpenPlane<T> make_open(const lbm_params& p, const int (&open_end)[2]) {
 }
 
 cudaStream_t cur_stream() { return (cudaStream_t)lbm_shim_stream(); }
+
+// torch's current stream, ordered after whatever this context enqueued on another stream before
+cudaStream_t use_stream(lbm_ctx* c) {
+  cudaStream_t st = cur_stream();
+  if (c->has_stream && st != c->last_stream) {
+    if (!c->order_ev) cudaEventCreateWithFlags(&c->order_ev, cudaEventDisableTiming);
+    if (c->order_ev) {
+      cudaEventRecord(c->order_ev, c->last_stream);
+      cudaStreamWaitEvent(st, c->order_ev, 0);
+    } else {
+      cudaStreamSynchronize(c->last_stream);
+    }
+  }
+  c->last_stream = st;
+  c->has_stream = true;
+  return st;
+}
+
+struct ProfOff {  // queries run their density / wall passes unprofiled; restored on every exit path
+  lbm_ctx* c; bool was;
+  explicit ProfOff(lbm_ctx* c_) : c(c_), was(c_->prof) { c->prof = false; }
+  ~ProfOff() { c->prof = was; }
+};
 
 struct Timed {  // brackets one launch with events when profiling is on
   lbm_ctx* c; cudaStream_t st; int kind; ProfEvent ev{};
@@ -285,8 +322,6 @@ void launch_psi(lbm_ctx* c, cudaStream_t st) {
 }
 
 
-// a3-a6: the fused pass.  Production = bulk-async staged tiles; the register kernel is kept as
-// an A/B reference (LBM_B200_COLLIDE=simple).
 // Apply a deferred open-plane fix now (getters that read the populations directly).
 template <typename T>
 void apply_pending_T(lbm_ctx* c, cudaStream_t st) {
@@ -300,17 +335,17 @@ void apply_pending(lbm_ctx* c, cudaStream_t st) {
   if (c->bits == 64) apply_pending_T<double>(c, st); else apply_pending_T<float>(c, st);
 }
 
+// a3-a6: the fused pass of the split step (bulk-async staged tiles).
 template <typename T, int TN, int MINB, int IDX>
 void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st, int part) {
   constexpr bool kRemainder = sizeof(T) == 4;
-  constexpr size_t smem = IDX == 1 ? collide16_smem_bytes<T, TN, (MINB >= 7)>() -
-                                         (MINB >= 8 ? (size_t)2 * TN * sizeof(T) : 0)
+  constexpr size_t smem = IDX == 1 ? collide16_smem_bytes<T, TN, (MINB >= 7)>()
                                    : collide_smem_bytes<T, TN>();
   static bool configured[64] = {};  // function attributes are per device
   if (!configured[c->device & 63]) {
-    cudaFuncSetAttribute(k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX>,
-                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured[c->device & 63] = true;
+    if (cudaFuncSetAttribute(k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX>,
+                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess)
+      configured[c->device & 63] = true;
   }
   Idx16 ix;
   ix.nbr16 = c->nbr16;
@@ -347,114 +382,93 @@ void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
 template <typename T>
 void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st,
                     int part = -1) {
-  constexpr bool kRemainder = sizeof(T) == 4;
-  if (c->collide_variant == 0) {  // A/B register kernel: no split, everything in part 0 (or -1)
-    if (part != 1)
-      k_collide_stream<T, kRemainder><<<blocks(c->nact, 256), 256, 0, st>>>(
-          fin, fout, (const Vec2<T>*)c->psi, c->nbr, c->nf, c->nact, c->npad, k);
-    return;
-  }
+  // fp32: 128-node tiles, 7 CTAs per SM at 72 registers (6 and 8 CTAs, 64- and 256-node tiles were
+  // measured slower); fp64 validation build: 2 CTAs per SM
   if constexpr (sizeof(T) == 4) {
-    if (c->idx16 == 2) {
-      if (c->tile == 1287) launch_bulk<T, 128, 7, 2>(c, fin, fout, k, st, part);
-      else launch_bulk<T, 128, 6, 2>(c, fin, fout, k, st, part);
-      return;
-    }
-    if (c->idx16) {
-      if (c->tile == 1285) launch_bulk<T, 128, 5, 1>(c, fin, fout, k, st, part);
-      else if (c->tile == 1287) launch_bulk<T, 128, 7, 1>(c, fin, fout, k, st, part);
-      else if (c->tile == 1288) launch_bulk<T, 128, 8, 1>(c, fin, fout, k, st, part);
-      else launch_bulk<T, 128, 6, 1>(c, fin, fout, k, st, part);
-      return;
-    }
-    switch (c->tile) {
-      case 1285: launch_bulk<T, 128, 5, 0>(c, fin, fout, k, st, part); break;
-      case 2563: launch_bulk<T, 256, 3, 0>(c, fin, fout, k, st, part); break;
-      default: launch_bulk<T, 128, 6, 0>(c, fin, fout, k, st, part); break;
-    }
+    if (c->idx16 == 2) launch_bulk<T, 128, 7, 2>(c, fin, fout, k, st, part);
+    else launch_bulk<T, 128, 7, 1>(c, fin, fout, k, st, part);
   } else {
     if (c->idx16 == 2) launch_bulk<T, 128, 2, 2>(c, fin, fout, k, st, part);
-    else if (c->idx16) launch_bulk<T, 128, 2, 1>(c, fin, fout, k, st, part);
-    else launch_bulk<T, 128, 2, 0>(c, fin, fout, k, st, part);
+    else launch_bulk<T, 128, 2, 1>(c, fin, fout, k, st, part);
   }
 }
 
-// One cooperative launch of the fused persistent step kernel (a1-a6 in one kernel).
+// One launch of the single-kernel window step (a0-a6 of one time step; kernels.cuh k_step_window).
 template <typename T, int MINB>
-int launch_fused(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
+int launch_window(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
   constexpr int TN = 128;
   constexpr bool kRemainder = sizeof(T) == 4;
-  constexpr size_t smem = collide_smem_bytes<T, TN>();
-  auto kern = k_step_fused<T, TN, MINB, kRemainder>;
+  constexpr size_t smem = collide16_smem_bytes<T, TN, (MINB >= 7)>();
+  auto kern = k_step_window<T, TN, MINB, kRemainder>;
   static int grid_cache_dev[64] = {};  // per device
   int& grid_cache = grid_cache_dev[c->device & 63];
   if (grid_cache == 0) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TN, smem));
-    if (per_sm < 1) return fail(LBM_ECUDA, "fused kernel does not fit on an SM");
+    if (per_sm < 1) return fail(LBM_ECUDA, "window kernel does not fit on an SM");
     grid_cache = per_sm * c->num_sms;
   }
-  c->fused_grid = grid_cache;
-  FusedSched sc;
-  sc.flags_d = c->fused_flags;
-  sc.flags_w = c->fused_flags + c->sched_ntf;
-  sc.epoch = ++c->fused_epoch;
-  sc.items = c->sched_items;
-  sc.nitems = c->sched_nitems;
-  Vec2<T>* psi = (Vec2<T>*)c->psi;
-  const int* nbr = c->nbr;
-  const int* wall_nbr = c->wall_nbr;
-  const T* inv_den = (const T*)c->wall_inv_den;
-  int nf = c->nf, nw = c->nw;
-  size_t npad = c->npad, nwpad = c->nwpad;
-  Consts<T> kk = k;
-  int* ctr = c->fused_ctr + 4 * c->fused_parity;
-  int* ctr_next = c->fused_ctr + 4 * (c->fused_parity ^ 1);
-  c->fused_parity ^= 1;
-  void* args[] = {(void*)&fin, (void*)&fout, (void*)&psi, (void*)&nbr, (void*)&wall_nbr,
-                  (void*)&inv_den, (void*)&nf, (void*)&nw, (void*)&npad, (void*)&nwpad,
-                  (void*)&kk, (void*)&sc, (void*)&ctr, (void*)&ctr_next};
-  CU(cudaLaunchCooperativeKernel((const void*)kern, dim3(grid_cache), dim3(TN), args, smem, st));
+  c->win_grid = std::min(grid_cache, c->win_nitems);
+  Idx16 ix;
+  ix.nbr16 = c->nbr16;
+  ix.meta = c->nbr16_meta;
+  ix.np_lo = c->open_end[0] ? c->np : 0;
+  ix.np_hi = c->open_end[1] ? c->np : 0;
+  ix.reverse = 0;
+  ix.nact = c->nact;
+  ix.bits = nullptr; ix.coord = nullptr;
+  ix.nx = c->nx; ix.ny = c->ny; ix.nz = c->nz; ix.words = 0;
+  ix.tile0 = 0; ix.split = 0; ix.tile1 = 0;
+  WinSched sc;
+  sc.items = c->win_items;
+  sc.nitems = c->win_nitems;
+  sc.flags_d = c->win_flags;
+  sc.flags_w = c->win_flags + c->win_ntf;
+  sc.flags_c = c->win_ntp ? c->win_flags + c->win_ntf + c->win_ntw : nullptr;
+  sc.epoch = ++c->win_epoch;
+  sc.np = c->np;
+  sc.ntp = c->win_ntp;
+  int* ctr = c->win_ctr + 4 * c->win_parity;
+  int* ctr_next = c->win_ctr + 4 * (c->win_parity ^ 1);
+  c->win_parity ^= 1;
+  kern<<<c->win_grid, TN, smem, st>>>(fin, fout, (Vec2<T>*)c->psi, (const int*)c->nbr,
+                                      (const int*)c->wall_nbr, (const T*)c->wall_inv_den,
+                                      (const T*)c->frozen, c->nf, c->nw, c->npad, c->nwpad, k, ix,
+                                      make_open<T>(c->p, c->open_end), sc, ctr, ctr_next);
   return LBM_OK;
 }
 
 template <typename T>
 int step_T(lbm_ctx* c, int n, cudaStream_t st) {
   const Consts<T> k = make_consts<T>(c->p);
-  const OpenPlane<T> op = make_open<T>(c->p, c->open_end);
   for (int it = 0; it < n; ++it) {
     const T* fin = (const T*)c->f[c->cur];
     T* fout = (T*)c->f[c->cur ^ 1];
     if (c->step_variant == 1) {
-      apply_pending_T<T>(c, st);
+      apply_pending_T<T>(c, st);  // left by a split step (not in a run of window steps)
       Timed t(c, st, 2);
       int rc;
-      if constexpr (sizeof(T) == 4) rc = launch_fused<T, 6>(c, fin, fout, k, st);
-      else rc = launch_fused<T, 2>(c, fin, fout, k, st);
+      if constexpr (sizeof(T) == 4) {
+        rc = c->win_ctas == 6 ? launch_window<T, 6>(c, fin, fout, k, st)
+                              : launch_window<T, 7>(c, fin, fout, k, st);
+      } else {
+        rc = launch_window<T, 2>(c, fin, fout, k, st);
+      }
       if (rc) return rc;
+      c->cur ^= 1;               // the open-plane fix is part of the kernel: the state is complete
     } else {
       launch_psi<T>(c, st);
       Timed t(c, st, 2);
       launch_collide<T>(c, fin, fout, k, st);
-    }
-    c->cur ^= 1;
-    if (c->p.z_open) {
-      if (c->step_variant == 1) {
-        Timed t(c, st, 3);
-        k_open_planes<T><<<blocks(2LL * c->np, 128), 128, 0, st>>>(fout, (const T*)c->frozen,
-                                                                   c->nf, c->np, c->npad, op);
-      } else {
-        c->open_pending = true;  // a0 is folded into the next density pass
-      }
+      c->cur ^= 1;
+      if (c->p.z_open) c->open_pending = true;  // a0 is folded into the next density pass
     }
   }
   CU(cudaPeekAtLastError());
   return LBM_OK;
 }
 
-constexpr int kGraphSteps = 16;            // even: the buffer parity returns to its start
-constexpr int kGraphAutoNodes = 600000;    // above this a step is long enough to hide the launches
 
 // n steps, through graph replays where that pays (see lbm_ctx::graph_mode)
 template <typename T>
@@ -463,7 +477,10 @@ int step_graphed_T(lbm_ctx* c, int n, cudaStream_t st) {
   const bool open = c->open_end[0] || c->open_end[1];
   // the first steps run directly: they configure the kernels' attributes and bring the deferred
   // open-plane fix into its steady state (pending at the start of every step)
-  if (!want || c->prof || c->step_variant != 0 || c->slab) return step_T<T>(c, n, st);
+  if (!want || c->prof || c->step_variant != 0 || c->slab) {
+    c->steps_done += n;
+    return step_T<T>(c, n, st);
+  }
   if (c->steps_done == 0 || (open && !c->open_pending)) {
     if (n == 0) return LBM_OK;
     if (int rc = step_T<T>(c, 1, st)) return rc;
@@ -564,14 +581,14 @@ int lbm_build_index(const uint8_t* solid, int nx, int ny, int nz, int z_open, in
   return LBM_OK;
 }
 
-int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open, int tile,
-                       int lead, int32_t* records, long long cap_items, long long* n_items) {
+int lbm_build_window(const uint8_t* solid, int nx, int ny, int nz, int z_open, int tile,
+                     int lead, int32_t* records, long long cap_items, long long* n_items) {
   if (!solid || !records || !n_items) return fail(LBM_EINVAL, "NULL argument");
   lbmgeo::Geometry g;
   const int rc = lbmgeo::build(g, solid, nx, ny, nz, z_open, true);
   if (rc) return fail(rc, "geometry build failed (%d)", rc);
-  lbmgeo::Schedule s;
-  if (lbmgeo::build_schedule(g, tile, lead < 0 ? 0 : lead, s) != 0)
+  lbmgeo::Window s;
+  if (lbmgeo::build_window(g, tile, lead < 0 ? 0 : lead, s) != 0)
     return fail(LBM_EINVAL, "schedule build failed");
   *n_items = (long long)s.nitems();
   if ((long long)s.nitems() > cap_items) return fail(LBM_EINVAL, "records capacity too small");
@@ -579,9 +596,41 @@ int lbm_build_schedule(const uint8_t* solid, int nx, int ny, int nz, int z_open,
   return LBM_OK;
 }
 
+void lbm_options_default(lbm_options* o) {
+  if (!o) return;
+  o->step = LBM_STEP_AUTO;
+  o->index = LBM_INDEX_16;
+  o->graph = -1;
+  o->pdl = 1;
+  o->reverse = 1;
+  o->keep_psi_mb = 48;
+  o->window_slack = 0;
+  o->window_ctas = 0;
+}
+
+static int validate_options(const lbm_options* o) {
+  if (o->step < LBM_STEP_AUTO || o->step > LBM_STEP_WINDOW)
+    return fail(LBM_EINVAL, "options.step must be LBM_STEP_AUTO, LBM_STEP_SPLIT or LBM_STEP_WINDOW");
+  if (o->index != LBM_INDEX_16 && o->index != LBM_INDEX_BITS)
+    return fail(LBM_EINVAL, "options.index must be LBM_INDEX_16 or LBM_INDEX_BITS");
+  if (o->graph < -1 || o->graph > 1) return fail(LBM_EINVAL, "options.graph must be -1, 0 or 1");
+  if ((o->pdl != 0 && o->pdl != 1) || (o->reverse != 0 && o->reverse != 1))
+    return fail(LBM_EINVAL, "options.pdl and options.reverse must be 0 or 1");
+  if (o->keep_psi_mb < 0 || o->window_slack < 0)
+    return fail(LBM_EINVAL, "options.keep_psi_mb and options.window_slack must be >= 0");
+  if (o->window_ctas != 0 && o->window_ctas != 6 && o->window_ctas != 7)
+    return fail(LBM_EINVAL, "options.window_ctas must be 0 (default), 6 or 7");
+  return LBM_OK;
+}
+
 static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz,
-                       const lbm_params* p, bool slab, int halo_lo, int halo_hi) {
+                       const lbm_params* p, const lbm_options* opt, bool slab, int halo_lo,
+                       int halo_hi) {
   if (!out || !solid || !p) return fail(LBM_EINVAL, "NULL argument");
+  lbm_options o;
+  lbm_options_default(&o);
+  if (opt) o = *opt;
+  if (int rc = validate_options(&o)) return rc;
   if (nx < 1 || ny < 1 || nz < 1) return fail(LBM_EINVAL, "box dimensions must be positive");
   if (int rc = validate_params(p, nz)) return rc;
   if (slab && ((halo_lo != 0 && halo_lo != 1) || (halo_hi != 0 && halo_hi != 1)))
@@ -618,16 +667,12 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   c->nact = (int)g.nact; c->slab = slab ? 1 : 0;
   c->open_end[0] = g.open_lo; c->open_end[1] = g.open_hi;
   c->bits = p->storage_bits; c->esz = p->storage_bits / 8;
-  if (const char* e = std::getenv("LBM_B200_COLLIDE")) c->collide_variant = !std::strcmp(e, "simple") ? 0 : 1;
-  if (const char* e = std::getenv("LBM_B200_TILE")) c->tile = std::atoi(e);
-  if (const char* e = std::getenv("LBM_B200_REVERSE")) c->reverse = std::atoi(e) != 0;
-  if (const char* e = std::getenv("LBM_B200_PDL")) c->pdl = std::atoi(e) != 0;
-  if (const char* e = std::getenv("LBM_B200_GRAPH")) c->graph_mode = std::atoi(e) != 0;
-  if (const char* e = std::getenv("LBM_B200_KEEP_PSI_MB")) c->keep_psi_mb = std::atoi(e);
-  if (const char* e = std::getenv("LBM_B200_IDX"))
-    c->idx16 = !std::strcmp(e, "bits") ? 2 : (std::atoi(e) == 32 ? 0 : 1);
-  if (const char* e = std::getenv("LBM_B200_STEP")) c->step_variant = !std::strcmp(e, "split") ? 0 : 1;
-  if (c->slab) c->step_variant = 0;
+  c->reverse = o.reverse;
+  c->pdl = o.pdl;
+  c->graph_mode = o.graph;
+  c->keep_psi_mb = o.keep_psi_mb;
+  c->idx16 = o.index == LBM_INDEX_BITS ? 2 : 1;
+  if (o.window_ctas) c->win_ctas = o.window_ctas;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
   // pair-slot indices i * npad + k and psi indices npad + w are 32-bit
   if ((size_t)19 * c->npad >= ((size_t)1 << 31) || c->npad + c->nwpad >= ((size_t)1 << 31)) {
@@ -637,7 +682,7 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   c->zstart.assign(nz + 1, 0);
   for (long long n = 0; n < g.nact; ++n) ++c->zstart[g.node_vox[n] / c->np + 1];
   for (int z = 0; z < nz; ++z) c->zstart[z + 1] += c->zstart[z];
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   const size_t fbytes = (size_t)2 * 19 * c->npad * c->esz;
   const size_t psibytes = (c->npad + c->nwpad) * 2 * c->esz;  // wall part starts at npad
   const size_t nbrbytes = (size_t)18 * c->npad * sizeof(int);
@@ -676,15 +721,26 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   if (e == cudaSuccess) e = cudaMemsetAsync(c->psi, 0, psibytes, st);
   if (e == cudaSuccess && frozenbytes) e = cudaMemsetAsync(c->frozen, 0, frozenbytes, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->nbr, 0, nbrbytes, st);
-  // Fused-step schedule (built from the raw ids), then re-base wall ids from nf+w to npad+w so
-  // that the wall part of psi starts on a tile boundary.
-  lbmgeo::Schedule sch;
+  // Window-step schedule (built from the raw ids; only when that step is selected), then re-base
+  // wall ids from nf+w to npad+w so that the wall part of psi starts on a tile boundary.
+  // LBM_STEP_AUTO: the window step when the box is large enough that launch gaps do not matter and
+  // the distance by which the density items lead the fused items (one z-plane of tiles plus twice
+  // the slack) is a window the L2 holds.
+  lbmgeo::Window win;
   {
-    int lead = 256;
-    if (const char* e = std::getenv("LBM_B200_LEAD")) lead = std::atoi(e);
-    if (lbmgeo::build_schedule(g, 128, lead < 0 ? 0 : lead, sch) != 0) {
-      delete c;
-      return fail(LBM_ENOMEM, "schedule build failed");
+    const int slack = o.window_slack > 0 ? o.window_slack : kWindowSlackTiles;
+    const long long plane_tiles = ((long long)nx * ny + 127) / 128;   // a solid-free plane
+    const long long lead = plane_tiles + 2 * slack;
+    const bool fits = lead * 128 * 19 * 2 * (long long)c->esz <= kWindowMaxBytes;
+    const bool want = !c->slab && c->idx16 == 1 &&
+                      (o.step == LBM_STEP_WINDOW ||
+                       (o.step == LBM_STEP_AUTO && kWindowAuto && g.nf > kGraphAutoNodes && fits));
+    if (want) {
+      if (lbmgeo::build_window(g, 128, slack, win) != 0) {
+        delete c;
+        return fail(LBM_ENOMEM, "window schedule build failed");
+      }
+      c->step_variant = 1;
     }
   }
   lbmgeo::Index16 i16;
@@ -721,23 +777,26 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   up(c->nbr16, i16.nbr16.data(), i16.nbr16.size() * sizeof(uint16_t));
   up(c->nbr16_meta, i16.meta.data(), i16.meta.size() * sizeof(int32_t));
   c->bytes[2] += (long long)(i16.nbr16.size() * 2 + i16.meta.size() * 4);
-  // fused-step schedule records, completion flags and counters
-  {
-    c->sched_nitems = (int)sch.nitems();
-    c->sched_ntf = sch.ntf;
-    c->sched_ntw = sch.ntw;
-    const size_t nflags = (size_t)sch.ntf + sch.ntw;
-    c->sched_items = (int4*)lbm_shim_alloc(sch.records.size() * sizeof(int32_t));
-    c->fused_ctr = (int*)lbm_shim_alloc(8 * sizeof(int));
-    c->fused_flags = (int*)lbm_shim_alloc(nflags * sizeof(int));
-    if (!c->sched_items || !c->fused_ctr || !c->fused_flags) {
+  // window-step schedule records, completion flags and counters
+  if (c->step_variant == 1) {
+    c->win_nitems = (int)win.nitems();
+    c->win_ntf = win.ntf;
+    c->win_ntw = win.ntw;
+    c->win_ntp = win.ntp;
+    c->win_reach = win.reach;
+    c->win_slack = win.slack;
+    const size_t nflags = (size_t)2 * win.ntf + win.ntw;
+    c->win_items = (int4*)lbm_shim_alloc(win.records.size() * sizeof(int32_t));
+    c->win_ctr = (int*)lbm_shim_alloc(8 * sizeof(int));
+    c->win_flags = (int*)lbm_shim_alloc(nflags * sizeof(int));
+    if (!c->win_items || !c->win_ctr || !c->win_flags) {
       delete c;
-      return fail(LBM_ENOMEM, "device allocation failed (schedule)");
+      return fail(LBM_ENOMEM, "device allocation failed (window schedule)");
     }
-    up(c->sched_items, sch.records.data(), sch.records.size() * sizeof(int32_t));
-    if (e == cudaSuccess) e = cudaMemsetAsync(c->fused_ctr, 0, 8 * sizeof(int), st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(c->fused_flags, 0, nflags * sizeof(int), st);
-    c->bytes[2] += (long long)(sch.records.size() * 4 + nflags * 4);
+    up(c->win_items, win.records.data(), win.records.size() * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->win_ctr, 0, 8 * sizeof(int), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->win_flags, 0, nflags * sizeof(int), st);
+    c->bytes[2] += (long long)(win.records.size() * 4 + nflags * 4);
   }
   lbmgeo::BitIndex bix;  // upload source until the sync below
   if (c->idx16 == 2) {
@@ -850,12 +909,31 @@ int lbm_build_slab_halo(const uint8_t* solid_local, int nx, int ny, int nz_local
 }
 
 int lbm_create(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz, const lbm_params* p) {
-  return create_impl(out, solid, nx, ny, nz, p, false, 0, 0);
+  return create_impl(out, solid, nx, ny, nz, p, nullptr, false, 0, 0);
+}
+
+int lbm_create_opt(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz,
+                   const lbm_params* p, const lbm_options* opt) {
+  return create_impl(out, solid, nx, ny, nz, p, opt, false, 0, 0);
 }
 
 int lbm_create_slab(lbm_ctx** out, const uint8_t* solid_local, int nx, int ny, int nz_local,
                     const lbm_params* p, int halo_lo, int halo_hi) {
-  return create_impl(out, solid_local, nx, ny, nz_local, p, true, halo_lo, halo_hi);
+  return create_impl(out, solid_local, nx, ny, nz_local, p, nullptr, true, halo_lo, halo_hi);
+}
+
+int lbm_create_slab_opt(lbm_ctx** out, const uint8_t* solid_local, int nx, int ny, int nz_local,
+                        const lbm_params* p, const lbm_options* opt, int halo_lo, int halo_hi) {
+  return create_impl(out, solid_local, nx, ny, nz_local, p, opt, true, halo_lo, halo_hi);
+}
+
+int lbm_step_info(lbm_ctx* c, int info[8]) {
+  if (!c || !info) return fail(LBM_EINVAL, "NULL argument");
+  info[0] = c->step_variant == 1 ? LBM_STEP_WINDOW : LBM_STEP_SPLIT;
+  info[1] = c->idx16 == 2 ? LBM_INDEX_BITS : LBM_INDEX_16;
+  info[2] = c->win_slack; info[3] = c->win_reach; info[4] = 0;
+  info[5] = c->win_nitems; info[6] = c->win_grid; info[7] = (int)c->wide_tiles;
+  return LBM_OK;
 }
 
 long long lbm_num_owned(lbm_ctx* c) { return c ? c->nact : -1; }
@@ -867,7 +945,7 @@ int lbm_slab_density(lbm_ctx* c, int part) {
   // part 0 may restart a step that stopped after its density pass (getters do that)
   if (part == 0 ? c->slab_phase > 2 : c->slab_phase != 1)
     return fail(LBM_EINVAL, "slab calls out of order (expected phase %d)", c->slab_phase);
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   if (c->bits == 64) launch_density<double>(c, st, part); else launch_density<float>(c, st, part);
   CU(cudaPeekAtLastError());
   c->slab_phase = part + 1;
@@ -905,7 +983,7 @@ int lbm_slab_collide(lbm_ctx* c, int part) {
   if (part != 0 && part != 1) return fail(LBM_EINVAL, "part must be 0 or 1");
   if (c->slab_phase != 2 + part)
     return fail(LBM_EINVAL, "slab calls out of order (expected phase %d)", c->slab_phase);
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   if (int rc = c->bits == 64 ? slab_collide_T<double>(c, part, st) : slab_collide_T<float>(c, part, st))
     return rc;
   c->slab_phase = 3 + part;
@@ -917,7 +995,7 @@ int lbm_slab_unpack(lbm_ctx* c) {
   if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
   if (c->slab_phase != 4)
     return fail(LBM_EINVAL, "slab calls out of order (expected phase %d)", c->slab_phase);
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   const int nu = c->n_unpack[0] + c->n_unpack[1];
   const int* slots = c->halo_slots + c->n_pack[0] + c->n_pack[1];
   if (nu) {
@@ -941,7 +1019,7 @@ int lbm_slab_ccl_begin(lbm_ctx* c, int comp, int mark_lo, int mark_hi) {
   if (c->slab_phase != 2)
     return fail(LBM_EINVAL, "slab context: lbm_slab_ccl_begin needs both lbm_slab_density parts and "
                             "the psi exchange on the current state");
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   const int na = c->nact;
   int* parent = c->ccl;
   int* flag = parent + na;
@@ -963,7 +1041,7 @@ int lbm_slab_ccl_begin(lbm_ctx* c, int comp, int mark_lo, int mark_hi) {
 int lbm_slab_ccl_export(lbm_ctx* c) {
   if (int rc = check_ctx(c)) return rc;
   if (!c->slab || c->ccl_comp < 0) return fail(LBM_EINVAL, "no lbm_slab_ccl_begin on this context");
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   const int na = c->nact;
   int* parent = c->ccl;
   int* flag = parent + na;
@@ -983,7 +1061,7 @@ int lbm_slab_ccl_import(lbm_ctx* c, int use_lo, int use_hi, int* changed) {
   if (int rc = check_ctx(c)) return rc;
   if (!changed) return fail(LBM_EINVAL, "NULL argument");
   if (!c->slab || c->ccl_comp < 0) return fail(LBM_EINVAL, "no lbm_slab_ccl_begin on this context");
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   const int na = c->nact;
   int* parent = c->ccl;
   int* flag = parent + na;
@@ -1009,7 +1087,7 @@ int lbm_slab_ccl_finish(lbm_ctx* c, int z0, int z1, long long* nodes, double* ma
   if (int rc = check_ctx(c)) return rc;
   if (!nodes || !mass || z0 < 0 || z1 > c->nz || z0 > z1) return fail(LBM_EINVAL, "bad argument");
   if (!c->slab || c->ccl_comp < 0) return fail(LBM_EINVAL, "no lbm_slab_ccl_begin on this context");
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   const int na = c->nact, comp = c->ccl_comp;
   int* parent = c->ccl;
   int* flag = parent + na;
@@ -1074,7 +1152,9 @@ int lbm_slab_buffer(lbm_ctx* c, int which, void** dev, long long* bytes) {
 void lbm_destroy(lbm_ctx* c) {
   if (!c) return;
   cudaSetDevice(c->device);
-  cudaStreamSynchronize(cur_stream());
+  // kernels of this context may be in flight on any stream it was used from: the buffers go back to
+  // torch's caching allocator, which would hand them out again at once
+  cudaDeviceSynchronize();
   delete c;
 }
 
@@ -1095,7 +1175,7 @@ int lbm_set_boundary(lbm_ctx* c, double inlet_value, double outlet_rho) {
   if (!std::isfinite(inlet_value) || !std::isfinite(outlet_rho))
     return fail(LBM_EINVAL, "boundary values must be finite");
   if (int rc = check_ctx(c)) return rc;
-  apply_pending(c, cur_stream());  // the last step's fix uses the values it was run with
+  apply_pending(c, use_stream(c));  // the last step's fix uses the values it was run with
   c->drop_graphs();                // the boundary values are kernel arguments
   if (c->p.inlet_kind == 1 || c->p.inlet_kind == 3) c->p.inlet_rho = inlet_value;
   else c->p.inlet_uz = inlet_value;
@@ -1105,7 +1185,7 @@ int lbm_set_boundary(lbm_ctx* c, double inlet_value, double outlet_rho) {
 
 int lbm_sync(lbm_ctx* c) {
   if (int rc = check_ctx(c)) return rc;
-  CU(cudaStreamSynchronize(cur_stream()));
+  CU(cudaStreamSynchronize(use_stream(c)));
   return LBM_OK;
 }
 
@@ -1115,7 +1195,7 @@ int lbm_step(lbm_ctx* c, int n) {
   if (c->slab)
     return fail(LBM_EINVAL, "slab context: a step is lbm_slab_density, psi exchange, "
                             "lbm_slab_collide, population exchange, lbm_slab_unpack");
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   if (c->prof) {
     for (auto& e : c->prof_events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     c->prof_events.clear();
@@ -1136,7 +1216,7 @@ int lbm_set_profiling(lbm_ctx* c, int on) {
 int lbm_last_step_profile(lbm_ctx* c, double ms[4], long long* launches) {
   if (int rc = check_ctx(c)) return rc;
   if (!ms || !launches) return fail(LBM_EINVAL, "NULL argument");
-  CU(cudaStreamSynchronize(cur_stream()));
+  CU(cudaStreamSynchronize(use_stream(c)));
   for (int k = 0; k < 4; ++k) ms[k] = 0.0;
   for (auto& e : c->prof_events) {
     float t = 0.f;
@@ -1150,7 +1230,7 @@ int lbm_last_step_profile(lbm_ctx* c, double ms[4], long long* launches) {
 int lbm_set_density(lbm_ctx* c, const double* rhoA, const double* rhoB) {
   if (int rc = check_ctx(c)) return rc;
   if (!rhoA || !rhoB) return fail(LBM_EINVAL, "NULL argument");
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   c->open_pending = false;  // the whole state is replaced
   const size_t bytes = (size_t)c->nvox * sizeof(double);
   DevBuf a(bytes), b(bytes);
@@ -1174,7 +1254,7 @@ int lbm_set_density(lbm_ctx* c, const double* rhoA, const double* rhoB) {
 int lbm_set_populations(lbm_ctx* c, int comp, const double* f) {
   if (int rc = check_ctx(c)) return rc;
   if (!f || comp < 0 || comp > 1) return fail(LBM_EINVAL, "bad argument");
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   apply_pending(c, st);  // the other component keeps its (completed) state
   const size_t bytes = (size_t)c->nvox * sizeof(double);
   DevBuf d(bytes);
@@ -1201,7 +1281,7 @@ int lbm_set_populations(lbm_ctx* c, int comp, const double* f) {
 int lbm_get_populations(lbm_ctx* c, int comp, double* f) {
   if (int rc = check_ctx(c)) return rc;
   if (!f || comp < 0 || comp > 1) return fail(LBM_EINVAL, "bad argument");
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   apply_pending(c, st);
   const size_t bytes = (size_t)c->nvox * sizeof(double);
   DevBuf d(bytes);
@@ -1227,14 +1307,14 @@ int lbm_get_macroscopic(lbm_ctx* c, double* rhoA, double* rhoB, double* ux, doub
   if (c->slab && c->slab_phase != 2)
     return fail(LBM_EINVAL, "slab context: lbm_get_macroscopic needs both lbm_slab_density parts "
                             "and the psi exchange on the current state");
-  cudaStream_t st = cur_stream();
-  const bool was = c->prof;
-  c->prof = false;
+  cudaStream_t st = use_stream(c);
   const int na = c->nact;  // owned nodes (all fluid nodes unless slab mode)
   DevBuf m((size_t)6 * na * sizeof(double));
   const size_t bytes = (size_t)c->nvox * sizeof(double);
   DevBuf d(bytes);
-  if (!m.p || !d.p) { c->prof = was; return fail(LBM_ENOMEM, "device staging allocation failed"); }
+  if (!m.p || !d.p) return fail(LBM_ENOMEM, "device staging allocation failed");
+  {
+  ProfOff guard(c);
   if (c->bits == 64) {
     launch_psi<double>(c, st);
     k_macroscopic<double><<<blocks(na, 256), 256, 0, st>>>(
@@ -1246,7 +1326,7 @@ int lbm_get_macroscopic(lbm_ctx* c, double* rhoA, double* rhoB, double* ux, doub
         (const float*)c->f[c->cur], (const Vec2<float>*)c->psi, c->nbr, (double*)m.p, na,
         c->npad, make_consts<float>(c->p));
   }
-  c->prof = was;
+  }
   CU(cudaPeekAtLastError());
   double* outs[6] = {rhoA, rhoB, ux, uy, uz, P};
   for (int q = 0; q < 6; ++q) {
@@ -1264,7 +1344,7 @@ int lbm_get_macroscopic(lbm_ctx* c, double* rhoA, double* rhoB, double* ux, doub
 int lbm_diagnostics(lbm_ctx* c, double mass[2], double momentum[3]) {
   if (int rc = check_ctx(c)) return rc;
   if (!mass || !momentum) return fail(LBM_EINVAL, "NULL argument");
-  cudaStream_t st = cur_stream();
+  cudaStream_t st = use_stream(c);
   apply_pending(c, st);
   const int nb = c->diag_blocks;
   if (c->bits == 64)
@@ -1294,9 +1374,8 @@ int lbm_saturation(lbm_ctx* c, int comp, int z0, int z1, double* S) {
     return fail(LBM_EINVAL, "bad argument");
   const int n0 = c->zstart[z0], n1 = c->zstart[z1];
   if (n1 <= n0) return fail(LBM_ENOFLUID, "no fluid node in the z-range");
-  cudaStream_t st = cur_stream();
-  const bool was = c->prof;
-  c->prof = false;
+  cudaStream_t st = use_stream(c);
+  ProfOff guard(c);
   unsigned long long* cnt = (unsigned long long*)(c->diag_out + 7);
   CU(cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), st));
   if (c->bits == 64) {
@@ -1308,7 +1387,6 @@ int lbm_saturation(lbm_ctx* c, int comp, int z0, int z1, double* S) {
     k_count_phase<float><<<blocks(n1 - n0, 256), 256, 0, st>>>((const Vec2<float>*)c->psi, n0, n1,
                                                                comp, cnt);
   }
-  c->prof = was;
   CU(cudaPeekAtLastError());
   unsigned long long h = 0;
   CU(cudaMemcpyAsync(&h, cnt, sizeof h, cudaMemcpyDeviceToHost, st));
@@ -1322,11 +1400,11 @@ int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, d
   if (c->slab) return fail(LBM_EINVAL, "lbm_trapped_volume is not available on a slab context");
   if (!nodes || !mass || comp < 0 || comp > 1 || z0 < 0 || z1 > c->nz || z0 >= z1)
     return fail(LBM_EINVAL, "bad argument");
-  cudaStream_t st = cur_stream();
-  const bool was = c->prof;
-  c->prof = false;
-  if (c->bits == 64) launch_psi<double>(c, st); else launch_psi<float>(c, st);
-  c->prof = was;
+  cudaStream_t st = use_stream(c);
+  {
+    ProfOff guard(c);
+    if (c->bits == 64) launch_psi<double>(c, st); else launch_psi<float>(c, st);
+  }
   CU(cudaPeekAtLastError());
   const int nf = c->nf, nz = c->nz;
   const int n0 = c->zstart[z0], n1 = c->zstart[z1];
@@ -1376,11 +1454,11 @@ int lbm_mean_pressure(lbm_ctx* c, int z0, int z1, double* P) {
   if (!P || z0 < 0 || z1 > c->nz || z0 >= z1) return fail(LBM_EINVAL, "bad argument");
   const int n0 = c->zstart[z0], n1 = c->zstart[z1];
   if (n1 <= n0) return fail(LBM_ENOFLUID, "no fluid node in the z-range");
-  cudaStream_t st = cur_stream();
-  const bool was = c->prof;
-  c->prof = false;
-  if (c->bits == 64) launch_psi<double>(c, st); else launch_psi<float>(c, st);
-  c->prof = was;
+  cudaStream_t st = use_stream(c);
+  {
+    ProfOff guard(c);
+    if (c->bits == 64) launch_psi<double>(c, st); else launch_psi<float>(c, st);
+  }
   CU(cudaPeekAtLastError());
   const int chunk = std::max(kCclBlock, (int)(((long long)(n1 - n0) + 1183) / 1184));
   const int nb = blocks(n1 - n0, chunk);

@@ -22,7 +22,8 @@ SYMBOLS = [
     "lbm_set_boundary", "lbm_step", "lbm_sync", "lbm_get_macroscopic", "lbm_diagnostics",
     "lbm_saturation", "lbm_trapped_volume", "lbm_mean_pressure", "lbm_num_fluid", "lbm_num_wall_solid",
     "lbm_memory_bytes", "lbm_set_profiling", "lbm_last_step_profile", "lbm_last_error",
-    "lbm_build_index", "lbm_build_schedule",
+    "lbm_build_index", "lbm_build_window",
+    "lbm_options_default", "lbm_create_opt", "lbm_create_slab_opt", "lbm_step_info",
     "lbm_create_slab", "lbm_slab_density", "lbm_slab_collide", "lbm_slab_unpack", "lbm_slab_buffer",
     "lbm_num_owned", "lbm_build_slab_halo",
     "lbm_slab_ccl_begin", "lbm_slab_ccl_export", "lbm_slab_ccl_import", "lbm_slab_ccl_finish",
@@ -42,6 +43,17 @@ class lbm_params(C.Structure):
                 ("outlet_kind", C.c_int), ("outlet_comp", C.c_int), ("outlet_rho", C.c_double),
                 ("storage_bits", C.c_int), ("half_force", C.c_int)]
 
+
+class lbm_options(C.Structure):
+    _fields_ = [("step", C.c_int), ("index", C.c_int), ("graph", C.c_int), ("pdl", C.c_int),
+                ("reverse", C.c_int), ("keep_psi_mb", C.c_int), ("window_slack", C.c_int),
+                ("window_ctas", C.c_int)]
+
+
+LBM_STEP_AUTO, LBM_STEP_SPLIT, LBM_STEP_WINDOW = 0, 1, 2
+LBM_INDEX_16, LBM_INDEX_BITS = 0, 1
+_STEP = {"auto": LBM_STEP_AUTO, "split": LBM_STEP_SPLIT, "window": LBM_STEP_WINDOW}
+_INDEX = {"16": LBM_INDEX_16, "bits": LBM_INDEX_BITS}
 
 _lib = None
 
@@ -86,7 +98,14 @@ def load():
     lib.lbm_last_error.argtypes = []
     lib.lbm_last_error.restype = C.c_char_p
     lib.lbm_build_index.argtypes = [V, I, I, I, I, V, V, LL, C.POINTER(LL), C.POINTER(LL)]
-    lib.lbm_build_schedule.argtypes = [V, I, I, I, I, I, I, V, LL, C.POINTER(LL)]
+    lib.lbm_build_window.argtypes = [V, I, I, I, I, I, I, V, LL, C.POINTER(LL)]
+    lib.lbm_options_default.argtypes = [C.POINTER(lbm_options)]
+    lib.lbm_options_default.restype = None
+    lib.lbm_create_opt.argtypes = [C.POINTER(P), V, I, I, I, C.POINTER(lbm_params),
+                                   C.POINTER(lbm_options)]
+    lib.lbm_create_slab_opt.argtypes = [C.POINTER(P), V, I, I, I, C.POINTER(lbm_params),
+                                        C.POINTER(lbm_options), I, I]
+    lib.lbm_step_info.argtypes = [P, C.POINTER(I)]
     lib.lbm_create_slab.argtypes = [C.POINTER(P), V, I, I, I, C.POINTER(lbm_params), I, I]
     lib.lbm_slab_density.argtypes = [P, I]
     lib.lbm_slab_collide.argtypes = [P, I]
@@ -110,7 +129,7 @@ def load():
                "lbm_diagnostics", "lbm_saturation", "lbm_trapped_volume", "lbm_mean_pressure",
                "lbm_memory_bytes",
                "lbm_set_profiling", "lbm_last_step_profile", "lbm_build_index",
-               "lbm_build_schedule"):
+               "lbm_build_window", "lbm_create_opt", "lbm_create_slab_opt", "lbm_step_info"):
         getattr(lib, fn).restype = I
     _lib = lib
     return lib
@@ -129,6 +148,22 @@ def make_params(p):
         setattr(s, k, int(p[k]))
     for k in ("inlet_rho", "inlet_uz", "outlet_rho"):
         setattr(s, k, float(p[k]))
+    return s
+
+
+def make_options(o=None):
+    """dict -> lbm_options: the library's defaults (lbm_options_default) with the given fields
+    replaced; step may be "auto" | "split" | "window", index "16" | "bits"."""
+    s = lbm_options()
+    load().lbm_options_default(C.byref(s))
+    for k, v in (o or {}).items():
+        if k == "step" and isinstance(v, str):
+            v = _STEP[v]
+        if k == "index" and isinstance(v, str):
+            v = _INDEX[v]
+        if k not in dict(lbm_options._fields_):
+            raise KeyError(f"unknown option {k!r}")
+        setattr(s, k, int(v))
     return s
 
 
@@ -153,17 +188,17 @@ def lbm_build_index(mask, z_open=0, with_nbr=True):
     return vox2id, (nbr[:, :nf.value] if with_nbr else None), nf.value, nw.value
 
 
-def lbm_build_schedule(mask, z_open=0, tile=128, lead=256):
-    """Host-only: the fused-step work schedule lbm_create builds. Returns records[n_items, 16]."""
+def lbm_build_window(mask, z_open=0, tile=128, lead=256):
+    """Host-only: the window-step work schedule lbm_create builds. Returns records[n_items, 16]."""
     lib = load()
     mask = np.ascontiguousarray(mask, np.uint8)
     nz, ny, nx = mask.shape
     nf = int((mask == 0).sum())
-    cap = 2 * (nf // tile + 1) + (int((mask != 0).sum()) // tile + 1)
+    cap = 2 * (nf // tile + 1) + (int((mask != 0).sum()) // tile + 1) + 2 * (nx * ny // tile + 1)
     rec = np.zeros((cap, 16), np.int32)
     n = C.c_longlong()
-    _chk(lib.lbm_build_schedule(mask.ctypes.data, nx, ny, nz, int(z_open), int(tile), int(lead),
-                                rec.ctypes.data, cap, C.byref(n)), "lbm_build_schedule")
+    _chk(lib.lbm_build_window(mask.ctypes.data, nx, ny, nz, int(z_open), int(tile), int(lead),
+                              rec.ctypes.data, cap, C.byref(n)), "lbm_build_window")
     return rec[:n.value]
 
 
@@ -196,7 +231,7 @@ class Lbm:
     slab=True: a z-slab context (lbm_create_slab; mask = owned planes + 2 halo planes per cut
     end; halo = (low, high) flags, 0 only at the ends of a z-open box)."""
 
-    def __init__(self, mask, params, slab=False, halo=(1, 1)):
+    def __init__(self, mask, params, slab=False, halo=(1, 1), options=None):
         lib = load()
         import torch
         if torch.cuda.is_available():
@@ -211,12 +246,23 @@ class Lbm:
         self._h = C.c_void_p()
         ps = make_params(params)
         self.slab = bool(slab)
-        if slab:
-            _chk(lib.lbm_create_slab(C.byref(self._h), mask.ctypes.data, nx, ny, nz,
-                                     C.byref(ps), int(halo[0]), int(halo[1])), "lbm_create_slab")
+        if options is None:
+            if slab:
+                _chk(lib.lbm_create_slab(C.byref(self._h), mask.ctypes.data, nx, ny, nz,
+                                         C.byref(ps), int(halo[0]), int(halo[1])),
+                     "lbm_create_slab")
+            else:
+                _chk(lib.lbm_create(C.byref(self._h), mask.ctypes.data, nx, ny, nz, C.byref(ps)),
+                     "lbm_create")
         else:
-            _chk(lib.lbm_create(C.byref(self._h), mask.ctypes.data, nx, ny, nz, C.byref(ps)),
-                 "lbm_create")
+            po = make_options(options)
+            if slab:
+                _chk(lib.lbm_create_slab_opt(C.byref(self._h), mask.ctypes.data, nx, ny, nz,
+                                             C.byref(ps), C.byref(po), int(halo[0]),
+                                             int(halo[1])), "lbm_create_slab_opt")
+            else:
+                _chk(lib.lbm_create_opt(C.byref(self._h), mask.ctypes.data, nx, ny, nz,
+                                        C.byref(ps), C.byref(po)), "lbm_create_opt")
         self.num_owned = int(lib.lbm_num_owned(self._h))
         self.num_fluid = int(lib.lbm_num_fluid(self._h))
         self.num_wall_solid = int(lib.lbm_num_wall_solid(self._h))
@@ -297,6 +343,14 @@ class Lbm:
              "lbm_slab_buffer")
         return int(ptr.value or 0), int(n.value)
 
+    def step_info(self):
+        v = (C.c_int * 8)()
+        _chk(load().lbm_step_info(self._h, v), "lbm_step_info")
+        return {"step": {LBM_STEP_SPLIT: "split", LBM_STEP_WINDOW: "window"}[v[0]],
+                "index": {LBM_INDEX_16: "16", LBM_INDEX_BITS: "bits"}[v[1]],
+                "window_slack": v[2], "window_reach": v[3],
+                "window_items": v[5], "window_grid": v[6], "wide_tiles": v[7]}
+
     def sync(self):
         _chk(load().lbm_sync(self._h), "lbm_sync")
 
@@ -307,7 +361,12 @@ class Lbm:
         for k in names:
             if k in fields:
                 res[k] = out[k] if out is not None else np.empty(self.shape, np.float64)
-                ptrs.append(res[k].ctypes.data)
+                a = res[k]
+                if (not isinstance(a, np.ndarray) or a.dtype != np.float64 or a.shape != self.shape
+                        or not a.flags["C_CONTIGUOUS"] or not a.flags["WRITEABLE"]):
+                    raise ValueError(f"out[{k!r}] must be a writeable C-contiguous float64 array "
+                                     f"of shape {self.shape}")
+                ptrs.append(a.ctypes.data)
             else:
                 ptrs.append(None)
         _chk(load().lbm_get_macroscopic(self._h, *ptrs), "lbm_get_macroscopic")

@@ -150,30 +150,31 @@ def test_compact_index_on_config_geometries():
     assert nf == int((c["mask"] == 0).sum())
 
 
-# ------------------------------------------------------------------ fused-step schedule (host)
+# ------------------------------------------------------------------ window-step schedule (host)
 
-@pytest.mark.parametrize("z_open,lead", [(0, 0), (1, 4), (0, 16)])
-def test_fused_schedule_is_a_valid_topological_order(z_open, lead):
-    """Every D/W/C item appears exactly once and every tile an item waits for (its dependency
-    ranges) was issued earlier in the schedule; the ranges cover the true psi stencil."""
+@pytest.mark.parametrize("z_open,slack", [(0, 0), (1, 4), (0, 16)])
+def test_window_schedule_is_a_valid_topological_order(z_open, slack):
+    """Every D/W/C/P item appears exactly once and every tile an item waits for (its dependency
+    ranges) was issued earlier in the schedule; the ranges of a C item cover its true psi stencil."""
     rng = np.random.Generator(np.random.PCG64(23))
     mask = (rng.uniform(size=(12, 20, 24)) < 0.35).astype(np.uint8)
     if z_open:
         mask[:2] = 0
         mask[-2:] = 0
     tile = 32
-    rec = lbm.lbm_build_schedule(mask, z_open, tile, lead)
+    rec = lbm.lbm_build_window(mask, z_open, tile, slack)
     vox2id, nbr, nf, nw = lbm.lbm_build_index(mask, z_open)
     ntf, ntw = -(-nf // tile), -(-nw // tile)
-    typ = rec[:, 0].astype(np.uint32) >> 30
-    til = rec[:, 0] & 0x3FFFFFFF
-    assert len(rec) == 2 * ntf + ntw
-    for k, n in ((0, ntf), (1, ntw), (2, ntf)):
+    ntp = -(-(20 * 24) // tile) if z_open else 0
+    typ = rec[:, 0].astype(np.uint32) >> 28
+    til = rec[:, 0] & 0x0FFFFFFF
+    assert len(rec) == 2 * ntf + ntw + 2 * ntp
+    for k, n in ((0, ntf), (1, ntw), (2, ntf), (3, 2 * ntp)):
         assert sorted(til[typ == k]) == list(range(n))
-    pos_d = np.empty(ntf, np.int64)
-    pos_d[til[typ == 0]] = np.nonzero(typ == 0)[0]
-    pos_w = np.empty(max(ntw, 1), np.int64)
-    pos_w[til[typ == 1]] = np.nonzero(typ == 1)[0]
+    pos = {}
+    for k, n in ((0, ntf), (1, ntw), (2, ntf)):
+        pos[k] = np.empty(max(n, 1), np.int64)
+        pos[k][til[typ == k]] = np.nonzero(typ == k)[0]
 
     def covered(r):
         out = set()
@@ -183,10 +184,24 @@ def test_fused_schedule_is_a_valid_topological_order(z_open, lead):
 
     ids = np.where(nbr < 0, -nbr - 1, nbr)                  # mirror ids beyond open planes
     for k in range(len(rec)):
-        d, w = covered(rec[k, 1:7]), covered(rec[k, 7:13])
-        assert all(pos_d[t] < k for t in d) and all(pos_w[j] < k for j in w)
+        a, b = covered(rec[k, 1:7]), covered(rec[k, 7:13])
+        first = 2 if typ[k] == 3 else 0                      # P items wait for C tiles
+        assert all(pos[first][t] < k for t in a) and all(pos[1][j] < k for j in b)
+        if typ[k] == 0:
+            assert not a and not b
         if typ[k] == 2:                                      # C item: ranges cover its psi stencil
             cols = ids[:, til[k] * tile:(til[k] + 1) * tile]
             need_d = set((cols[cols < nf] // tile).tolist())
             need_w = set(((cols[cols >= nf] - nf) // tile).tolist())
-            assert need_d <= d and need_w <= w
+            assert need_d <= a and need_w <= b
+        if typ[k] == 3:                                      # P item: every tile that writes into
+            plane, chunk = divmod(til[k], ntp)               # its plane nodes / their inner neighbours
+            npl = 20 * 24
+            q = np.arange(chunk * tile, min(npl, (chunk + 1) * tile))
+            vb = q if plane == 0 else nf - npl + q
+            vf = npl + q if plane == 0 else nf - 2 * npl + q
+            need = set((np.concatenate([vb, vf]) // tile).tolist())
+            for v in np.concatenate([vb, vf]):
+                src = nbr[:, v]
+                need |= set((src[(src >= 0) & (src < nf)] // tile).tolist())
+            assert need <= a
