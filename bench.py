@@ -46,10 +46,6 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "slab"])
-    ap.add_argument("--step", default=None, choices=["auto", "split", "window"],
-                    help="lbm_options.step (default: the library's choice)")
-    ap.add_argument("--slack", type=int, default=0, help="lbm_options.window_slack (tiles)")
-    ap.add_argument("--ctas", type=int, default=0, help="lbm_options.window_ctas")
     return ap.parse_args()
 
 
@@ -201,14 +197,7 @@ def run_ours(args):
     K = args.steps if args.steps is not None else 500
     W = args.warmup if args.warmup is not None else 20
     cfg = workload(args)
-    opts = {}
-    if args.step:
-        opts["step"] = args.step
-    if args.slack:
-        opts["window_slack"] = args.slack
-    if args.ctas:
-        opts["window_ctas"] = args.ctas
-    sim = Lbm(cfg["mask"], cfg["params"], options=opts or None)
+    sim = Lbm(cfg["mask"], cfg["params"])
     sim.set_density(cfg["rhoA"], cfg["rhoB"])
     nf = sim.num_fluid
     mem = sim.memory_bytes()

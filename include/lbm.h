@@ -69,31 +69,18 @@ typedef struct {
 /* Execution options (plain data, copied by lbm_create_opt; every combination computes the same
  * numbers bit for bit -- tests/test_gpu_parity.py -- they select how the step is scheduled).
  * lbm_options_default fills in the defaults; lbm_create uses them. */
-enum { LBM_STEP_AUTO = 0, LBM_STEP_SPLIT = 1, LBM_STEP_WINDOW = 2 };
 enum { LBM_INDEX_16 = 0, LBM_INDEX_BITS = 1 };
 typedef struct {
-  int step;         /* LBM_STEP_SPLIT: one kernel per pass (density, virtual solid, fused
-                       force+collide+stream), chained by programmatic dependent launch.
-                       LBM_STEP_WINDOW: the whole step (a0-a6) as ONE persistent kernel in which the
-                       density pass runs a fixed distance ahead of the fused pass, so that the fused
-                       pass finds the populations in L2.
-                       LBM_STEP_AUTO (default): WINDOW for boxes above 600 000 fluid nodes whose
-                       lead window fits the L2, SPLIT otherwise (small boxes replay a CUDA graph)   */
   int index;        /* neighbour index of the fused pass: LBM_INDEX_16 (default) 16-bit tile-relative
                        rows, 37 B per node; LBM_INDEX_BITS per-row bitmasks + prefix ids, 0.5 B per
-                       voxel + 4 B per node (low-memory option, split step only, ~2.5 % slower)     */
-  int graph;        /* split step: -1 (default) replay a captured CUDA graph of 16 steps on boxes of
+                       voxel + 4 B per node (low-memory option, ~2.5 % slower)                      */
+  int graph;        /* -1 (default) replay a captured CUDA graph of 16 steps on boxes of
                        <= 600 000 fluid nodes, 0 never, 1 always                                    */
-  int pdl;          /* split step: 1 (default) programmatic dependent launch of the three passes    */
-  int reverse;      /* split step: 1 (default) the fused pass walks the tiles backwards (L2 reuse
+  int pdl;          /* 1 (default) programmatic dependent launch of the three passes    */
+  int reverse;      /* 1 (default) the fused pass walks the tiles backwards (L2 reuse
                        across the two passes)                                                       */
-  int keep_psi_mb;  /* split step: L2 budget in MB for psi stored with evict_last priority
+  int keep_psi_mb;  /* L2 budget in MB for psi stored with evict_last priority
                        (default 48; 0: plain stores)                                                */
-  int window_slack; /* window step: how many fluid tiles (of 128 nodes) before its first consumer a
-                       producer item is issued; 0 (default) = 450.  The density items then lead the
-                       fused items by one z-plane of tiles + twice this                             */
-  int window_ctas;  /* window step, fp32: resident CTAs per SM the kernel is compiled for: 0 (default)
-                       = 7 (72 registers), 6 (80 registers)                                        */
 } lbm_options;
 void lbm_options_default(lbm_options* o);
 
@@ -109,10 +96,10 @@ int lbm_create_opt(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz,
 /* Synchronises the device (kernels of the context may be in flight on any stream it was used
  * from), then releases everything.  NULL is allowed. */
 void lbm_destroy(lbm_ctx* c);
-/* What lbm_create chose: info[0] step (LBM_STEP_SPLIT / LBM_STEP_WINDOW), [1] index form,
- * [2] slack and [3] largest stencil reach of the window schedule (tiles), [4] unused, [5] its item count,
- * [6] CTAs of the window kernel (0 before the first step), [7] tiles that fall back to int32
- * index rows. */
+/* What lbm_create chose: info[0] index form (LBM_INDEX_16 / LBM_INDEX_BITS; a box edge above
+ * 1024 falls back to LBM_INDEX_16), [1] 1 if lbm_step replays CUDA graphs, [2] pdl, [3] reverse,
+ * [4] share of the psi lines stored with evict_last priority, in 1/1000, [5] tiles that read the
+ * int32 index rows instead of the 16-bit ones, [6], [7] reserved (0). */
 int lbm_step_info(lbm_ctx* c, int info[8]);
 
 /* f_i^sigma = w_i * rho_sigma (reading R11); dense double arrays of nx*ny*nz.  Also records the
@@ -130,7 +117,7 @@ int lbm_set_boundary(lbm_ctx* c, double inlet_value, double outlet_rho);
  * 9), streaming with halfway bounce-back, open-plane fix (L147-157).
  * Asynchronous on torch's current stream; n >= 0.  A context may be used from different streams
  * in turn: a call on another stream than the previous call's first waits for the work enqueued
- * there.  In the split step the open-plane fix of the last step is deferred: it is applied by the
+ * there.  The open-plane fix of the last step is deferred: it is applied by the
  * next lbm_step (inside its density pass) or by the next getter, whichever comes first, with the
  * boundary values that were in force when the step ran; callers always observe a complete state. */
 int lbm_step(lbm_ctx* c, int n);
@@ -166,7 +153,7 @@ int lbm_memory_bytes(lbm_ctx* c, long long bytes[4]);
 /* Device time (ms) of the kernels of the last lbm_step call, by kind, measured with CUDA events
  * on the launching stream when profiling is enabled with lbm_set_profiling(c, 1):
  * ms[0] density pass (in the default path it carries the open-plane fix of the previous step),
- * [1] virtual-solid pass, [2] collide+stream (the whole step in the window step),
+ * [1] virtual-solid pass, [2] collide+stream,
  * [3] open-plane fix when it is launched on its own; launches = number of kernel launches of that
  * call.  Synchronises. */
 int lbm_set_profiling(lbm_ctx* c, int on);
@@ -181,18 +168,6 @@ const char* lbm_last_error(void);
  * x+e_i lies beyond an open plane.  Returns N_f through *nf and N_w through *nw. */
 int lbm_build_index(const uint8_t* solid, int nx, int ny, int nz, int z_open, int32_t* vox2id,
                     int32_t* nbr, long long nbr_cap, long long* nf, long long* nw);
-
-/* Host-only helper (no GPU needed): the work schedule of the window step exactly as lbm_create
- * builds it.  records: caller-allocated, cap_items*16 int32; item k is
- * records[16k..16k+15] = {type<<28 | tile, 3 x (lo,cnt) dependency ranges of a first kind,
- * 3 x (lo,cnt) of a second kind, 0, 0, 0}: type 0 = D, density pass on a fluid tile (no
- * dependencies); 1 = W, virtual-solid pass on a wall tile (first kind: D tiles); 2 = C, fused
- * collide+stream pass on a fluid tile (first kind: D tiles, second kind: W tiles); 3 = P,
- * open-plane fix on `tile` nodes of plane tile / ntp (first kind: C tiles).  Tiles are `tile`
- * consecutive ids.  Every item follows the items it depends on.  *n_items receives the item
- * count. */
-int lbm_build_window(const uint8_t* solid, int nx, int ny, int nz, int z_open, int tile,
-                     int lead, int32_t* records, long long cap_items, long long* n_items);
 
 /* ---- z-slab sharding across GPUs --------
  * The step has two grid-wide dependencies (Eq. 11/13: every node's force needs its

@@ -130,211 +130,6 @@ int build(Geometry& g, const uint8_t* solid, int nx, int ny, int nz, int z_open,
   return 0;
 }
 
-namespace {
-
-// Compress a sorted list of distinct tile ids into at most kDepRanges (lo,cnt) ranges by closing
-// the smallest gaps first (a range may then cover tiles that are not strictly needed).
-void to_ranges(std::vector<int32_t>& ids, int32_t* out /* 2*kDepRanges */) {
-  for (int k = 0; k < 2 * kDepRanges; ++k) out[k] = 0;
-  if (ids.empty()) return;
-  std::sort(ids.begin(), ids.end());
-  ids.erase(std::unique(ids.begin(), ids.end()), ids.end());
-  std::vector<std::pair<int32_t, int32_t>> r;  // [lo, hi]
-  for (int32_t v : ids) {
-    if (!r.empty() && v == r.back().second + 1) r.back().second = v;
-    else r.emplace_back(v, v);
-  }
-  while ((int)r.size() > kDepRanges) {
-    size_t best = 0;
-    int32_t gap = r[1].first - r[0].second;
-    for (size_t k = 1; k + 1 < r.size(); ++k)
-      if (r[k + 1].first - r[k].second < gap) { gap = r[k + 1].first - r[k].second; best = k; }
-    r[best].second = r[best + 1].second;
-    r.erase(r.begin() + best + 1);
-  }
-  for (size_t k = 0; k < r.size(); ++k) {
-    out[2 * k] = r[k].first;
-    out[2 * k + 1] = r[k].second - r[k].first + 1;
-  }
-}
-
-}  // namespace
-
-int build_window(const Geometry& g, int tile, int lead, Window& s) {
-  if (tile < 32 || g.nf <= 0 || g.nbr.empty() || g.nact != g.nf) return -1;
-  const long long nf = g.nf, nw = g.nw, np = (long long)g.nx * g.ny;
-  s.tile = tile;
-  s.ntf = (int)((nf + tile - 1) / tile);
-  s.ntw = (int)((nw + tile - 1) / tile);
-  s.ntp = (g.open_lo || g.open_hi) ? (int)((np + tile - 1) / tile) : 0;
-  const int ntf = s.ntf, ntw = s.ntw, ntp = s.ntp;
-  try {
-    // dependency ranges: C(t) -> D, W tiles of its psi stencil; W(j) -> D tiles of its fluid
-    // neighbours; P(k) -> C tiles that write into its plane nodes and their interior neighbours
-    std::vector<int32_t> dep_c((size_t)ntf * 4 * kDepRanges), dep_w((size_t)ntw * 2 * kDepRanges);
-    std::vector<int32_t> dep_p((size_t)2 * ntp * 2 * kDepRanges, 0);
-#pragma omp parallel
-    {
-      std::vector<int32_t> ds, ws;
-#pragma omp for schedule(static)
-      for (int t = 0; t < ntf; ++t) {
-        ds.clear(); ws.clear();
-        const long long n1 = std::min<long long>(nf, (long long)(t + 1) * tile);
-        for (int i = 0; i < 18; ++i)
-          for (long long n = (long long)t * tile; n < n1; ++n) {
-            int32_t id = g.nbr[(size_t)i * nf + n];
-            if (id < 0) id = -id - 1;
-            const int32_t k = id < nf ? id / tile : (int32_t)((id - nf) / tile);
-            std::vector<int32_t>& v = id < nf ? ds : ws;
-            if (v.empty() || v.back() != k) v.push_back(k);
-          }
-        to_ranges(ds, &dep_c[(size_t)t * 4 * kDepRanges]);
-        to_ranges(ws, &dep_c[(size_t)t * 4 * kDepRanges + 2 * kDepRanges]);
-      }
-#pragma omp for schedule(static)
-      for (int j = 0; j < ntw; ++j) {
-        ds.clear();
-        const long long w1 = std::min<long long>(nw, (long long)(j + 1) * tile);
-        for (int i = 0; i < 18; ++i)
-          for (long long w = (long long)j * tile; w < w1; ++w) {
-            const int32_t id = g.wall_nbr[(size_t)i * nw + w];
-            if (id < 0) continue;
-            const int32_t k = id / tile;
-            if (ds.empty() || ds.back() != k) ds.push_back(k);
-          }
-        to_ranges(ds, &dep_w[(size_t)j * 2 * kDepRanges]);
-      }
-#pragma omp for schedule(static)
-      for (int k = 0; k < 2 * ntp; ++k) {
-        const int plane = k / ntp;
-        if (!(plane == 0 ? g.open_lo : g.open_hi)) continue;
-        ds.clear();
-        const long long q0 = (long long)(k - plane * ntp) * tile, q1 = std::min(np, q0 + tile);
-        for (long long q = q0; q < q1; ++q) {
-          // open planes and their interior neighbours are solid-free: ids q, np+q / nf-np+q, nf-2np+q
-          const long long v2[2] = {plane == 0 ? q : nf - np + q, plane == 0 ? np + q : nf - 2 * np + q};
-          for (long long v : v2) {
-            ds.push_back((int32_t)(v / tile));
-            for (int i = 1; i < kQ; ++i) {  // population i of v is pushed by the node at v - e_i
-              const int32_t src = g.nbr[(size_t)(kOpp[i] - 1) * nf + v];
-              if (src >= 0 && src < nf) ds.push_back((int32_t)(src / tile));
-            }
-          }
-        }
-        to_ranges(ds, &dep_p[(size_t)k * 2 * kDepRanges]);
-      }
-    }
-    // furthest tile of 3 ranges that is not a periodic wrap-around seen from `from` (-1 if none)
-    auto far_of = [&](const int32_t* r, int from, int n) {
-      int far = -1;
-      for (int k = 0; k < kDepRanges; ++k) {
-        const int hi = r[2 * k] + r[2 * k + 1] - 1;
-        if (r[2 * k + 1] > 0 && hi > far && hi - from < n / 2 + 1) far = hi;
-      }
-      return far;
-    };
-    // Issue time of every item, in units of fluid tiles: C(t) is issued at time t.  A producer
-    // is issued `slack` before its first consumer, so that it has normally completed (and its
-    // flag need not be waited for) when the consumer starts: W(j) at (first C tile that reads
-    // it) - slack, D(k) at min(first C tile that reads it, issue time of the first W tile that
-    // reads it) - slack.  D(k) thus leads C(k) by (local reach of the psi stencil, about one
-    // z-plane of tiles) + 2 * slack: the window of populations the L2 has to hold.
-    const int slack = std::max(0, lead);
-    const long long kNever = (long long)4 * ntf + 8;
-    std::vector<long long> time_d(ntf, kNever), time_w(ntw, kNever);
-    for (int t = ntf - 1; t >= 0; --t) {  // first consumer = smallest t: walk down, overwrite
-      const int32_t* d = &dep_c[(size_t)t * 4 * kDepRanges];
-      const int32_t* w = d + 2 * kDepRanges;
-      for (int k = 0; k < kDepRanges; ++k) {
-        for (int q = 0; q < d[2 * k + 1]; ++q) time_d[d[2 * k] + q] = t;
-        for (int q = 0; q < w[2 * k + 1]; ++q) time_w[w[2 * k] + q] = t;
-      }
-    }
-    for (int j = 0; j < ntw; ++j) time_w[j] -= slack;   // a wall tile nobody reads goes last
-    for (int k = 0; k < ntf; ++k) time_d[k] -= slack;
-    for (int j = 0; j < ntw; ++j) {
-      const int32_t* d = &dep_w[(size_t)j * 2 * kDepRanges];
-      for (int k = 0; k < kDepRanges; ++k)
-        for (int q = 0; q < d[2 * k + 1]; ++q)
-          time_d[d[2 * k] + q] = std::min(time_d[d[2 * k] + q], time_w[j] - slack);
-    }
-    int reach = 0;
-    for (int t = 0; t < ntf; ++t)
-      reach = std::max(reach, far_of(&dep_c[(size_t)t * 4 * kDepRanges], t, ntf) - t);
-    s.reach = reach;
-    s.slack = slack;
-    struct Item { long long key; int type, idx; };
-    std::vector<Item> order;
-    order.reserve((size_t)2 * ntf + ntw + 2 * ntp);
-    for (int j = 0; j < ntf; ++j) order.push_back({time_d[j], 0, j});
-    for (int j = 0; j < ntw; ++j) order.push_back({time_w[j], 1, j});
-    for (int t = 0; t < ntf; ++t) order.push_back({(long long)t, 2, t});
-    for (int k = 0; k < 2 * ntp; ++k) {
-      const int plane = k / ntp;
-      if (!(plane == 0 ? g.open_lo : g.open_hi)) continue;
-      const int32_t* d = &dep_p[(size_t)k * 2 * kDepRanges];
-      int far = 0;
-      for (int q = 0; q < kDepRanges; ++q)
-        if (d[2 * q + 1] > 0) far = std::max(far, d[2 * q] + d[2 * q + 1] - 1);
-      order.push_back({(long long)far + std::max(slack, 1), 3, k});
-    }
-    std::stable_sort(order.begin(), order.end(),
-                     [](const Item& a, const Item& b) { return a.key < b.key; });
-    // emit in that order; an item whose dependency has not been emitted yet (periodic wrap, tiny
-    // boxes) pulls it in front of itself, so every item follows what it waits for
-    s.records.clear();
-    s.records.reserve(order.size() * kWinRecordInts);
-    std::vector<uint8_t> done_d(ntf, 0), done_w(ntw, 0), done_c(ntf, 0);
-    auto push = [&](int type, int t, const int32_t* a, const int32_t* b) {
-      const size_t base = s.records.size();
-      s.records.resize(base + kWinRecordInts, 0);
-      s.records[base] = (int32_t)(((uint32_t)type << 28) | (uint32_t)t);
-      for (int k = 0; k < 2 * kDepRanges; ++k) {
-        s.records[base + 1 + k] = a ? a[k] : 0;
-        s.records[base + 1 + 2 * kDepRanges + k] = b ? b[k] : 0;
-      }
-    };
-    auto emit_d = [&](int t) {
-      if (done_d[t]) return;
-      done_d[t] = 1;
-      push(0, t, nullptr, nullptr);
-    };
-    auto emit_w = [&](int j) {
-      if (done_w[j]) return;
-      done_w[j] = 1;
-      const int32_t* d = &dep_w[(size_t)j * 2 * kDepRanges];
-      for (int k = 0; k < kDepRanges; ++k)
-        for (int q = 0; q < d[2 * k + 1]; ++q) emit_d(d[2 * k] + q);
-      push(1, j, d, nullptr);
-    };
-    auto emit_c = [&](int t) {
-      if (done_c[t]) return;
-      done_c[t] = 1;
-      const int32_t* d = &dep_c[(size_t)t * 4 * kDepRanges];
-      const int32_t* w = d + 2 * kDepRanges;
-      for (int k = 0; k < kDepRanges; ++k) {
-        for (int q = 0; q < w[2 * k + 1]; ++q) emit_w(w[2 * k] + q);
-        for (int q = 0; q < d[2 * k + 1]; ++q) emit_d(d[2 * k] + q);
-      }
-      push(2, t, d, w);
-    };
-    for (const Item& it : order) {
-      if (it.type == 0) emit_d(it.idx);
-      else if (it.type == 1) emit_w(it.idx);
-      else if (it.type == 2) emit_c(it.idx);
-      else {
-        const int32_t* d = &dep_p[(size_t)it.idx * 2 * kDepRanges];
-        for (int k = 0; k < kDepRanges; ++k)
-          for (int q = 0; q < d[2 * k + 1]; ++q) emit_c(d[2 * k] + q);
-        push(3, it.idx, d, nullptr);
-      }
-    }
-  } catch (const std::bad_alloc&) {
-    return -4;
-  }
-  return 0;
-}
-
 int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Index16& out) {
   if (g.nf <= 0 || g.nbr.empty()) return -1;
   const long long nf = g.nf;

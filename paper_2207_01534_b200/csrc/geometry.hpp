@@ -39,28 +39,6 @@ struct Geometry {
   std::vector<double> wall_inv_den;
 };
 
-// Work schedule of the single-kernel ("window") step.  The step is cut into
-// items over tiles of `tile` consecutive ids -- D(t): density pass on fluid tile t, W(j):
-// virtual-solid pass on wall tile j, C(t): fused force+collide+stream pass on fluid tile t, P(k):
-// open-plane fix on `tile` nodes of an open plane (k = plane * ntp + chunk) -- and the items are
-// put in ONE global order in which every item comes after the items it depends on.  Dependencies
-// are explicit: each item lists up to kDepRanges (lo,cnt) ranges of completion flags of a first
-// kind (D tiles for W and C items, C tiles for P items) and of a second kind (W tiles, C items
-// only); a range may cover more tiles than strictly needed.  Every producer is issued `slack`
-// fluid tiles before its first consumer, so D(j) runs (local stencil reach + 2 * slack) tiles ahead
-// of C(j): the populations D(j) reads are then still in L2 when C(j) reads them again.
-constexpr int kDepRanges = 3;
-constexpr int kWinRecordInts = 16;  // {type<<28|tile, first kind: 3 x (lo,cnt), second kind: 3 x (lo,cnt), 0, 0, 0}
-struct Window {
-  int tile = 128;
-  int ntf = 0, ntw = 0, ntp = 0;  // fluid tiles, wall tiles, P items per open plane (0: z periodic)
-  int reach = 0;                  // largest distance (tiles) a C tile's psi stencil reaches ahead of it
-  int slack = 0;                  // issue distance between a producer and its first consumer
-  std::vector<int32_t> records;   // [nitems * kWinRecordInts]; type 0 = D, 1 = W, 2 = C, 3 = P
-  size_t nitems() const { return records.size() / kWinRecordInts; }
-};
-int build_window(const Geometry& g, int tile, int slack, Window& s);
-
 // 16-bit tile-relative form of the neighbour index (halves the index traffic of the fused pass).
 // For tile t (kIdxTile consecutive fluid ids) and direction i the entries of nbr are written as
 //   bit 15 = 0: fluid id (or mirror node)  = meta[t][i-1]      + (e & 0x7fff)

@@ -86,8 +86,8 @@ __device__ __forceinline__ void store_vec2(Vec2<double>* p, Vec2<double> v, uint
 }
 
 // Explicitly rounded scalar operations.  The same device function is inlined into several kernels
-// (the open-plane fix runs in k_open_planes, k_density_open and k_step_window; the virtual-solid
-// sum in k_wallpsi and k_step_window); left to the compiler, whether a*b+c becomes one FMA or a
+// (the open-plane fix runs in k_open_planes and k_density_open; the tile function in the fp32 and
+// fp64 fused passes of every index form); left to the compiler, whether a*b+c becomes one FMA or a
 // multiply and an add depends on the surrounding code, and the kernels would differ in the last
 // bit.  Every product-sum of such shared code is therefore spelled out.
 __device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
@@ -403,61 +403,11 @@ __device__ __forceinline__ Pr<T> edot2(int i, Pr<T> x, Pr<T> y, Pr<T> z) {
   return r;
 }
 
-// L2 eviction policies and hinted accesses of the single-kernel step (k_step_window).  evict_last
-// on the density items' loads keeps a tile's populations in L2 until the fused item of the same
-// tile reads them again a short while later; evict_first on that second read and streaming stores
-// let them leave first.
-__device__ __forceinline__ uint64_t l2_policy_evict_last() {
-  uint64_t p;
-  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-  return p;
-}
-__device__ __forceinline__ uint64_t l2_policy_evict_first() {
-  uint64_t p;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-  return p;
-}
-__device__ __forceinline__ Vec2<float> load_vec2_keep(const Vec2<float>* p, uint64_t pol) {
-  Vec2<float> v;
-  asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;"
-               : "=f"(v.a), "=f"(v.b) : "l"(p), "l"(pol));
-  return v;
-}
-__device__ __forceinline__ Vec2<double> load_vec2_keep(const Vec2<double>* p, uint64_t pol) {
-  Vec2<double> v;
-  asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;"
-               : "=d"(v.a), "=d"(v.b) : "l"(p), "l"(pol));
-  return v;
-}
-__device__ __forceinline__ void bulk_g2s_hint(void* dst, const void* src, uint32_t bytes,
-                                              uint64_t* bar, uint64_t pol) {
-  asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
-      "[%0], [%1], %2, [%3], %4;" ::"r"(smem_u32(dst)),
-      "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
-      : "memory");
-}
-// one (A, B) pair of a population; CS: streaming store
-template <bool CS>
-__device__ __forceinline__ void store_pair(Pr<float>* p, Pr<float> v) {
-  if constexpr (CS)
-    asm volatile("st.global.cs.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.a), "f"(v.b) : "memory");
-  else
-    *p = v;
-}
-template <bool CS>
-__device__ __forceinline__ void store_pair(Pr<double>* p, Pr<double> v) {
-  if constexpr (CS)
-    asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.a), "d"(v.b) : "memory");
-  else
-    *p = v;
-}
-
 // Per-thread work of the fused pass on a staged tile: sf = [38][TN] populations, sid = [18][TN]
 // neighbour ids in shared memory; tid = column of this thread in the tile; n = its node id.
 // Threads of the ragged last tile (valid = false) compute on the zero padding and only their
-// stores are predicated off, so control flow stays warp-uniform.  CS: streaming push stores.
-template <typename T, int TN, bool REMAINDER, bool CS = false>
+// stores are predicated off, so control flow stays warp-uniform.
+template <typename T, int TN, bool REMAINDER>
 __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
                                                     const int* __restrict__ sid, const int tid,
                                                     const int n, const bool valid,
@@ -551,13 +501,13 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
       const int k = sidc[(ip - 1) * TN];
       const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)ip * np32 + (unsigned)k
                                                        : (unsigned)im * np32 + (unsigned)n;
-      if (valid && k >= 0) store_pair<CS>(fo + slot, vp);
+      if (valid && k >= 0) fo[slot] = vp;
     }
     {
       const int k = sidc[(im - 1) * TN];
       const unsigned slot = (unsigned)k < (unsigned)nf ? (unsigned)im * np32 + (unsigned)k
                                                        : (unsigned)ip * np32 + (unsigned)n;
-      if (valid && k >= 0) store_pair<CS>(fo + slot, vm);
+      if (valid && k >= 0) fo[slot] = vm;
     }
   }
   // rest population: Eq. (1) with e_0 = 0, or the remainder rho - sum_{i>=1} f*_i (fp32 build)
@@ -569,7 +519,7 @@ __device__ __forceinline__ void collide_tile_thread(const T* __restrict__ sf,
     const P f0 = sfp[0];
     v0 = pfma(pbc(c1), f0, pfma(pbc(mul_rn(mul_rn(om, w0), k0)), R, pmul(pbc(mul_rn(cS, w0)), M3UF)));
   }
-  if (valid) store_pair<CS>(fo + n, v0);
+  if (valid) fo[n] = v0;
 }
 
 // 16-bit tile-relative neighbour index (geometry.hpp Index16): per tile 18 rows of TN uint16 plus
@@ -620,25 +570,18 @@ struct TileSmem {
 
 // Stage one tile: 19 population rows of TN (A, B) pairs, 18 rows of 16-bit index, the tile's
 // record of bases -> shared memory, completion on `bar`.  Call from one converged warp.
-// HINT: the population rows are read with the L2 policy `pol`.
-template <typename T, int TN, bool ALIAS, bool HINT>
+template <typename T, int TN, bool ALIAS>
 __device__ __forceinline__ void stage_tile16(const TileSmem<T, TN, ALIAS> sm,
                                              const T* __restrict__ fin, const Idx16& ix,
-                                             size_t npad, unsigned tile, uint64_t* bar,
-                                             uint64_t pol) {
+                                             size_t npad, unsigned tile, uint64_t* bar) {
   const size_t t0 = (size_t)tile * TN;
   if (elect_one()) {
     mbar_expect_tx(bar, (uint32_t)((size_t)2 * Q * TN * sizeof(T) +
                                    (size_t)18 * TN * sizeof(uint16_t) + kIdxMeta * sizeof(int)));
 #pragma unroll
-    for (int r = 0; r < Q; ++r) {  // one row of TN (A, B) pairs per direction
-      if constexpr (HINT)
-        bulk_g2s_hint(sm.sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2,
-                      2 * TN * sizeof(T), bar, pol);
-      else
-        bulk_g2s(sm.sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2,
-                 2 * TN * sizeof(T), bar);
-    }
+    for (int r = 0; r < Q; ++r)  // one row of TN (A, B) pairs per direction
+      bulk_g2s(sm.sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2,
+               2 * TN * sizeof(T), bar);
 #pragma unroll
     for (int r = 0; r < 18; ++r)
       bulk_g2s(sm.s16 + (size_t)r * TN, ix.nbr16 + (size_t)r * npad + t0, TN * sizeof(uint16_t),
@@ -653,7 +596,7 @@ __device__ __forceinline__ void stage_tile16(const TileSmem<T, TN, ALIAS> sm,
 // recognised from the node's plane and e_z.  Rare "wide" tiles (an offset range does not fit 15
 // bits) take the int32 rows with a second round of bulk copies (one more phase of `bar`).
 // Called by every thread of the CTA.
-template <typename T, int TN, bool ALIAS, bool REREAD = false>
+template <typename T, int TN, bool ALIAS>
 __device__ __forceinline__ void decode_tile16(const TileSmem<T, TN, ALIAS> sm,
                                               const int* __restrict__ nbr, const Idx16& ix,
                                               size_t npad, size_t t0, int n, int tid, int warp,
@@ -688,13 +631,9 @@ __device__ __forceinline__ void decode_tile16(const TileSmem<T, TN, ALIAS> sm,
       sm.sid[(i - 1) * TN + tid] = k;
     }
   }
-  // REREAD: the tile function re-reads the ids from shared memory where it needs them; without
-  // this compiler barrier the 18 decoded ids are forwarded in registers across the psi gathers
-  // (fine in the one-tile kernel, more spills in the persistent one)
-  if constexpr (REREAD) asm volatile("" ::: "memory");
 }
 
-// The fused pass of the split step (one kernel per pass): one CTA per tile.
+// The fused pass (a3-a6): one CTA per tile.
 // IDX: 1 = 16-bit tile-relative rows (default), 2 = geometric (bitmask) index (low-memory option)
 template <typename T, int TN, int MINB, bool REMAINDER, int IDX>
 __global__ void __launch_bounds__(TN, MINB)
@@ -773,7 +712,7 @@ __global__ void __launch_bounds__(TN, MINB)
     mbar_wait(&bar, phase);
     phase ^= 1u;
   } else {
-    if (warp == 0) stage_tile16<T, TN, kAlias, false>(sm, fin, ix, npad, tile, &bar, 0);
+    if (warp == 0) stage_tile16<T, TN, kAlias>(sm, fin, ix, npad, tile, &bar);
     // the bulk copies above read the populations (complete since the previous step; the density
     // pass that fixed the open planes finished before the wall pass began) and the static index;
     // psi and the wall psi are this step's
@@ -968,208 +907,6 @@ __global__ void __launch_bounds__(256, 4)
     if (op.kind[plane] == 0) return;
     store_vec2(psi + (plane == 0 ? q : nf - np + q),
                open_plane_node<T>(f, frozen, nf, np, npad, op, plane, q), pol);
-  }
-}
-
-// ---------------------------------------------------------------------------------------------
-// Single-kernel step ("window" step).  The two grid-wide dependencies of a step -- every node's
-// force needs its neighbours' rho(t) (Eq. 11/13), every wall solid's rho~(t) needs its fluid
-// neighbours' rho(t) (Eq. 15) -- are resolved INSIDE one persistent kernel instead of by kernel
-// boundaries, so that the density pass runs only a short, fixed distance (the "lead", ~20 MB of
-// populations) ahead of the fused pass: the populations it has just read are then still in the
-// 126 MB L2 when the fused pass reads them again, and the second 152 B/node DRAM read of the
-// two-pass method disappears (472 -> ~320 B/node of DRAM traffic).
-//
-// Work items over tiles of TN consecutive ids, in ONE host-built order (geometry.hpp Window) in
-// which every item follows the items it depends on:
-//   D(t)  a1 on fluid tile t             publishes flags_d[t]
-//   W(j)  a2 on wall tile j              needs D of its fluid neighbours; publishes flags_w[j]
-//   C(t)  a3-a6 on fluid tile t          needs D and W of its psi stencil; publishes flags_c[t]
-//   P(k)  a0 on TN nodes of an open plane (after streaming, as PAPER.md L147-157 has it)
-//                                        needs C of every tile that pushes into those nodes or
-//                                        into their interior neighbours
-// CTAs take items with an atomic ticket, in that order.  A ticket holder waits only on items with
-// smaller tickets, which are finished or held by running CTAs, so the scheme cannot deadlock and
-// needs no co-residency guarantee.  An item's dependencies are at most 6 (lo,cnt) ranges of flags
-// (a psi stencil touches ~10 D tiles in three id ranges, one per z-plane); one warp loads all of
-// them at once and spins until each carries this step's epoch.  Producers run far enough ahead
-// (lead) that the flags are normally already set.
-//
-// Visibility.  A producer's stores are followed by the CTA barrier at the end of the item and a
-// gpu-scope release store of the flag by thread 0 (release is cumulative over the barrier).  The
-// consumer's warp 0 polls with relaxed gpu-scope loads (served by L2), and the CTA barrier that
-// follows orders every thread's loads after the poll.  No acquire fence is used: a gpu-scope
-// acquire invalidates the SM's whole L1 (CCTL.IVALL), which seven co-resident CTAs would pay on
-// every item, and it is not needed -- within one launch every psi / fout line is written once,
-// a line can only enter an L1 after the flag of its (line-aligned) tile was seen set, i.e. with
-// final data, and L1 does not survive a kernel boundary.
-__device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
-  int v;
-  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st_release_gpu(int* p, int v) {
-  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
-constexpr int kWinRecordInts = 16;  // geometry.hpp kWinRecordInts
-// rec[1..12] = 6 x (lo,cnt): ranges 0-2 index fa, ranges 3-5 index fb.  Call from all 32 lanes of
-// one warp.
-__device__ __forceinline__ void wait_flags(const int* __restrict__ fa, const int* __restrict__ fb,
-                                           const int* rec, int epoch) {
-  const int lane = threadIdx.x & 31;
-  int total = 0;
-#pragma unroll
-  for (int r = 0; r < 6; ++r) total += rec[2 + 2 * r];
-  for (int base = 0; base < total; base += 32) {
-    const int k = base + lane;
-    const int* p = nullptr;
-    int c0 = 0;
-#pragma unroll
-    for (int r = 0; r < 6; ++r) {
-      const int cnt = rec[2 + 2 * r];
-      if (k >= c0 && k < c0 + cnt) p = (r < 3 ? fa : fb) + rec[1 + 2 * r] + (k - c0);
-      c0 += cnt;
-    }
-    while (true) {
-      const int ok = p == nullptr || ld_relaxed_gpu(p) == epoch;
-      if (__all_sync(0xffffffffu, ok)) break;
-      __nanosleep(32);
-    }
-  }
-}
-
-struct WinSched {
-  const int4* items;   // [nitems][4]: 16 ints per item = {type << 28 | tile, 6 x (lo,cnt), 0, 0, 0}
-  int nitems;
-  int* flags_d;        // [fluid tiles]  epoch of the last step in which D(t) completed
-  int* flags_w;        // [wall tiles]
-  int* flags_c;        // [fluid tiles]  (used by the P items: only in z-open boxes)
-  int epoch;           // this step's epoch (> 0, increases by one per step)
-  int np;              // nodes per z-plane; P item k covers plane k / ntp, nodes (k % ntp)*TN ...
-  int ntp;             // P items per open plane
-};
-
-template <typename T, int TN, int MINB, bool REMAINDER>
-__global__ void __launch_bounds__(TN, MINB)
-    k_step_window(const T* __restrict__ fin, T* __restrict__ fout, Vec2<T>* __restrict__ psi,
-                  const int* __restrict__ nbr, const int* __restrict__ wall_nbr,
-                  const T* __restrict__ inv_den, const T* __restrict__ frozen, int nf, int nw,
-                  size_t npad, size_t nwpad, Consts<T> c, Idx16 ix, OpenPlane<T> op, WinSched sc,
-                  int* __restrict__ ctr, int* __restrict__ ctr_next) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  constexpr bool kAlias = MINB >= 7;
-  const TileSmem<T, TN, kAlias> sm(smem_raw);
-  __shared__ uint64_t bar;
-  __shared__ __align__(16) int s_rec[2][kWinRecordInts];  // double-buffered item record
-  const int tid = threadIdx.x;
-  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // compiler-visible warp-uniform value
-  if (tid == 0) mbar_init(&bar, 1);
-  // Thread 0 draws a ticket, threads 0-3 fetch its record; the NEXT ticket is drawn while the CTA
-  // works on the current item.
-  if (tid < 4) {
-    int k = 0;
-    if (tid == 0) k = atomicAdd(&ctr[0], 1);
-    k = __shfl_sync(0xfu, k, 0);
-    reinterpret_cast<int4*>(s_rec[0])[tid] =
-        k < sc.nitems ? __ldg(sc.items + (size_t)4 * k + tid) : make_int4(-1, 0, 0, 0);
-    if (blockIdx.x == 0 && tid == 0) ctr_next[0] = 0;  // the other step's counter is idle now
-  }
-  __syncthreads();
-  uint32_t phase = 0;
-  int buf = 0;
-  while (true) {
-    const int* rec = s_rec[buf];
-    const int head = __shfl_sync(0xffffffffu, rec[0], 0);
-    if (head == -1) break;
-    if (tid < 4) {
-      int k = 0;
-      if (tid == 0) k = atomicAdd(&ctr[0], 1);
-      k = __shfl_sync(0xfu, k, 0);
-      reinterpret_cast<int4*>(s_rec[buf ^ 1])[tid] =
-          k < sc.nitems ? __ldg(sc.items + (size_t)4 * k + tid) : make_int4(-1, 0, 0, 0);
-    }
-    const int type = (int)((unsigned)head >> 28), t = head & 0x0fffffff;
-    if (type == 0) {
-#ifndef WIN_NO_D
-      // ---- D(t): a1 on fluid tile t, summed in direction order exactly as k_density does
-      const int n = t * TN + tid;  // < npad; the padding holds zeros
-      const Vec2<T>* f2 = reinterpret_cast<const Vec2<T>*>(fin);
-      const uint64_t keep = l2_policy_evict_last();
-      Vec2<T> v[Q];
-#pragma unroll
-      for (int i = 0; i < Q; ++i) v[i] = load_vec2_keep(f2 + (size_t)i * npad + n, keep);
-      T ra = v[0].a, rb = v[0].b;
-#pragma unroll
-      for (int i = 1; i < Q; ++i) { ra += v[i].a; rb += v[i].b; }
-      Vec2<T> o; o.a = ra; o.b = rb;
-      psi[n] = o;
-#endif
-    } else if (type == 1) {
-#ifndef WIN_NO_W
-      // ---- W(j): a2 on wall tile t (Eq. 14-15), as k_wallpsi
-      const int w = t * TN + tid;
-      const bool live = w < nw;
-      int id[Q];
-#pragma unroll
-      for (int i = 1; i < Q; ++i) id[i] = live ? wall_nbr[(size_t)(i - 1) * nwpad + w] : -1;
-      const T s = live ? inv_den[w] : T(0);
-      if (warp == 0) wait_flags(sc.flags_d, sc.flags_d, rec, sc.epoch);
-      __syncthreads();
-      if (live) {
-        T na = T(0), nb = T(0);
-#pragma unroll
-        for (int i = 1; i < Q; ++i) {
-          if (id[i] >= 0) {
-            const Vec2<T> p = psi[id[i]];
-            na = fma_rn(wgt<T>(i), p.a, na);
-            nb = fma_rn(wgt<T>(i), p.b, nb);
-          }
-        }
-        Vec2<T> o; o.a = mul_rn(mul_rn(c.chiA, na), s); o.b = mul_rn(mul_rn(c.chiB, nb), s);
-        psi[npad + w] = o;
-      }
-#endif
-    } else if (type == 2) {
-      // ---- C(t): a3-a6 on fluid tile t.  The tile's populations and index do not depend on
-      // psi: their bulk copies are in flight while warp 0 checks the flags.
-      // (the row stride is laundered through an empty asm so that the compiler does not hoist the
-      // 37 row offsets out of the item loop and then spill them)
-      size_t np_it = npad;
-      asm volatile("" : "+l"(np_it));
-      if (warp == 0) {
-        stage_tile16<T, TN, kAlias, true>(sm, fin, ix, np_it, (unsigned)t, &bar,
-                                          l2_policy_evict_first());
-        wait_flags(sc.flags_d, sc.flags_w, rec, sc.epoch);
-      }
-      __syncthreads();
-      mbar_wait(&bar, phase);
-      phase ^= 1u;
-      const size_t t0 = (size_t)t * TN;
-      const int n = (int)t0 + tid;
-      decode_tile16<T, TN, kAlias, true>(sm, nbr, ix, np_it, t0, n, tid, warp, &bar, phase);
-      collide_tile_thread<T, TN, REMAINDER, true>(sm.sf, sm.sid, tid, n, n < nf, fout, psi, nf,
-                                                  np_it, c);
-      // the decoded ids were written through the generic proxy; the next item's bulk copies write
-      // the same shared memory through the async proxy
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    } else {
-      // ---- P(k): a0 on TN nodes of an open plane of the NEW buffer (reading R12)
-#ifndef WIN_NO_P
-      if (warp == 0) wait_flags(sc.flags_c, sc.flags_c, rec, sc.epoch);
-      __syncthreads();
-      const int plane = t / sc.ntp, q = (t - plane * sc.ntp) * TN + tid;
-      if (q < sc.np && op.kind[plane] != 0)
-        open_plane_node<T>(fout, frozen, nf, sc.np, npad, op, plane, q);
-#endif
-    }
-    __syncthreads();  // the item's stores are issued; the stage is free; the next record is in place
-    if (tid == 0) {
-      int* flag = type == 0 ? sc.flags_d + t : type == 1 ? sc.flags_w + t
-                  : (type == 2 && sc.flags_c) ? sc.flags_c + t : nullptr;
-      if (flag) st_release_gpu(flag, sc.epoch);
-    }
-    buf ^= 1;
   }
 }
 

@@ -113,20 +113,10 @@ struct lbm_ctx {
   uint16_t* nbr16 = nullptr;         // [18][npad]
   int* nbr16_meta = nullptr;         // [tiles][kIdxMeta]
   long long wide_tiles = 0;
-  int reverse = 1;          // fused pass of the split step walks the tiles backwards (L2 reuse across passes)
-  int step_variant = 0;     // 0: one kernel per pass (split), 1: single-kernel window step
-  int win_grid = 0;         // CTAs of the window kernel (resident CTAs per SM x SMs)
-  int win_reach = 0, win_slack = 0;
-  int win_ctas = 7;         // resident CTAs per SM the fp32 window kernel is compiled for (6: 80 registers)
-  int4* win_items = nullptr;         // window-step schedule records (geometry.hpp Window)
-  int win_nitems = 0, win_ntf = 0, win_ntw = 0, win_ntp = 0;
-  int* win_ctr = nullptr;            // [2][4] ticket counters, alternating per step
-  int* win_flags = nullptr;          // [ntf | ntw | ntf] completion epochs of D, W, C items
-  int win_epoch = 0;
-  int win_parity = 0;
+  int reverse = 1;          // the fused pass walks the tiles backwards (L2 reuse across the passes)
   float keep_psi = 0.f;     // share of the psi lines stored with L2 evict_last priority, from
   int keep_psi_mb = 48;     // this budget: min(1, MB / psi bytes) (0: off)
-  int pdl = 1;              // programmatic dependent launch of the three passes of the split step
+  int pdl = 1;              // programmatic dependent launch of the three passes
   // Launch-bound boxes (a step of config 1 or 2 is three kernels of 3-8 us each): lbm_step replays
   // a captured CUDA graph of kGraphSteps steps (programmatic-dependent-launch edges included)
   // instead of launching every kernel from the host.  One graph per starting buffer parity;
@@ -163,9 +153,8 @@ struct lbm_ctx {
     lbm_shim_free(f[0]); lbm_shim_free(f[1]); lbm_shim_free(psi); lbm_shim_free(nbr);
     lbm_shim_free(wall_nbr); lbm_shim_free(wall_inv_den); lbm_shim_free(node_vox_d);
     lbm_shim_free(frozen); lbm_shim_free(partial); lbm_shim_free(diag_out);
-    lbm_shim_free(win_items); lbm_shim_free(win_ctr); lbm_shim_free(nbr16);
+    lbm_shim_free(nbr16);
     lbm_shim_free(nbr16_meta);
-    lbm_shim_free(win_flags);
     lbm_shim_free(halo_slots); lbm_shim_free(halo_send); lbm_shim_free(halo_recv);
     lbm_shim_free(ccl);
     lbm_shim_free(bit_rec); lbm_shim_free(bit_coord);
@@ -188,14 +177,6 @@ Consts<T> make_consts(const lbm_params& p) {
 
 constexpr int kGraphSteps = 16;            // even: the buffer parity returns to its start
 constexpr int kGraphAutoNodes = 600000;    // above this a step is long enough to hide the launches
-// Window step: a producer item is issued this many fluid tiles before its first consumer (about
-// the number of items in flight on 148 SMs x 7 CTAs, in tile units); LBM_STEP_AUTO takes the
-// window step only if the resulting lead is a window of populations the L2 holds beside the
-// step's write stream.
-constexpr int kWindowSlackTiles = 450;
-constexpr long long kWindowMaxBytes = 40LL << 20;
-constexpr bool kWindowAuto = true;
-
 template <typename T>
 OpenPlane<T> make_open(const lbm_params& p, const int (&open_end)[2]) {
   OpenPlane<T> o;
@@ -393,82 +374,23 @@ void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaS
   }
 }
 
-// One launch of the single-kernel window step (a0-a6 of one time step; kernels.cuh k_step_window).
-template <typename T, int MINB>
-int launch_window(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStream_t st) {
-  constexpr int TN = 128;
-  constexpr bool kRemainder = sizeof(T) == 4;
-  constexpr size_t smem = collide16_smem_bytes<T, TN, (MINB >= 7)>();
-  auto kern = k_step_window<T, TN, MINB, kRemainder>;
-  static int grid_cache_dev[64] = {};  // per device
-  int& grid_cache = grid_cache_dev[c->device & 63];
-  if (grid_cache == 0) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int per_sm = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TN, smem));
-    if (per_sm < 1) return fail(LBM_ECUDA, "window kernel does not fit on an SM");
-    grid_cache = per_sm * c->num_sms;
-  }
-  c->win_grid = std::min(grid_cache, c->win_nitems);
-  Idx16 ix;
-  ix.nbr16 = c->nbr16;
-  ix.meta = c->nbr16_meta;
-  ix.np_lo = c->open_end[0] ? c->np : 0;
-  ix.np_hi = c->open_end[1] ? c->np : 0;
-  ix.reverse = 0;
-  ix.nact = c->nact;
-  ix.bits = nullptr; ix.coord = nullptr;
-  ix.nx = c->nx; ix.ny = c->ny; ix.nz = c->nz; ix.words = 0;
-  ix.tile0 = 0; ix.split = 0; ix.tile1 = 0;
-  WinSched sc;
-  sc.items = c->win_items;
-  sc.nitems = c->win_nitems;
-  sc.flags_d = c->win_flags;
-  sc.flags_w = c->win_flags + c->win_ntf;
-  sc.flags_c = c->win_ntp ? c->win_flags + c->win_ntf + c->win_ntw : nullptr;
-  sc.epoch = ++c->win_epoch;
-  sc.np = c->np;
-  sc.ntp = c->win_ntp;
-  int* ctr = c->win_ctr + 4 * c->win_parity;
-  int* ctr_next = c->win_ctr + 4 * (c->win_parity ^ 1);
-  c->win_parity ^= 1;
-  kern<<<c->win_grid, TN, smem, st>>>(fin, fout, (Vec2<T>*)c->psi, (const int*)c->nbr,
-                                      (const int*)c->wall_nbr, (const T*)c->wall_inv_den,
-                                      (const T*)c->frozen, c->nf, c->nw, c->npad, c->nwpad, k, ix,
-                                      make_open<T>(c->p, c->open_end), sc, ctr, ctr_next);
-  return LBM_OK;
-}
-
 template <typename T>
 int step_T(lbm_ctx* c, int n, cudaStream_t st) {
   const Consts<T> k = make_consts<T>(c->p);
   for (int it = 0; it < n; ++it) {
     const T* fin = (const T*)c->f[c->cur];
     T* fout = (T*)c->f[c->cur ^ 1];
-    if (c->step_variant == 1) {
-      apply_pending_T<T>(c, st);  // left by a split step (not in a run of window steps)
-      Timed t(c, st, 2);
-      int rc;
-      if constexpr (sizeof(T) == 4) {
-        rc = c->win_ctas == 6 ? launch_window<T, 6>(c, fin, fout, k, st)
-                              : launch_window<T, 7>(c, fin, fout, k, st);
-      } else {
-        rc = launch_window<T, 2>(c, fin, fout, k, st);
-      }
-      if (rc) return rc;
-      c->cur ^= 1;               // the open-plane fix is part of the kernel: the state is complete
-    } else {
-      launch_psi<T>(c, st);
+    launch_psi<T>(c, st);
+    {
       Timed t(c, st, 2);
       launch_collide<T>(c, fin, fout, k, st);
-      c->cur ^= 1;
-      if (c->p.z_open) c->open_pending = true;  // a0 is folded into the next density pass
     }
+    c->cur ^= 1;
+    if (c->p.z_open) c->open_pending = true;  // a0 is folded into the next density pass
   }
   CU(cudaPeekAtLastError());
   return LBM_OK;
 }
-
 
 // n steps, through graph replays where that pays (see lbm_ctx::graph_mode)
 template <typename T>
@@ -477,7 +399,7 @@ int step_graphed_T(lbm_ctx* c, int n, cudaStream_t st) {
   const bool open = c->open_end[0] || c->open_end[1];
   // the first steps run directly: they configure the kernels' attributes and bring the deferred
   // open-plane fix into its steady state (pending at the start of every step)
-  if (!want || c->prof || c->step_variant != 0 || c->slab) {
+  if (!want || c->prof || c->slab) {
     c->steps_done += n;
     return step_T<T>(c, n, st);
   }
@@ -581,45 +503,22 @@ int lbm_build_index(const uint8_t* solid, int nx, int ny, int nz, int z_open, in
   return LBM_OK;
 }
 
-int lbm_build_window(const uint8_t* solid, int nx, int ny, int nz, int z_open, int tile,
-                     int lead, int32_t* records, long long cap_items, long long* n_items) {
-  if (!solid || !records || !n_items) return fail(LBM_EINVAL, "NULL argument");
-  lbmgeo::Geometry g;
-  const int rc = lbmgeo::build(g, solid, nx, ny, nz, z_open, true);
-  if (rc) return fail(rc, "geometry build failed (%d)", rc);
-  lbmgeo::Window s;
-  if (lbmgeo::build_window(g, tile, lead < 0 ? 0 : lead, s) != 0)
-    return fail(LBM_EINVAL, "schedule build failed");
-  *n_items = (long long)s.nitems();
-  if ((long long)s.nitems() > cap_items) return fail(LBM_EINVAL, "records capacity too small");
-  std::memcpy(records, s.records.data(), s.records.size() * sizeof(int32_t));
-  return LBM_OK;
-}
-
 void lbm_options_default(lbm_options* o) {
   if (!o) return;
-  o->step = LBM_STEP_AUTO;
   o->index = LBM_INDEX_16;
   o->graph = -1;
   o->pdl = 1;
   o->reverse = 1;
   o->keep_psi_mb = 48;
-  o->window_slack = 0;
-  o->window_ctas = 0;
 }
 
 static int validate_options(const lbm_options* o) {
-  if (o->step < LBM_STEP_AUTO || o->step > LBM_STEP_WINDOW)
-    return fail(LBM_EINVAL, "options.step must be LBM_STEP_AUTO, LBM_STEP_SPLIT or LBM_STEP_WINDOW");
   if (o->index != LBM_INDEX_16 && o->index != LBM_INDEX_BITS)
     return fail(LBM_EINVAL, "options.index must be LBM_INDEX_16 or LBM_INDEX_BITS");
   if (o->graph < -1 || o->graph > 1) return fail(LBM_EINVAL, "options.graph must be -1, 0 or 1");
   if ((o->pdl != 0 && o->pdl != 1) || (o->reverse != 0 && o->reverse != 1))
     return fail(LBM_EINVAL, "options.pdl and options.reverse must be 0 or 1");
-  if (o->keep_psi_mb < 0 || o->window_slack < 0)
-    return fail(LBM_EINVAL, "options.keep_psi_mb and options.window_slack must be >= 0");
-  if (o->window_ctas != 0 && o->window_ctas != 6 && o->window_ctas != 7)
-    return fail(LBM_EINVAL, "options.window_ctas must be 0 (default), 6 or 7");
+  if (o->keep_psi_mb < 0) return fail(LBM_EINVAL, "options.keep_psi_mb must be >= 0");
   return LBM_OK;
 }
 
@@ -672,7 +571,6 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   c->graph_mode = o.graph;
   c->keep_psi_mb = o.keep_psi_mb;
   c->idx16 = o.index == LBM_INDEX_BITS ? 2 : 1;
-  if (o.window_ctas) c->win_ctas = o.window_ctas;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
   // pair-slot indices i * npad + k and psi indices npad + w are 32-bit
   if ((size_t)19 * c->npad >= ((size_t)1 << 31) || c->npad + c->nwpad >= ((size_t)1 << 31)) {
@@ -721,28 +619,7 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   if (e == cudaSuccess) e = cudaMemsetAsync(c->psi, 0, psibytes, st);
   if (e == cudaSuccess && frozenbytes) e = cudaMemsetAsync(c->frozen, 0, frozenbytes, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->nbr, 0, nbrbytes, st);
-  // Window-step schedule (built from the raw ids; only when that step is selected), then re-base
-  // wall ids from nf+w to npad+w so that the wall part of psi starts on a tile boundary.
-  // LBM_STEP_AUTO: the window step when the box is large enough that launch gaps do not matter and
-  // the distance by which the density items lead the fused items (one z-plane of tiles plus twice
-  // the slack) is a window the L2 holds.
-  lbmgeo::Window win;
-  {
-    const int slack = o.window_slack > 0 ? o.window_slack : kWindowSlackTiles;
-    const long long plane_tiles = ((long long)nx * ny + 127) / 128;   // a solid-free plane
-    const long long lead = plane_tiles + 2 * slack;
-    const bool fits = lead * 128 * 19 * 2 * (long long)c->esz <= kWindowMaxBytes;
-    const bool want = !c->slab && c->idx16 == 1 &&
-                      (o.step == LBM_STEP_WINDOW ||
-                       (o.step == LBM_STEP_AUTO && kWindowAuto && g.nf > kGraphAutoNodes && fits));
-    if (want) {
-      if (lbmgeo::build_window(g, 128, slack, win) != 0) {
-        delete c;
-        return fail(LBM_ENOMEM, "window schedule build failed");
-      }
-      c->step_variant = 1;
-    }
-  }
+  // Re-base wall ids from nf+w to npad+w so that the wall part of psi starts on a tile boundary.
   lbmgeo::Index16 i16;
   if (lbmgeo::build_index16(g, (long long)c->npad, c->npad, i16) != 0) {
     delete c;
@@ -777,27 +654,6 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   up(c->nbr16, i16.nbr16.data(), i16.nbr16.size() * sizeof(uint16_t));
   up(c->nbr16_meta, i16.meta.data(), i16.meta.size() * sizeof(int32_t));
   c->bytes[2] += (long long)(i16.nbr16.size() * 2 + i16.meta.size() * 4);
-  // window-step schedule records, completion flags and counters
-  if (c->step_variant == 1) {
-    c->win_nitems = (int)win.nitems();
-    c->win_ntf = win.ntf;
-    c->win_ntw = win.ntw;
-    c->win_ntp = win.ntp;
-    c->win_reach = win.reach;
-    c->win_slack = win.slack;
-    const size_t nflags = (size_t)2 * win.ntf + win.ntw;
-    c->win_items = (int4*)lbm_shim_alloc(win.records.size() * sizeof(int32_t));
-    c->win_ctr = (int*)lbm_shim_alloc(8 * sizeof(int));
-    c->win_flags = (int*)lbm_shim_alloc(nflags * sizeof(int));
-    if (!c->win_items || !c->win_ctr || !c->win_flags) {
-      delete c;
-      return fail(LBM_ENOMEM, "device allocation failed (window schedule)");
-    }
-    up(c->win_items, win.records.data(), win.records.size() * sizeof(int32_t));
-    if (e == cudaSuccess) e = cudaMemsetAsync(c->win_ctr, 0, 8 * sizeof(int), st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(c->win_flags, 0, nflags * sizeof(int), st);
-    c->bytes[2] += (long long)(win.records.size() * 4 + nflags * 4);
-  }
   lbmgeo::BitIndex bix;  // upload source until the sync below
   if (c->idx16 == 2) {
     if (lbmgeo::build_bitindex(g, (long long)c->npad, bix) != 0) {
@@ -929,10 +785,13 @@ int lbm_create_slab_opt(lbm_ctx** out, const uint8_t* solid_local, int nx, int n
 
 int lbm_step_info(lbm_ctx* c, int info[8]) {
   if (!c || !info) return fail(LBM_EINVAL, "NULL argument");
-  info[0] = c->step_variant == 1 ? LBM_STEP_WINDOW : LBM_STEP_SPLIT;
-  info[1] = c->idx16 == 2 ? LBM_INDEX_BITS : LBM_INDEX_16;
-  info[2] = c->win_slack; info[3] = c->win_reach; info[4] = 0;
-  info[5] = c->win_nitems; info[6] = c->win_grid; info[7] = (int)c->wide_tiles;
+  const bool graph = c->graph_mode == 1 || (c->graph_mode < 0 && c->nf <= kGraphAutoNodes);
+  info[0] = c->idx16 == 2 ? LBM_INDEX_BITS : LBM_INDEX_16;
+  info[1] = graph && !c->slab ? 1 : 0;
+  info[2] = c->pdl; info[3] = c->reverse;
+  info[4] = (int)(c->keep_psi * 1000.f + 0.5f);
+  info[5] = (int)std::min<long long>(c->wide_tiles, 2147483647LL);
+  info[6] = 0; info[7] = 0;
   return LBM_OK;
 }
 

@@ -22,7 +22,7 @@ SYMBOLS = [
     "lbm_set_boundary", "lbm_step", "lbm_sync", "lbm_get_macroscopic", "lbm_diagnostics",
     "lbm_saturation", "lbm_trapped_volume", "lbm_mean_pressure", "lbm_num_fluid", "lbm_num_wall_solid",
     "lbm_memory_bytes", "lbm_set_profiling", "lbm_last_step_profile", "lbm_last_error",
-    "lbm_build_index", "lbm_build_window",
+    "lbm_build_index",
     "lbm_options_default", "lbm_create_opt", "lbm_create_slab_opt", "lbm_step_info",
     "lbm_create_slab", "lbm_slab_density", "lbm_slab_collide", "lbm_slab_unpack", "lbm_slab_buffer",
     "lbm_num_owned", "lbm_build_slab_halo",
@@ -45,14 +45,11 @@ class lbm_params(C.Structure):
 
 
 class lbm_options(C.Structure):
-    _fields_ = [("step", C.c_int), ("index", C.c_int), ("graph", C.c_int), ("pdl", C.c_int),
-                ("reverse", C.c_int), ("keep_psi_mb", C.c_int), ("window_slack", C.c_int),
-                ("window_ctas", C.c_int)]
+    _fields_ = [("index", C.c_int), ("graph", C.c_int), ("pdl", C.c_int), ("reverse", C.c_int),
+                ("keep_psi_mb", C.c_int)]
 
 
-LBM_STEP_AUTO, LBM_STEP_SPLIT, LBM_STEP_WINDOW = 0, 1, 2
 LBM_INDEX_16, LBM_INDEX_BITS = 0, 1
-_STEP = {"auto": LBM_STEP_AUTO, "split": LBM_STEP_SPLIT, "window": LBM_STEP_WINDOW}
 _INDEX = {"16": LBM_INDEX_16, "bits": LBM_INDEX_BITS}
 
 _lib = None
@@ -98,7 +95,6 @@ def load():
     lib.lbm_last_error.argtypes = []
     lib.lbm_last_error.restype = C.c_char_p
     lib.lbm_build_index.argtypes = [V, I, I, I, I, V, V, LL, C.POINTER(LL), C.POINTER(LL)]
-    lib.lbm_build_window.argtypes = [V, I, I, I, I, I, I, V, LL, C.POINTER(LL)]
     lib.lbm_options_default.argtypes = [C.POINTER(lbm_options)]
     lib.lbm_options_default.restype = None
     lib.lbm_create_opt.argtypes = [C.POINTER(P), V, I, I, I, C.POINTER(lbm_params),
@@ -129,7 +125,7 @@ def load():
                "lbm_diagnostics", "lbm_saturation", "lbm_trapped_volume", "lbm_mean_pressure",
                "lbm_memory_bytes",
                "lbm_set_profiling", "lbm_last_step_profile", "lbm_build_index",
-               "lbm_build_window", "lbm_create_opt", "lbm_create_slab_opt", "lbm_step_info"):
+               "lbm_create_opt", "lbm_create_slab_opt", "lbm_step_info"):
         getattr(lib, fn).restype = I
     _lib = lib
     return lib
@@ -153,12 +149,10 @@ def make_params(p):
 
 def make_options(o=None):
     """dict -> lbm_options: the library's defaults (lbm_options_default) with the given fields
-    replaced; step may be "auto" | "split" | "window", index "16" | "bits"."""
+    replaced; index may be "16" | "bits"."""
     s = lbm_options()
     load().lbm_options_default(C.byref(s))
     for k, v in (o or {}).items():
-        if k == "step" and isinstance(v, str):
-            v = _STEP[v]
         if k == "index" and isinstance(v, str):
             v = _INDEX[v]
         if k not in dict(lbm_options._fields_):
@@ -186,20 +180,6 @@ def lbm_build_index(mask, z_open=0, with_nbr=True):
                              nbr.ctypes.data if with_nbr else None, 18 * max(nfluid, 1),
                              C.byref(nf), C.byref(nw)), "lbm_build_index")
     return vox2id, (nbr[:, :nf.value] if with_nbr else None), nf.value, nw.value
-
-
-def lbm_build_window(mask, z_open=0, tile=128, lead=256):
-    """Host-only: the window-step work schedule lbm_create builds. Returns records[n_items, 16]."""
-    lib = load()
-    mask = np.ascontiguousarray(mask, np.uint8)
-    nz, ny, nx = mask.shape
-    nf = int((mask == 0).sum())
-    cap = 2 * (nf // tile + 1) + (int((mask != 0).sum()) // tile + 1) + 2 * (nx * ny // tile + 1)
-    rec = np.zeros((cap, 16), np.int32)
-    n = C.c_longlong()
-    _chk(lib.lbm_build_window(mask.ctypes.data, nx, ny, nz, int(z_open), int(tile), int(lead),
-                              rec.ctypes.data, cap, C.byref(n)), "lbm_build_window")
-    return rec[:n.value]
 
 
 def lbm_build_slab_halo(mask_local, z_open=0, halo=(1, 1)):
@@ -346,10 +326,9 @@ class Lbm:
     def step_info(self):
         v = (C.c_int * 8)()
         _chk(load().lbm_step_info(self._h, v), "lbm_step_info")
-        return {"step": {LBM_STEP_SPLIT: "split", LBM_STEP_WINDOW: "window"}[v[0]],
-                "index": {LBM_INDEX_16: "16", LBM_INDEX_BITS: "bits"}[v[1]],
-                "window_slack": v[2], "window_reach": v[3],
-                "window_items": v[5], "window_grid": v[6], "wide_tiles": v[7]}
+        return {"index": {LBM_INDEX_16: "16", LBM_INDEX_BITS: "bits"}[v[0]], "graph": bool(v[1]),
+                "pdl": bool(v[2]), "reverse": bool(v[3]), "keep_psi": v[4] / 1000.0,
+                "wide_tiles": v[5]}
 
     def sync(self):
         _chk(load().lbm_sync(self._h), "lbm_sync")

@@ -191,7 +191,7 @@ class SlabLbm:
     Global arrays are [z, y, x]; `get_macroscopic` returns the owned planes of this process
     (all planes when world is None)."""
 
-    def __init__(self, mask, params, parts=None, rank=None, world=None, group=None):
+    def __init__(self, mask, params, parts=None, rank=None, world=None, group=None, options=None):
         mask = np.ascontiguousarray(mask, np.uint8)
         self.shape = mask.shape
         self.world = world
@@ -201,7 +201,7 @@ class SlabLbm:
         self.mine = [rank] if world is not None else list(range(nparts))
         self.halo = [halo_flags(r, nparts, self.z_open) for r in range(nparts)]
         self.sims = [Lbm(local_box(mask, *self.ranges[r], self.halo[r]), params, slab=True,
-                         halo=self.halo[r]) for r in self.mine]
+                         halo=self.halo[r], options=options) for r in self.mine]
         # fluid nodes per global plane (host copy of the mask statistics the queries weight with)
         self._plane_fluid = (mask.reshape(mask.shape[0], -1) == 0).sum(axis=1).astype(np.int64)
         self.num_fluid = sum(s.num_owned for s in self.sims)

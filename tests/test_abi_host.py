@@ -150,58 +150,33 @@ def test_compact_index_on_config_geometries():
     assert nf == int((c["mask"] == 0).sum())
 
 
-# ------------------------------------------------------------------ window-step schedule (host)
+def test_library_has_no_global_knobs():
+    """no global state, no environment variables.  The shared object neither
+    imports getenv nor carries an LBM_B200_* string; execution options travel in lbm_options."""
+    import subprocess
+    path = binding.library_path()
+    lbm.load()
+    und = subprocess.run(["nm", "-D", "--undefined-only", path], capture_output=True, text=True).stdout
+    assert "getenv" not in und
+    assert b"LBM_B200_" not in open(path, "rb").read()
+    src = "".join(open(os.path.join(ROOT, "paper_2207_01534_b200", "csrc", f)).read()
+                  for f in ("lbm.cu", "kernels.cuh", "geometry.cpp", "torch_shim.cpp"))
+    assert "getenv" not in src
 
-@pytest.mark.parametrize("z_open,slack", [(0, 0), (1, 4), (0, 16)])
-def test_window_schedule_is_a_valid_topological_order(z_open, slack):
-    """Every D/W/C/P item appears exactly once and every tile an item waits for (its dependency
-    ranges) was issued earlier in the schedule; the ranges of a C item cover its true psi stencil."""
-    rng = np.random.Generator(np.random.PCG64(23))
-    mask = (rng.uniform(size=(12, 20, 24)) < 0.35).astype(np.uint8)
-    if z_open:
-        mask[:2] = 0
-        mask[-2:] = 0
-    tile = 32
-    rec = lbm.lbm_build_window(mask, z_open, tile, slack)
-    vox2id, nbr, nf, nw = lbm.lbm_build_index(mask, z_open)
-    ntf, ntw = -(-nf // tile), -(-nw // tile)
-    ntp = -(-(20 * 24) // tile) if z_open else 0
-    typ = rec[:, 0].astype(np.uint32) >> 28
-    til = rec[:, 0] & 0x0FFFFFFF
-    assert len(rec) == 2 * ntf + ntw + 2 * ntp
-    for k, n in ((0, ntf), (1, ntw), (2, ntf), (3, 2 * ntp)):
-        assert sorted(til[typ == k]) == list(range(n))
-    pos = {}
-    for k, n in ((0, ntf), (1, ntw), (2, ntf)):
-        pos[k] = np.empty(max(n, 1), np.int64)
-        pos[k][til[typ == k]] = np.nonzero(typ == k)[0]
 
-    def covered(r):
-        out = set()
-        for q in range(3):
-            out.update(range(r[2 * q], r[2 * q] + r[2 * q + 1]))
-        return out
-
-    ids = np.where(nbr < 0, -nbr - 1, nbr)                  # mirror ids beyond open planes
-    for k in range(len(rec)):
-        a, b = covered(rec[k, 1:7]), covered(rec[k, 7:13])
-        first = 2 if typ[k] == 3 else 0                      # P items wait for C tiles
-        assert all(pos[first][t] < k for t in a) and all(pos[1][j] < k for j in b)
-        if typ[k] == 0:
-            assert not a and not b
-        if typ[k] == 2:                                      # C item: ranges cover its psi stencil
-            cols = ids[:, til[k] * tile:(til[k] + 1) * tile]
-            need_d = set((cols[cols < nf] // tile).tolist())
-            need_w = set(((cols[cols >= nf] - nf) // tile).tolist())
-            assert need_d <= a and need_w <= b
-        if typ[k] == 3:                                      # P item: every tile that writes into
-            plane, chunk = divmod(til[k], ntp)               # its plane nodes / their inner neighbours
-            npl = 20 * 24
-            q = np.arange(chunk * tile, min(npl, (chunk + 1) * tile))
-            vb = q if plane == 0 else nf - npl + q
-            vf = npl + q if plane == 0 else nf - 2 * npl + q
-            need = set((np.concatenate([vb, vf]) // tile).tolist())
-            for v in np.concatenate([vb, vf]):
-                src = nbr[:, v]
-                need |= set((src[(src >= 0) & (src < nf)] // tile).tolist())
-            assert need <= a
+def test_options_struct_and_defaults():
+    assert C.sizeof(lbm.lbm_options) == 20
+    o = lbm.make_options()
+    assert (o.index, o.graph, o.pdl, o.reverse, o.keep_psi_mb) == (0, -1, 1, 1, 48)
+    o = lbm.make_options({"index": "bits", "graph": 0})
+    assert (o.index, o.graph) == (1, 0)
+    with pytest.raises(KeyError):
+        lbm.make_options({"tile": 1287})
+    # bad option values are rejected before any device is needed
+    h = C.c_void_p()
+    m = np.zeros((4, 4, 4), np.uint8)
+    ps = lbm.make_params(default_params())
+    for bad in ({"index": 5}, {"graph": 3}, {"pdl": 2}, {"keep_psi_mb": -1}):
+        po = lbm.make_options(bad)
+        rc = lbm.load().lbm_create_opt(C.byref(h), m.ctypes.data, 4, 4, 4, C.byref(ps), C.byref(po))
+        assert rc == binding.LBM_EINVAL

@@ -265,35 +265,6 @@ def test_set_boundary_changes_inlet_density():
     assert np.allclose(m["rhoA"][-1], 0.98, atol=1e-12)     # outlet Dirichlet on A
 
 
-def test_fused_single_kernel_step_matches_split_and_oracle(monkeypatch):
-    """The experimental fused persistent step kernel (LBM_B200_STEP=fused: density, virtual-solid
-    and collide+stream items of one step in one cooperative launch, ordered by completion flags)
-    runs the same per-node arithmetic as the default one-kernel-per-pass path: bit-identical."""
-    c = make_config(4, size=48, storage_bits=64)
-    monkeypatch.setenv("LBM_B200_STEP", "fused")
-    monkeypatch.setenv("LBM_B200_LEAD", "8")
-    a = Lbm(c["mask"], c["params"])
-    monkeypatch.setenv("LBM_B200_STEP", "split")
-    b = Lbm(c["mask"], c["params"])
-    o = LbmRef(c["mask"], c["params"])
-    for s in (a, b, o):
-        s.set_density(c["rhoA"], c["rhoB"])
-        s.step(40)
-    for comp in (0, 1):
-        assert np.array_equal(a.get_populations(comp), b.get_populations(comp))
-    assert _pop_rel(o, a, c["mask"]) <= 1e-10
-    c32 = make_config(5, size=48)
-    monkeypatch.setenv("LBM_B200_STEP", "fused")
-    a = Lbm(c32["mask"], c32["params"])
-    monkeypatch.setenv("LBM_B200_STEP", "split")
-    b = Lbm(c32["mask"], c32["params"])
-    for s in (a, b):
-        s.set_density(c32["rhoA"], c32["rhoB"])
-        s.step(25)
-    for comp in (0, 1):
-        assert np.array_equal(a.get_populations(comp), b.get_populations(comp))
-
-
 @pytest.mark.parametrize("shape", [(1, 1, 64), (1, 40, 41), (3, 1, 5), (2, 2, 2)])
 def test_degenerate_box_shapes_fp64(shape):
     """Boxes that are one voxel thick along one or two axes (a voxel is then its own periodic
@@ -342,58 +313,83 @@ def test_velocity_inlet_on_component_b_and_extreme_parameters_fp64():
     assert _pop_rel(o, g, c["mask"]) <= 1e-10
 
 
-def test_register_kernel_and_int32_index_paths_agree_with_production(monkeypatch):
-    """A/B paths kept in the library: the one-node-per-thread register kernel
-    (LBM_B200_COLLIDE=simple: direction-by-direction collision, no pairing) and the int32 index
-    rows (LBM_B200_IDX=32) against the production fused pass, fp64, and all against the oracle."""
-    c = make_config(3, size=32, storage_bits=64)
+@pytest.mark.parametrize("bits", [64, 32])
+def test_execution_options_are_bit_identical(bits):
+    """lbm_options select how the step is scheduled and which index form the fused pass reads --
+    never what is computed: the geometric (bitmask) index, forward tile order, no programmatic
+    dependent launch, no L2 priority for psi, CUDA-graph replay all give the default path's
+    populations bit for bit (fp64 and fp32 builds), and those match the oracle."""
+    c = make_config(3, size=32, storage_bits=bits)
     sims = {}
-    for name, env in (("prod", {}), ("simple", {"LBM_B200_COLLIDE": "simple"}),
-                      ("idx32", {"LBM_B200_IDX": "32"}), ("bits", {"LBM_B200_IDX": "bits"}),
-                      ("cta6", {"LBM_B200_TILE": "1286"}), ("cta8", {"LBM_B200_TILE": "1288"}),
-                      ("fwd", {"LBM_B200_REVERSE": "0"}),
-                      ("nopdl", {"LBM_B200_PDL": "0"}), ("nokeep", {"LBM_B200_KEEP_PSI_MB": "0"})):
-        for k in ("LBM_B200_COLLIDE", "LBM_B200_IDX", "LBM_B200_REVERSE", "LBM_B200_PDL",
-                  "LBM_B200_KEEP_PSI_MB", "LBM_B200_TILE"):
-            monkeypatch.delenv(k, raising=False)
-        for k, v in env.items():
-            monkeypatch.setenv(k, v)
-        g = Lbm(c["mask"], c["params"])
+    for name, opt in (("prod", None), ("bits", {"index": "bits"}), ("fwd", {"reverse": 0}),
+                      ("nopdl", {"pdl": 0}), ("nokeep", {"keep_psi_mb": 0}), ("graph", {"graph": 1}),
+                      ("nograph", {"graph": 0})):
+        g = Lbm(c["mask"], c["params"], options=opt)
         g.set_density(c["rhoA"], c["rhoB"])
         g.step(30)
+        info = g.step_info()
+        assert info["index"] == ("bits" if name == "bits" else "16")
+        assert info["pdl"] == (name != "nopdl") and info["reverse"] == (name != "fwd")
         sims[name] = [g.get_populations(s) for s in (0, 1)]
         g.close()
-    fl = c["mask"] == 0
-    for s in (0, 1):
-        assert np.array_equal(sims["prod"][s], sims["idx32"][s])      # same arithmetic, other index
-        assert np.array_equal(sims["prod"][s], sims["bits"][s])       # ... ids from the bitmask tables
-        assert np.array_equal(sims["prod"][s], sims["fwd"][s])        # tile order is irrelevant
-        assert np.array_equal(sims["prod"][s], sims["cta6"][s])       # so is the CTA residency
-        assert np.array_equal(sims["prod"][s], sims["cta8"][s])       # (fp64 build: same kernel)
-        assert np.array_equal(sims["prod"][s], sims["nopdl"][s])      # launch overlap is irrelevant
-        assert np.array_equal(sims["prod"][s], sims["nokeep"][s])     # so is the L2 priority of psi
-        a, b = sims["simple"][s][:, fl], sims["prod"][s][:, fl]
-        assert (np.abs(a - b) / np.abs(b)).max() < 1e-11              # different operation order
+    for name in sims:
+        for s in (0, 1):
+            assert np.array_equal(sims["prod"][s], sims[name][s]), name
     o = LbmRef(c["mask"], c["params"])
     o.set_density(c["rhoA"], c["rhoB"])
     o.step(30)
+    fl = c["mask"] == 0
     for s in (0, 1):
         b = o.get_populations(s)[:, fl]
-        assert (np.abs(sims["simple"][s][:, fl] - b) / np.abs(b)).max() < 1e-10
+        assert (np.abs(sims["prod"][s][:, fl] - b) / np.abs(b)).max() < (1e-10 if bits == 64 else 1e-4)
+
+
+def test_options_are_validated():
+    from paper_2207_01534_b200 import LbmError
+    c = make_config(1, size=8)
+    for bad in ({"index": 7}, {"graph": 2}, {"pdl": 3}, {"reverse": -1}, {"keep_psi_mb": -5}):
+        with pytest.raises(LbmError) as e:
+            Lbm(c["mask"], c["params"], options=bad)
+        assert e.value.code == -1
+
+
+def test_context_used_from_several_streams():
+    """A context may be stepped and queried from different torch streams in turn (each call is
+    ordered after the work the context enqueued before, on whatever stream) and destroyed while
+    another stream than the current one holds its last kernels."""
+    import torch
+    c = make_config(4, size=32, storage_bits=64)
+    ref = Lbm(c["mask"], c["params"])
+    ref.set_density(c["rhoA"], c["rhoB"])
+    ref.step(24)
+    want = [ref.get_populations(s) for s in (0, 1)]
+    ref.close()
+    g = Lbm(c["mask"], c["params"])
+    g.set_density(c["rhoA"], c["rhoB"])
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    for k in range(6):
+        with torch.cuda.stream(s1 if k % 2 == 0 else s2):
+            g.step(4)
+    got = [g.get_populations(s) for s in (0, 1)]        # on the default stream
+    for a, b in zip(want, got):
+        assert np.array_equal(a, b)
+    with torch.cuda.stream(s1):
+        g.step(50)
+    g.close()                                            # outside the stream block
+    torch.cuda.synchronize()
 
 
 # ------------------------------------------------------------------ CUDA-graph replay of lbm_step
 
 @pytest.mark.parametrize("k,bits", [(1, 64), (3, 32), (4, 64)])
-def test_graph_replay_is_bit_identical_to_host_launches(k, bits, monkeypatch):
+def test_graph_replay_is_bit_identical_to_host_launches(k, bits):
     """lbm_step through replayed CUDA graphs of 16 steps (the default on launch-bound boxes) gives
     the populations of plain host launches bit for bit: periodic and open boxes, with getters and
     a boundary change (which drops the captured graphs) in between, odd step counts."""
     c = make_config(k, size=32 if k == 1 else 36, storage_bits=bits)
     res = []
-    for mode in ("0", "1"):
-        monkeypatch.setenv("LBM_B200_GRAPH", mode)
-        g = Lbm(c["mask"], c["params"])
+    for mode in (0, 1):
+        g = Lbm(c["mask"], c["params"], options={"graph": mode})
         g.set_density(c["rhoA"], c["rhoB"])
         g.step(53)                       # 1 direct + 3 graphs + 4 direct
         m1, _ = g.diagnostics()          # applies a pending open-plane fix: next step runs direct
@@ -411,22 +407,3 @@ def test_graph_replay_is_bit_identical_to_host_launches(k, bits, monkeypatch):
         g.close()
     for a, b in zip(res[0], res[1]):
         assert np.array_equal(a, b)
-
-
-def test_fp32_cta_residency_variants_are_bit_identical(monkeypatch):
-    """LBM_B200_TILE selects how many CTAs of the fused pass share an SM (5, 6, 7 = default, 8) and
-    with it the shared-memory layout (7: 16-bit index rows staged inside the id array; 8: rest
-    populations from a register instead of a staged row).  Same arithmetic: identical populations."""
-    c = make_config(4, size=40, storage_bits=32)
-    res = {}
-    for tile in ("1287", "1285", "1286", "1288"):
-        monkeypatch.setenv("LBM_B200_TILE", tile)
-        g = Lbm(c["mask"], c["params"])
-        g.set_density(c["rhoA"], c["rhoB"])
-        g.step(40)
-        res[tile] = [g.get_populations(s) for s in (0, 1)]
-        g.close()
-    monkeypatch.delenv("LBM_B200_TILE")
-    for tile in ("1285", "1286", "1288"):
-        for a, b in zip(res["1287"], res[tile]):
-            assert np.array_equal(a, b), tile
