@@ -78,3 +78,25 @@ def test_bad_arguments(kw):
     args.update(kw)
     with pytest.raises(ValueError):
         primary_drainage(_Scripted(), [1.0], 1.0, **args)
+
+
+def test_displacement_run_sequences_queries():
+    """paper_2207_01534_b200/displacement.py: samples at step 0 and after every block, the last
+    block shortened to the step count; saturations over the rock only (R29), P_c from the two end
+    planes (R28), trapped volume of the DISPLACED component (R15)."""
+    from paper_2207_01534_b200.displacement import displacement_run
+
+    class S(_Scripted):
+        def diagnostics(self):
+            return (1.0, 2.0), (0.0, 0.0, 0.0)
+
+    sim = S(nz=40)
+    seen = []
+    samples, final = displacement_run(sim, 2500, 1000, invading_comp=1, layers=8,
+                                      on_sample=lambda k, s, pc: seen.append(k))
+    assert [k for k, _, _ in samples] == [0, 1000, 2000, 2500] == seen
+    assert [c for c in sim.calls if c[0] == "step"] == [("step", 1000), ("step", 1000), ("step", 500)]
+    assert all(c[2:] == (8, 32) for c in sim.calls if c[0] == "saturation")
+    assert ("mean_pressure", 0, 1) in sim.calls and ("mean_pressure", 39, 40) in sim.calls
+    assert ("trapped_volume", 0, 8, 32) in sim.calls
+    assert final["trapped_nodes"] == 7 and final["mass"] == (1.0, 2.0)
