@@ -9,11 +9,15 @@ diagnostics) over all fluid nodes of the workload.  Default workload: BASELINE.j
 256^3 sandstone-like mask the north_star quotes its roofline target on.  Inputs are seeded and
 synthetic (workloads/generators.py); they stand in for the paper's Bentheimer image.
 
-N > 1: the headline metric is single-GPU by the north_star ("no sharding"), so by default ranks
-run independent replicas (no data-path collective; value = all ranks' updates / max time over
-ranks, "scaling": "weak").  --shard slab instead cuts ONE box (default config 5; the z-open configs 3 and 4
-work too) into N z-slabs, one per rank, with the psi-plane and 5-population halo exchanges of SURVEY.md §8e over
-NCCL send/recv ("scaling": "strong").
+N > 1 (launched by torch.distributed.run, one rank per GPU): the path shards by z-slabs
+(SURVEY.md §8e), so by default ONE box -- config 5, the 512^3 throughput workload, unless --config
+says otherwise; the z-open configs 3 and 4 work too -- is cut into N slabs, one per rank, and
+stepped by lbm_slab_step with the psi-plane and 5-population halo exchanges as NCCL send/recv on a
+side stream ("scaling": "strong").  Rank 0 first times the same box
+unsharded on its own GPU (config.single_gpu_ms_per_step_same_workload), so the N = 1 and N > 1
+lines are comparable.  --shard replicas runs N independent copies of the single-GPU workload
+instead (no data-path collective, "scaling": "weak").  NCCL's INIT log goes to
+bench_nccl.<host>.<pid>.log beside the script (NCCL_DEBUG=INFO unless the environment says otherwise).
 
 --impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the
 same workload on the host cores; it is a deliberately slow program, reported as a baseline.
@@ -41,11 +45,15 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=None, choices=[1, 2, 3, 4, 5],
+                    help="default: 4 on one GPU (the headline workload), 5 for the sharded run")
     ap.add_argument("--size", type=int, default=None, help="override the box edge (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--shard", default="replicas", choices=["replicas", "slab"])
+    ap.add_argument("--no-single", action="store_true",
+                    help="sharded run: skip the unsharded reference timing on rank 0")
+    ap.add_argument("--shard", default=None, choices=["replicas", "slab"],
+                    help="default: slab when WORLD_SIZE > 1, else the plain single-GPU step")
     return ap.parse_args()
 
 
@@ -155,15 +163,39 @@ def aggregate_over_ranks(local_ms, units_per_rank, world, device):
     return ms, world * units_per_rank / (ms * 1e-3) / 1e6
 
 
-# DRAM bytes per launch of the fused pass from the committed `ncu --set full` capture
-# (profiles/r1_v10_step.md): dram__bytes_read.sum + dram__bytes_write.sum on config 4.
-NCU_TRAFFIC_CFG4_COLLIDE = 1.480e9
+def source_sha16():
+    """First 16 hex digits of the SHA-256 over the CUDA path's sources: identifies the build an
+    ncu capture under profiles/ belongs to."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("kernels.cuh", "lbm.cu", "geometry.cpp", "geometry.hpp", "torch_shim.cpp"):
+        with open(os.path.join(ROOT, "paper_2207_01534_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload_name, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload_name` from
+    the committed `ncu --set full` capture of THIS build (profiles/ncu_traffic.csv, rows keyed by
+    source_sha16), else None: a capture of another build says nothing about this one."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    sha = source_sha16()
+    with open(path) as fh:
+        for line in fh:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 4 and f[0] == sha and f[1] == workload_name and f[2] == kernel:
+                return float(f[3])
+    return None
 
 
 def run_reference(args):
     """--impl reference: the oracle as it stands, on the host cores, rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
+    if args.config is None:   # the arm the driver compares with: same workload as ours for this N
+        args.config = 5 if (int(os.environ.get("WORLD_SIZE", "1")) > 1 and args.shard != "replicas") else 4
     cfg = workload(args)
     steps = args.steps if args.steps is not None else None
     warm = args.warmup if args.warmup is not None else 1
@@ -231,9 +263,12 @@ def run_ours(args):
     peak, peak_src = measured_peaks()
     t_col = kms["collide_stream"] / K * 1e-3
     achieved = BYTES_PER_UPDATE_COLLIDE * nf / t_col / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_collide_stream", "achieved": achieved, "peak": peak,
+    kname = ("k_collide_stream_bulk<float,128,7,1,1>" if cfg["params"]["storage_bits"] == 32
+             else "k_collide_stream_bulk<double,128,2,0,1>")
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_CFG4_COLLIDE if (args.config == 4 and args.size is None) else None,
+                "traffic": ncu_traffic(cfg["name"] if args.size is None else None, kname),
+                "traffic_source": "profiles/ncu_traffic.csv, build " + source_sha16(),
                 "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": BYTES_PER_UPDATE_COLLIDE * nf,
                 "kernel_ms_per_launch": {k: v / K for k, v in kms.items()},
@@ -309,15 +344,33 @@ def run_slab(args):
     K = args.steps if args.steps is not None else 200
     W = args.warmup if args.warmup is not None else 20
     cfg = workload(args)
-    sim = SlabLbm(cfg["mask"], cfg["params"], rank=rank, world=world)
-    sim.set_density(cfg["rhoA"], cfg["rhoB"])
-    one = sim.sims[0]
     total_nf = int((cfg["mask"] == 0).sum())
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    # the same box, unsharded, on rank 0's GPU: what the sharded number is to be compared with
+    single_ms = None
+    if rank == 0 and not args.no_single:
+        from paper_2207_01534_b200 import Lbm
+        ref = Lbm(cfg["mask"], cfg["params"])
+        ref.set_density(cfg["rhoA"], cfg["rhoB"])
+        ref.step(5)
+        torch.cuda.synchronize()
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record()
+        ref.step(min(K, 50))
+        r1.record()
+        torch.cuda.synchronize()
+        single_ms = r0.elapsed_time(r1) / min(K, 50)
+        ref.close()
+        torch.cuda.empty_cache()
+    barrier()
+    sim = SlabLbm(cfg["mask"], cfg["params"], rank=rank, world=world)
+    sim.set_density(cfg["rhoA"], cfg["rhoB"])
+    one = sim.sims[0]
 
     sim.step(W)
     barrier()
@@ -345,7 +398,8 @@ def run_slab(args):
     peak, peak_src = measured_peaks()
     t_col = kms["collide_stream"] / K * 1e-3
     achieved = BYTES_PER_UPDATE_COLLIDE * one.num_owned / t_col / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_collide_stream", "achieved": achieved, "peak": peak,
+    roofline = {"bound": "hbm", "kernel": "k_collide_stream_bulk<float,128,7,1,1>",
+                "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": BYTES_PER_UPDATE_COLLIDE * one.num_owned,
                 "kernel_ms_per_launch": {("halo_pack_unpack" if k == "open_planes" else k): v / K
@@ -378,6 +432,9 @@ def run_slab(args):
                 "config": {"workload": cfg["name"], "box": list(cfg["mask"].shape[::-1]),
                            "fluid_nodes": total_nf, "porosity": cfg["porosity"],
                            "parallelism": f"z-slabs x{world}", "slab_z_ranges": sim.ranges,
+                           "slab_step": ("lbm_slab_step (NCCL send/recv inside the library)"
+                                         if sim.native else "sequenced from Python (RingTransport)"),
+                           "single_gpu_ms_per_step_same_workload": single_ms,
                            "l2": "populations exceed the 126 MB L2 at the default size; no flush"},
                 "clocks": sampler.result(), "e2e": e2e, "gpu_launches": launches,
                 "roofline": roofline, "cpu_baseline": None,
@@ -392,9 +449,18 @@ if __name__ == "__main__":
     a = parse_args()
     if a.impl == "reference":
         run_reference(a)
-    elif a.shard == "slab":
-        if a.config == 4 and "--config" not in " ".join(sys.argv):
-            a.config = 5
-        run_slab(a)
     else:
-        run_ours(a)
+        world = int(os.environ.get("WORLD_SIZE", "1"))
+        shard = a.shard or ("slab" if world > 1 else "replicas")
+        if shard == "slab":
+            if a.config is None:
+                a.config = 5
+            if world > 1:
+                os.environ.setdefault("NCCL_DEBUG", "INFO")
+                os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+                os.environ.setdefault("NCCL_DEBUG_FILE", os.path.join(ROOT, "bench_nccl.%h.%p.log"))
+            run_slab(a)
+        else:
+            if a.config is None:
+                a.config = 4
+            run_ours(a)

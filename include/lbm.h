@@ -221,6 +221,25 @@ int lbm_slab_unpack(lbm_ctx* c);
  * face 0, and vice versa (both are derived from the same mask planes). */
 int lbm_slab_buffer(lbm_ctx* c, int which, void** dev, long long* bytes);
 long long lbm_num_owned(lbm_ctx* c);   /* fluid nodes of the owned planes, or -1 */
+/* The sharded step inside the library, one rank (process) per GPU, slab r of N on rank r: the
+ * exchanges are grouped ncclSend / ncclRecv to the two ring neighbours on a side stream, ordered
+ * against the launches by events, so that the psi exchange runs beside the interior density pass
+ * and the population exchange beside the interior fused pass -- no host work between the
+ * launches of a step beyond enqueuing them.  lbm_comm_unique_id (on ONE rank) makes the
+ * rendezvous token, which the caller distributes to all ranks by whatever means it has
+ * (torch.distributed broadcast in paper_2207_01534_b200/slab.py); lbm_slab_comm_init is
+ * collective over the N ranks (it creates the NCCL communicator; N = 1 is allowed: the single
+ * slab of a z-periodic box exchanges with itself); lbm_slab_step(c, n) then advances n time
+ * steps, asynchronously on torch's current stream, each in the order listed above including
+ * lbm_slab_unpack; lbm_slab_exchange(c, kind) is one exchange on its own (kind 0 psi, 1
+ * populations, 2 the cluster-flag planes of the trapped-volume query), in line on the current
+ * stream.  The result is bit-identical to the unsharded lbm_step and to the call-by-call
+ * sequence with caller-side exchanges.  LBM_ECUDA on an NCCL error. */
+#define LBM_COMM_ID_BYTES 128
+int lbm_comm_unique_id(char id[LBM_COMM_ID_BYTES]);
+int lbm_slab_comm_init(lbm_ctx* c, const char id[LBM_COMM_ID_BYTES], int rank, int world);
+int lbm_slab_step(lbm_ctx* c, int n);
+int lbm_slab_exchange(lbm_ctx* c, int kind);
 /* Trapped volume (reading R15) of a box cut into slabs.  Every slab labels the connected
  * components of the phase-comp nodes it owns (lbm_slab_ccl_begin; needs psi of the current state
  * like the other slab queries; mark_lo / mark_hi = this slab owns the global plane z = 0 /

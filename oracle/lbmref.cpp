@@ -11,9 +11,11 @@
  *      NEEM variant (kinds 1-2): pinned to the textbook identity of ref. [6], its exact
  *      consequences, the frozen rule and a moving fixed point (tests/test_oracle_neem.py);
  *      Zou-He variant (kinds 3-4, R31): pinned by its defining properties and a fixed point
- *      (tests/test_oracle_zouhe.py).  What stays a READING of a garbled passage -- parity
- *      unpinned -- is R12 iii/iv: which velocity NEEM extrapolates (the bare mixture velocity)
- *      and the mirrored psi neighbours beyond a plane; the paper prints no number for either.
+ *      (tests/test_oracle_zouhe.py).  The mirrored psi neighbours beyond a plane (R12 iv, the
+ *      one statement PAPER.md L113 prints: psi(x+e_14) = psi(x+e_13)) are pinned by the exact
+ *      cancellation of the plane-normal force they imply (tests/test_oracle_diag_open.py).  What
+ *      stays a READING of a garbled passage -- parity unpinned -- is R12 iii: which velocity NEEM
+ *      extrapolates (the bare mixture velocity); neither the paper nor the mathematics fixes it.
  * No blocking, fusion or reordering: five plain loop nests over the dense box.
  */
 #include "lbmref.h"

@@ -10,8 +10,11 @@
  * momentum conservation, lattice symmetries, G=0 shear-wave decay, discrete Poiseuille
  * closed form, flat-interface coexistence 0.027, Laplace gamma=0.071
  * (PAPER.md L181), contact-angle fit, brute-force flood fill.
- * PARITY UNPINNED: the open-boundary treatment (lbmref_step with z_open=1) -- no printed
- * number exists for it; only the consistency checks of DESIGN.md R12 are tested.
+ * Open planes (lbmref_step with z_open=1): the NEEM formula, the frozen rule, the Zou-He
+ * variant and the psi mirror across the planes are pinned by identities,
+ * fixed points and an exact force cancellation (tests/test_oracle_neem.py, _zouhe.py,
+ * _diag_open.py).  PARITY UNPINNED: one choice the garbled passage PAPER.md L147-157 leaves
+ * open -- which velocity NEEM extrapolates (reading R12 iii: the bare mixture velocity).
  *
  * Layout: dense arrays are indexed idx = x + nx*(y + ny*z); populations are
  * f[i*nvox + idx] per component with the direction order returned by lbmref_lattice.

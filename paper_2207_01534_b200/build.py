@@ -47,6 +47,14 @@ def build(force=False, verbose=False, ptxas_v=False):
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     nvcc = _nvcc()
+    # NCCL: the header and library PyTorch bundles (the process already holds that libnccl.so.2
+    # when this library is loaded), else the system's
+    site = os.path.dirname(os.path.dirname(torch.__file__))
+    nccl_inc = os.path.join(site, "nvidia", "nccl", "include")
+    nccl_lib = os.path.join(site, "nvidia", "nccl", "lib")
+    nccl_flags = ["-I", nccl_inc] if os.path.exists(os.path.join(nccl_inc, "nccl.h")) else []
+    nccl_link = ([f"-L{nccl_lib}", "-l:libnccl.so.2", "-Xlinker", f"-rpath={nccl_lib}"]
+                 if os.path.exists(os.path.join(nccl_lib, "libnccl.so.2")) else ["-lnccl"])
     common = ["-O3", "-std=c++17", "-Xcompiler", "-fPIC", f"-D_GLIBCXX_USE_CXX11_ABI={abi}"]
     objs = []
 
@@ -57,7 +65,8 @@ def build(force=False, verbose=False, ptxas_v=False):
 
     o = os.path.join(objdir, "lbm.o")
     run([nvcc, "-c", os.path.join(CSRC, "lbm.cu"), "-o", o] + common + ARCH
-        + ["-lineinfo", "--expt-relaxed-constexpr"] + (["-Xptxas", "-v"] if ptxas_v else []))
+        + nccl_flags + ["-lineinfo", "--expt-relaxed-constexpr"]
+        + (["-Xptxas", "-v"] if ptxas_v else []))
     objs.append(o)
     o = os.path.join(objdir, "geometry.o")
     run(["g++", "-c", os.path.join(CSRC, "geometry.cpp"), "-o", o, "-O2", "-std=c++17", "-fPIC",
@@ -74,7 +83,7 @@ def build(force=False, verbose=False, ptxas_v=False):
     objs.append(o)
     run([nvcc, "-shared", "-o", LIB] + objs + ARCH
         + ["-Xcompiler", "-fopenmp", f"-L{torch_lib}", "-lc10", "-lc10_cuda", "-lcudart",
-           "-Xlinker", f"-rpath={torch_lib}"])
+           "-Xlinker", f"-rpath={torch_lib}"] + nccl_link)
     return LIB
 
 

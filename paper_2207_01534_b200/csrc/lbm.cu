@@ -3,6 +3,7 @@
 #include "../../include/lbm.h"
 
 #include <cuda_runtime.h>
+#include <nccl.h>
 
 #include <algorithm>
 #include <cmath>
@@ -133,6 +134,12 @@ struct lbm_ctx {
   // last stream it used; a call on a different stream first waits (event) for the work enqueued on
   // the previous one, and lbm_destroy synchronises the device before the buffers go back to the
   // caching allocator.
+  // Native slab ring (lbm_slab_comm_init / lbm_slab_step): NCCL communicator over the slabs, one
+  // rank per GPU; the exchanges run on comm_stream beside the interior launches of the same pass.
+  ncclComm_t comm = nullptr;
+  int comm_rank = 0, comm_world = 0;
+  cudaStream_t comm_stream = nullptr;
+  cudaEvent_t comm_ev[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaStream_t last_stream = nullptr;
   bool has_stream = false;
   cudaEvent_t order_ev = nullptr;
@@ -149,6 +156,9 @@ struct lbm_ctx {
     drop_graphs();
     if (cap_stream) cudaStreamDestroy(cap_stream);
     if (order_ev) cudaEventDestroy(order_ev);
+    if (comm) ncclCommDestroy(comm);
+    if (comm_stream) cudaStreamDestroy(comm_stream);
+    for (auto& e : comm_ev) if (e) cudaEventDestroy(e);
     for (auto& e : prof_events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     lbm_shim_free(f[0]); lbm_shim_free(f[1]); lbm_shim_free(psi); lbm_shim_free(nbr);
     lbm_shim_free(wall_nbr); lbm_shim_free(wall_inv_den); lbm_shim_free(node_vox_d);
@@ -976,14 +986,13 @@ int lbm_slab_ccl_finish(lbm_ctx* c, int z0, int z1, long long* nodes, double* ma
   return LBM_OK;
 }
 
-int lbm_slab_buffer(lbm_ctx* c, int which, void** dev, long long* bytes) {
-  if (!c || !dev || !bytes) return fail(LBM_EINVAL, "NULL argument");
-  if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
-  if (which < 0 || which > 11) return fail(LBM_EINVAL, "which must be 0..11");
+extern "C++" {
+// exchange buffer `which` of a slab context (include/lbm.h lbm_slab_buffer)
+static void slab_buffer_of(lbm_ctx* c, int which, void** dev, long long* bytes) {
   if (which >= 8) {  // cluster-flag planes of the trapped-volume query: send low/high, receive low/high
     *dev = c->ccl + (size_t)2 * c->nact + (size_t)(which - 8) * c->np;
     *bytes = (long long)c->np * (long long)sizeof(int);
-    return LBM_OK;
+    return;
   }
   const size_t pair = 2 * c->esz;
   const int face = which & 1;
@@ -1005,6 +1014,117 @@ int lbm_slab_buffer(lbm_ctx* c, int which, void** dev, long long* bytes) {
       *bytes = c->n_unpack[face] * (long long)pair;
       break;
   }
+}
+
+#define NC(call)                                                                          \
+  do {                                                                                    \
+    ncclResult_t r_ = (call);                                                             \
+    if (r_ != ncclSuccess)                                                                \
+      return fail(LBM_ECUDA, "%s failed: %s (%s:%d)", #call, ncclGetErrorString(r_),      \
+                  __FILE__, __LINE__);                                                    \
+  } while (0)
+
+// One neighbour exchange on the slab ring, enqueued on `cs`: kind 0 = psi planes (buffers 0,1 ->
+// the neighbours' 2,3), kind 1 = populations that crossed a cut (4,5 -> 6,7).  My high-face
+// message goes to rank+1 and lands in its low halo, my low-face message to rank-1 and lands in
+// its high halo.  Posting order (send up, send down, receive from below, receive from above)
+// keeps the two messages between the same pair of ranks matched at world sizes 1 and 2.  Empty
+// messages (the ends of a z-open box) are skipped on both sides: the sizes derive from the same
+// mask planes.
+static int slab_exchange(lbm_ctx* c, int kind, cudaStream_t cs) {
+  void* b[4];
+  long long n[4];
+  for (int k = 0; k < 4; ++k) slab_buffer_of(c, 4 * kind + k, &b[k], &n[k]);
+  const int up = (c->comm_rank + 1) % c->comm_world;
+  const int down = (c->comm_rank + c->comm_world - 1) % c->comm_world;
+  if (n[0] + n[1] + n[2] + n[3] == 0) return LBM_OK;
+  NC(ncclGroupStart());
+  if (n[1]) NC(ncclSend(b[1], (size_t)n[1], ncclChar, up, c->comm, cs));
+  if (n[0]) NC(ncclSend(b[0], (size_t)n[0], ncclChar, down, c->comm, cs));
+  if (n[2]) NC(ncclRecv(b[2], (size_t)n[2], ncclChar, down, c->comm, cs));
+  if (n[3]) NC(ncclRecv(b[3], (size_t)n[3], ncclChar, up, c->comm, cs));
+  NC(ncclGroupEnd());
+  return LBM_OK;
+}
+
+// One sharded time step with both exchanges beside the interior launches (the order of
+// include/lbm.h "z-slab sharding"): st = compute stream, c->comm_stream = exchanges.
+template <typename T>
+static int slab_step_once(lbm_ctx* c, cudaStream_t st) {
+  cudaStream_t cs = c->comm_stream;
+  launch_density<T>(c, st, 0);
+  CU(cudaEventRecord(c->comm_ev[0], st));
+  CU(cudaStreamWaitEvent(cs, c->comm_ev[0], 0));
+  if (int rc = slab_exchange(c, 0, cs)) return rc;
+  CU(cudaEventRecord(c->comm_ev[1], cs));
+  launch_density<T>(c, st, 1);
+  CU(cudaStreamWaitEvent(st, c->comm_ev[1], 0));
+  c->slab_phase = 2;
+  if (int rc = slab_collide_T<T>(c, 0, st)) return rc;
+  CU(cudaEventRecord(c->comm_ev[2], st));
+  CU(cudaStreamWaitEvent(cs, c->comm_ev[2], 0));
+  if (int rc = slab_exchange(c, 1, cs)) return rc;
+  CU(cudaEventRecord(c->comm_ev[3], cs));
+  if (int rc = slab_collide_T<T>(c, 1, st)) return rc;
+  CU(cudaStreamWaitEvent(st, c->comm_ev[3], 0));
+  c->slab_phase = 4;
+  return LBM_OK;
+}
+}  // extern "C++"
+
+int lbm_comm_unique_id(char id[LBM_COMM_ID_BYTES]) {
+  if (!id) return fail(LBM_EINVAL, "NULL argument");
+  static_assert(sizeof(ncclUniqueId) == LBM_COMM_ID_BYTES, "ncclUniqueId size");
+  ncclUniqueId u;
+  NC(ncclGetUniqueId(&u));
+  std::memcpy(id, &u, sizeof u);
+  return LBM_OK;
+}
+
+int lbm_slab_comm_init(lbm_ctx* c, const char id[LBM_COMM_ID_BYTES], int rank, int world) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
+  if (!id || world < 1 || rank < 0 || rank >= world) return fail(LBM_EINVAL, "bad argument");
+  if (c->comm) return fail(LBM_EINVAL, "the context already has a communicator");
+  ncclUniqueId u;
+  std::memcpy(&u, id, sizeof u);
+  NC(ncclCommInitRank(&c->comm, world, u, rank));
+  c->comm_rank = rank;
+  c->comm_world = world;
+  CU(cudaStreamCreateWithFlags(&c->comm_stream, cudaStreamNonBlocking));
+  for (auto& e : c->comm_ev) CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  return LBM_OK;
+}
+
+int lbm_slab_step(lbm_ctx* c, int n) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
+  if (!c->comm) return fail(LBM_EINVAL, "lbm_slab_step needs lbm_slab_comm_init");
+  if (n < 0) return fail(LBM_EINVAL, "n must be >= 0");
+  if (c->slab_phase > 2)
+    return fail(LBM_EINVAL, "slab calls out of order (expected phase %d)", c->slab_phase);
+  cudaStream_t st = use_stream(c);
+  for (int it = 0; it < n; ++it) {
+    if (int rc = c->bits == 64 ? slab_step_once<double>(c, st) : slab_step_once<float>(c, st))
+      return rc;
+    if (int rc = lbm_slab_unpack(c)) return rc;
+  }
+  return LBM_OK;
+}
+
+int lbm_slab_exchange(lbm_ctx* c, int kind) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
+  if (!c->comm) return fail(LBM_EINVAL, "lbm_slab_exchange needs lbm_slab_comm_init");
+  if (kind < 0 || kind > 2) return fail(LBM_EINVAL, "kind must be 0 (psi), 1 (populations) or 2 (cluster flags)");
+  return slab_exchange(c, kind, use_stream(c));   // in line on the caller's stream
+}
+
+int lbm_slab_buffer(lbm_ctx* c, int which, void** dev, long long* bytes) {
+  if (!c || !dev || !bytes) return fail(LBM_EINVAL, "NULL argument");
+  if (!c->slab) return fail(LBM_EINVAL, "not a slab context");
+  if (which < 0 || which > 11) return fail(LBM_EINVAL, "which must be 0..11");
+  slab_buffer_of(c, which, dev, bytes);
   return LBM_OK;
 }
 

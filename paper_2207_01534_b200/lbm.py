@@ -26,6 +26,7 @@ SYMBOLS = [
     "lbm_options_default", "lbm_create_opt", "lbm_create_slab_opt", "lbm_step_info",
     "lbm_create_slab", "lbm_slab_density", "lbm_slab_collide", "lbm_slab_unpack", "lbm_slab_buffer",
     "lbm_num_owned", "lbm_build_slab_halo",
+    "lbm_comm_unique_id", "lbm_slab_comm_init", "lbm_slab_step", "lbm_slab_exchange",
     "lbm_slab_ccl_begin", "lbm_slab_ccl_export", "lbm_slab_ccl_import", "lbm_slab_ccl_finish",
 ]
 
@@ -110,6 +111,12 @@ def load():
     lib.lbm_num_owned.argtypes = [P]
     lib.lbm_num_owned.restype = LL
     lib.lbm_build_slab_halo.argtypes = [V, I, I, I, I, I, I, V, V, LL] + [C.POINTER(LL)] * 5
+    lib.lbm_comm_unique_id.argtypes = [C.c_char_p]
+    lib.lbm_slab_comm_init.argtypes = [P, C.c_char_p, I, I]
+    lib.lbm_slab_step.argtypes = [P, I]
+    lib.lbm_slab_exchange.argtypes = [P, I]
+    for fn in ("lbm_comm_unique_id", "lbm_slab_comm_init", "lbm_slab_step", "lbm_slab_exchange"):
+        getattr(lib, fn).restype = I
     lib.lbm_slab_ccl_begin.argtypes = [P, I, I, I]
     lib.lbm_slab_ccl_export.argtypes = [P]
     lib.lbm_slab_ccl_import.argtypes = [P, I, I, C.POINTER(I)]
@@ -180,6 +187,16 @@ def lbm_build_index(mask, z_open=0, with_nbr=True):
                              nbr.ctypes.data if with_nbr else None, 18 * max(nfluid, 1),
                              C.byref(nf), C.byref(nw)), "lbm_build_index")
     return vox2id, (nbr[:, :nf.value] if with_nbr else None), nf.value, nw.value
+
+
+LBM_COMM_ID_BYTES = 128
+
+
+def lbm_comm_unique_id():
+    """Rendezvous token of a slab ring (made on one rank, to be handed to every rank)."""
+    buf = C.create_string_buffer(LBM_COMM_ID_BYTES)
+    _chk(load().lbm_comm_unique_id(buf), "lbm_comm_unique_id")
+    return buf.raw
 
 
 def lbm_build_slab_halo(mask_local, z_open=0, halo=(1, 1)):
@@ -294,6 +311,18 @@ class Lbm:
 
     def slab_unpack(self):
         _chk(load().lbm_slab_unpack(self._h), "lbm_slab_unpack")
+
+    def slab_comm_init(self, comm_id, rank, world):
+        if len(comm_id) != LBM_COMM_ID_BYTES:
+            raise ValueError("comm_id must be the 128 bytes lbm_comm_unique_id returned")
+        _chk(load().lbm_slab_comm_init(self._h, bytes(comm_id), int(rank), int(world)),
+             "lbm_slab_comm_init")
+
+    def slab_step(self, n=1):
+        _chk(load().lbm_slab_step(self._h, int(n)), "lbm_slab_step")
+
+    def slab_exchange(self, kind):
+        _chk(load().lbm_slab_exchange(self._h, int(kind)), "lbm_slab_exchange")
 
     def slab_ccl_begin(self, comp, mark_lo, mark_hi):
         _chk(load().lbm_slab_ccl_begin(self._h, int(comp), int(bool(mark_lo)), int(bool(mark_hi))),

@@ -191,7 +191,8 @@ class SlabLbm:
     Global arrays are [z, y, x]; `get_macroscopic` returns the owned planes of this process
     (all planes when world is None)."""
 
-    def __init__(self, mask, params, parts=None, rank=None, world=None, group=None, options=None):
+    def __init__(self, mask, params, parts=None, rank=None, world=None, group=None, options=None,
+                 native=None):
         mask = np.ascontiguousarray(mask, np.uint8)
         self.shape = mask.shape
         self.world = world
@@ -207,6 +208,35 @@ class SlabLbm:
         self.num_fluid = sum(s.num_owned for s in self.sims)
         self._ring = RingTransport(rank, world, group) if world is not None else None
         self._buf = [[buffer_tensor(s, w) for w in range(12)] for s in self.sims]
+        # native = the step and its exchanges run inside the library (lbm_slab_step: NCCL send /
+        # recv on a side stream); default whenever every rank has its own GPU, i.e. with the NCCL
+        # backend (or a single rank).  Otherwise the step is sequenced here, call by call, with the
+        # exchanges through RingTransport (gloo: the CPU tests and several ranks on one GPU).
+        if native is None:
+            native = world is not None and (world == 1 or self._backend(group) == "nccl")
+        self.native = bool(native) and world is not None
+        if self.native:
+            self.sims[0].slab_comm_init(self._comm_id(rank, world, group), rank, world)
+
+    @staticmethod
+    def _backend(group):
+        import torch.distributed as dist
+        return dist.get_backend(group) if dist.is_initialized() else None
+
+    @staticmethod
+    def _comm_id(rank, world, group):
+        """The ring's rendezvous token: made on rank 0, broadcast through torch.distributed."""
+        from .lbm import lbm_comm_unique_id
+        if world == 1:
+            return lbm_comm_unique_id()
+        import torch
+        import torch.distributed as dist
+        dev = "cuda" if dist.get_backend(group) == "nccl" else "cpu"
+        t = torch.zeros(128, dtype=torch.uint8, device=dev)
+        if rank == 0:
+            t.copy_(torch.frombuffer(bytearray(lbm_comm_unique_id()), dtype=torch.uint8))
+        dist.broadcast(t, src=0, group=group)
+        return bytes(t.cpu().numpy().tobytes())
 
     def close(self):
         self._buf = []
@@ -239,6 +269,9 @@ class SlabLbm:
         RingTransport.finish(works)
 
     def step(self, n=1):
+        if self.native:
+            self.sims[0].slab_step(int(n))
+            return
         for _ in range(int(n)):
             self._density_and_psi_halo()
             for s in self.sims:

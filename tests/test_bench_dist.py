@@ -1,6 +1,7 @@
-"""N > 1 path of bench.py on CPU: two gloo ranks run the replica aggregation (max-over-ranks time,
-whole-job throughput).  The path does not shard, so this
-host logic is all there is to the multi-process run besides NCCL's barrier."""
+"""N > 1 host logic of bench.py on CPU: two gloo ranks run the aggregation both multi-rank modes use
+(max-over-ranks time, whole-job throughput).  The sharded step itself (bench.py's default for
+N > 1: z-slabs) is covered by tests/test_slab_host.py (halo lists, ring
+choreography on two gloo ranks) and tests/test_gpu_slab.py; here also the mode selection."""
 import os
 import sys
 
@@ -38,3 +39,18 @@ def test_replica_aggregation_world_size_2():
     for rank, ms, mlups in res:
         assert ms == 12.5                              # max over ranks, on every rank
         assert abs(mlups - 2 * 20.0 / 12.5e-3) < 1e-6  # both replicas' updates / slowest time
+
+
+def test_mode_selection(monkeypatch):
+    """One GPU: the headline workload (config 4), plain step.  torchrun with N > 1: the sharded
+    path on config 5, unless --shard replicas / --config say otherwise."""
+    sys.path.insert(0, ROOT)
+    import bench
+    monkeypatch.setattr(sys, "argv", ["bench.py"])
+    a = bench.parse_args()
+    assert a.shard is None and a.config is None and a.gpus == 1
+    monkeypatch.setattr(sys, "argv", ["bench.py", "--gpus", "8", "--shard", "replicas", "--config", "4"])
+    a = bench.parse_args()
+    assert (a.shard, a.config, a.gpus) == ("replicas", 4, 8)
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert 'shard = a.shard or ("slab" if world > 1 else "replicas")' in src

@@ -120,10 +120,15 @@ def test_laplace_paper_size_128_cubed():
         assert abs(dP * R / 2.0 / g1 - 1.0) < 0.03, (tau, dP * R / 2.0, g1)
 
 
+PAPER_FIT = (47.4136, -23.4513, 89.7938, 91.2324)           # cubic, linear ... constant
+
+
 def test_contact_angle_calibration_paper_size():
     """PAPER.md Sec. 3.2 at the paper's own size and viscosity ratio: 200 x 100 x 200 (wall-normal
-    extent 100), droplet r0 = 30 on the bottom wall, M = 25 (tau = 3.5 / 0.62), G = 3.5.  theta
-    (through component 2) against the printed cubic (L199) over xi in [-0.4, 0.4]."""
+    extent 100), droplet r0 = 30 on the bottom wall, M = 25 (tau = 3.5 / 0.62), G = 3.5, over the
+    paper's whole range xi in [-0.5, 0.5] (Fig. 2).  theta (through component 2) against the
+    printed cubic (L199) point by point, and the cubic re-fitted from these runs against the
+    printed coefficients ("regenerating ... cubic coefficients")."""
     nz, ny, nx = 100, 200, 200
     shape = (nz, ny, nx)
     mask = np.zeros(shape, np.uint8)
@@ -132,13 +137,23 @@ def test_contact_angle_calibration_paper_size():
     rA = np.where(mask == 0, rA, 0.0)
     rB = np.where(mask == 0, 1.027 - rA, 0.0)
     got = {}
-    for xi in (-0.4, -0.2, 0.0, 0.2, 0.4):
+    for xi in (-0.5, -0.4, -0.3, -0.2, -0.1, 0.0, 0.1, 0.2, 0.3, 0.4, 0.5):
         g = Lbm(mask, default_params(G=3.5, tau=(3.5, 0.62), xi=xi, storage_bits=32))
         g.set_density(rA, rB)
-        g.step(15000)
+        g.step(15000 if abs(xi) < 0.45 else 30000)          # the far ends spread / retract furthest
         m = g.get_macroscopic(fields=("rhoA", "rhoB"))
         g.close()
         assert np.isfinite(m["rhoA"]).all()
         got[xi] = _cap_angle_through_B(m["rhoA"], m["rhoB"])
+    print("contact angles (xi: theta, paper fit):",
+          {xi: (round(th, 2), round(_paper_fit(xi), 2)) for xi, th in got.items()})
     for xi, th in got.items():
-        assert abs(th - _paper_fit(xi)) < 3.0, got
+        assert abs(th - _paper_fit(xi)) < (3.0 if abs(xi) < 0.45 else 4.0), got
+    xs = np.array(sorted(got))
+    coef = np.polyfit(xs, np.array([got[x] for x in xs]), 3)
+    print("re-fitted cubic:", coef, "paper:", PAPER_FIT)
+    assert abs(coef[3] - PAPER_FIT[3]) < 1.5, coef           # theta(0): neutral wetting, ~91 degrees
+    assert abs(coef[2] / PAPER_FIT[2] - 1.0) < 0.05, coef    # slope at xi = 0 within 5 %
+    assert abs(coef[1] - PAPER_FIT[1]) < 12.0 and abs(coef[0] - PAPER_FIT[0]) < 25.0, coef
+    grid = np.linspace(-0.5, 0.5, 41)                        # the two curves agree over the range
+    assert np.max(np.abs(np.polyval(coef, grid) - np.polyval(PAPER_FIT, grid))) < 3.0, coef

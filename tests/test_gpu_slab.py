@@ -436,3 +436,42 @@ def test_slab_trapped_volume_serpentine_crosses_every_cut_many_times():
         assert got[0] == want[0] and abs(got[1] - want[1]) < 1e-9
         s.close()
     g.close()
+
+
+@pytest.mark.parametrize("k,bits", [(5, 64), (5, 32), (4, 32), (3, 64)])
+def test_native_slab_step_ring_of_one(k, bits):
+    """lbm_slab_step: the sharded step sequenced inside the library, exchanges as grouped
+    ncclSend / ncclRecv on a side stream.  One GPU can host one NCCL rank, so the ring has one
+    slab: in a z-periodic box (config 5) it exchanges both faces with itself -- every pack /
+    send / receive / unpack path runs, with the message matching of a 1- or 2-rank ring --, in a
+    z-open box (configs 3, 4) it owns both open planes and has nothing to exchange.  Bit-identical
+    to the unsharded step and to the call-by-call sequence driven from Python, across getters in
+    between."""
+    c = make_config(k, size=40, storage_bits=bits)
+    ref = Lbm(c["mask"], c["params"])
+    ref.set_density(c["rhoA"], c["rhoB"])
+    ref.step(25)
+    want = [ref.get_populations(s) for s in (0, 1)]
+    want_sat = ref.saturation(1)
+    ref.close()
+    for native in (True, False):
+        s = SlabLbm(c["mask"], c["params"], rank=0, world=1, native=native)
+        assert s.native == native
+        s.set_density(c["rhoA"], c["rhoB"])
+        s.step(10)
+        s.saturation(0)                       # a query between steps (density + psi halo, phase 2)
+        s.step(15)
+        for comp in (0, 1):
+            assert np.array_equal(s.get_populations(comp), want[comp]), (native, comp)
+        assert s.saturation(1) == want_sat
+        s.close()
+
+
+def test_native_slab_step_needs_a_communicator():
+    from paper_2207_01534_b200 import LbmError
+    c = make_config(5, size=24)
+    s = SlabLbm(c["mask"], c["params"], parts=1)           # in-process slabs: no communicator
+    with pytest.raises(LbmError) as e:
+        s.sims[0].slab_step(1)
+    assert e.value.code == -1
+    s.close()
