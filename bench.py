@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--size", type=int, default=None, help="override the box edge (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="lbm_options field, e.g. --opt index=bits --opt graph=0 (repeatable)")
     ap.add_argument("--no-single", action="store_true",
                     help="sharded run: skip the unsharded reference timing on rank 0")
     ap.add_argument("--shard", default=None, choices=["replicas", "slab"],
@@ -229,7 +231,9 @@ def run_ours(args):
     K = args.steps if args.steps is not None else 500
     W = args.warmup if args.warmup is not None else 20
     cfg = workload(args)
-    sim = Lbm(cfg["mask"], cfg["params"])
+    opts = {k: (v if not v.lstrip("-").isdigit() else int(v))
+            for k, v in (kv.split("=", 1) for kv in args.opt)}
+    sim = Lbm(cfg["mask"], cfg["params"], options=opts or None)
     sim.set_density(cfg["rhoA"], cfg["rhoB"])
     nf = sim.num_fluid
     mem = sim.memory_bytes()

@@ -407,3 +407,73 @@ def test_graph_replay_is_bit_identical_to_host_launches(k, bits):
         g.close()
     for a, b in zip(res[0], res[1]):
         assert np.array_equal(a, b)
+
+
+# ------------------------------------------------------------------ the pins of R12 iv and R14, through the C ABI
+
+def test_open_plane_psi_mirror_on_gpu():
+    """The oracle pin of reading R12 iv (tests/test_oracle_diag_open.py) through
+    lbm_get_macroscopic: with f = w_i rho on a solid-free open box the plane-normal force cancels
+    term by term on both open planes, so u_z = 0 there for any density field; fp64 and fp32."""
+    rng = np.random.Generator(np.random.PCG64(113))
+    shape = (9, 6, 7)
+    rA = rng.uniform(0.05, 1.0, shape)
+    rB = rng.uniform(0.05, 1.0, shape)
+    for bits, zero in ((64, 1e-15), (32, 2e-7)):
+        p = default_params(G=3.5, tau=(1.0, 1.0), z_open=1, inlet_kind=1, inlet_comp=0,
+                           inlet_rho=1.0, outlet_kind=1, outlet_comp=0, outlet_rho=1.0,
+                           storage_bits=bits)
+        g = Lbm(np.zeros(shape, np.uint8), p)
+        g.set_density(rA, rB)
+        m = g.get_macroscopic()
+        o = LbmRef(np.zeros(shape, np.uint8), p)
+        o.set_density(rA, rB)
+        mo = o.get_macroscopic()
+        for z in (0, shape[0] - 1):
+            assert np.max(np.abs(m["uz"][z])) < zero
+            assert np.max(np.abs(m["ux"][z])) > 1e-3
+        assert np.max(np.abs(m["uz"][1])) > 1e-3
+        for k in ("ux", "uy", "uz"):
+            assert np.max(np.abs(m[k] - mo[k])) < (1e-13 if bits == 64 else 1e-6)
+        g.close()
+
+
+def test_saturation_tie_goes_to_component_one_on_gpu():
+    """Reading R14 through lbm_saturation and lbm_trapped_volume: identical populations of the two
+    components on a node (an exact tie) count for component index 1, never for index 0."""
+    rng = np.random.Generator(np.random.PCG64(14))
+    shape = (6, 5, 4)
+    mask = np.zeros(shape, np.uint8)
+    mask[2, 1, 1] = 1
+    f = rng.uniform(0.01, 0.1, (19,) + shape)
+    clear_a = rng.uniform(size=shape) < 0.3
+    clear_b = ~clear_a & (rng.uniform(size=shape) < 0.4)
+    gpop = f.copy()
+    gpop[:, clear_a] *= 0.5
+    gpop[:, clear_b] *= 2.0
+    fluid = mask == 0
+    tie = fluid & ~clear_a & ~clear_b
+    tot = fluid.sum()
+    for bits in (64, 32):
+        g = Lbm(mask, default_params(storage_bits=bits))
+        o = LbmRef(mask, default_params(storage_bits=bits))
+        for s in (g, o):
+            s.set_populations(0, f)
+            s.set_populations(1, gpop)
+        assert g.saturation(0) == (fluid & clear_a).sum() / tot == o.saturation(0)
+        assert g.saturation(1) == ((fluid & clear_b).sum() + tie.sum()) / tot == o.saturation(1)
+        g.set_populations(1, f)
+        assert g.saturation(0) == 0.0 and g.saturation(1) == 1.0
+        assert g.trapped_volume(0)[0] == 0 and g.trapped_volume(1)[0] == 0
+        g.close()
+
+
+def test_get_macroscopic_validates_output_arrays():
+    c = make_config(1, size=8)
+    g = Lbm(c["mask"], c["params"])
+    g.set_density(c["rhoA"], c["rhoB"])
+    for bad in (np.empty(c["mask"].shape, np.float32), np.empty((8, 8, 9)),
+                np.empty((8, 8, 16))[:, :, ::2]):
+        with pytest.raises(ValueError):
+            g.get_macroscopic(fields=("rhoA",), out={"rhoA": bad})
+    g.close()
