@@ -81,8 +81,6 @@ typedef struct {
                        across the two passes)                                                       */
   int keep_psi_mb;  /* L2 budget in MB for psi stored with evict_last priority
                        (default 48; 0: plain stores)                                                */
-  int chunks;       /* EXPERIMENT: > 1 = run the three passes in this many id chunks, the density pass
-                       two z-planes ahead of the fused pass (L2 reuse of the populations)         */
 } lbm_options;
 void lbm_options_default(lbm_options* o);
 

@@ -144,10 +144,9 @@ template <typename T>
 __global__ void __launch_bounds__(256) k_wallpsi(Vec2<T>* __restrict__ psi,
                                                  const int* __restrict__ wall_nbr,
                                                  const T* __restrict__ inv_den,
-                                                 size_t wall_base, int w0, int nw, size_t nwpad,
-                                                 T chiA, T chiB, float keep_psi) {
-  // wall solids [w0, nw) (whole pass: w0 = 0)
-  const int w = w0 + blockIdx.x * blockDim.x + threadIdx.x;
+                                                 size_t wall_base, int nw, size_t nwpad, T chiA,
+                                                 T chiB, float keep_psi) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
   const bool live = w < nw;
   int id[Q];
 #pragma unroll

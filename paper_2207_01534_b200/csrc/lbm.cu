@@ -115,9 +115,6 @@ struct lbm_ctx {
   int* nbr16_meta = nullptr;         // [tiles][kIdxMeta]
   long long wide_tiles = 0;
   int reverse = 1;          // the fused pass walks the tiles backwards (L2 reuse across the passes)
-  int chunks = 0;           // > 1: chunked step (experiment): the id range in this many chunks
-  int chunk_t0 = 0, chunk_t1 = 0;    // tile range of the chunk being launched
-  std::vector<int32_t> wzstart;      // [nz+1] first wall-solid id of every z-plane
   float keep_psi = 0.f;     // share of the psi lines stored with L2 evict_last priority, from
   int keep_psi_mb = 48;     // this budget: min(1, MB / psi bytes) (0: off)
   int pdl = 1;              // programmatic dependent launch of the three passes
@@ -303,39 +300,7 @@ void launch_wall(lbm_ctx* c, cudaStream_t st) {
   const bool pdl = c->pdl && !c->prof;
   Timed t(c, st, 1);
   launch_k(pdl, k_wallpsi<T>, blocks(c->nw, 256), 256, 0, st, (Vec2<T>*)c->psi,
-           (const int*)c->wall_nbr, (const T*)c->wall_inv_den, c->npad, 0, c->nw, c->nwpad,
-           (T)(1.0 + c->p.xi), (T)(1.0 - c->p.xi), c->keep_psi);
-}
-
-// ---- chunked step (experiment): the three passes in id chunks, density a little ahead ----------
-// a1 on ids [a, b) (a multiple of 256); `fix` = this launch also carries the deferred open-plane fix
-template <typename T>
-void launch_density_range(lbm_ctx* c, cudaStream_t st, int a, int b, bool fix) {
-  if (b <= a && !fix) return;
-  T* fin = (T*)c->f[c->cur];
-  const bool pdl = c->pdl && !c->prof;
-  Timed t(c, st, 0);
-  const unsigned grid = b > a ? blocks(b - a, 256) : 0;
-  NodeRange r{a, (int)grid, 0, b};
-  if (fix && c->open_pending) {
-    const unsigned nbp = blocks(2LL * c->np, 256);
-    launch_k(pdl, k_density_open<T>, nbp + grid, 256, 0, st, fin, (Vec2<T>*)c->psi,
-             (const T*)c->frozen, c->nact, c->np, c->npad, (int)nbp,
-             make_open<T>(c->p, c->open_end), c->keep_psi, r);
-    c->open_pending = false;
-  } else if (grid > 0) {
-    launch_k(pdl, k_density<T>, grid, 256, 0, st, (const T*)fin, (Vec2<T>*)c->psi, r, c->npad,
-             c->keep_psi);
-  }
-}
-// a2 on wall solids [w0, w1)
-template <typename T>
-void launch_wall_range(lbm_ctx* c, cudaStream_t st, int w0, int w1) {
-  if (w1 <= w0) return;
-  const bool pdl = c->pdl && !c->prof;
-  Timed t(c, st, 1);
-  launch_k(pdl, k_wallpsi<T>, blocks(w1 - w0, 256), 256, 0, st, (Vec2<T>*)c->psi,
-           (const int*)c->wall_nbr, (const T*)c->wall_inv_den, c->npad, w0, w1, c->nwpad,
+           (const int*)c->wall_nbr, (const T*)c->wall_inv_den, c->npad, c->nw, c->nwpad,
            (T)(1.0 + c->p.xi), (T)(1.0 - c->p.xi), c->keep_psi);
 }
 
@@ -346,7 +311,6 @@ void launch_psi(lbm_ctx* c, cudaStream_t st) {
   if (!c->slab) launch_density<T>(c, st);
   launch_wall<T>(c, st);
 }
-
 
 // Apply a deferred open-plane fix now (getters that read the populations directly).
 template <typename T>
@@ -396,10 +360,6 @@ void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
     ix.tile0 = lo1;
     grid = (unsigned)(hi0 - lo1);
     ix.split = (int)grid;
-  } else if (part == 2) {                        // chunked step: tiles [chunk_t0, chunk_t1)
-    ix.tile0 = c->chunk_t0;
-    grid = (unsigned)(c->chunk_t1 - c->chunk_t0);
-    ix.split = (int)grid;
   }
   if (grid == 0) return;
   // Overlap only behind the wall pass: its blocks trigger after their own wait, i.e. once the
@@ -429,43 +389,8 @@ int step_T(lbm_ctx* c, int n, cudaStream_t st) {
   for (int it = 0; it < n; ++it) {
     const T* fin = (const T*)c->f[c->cur];
     T* fout = (T*)c->f[c->cur ^ 1];
-    if (c->chunks > 1 && !c->slab) {
-      // chunk k = tiles [t0, t1); its fused pass needs psi of the planes zlo-1 .. zhi+1 of its
-      // nodes: fluid density through plane zhi+1, virtual solid density of the wall solids through
-      // plane zhi+1, which in turn needs fluid density through plane zhi+2
-      const int nz = c->nz, nf = c->nf, nw = c->nw;
-      const int ntiles = (int)blocks(nf, 128);
-      int d_done = 0, w_done = 0, d_end = nf, w_end = nw;
-      bool first = true;
-      if (!c->p.z_open) {      // periodic wrap: the first chunk reads the last plane's psi
-        const int a = c->zstart[std::max(0, nz - 2)] / 256 * 256;
-        launch_density_range<T>(c, st, a, nf, true);
-        first = false;
-        d_end = a;
-      }
-      for (int kc = 0; kc < c->chunks; ++kc) {
-        const int t0 = (int)((long long)ntiles * kc / c->chunks);
-        const int t1 = (int)((long long)ntiles * (kc + 1) / c->chunks);
-        if (t1 <= t0) continue;
-        const int nlast = std::min(nf, t1 * 128) - 1;
-        int zhi = (int)(std::upper_bound(c->zstart.begin(), c->zstart.end(), nlast) - c->zstart.begin()) - 1;
-        const int need_d = std::min(d_end, (int)pad256(c->zstart[std::min(nz, zhi + 3)]));
-        launch_density_range<T>(c, st, d_done, std::max(d_done, need_d), first);
-        first = false;
-        d_done = std::max(d_done, need_d);
-        if (kc == 0 && !c->p.z_open) {   // walls of the last plane (they read planes nz-2, nz-1, 0)
-          launch_wall_range<T>(c, st, c->wzstart[nz - 1], nw);
-          w_end = c->wzstart[nz - 1];
-        }
-        const int need_w = std::min(w_end, c->wzstart[std::min(nz, zhi + 2)]);
-        launch_wall_range<T>(c, st, w_done, std::max(w_done, need_w));
-        w_done = std::max(w_done, need_w);
-        c->chunk_t0 = t0; c->chunk_t1 = t1;
-        Timed t(c, st, 2);
-        launch_collide<T>(c, fin, fout, k, st, 2);
-      }
-    } else {
-      launch_psi<T>(c, st);
+    launch_psi<T>(c, st);
+    {
       Timed t(c, st, 2);
       launch_collide<T>(c, fin, fout, k, st);
     }
@@ -594,7 +519,6 @@ void lbm_options_default(lbm_options* o) {
   o->pdl = 1;
   o->reverse = 1;
   o->keep_psi_mb = 48;
-  o->chunks = 0;
 }
 
 static int validate_options(const lbm_options* o) {
@@ -604,7 +528,6 @@ static int validate_options(const lbm_options* o) {
   if ((o->pdl != 0 && o->pdl != 1) || (o->reverse != 0 && o->reverse != 1))
     return fail(LBM_EINVAL, "options.pdl and options.reverse must be 0 or 1");
   if (o->keep_psi_mb < 0) return fail(LBM_EINVAL, "options.keep_psi_mb must be >= 0");
-  if (o->chunks < 0) return fail(LBM_EINVAL, "options.chunks must be >= 0");
   return LBM_OK;
 }
 
@@ -657,7 +580,6 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   c->graph_mode = o.graph;
   c->keep_psi_mb = o.keep_psi_mb;
   c->idx16 = o.index == LBM_INDEX_BITS ? 2 : 1;
-  c->chunks = o.chunks;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
   // pair-slot indices i * npad + k and psi indices npad + w are 32-bit
   if ((size_t)19 * c->npad >= ((size_t)1 << 31) || c->npad + c->nwpad >= ((size_t)1 << 31)) {
@@ -667,9 +589,6 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   c->zstart.assign(nz + 1, 0);
   for (long long n = 0; n < g.nact; ++n) ++c->zstart[g.node_vox[n] / c->np + 1];
   for (int z = 0; z < nz; ++z) c->zstart[z + 1] += c->zstart[z];
-  c->wzstart.assign(nz + 1, 0);
-  for (long long w = 0; w < g.nw; ++w) ++c->wzstart[g.wall_vox[w] / c->np + 1];
-  for (int z = 0; z < nz; ++z) c->wzstart[z + 1] += c->wzstart[z];
   cudaStream_t st = use_stream(c);
   const size_t fbytes = (size_t)2 * 19 * c->npad * c->esz;
   const size_t psibytes = (c->npad + c->nwpad) * 2 * c->esz;  // wall part starts at npad

@@ -47,7 +47,7 @@ class lbm_params(C.Structure):
 
 class lbm_options(C.Structure):
     _fields_ = [("index", C.c_int), ("graph", C.c_int), ("pdl", C.c_int), ("reverse", C.c_int),
-                ("keep_psi_mb", C.c_int), ("chunks", C.c_int)]
+                ("keep_psi_mb", C.c_int)]
 
 
 LBM_INDEX_16, LBM_INDEX_BITS = 0, 1

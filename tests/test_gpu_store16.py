@@ -109,10 +109,11 @@ def errors_against_oracle(cfg, form, steps, oracle_state=None):
 
 
 def test_storage_experiment_verdict_on_a_droplet():
-    """The go/no-go of DESIGN.md section 10 on the smallest case: after 100 steps of a G = 3.5
+    """The go/no-go of profiles/r2_store16.md on the smallest case: after 100 steps of a G = 3.5
     droplet (interface densities 0.027 .. 1) the fp32 build meets the north-star tolerances, plain
-    fp16 / bf16 storage misses them by orders of magnitude, and the best 16-bit form (deviation from
-    the node's own previous density) still misses the 1e-4 density bar at the interface."""
+    fp16 storage misses them by more than an order of magnitude, the best 16-bit form (deviation
+    from the node's own previous density) still misses the velocity bar severalfold, and the same
+    form in 24 bits meets all three."""
     from workloads import default_params, tanh_profile
     n = 32
     shape = (n, n, n)
@@ -121,12 +122,12 @@ def test_storage_experiment_verdict_on_a_droplet():
     cfg = dict(mask=np.zeros(shape, np.uint8), rhoA=rA, rhoB=1.027 - rA,
                params=default_params(G=3.5, tau=(1.0, 1.0), storage_bits=32))
     res, state = {}, None
-    for form in ("fp32", "fp16", "dev16", "fix16"):
+    for form in ("fp32", "fp16", "dev16", "dev24"):
         res[form], state = errors_against_oracle(cfg, form, 100, state)
     assert res["fp32"][0] <= 1e-4 and res["fp32"][1] <= 1e-4 and res["fp32"][2] <= 1e-6, res
-    assert res["fp16"][0] > 1e-3, res                       # plain half: nowhere near
-    assert res["dev16"][0] < res["fp16"][0] and res["fix16"][0] < res["fp16"][0], res
-    assert min(res["dev16"][0], res["fix16"][0]) > 1e-4, res   # no-go: the 1e-4 bar is not met
+    assert res["fp16"][0] > 5e-4 and res["fp16"][1] > 2e-3, res      # plain half: nowhere near
+    assert res["dev16"][0] < res["fp16"][0] and res["dev16"][1] > 3e-4, res   # 16 bits: no-go
+    assert res["dev24"][0] <= 1e-4 and res["dev24"][1] <= 1e-4 and res["dev24"][2] <= 1e-6, res
 
 
 def main():
