@@ -139,6 +139,21 @@ int lbm_saturation(lbm_ctx* c, int comp, int z0, int z1, double* S);
  * lbm_saturation.  Runs on the GPU (lock-free union-find over the compact ids, 8 B per fluid
  * node of temporary device memory); an empty z-range gives 0.  Synchronises. */
 int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, double* mass);
+/* lbm_trapped_volume without any allocation: same query, same kernels, same result (node count
+ * and mass bit-identical), but the scratch of the connected-component labelling (8 B per fluid
+ * node + 19 KB of partial sums) lives in a file-scope device array of the library instead of a
+ * temporary buffer from the caching allocator.  The call performs no cudaMalloc / cudaFree and
+ * calls no allocating routine; it is for callers that cannot allocate (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc).  Limits and caveats:
+ *  - boxes of at most LBM_STATIC_MAX_NODES fluid nodes; more -> LBM_EINVAL with a message naming
+ *    the limit (use lbm_trapped_volume);
+ *  - every GPU that loads the library holds the array (8 MiB + 19 KB) until the process exits;
+ *  - ALL contexts on a device share the one array and it keeps the last call's contents (the call
+ *    rewrites every word it reads, nothing needs clearing): two calls that overlap on the GPU --
+ *    from different streams or host threads -- race.  One call at a time per device;
+ *  - not available on slab contexts.  Synchronises like lbm_trapped_volume. */
+#define LBM_STATIC_MAX_NODES 1048576
+int lbm_trapped_volume_static(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, double* mass);
 /* Mean over the fluid nodes with z in [z0,z1) of the pressure of Eq. (12) (reading R13):
  * P = (rho_A+rho_B)/3 + (G/3) rho_A rho_B.  The capillary pressure of the drainage protocol
  * is P_c = mean over the inlet layer - mean over the outlet layer.  Computed on

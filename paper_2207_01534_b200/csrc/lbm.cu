@@ -1424,6 +1424,84 @@ int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, d
   return LBM_OK;
 }
 
+// ---- lbm_trapped_volume_static: the trapped-volume query without any allocation ---------------
+// Scratch of the union-find kernels (parent[nf] | flag[nf] int32, then 2 * blocks + 2 doubles of
+// partial sums) in a file-scope device array instead of a buffer from the caching allocator, for
+// callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid
+// cudaMalloc).  Every GPU that loads the library holds the array (8 MiB + 19 KB) until exit.
+// In HOST code the array's name is a host-side stand-in, not a device address: the kernels get
+// the address cudaGetSymbolAddress returns, looked up once per device with that device current.
+constexpr long long kStaticMaxNodes = LBM_STATIC_MAX_NODES;
+constexpr int kStaticMaxBlocks = 1184;   // blocks of k_ccl_count: 8 per SM x 148
+constexpr size_t kStaticScratchBytes =
+    (size_t)kStaticMaxNodes * 2 * sizeof(int) + ((size_t)2 * kStaticMaxBlocks + 2) * sizeof(double);
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+int lbm_trapped_volume_static(lbm_ctx* c, int comp, int z0, int z1, long long* nodes,
+                              double* mass) {
+  if (int rc = check_ctx(c)) return rc;   // makes the context's device current
+  if (c->slab) return fail(LBM_EINVAL, "lbm_trapped_volume_static is not available on a slab context");
+  if (!nodes || !mass || comp < 0 || comp > 1 || z0 < 0 || z1 > c->nz || z0 >= z1)
+    return fail(LBM_EINVAL, "bad argument");
+  if ((long long)c->nf > kStaticMaxNodes)
+    return fail(LBM_EINVAL,
+                "lbm_trapped_volume_static: the box has %d fluid nodes, the static scratch serves at "
+                "most LBM_STATIC_MAX_NODES = %lld; use lbm_trapped_volume",
+                c->nf, kStaticMaxNodes);
+  // device address of g_static_scratch: looked up once per device, with that device current
+  static void* scratch_of_device[64] = {};
+  void* scratch = c->device < 64 ? scratch_of_device[c->device] : nullptr;
+  if (!scratch) {
+    CU(cudaGetSymbolAddress(&scratch, g_static_scratch));
+    if (!scratch) return fail(LBM_ECUDA, "cudaGetSymbolAddress returned a null address");
+    if (c->device < 64) scratch_of_device[c->device] = scratch;
+  }
+  cudaStream_t st = use_stream(c);
+  {
+    ProfOff guard(c);
+    if (c->bits == 64) launch_psi<double>(c, st); else launch_psi<float>(c, st);
+  }
+  CU(cudaPeekAtLastError());
+  const int nf = c->nf, nz = c->nz;
+  const int n0 = c->zstart[z0], n1 = c->zstart[z1];
+  const int chunk = std::max(kCclBlock, (int)(((long long)(n1 - n0) + kStaticMaxBlocks - 1) / kStaticMaxBlocks));
+  const int nb = n1 > n0 ? blocks(n1 - n0, chunk) : 0;   // <= kStaticMaxBlocks
+  const size_t ints = ((size_t)2 * nf + 1) & ~(size_t)1;
+  // The array keeps the previous call's contents.  Nothing has to be cleared: k_ccl_init writes
+  // parent[n] and flag[n] of every node before anything reads them, k_ccl_count every partial it
+  // is summed from, k_sum_pairs both results.
+  int* parent = (int*)scratch;
+  int* flag = parent + nf;
+  double* partial = (double*)(parent + ints);
+  double* out = partial + (size_t)2 * nb;
+  const int g = blocks(nf, 256);
+  if (c->bits == 64)
+    k_ccl_init<double><<<g, 256, 0, st>>>((const Vec2<double>*)c->psi, nf, comp, parent, flag);
+  else
+    k_ccl_init<float><<<g, 256, 0, st>>>((const Vec2<float>*)c->psi, nf, comp, parent, flag);
+  k_ccl_unite<<<g, 256, 0, st>>>(c->nbr, nf, c->npad, parent);
+  k_ccl_flatten<<<g, 256, 0, st>>>(nf, parent);
+  const int a0 = c->zstart[0], a1 = c->zstart[1], b0 = c->zstart[nz - 1], b1 = c->zstart[nz];
+  if ((a1 - a0) + (b1 - b0) > 0)
+    k_ccl_mark<<<blocks((a1 - a0) + (b1 - b0), 256), 256, 0, st>>>(parent, a0, a1, b0, b1, flag);
+  if (nb > 0) {
+    if (c->bits == 64)
+      k_ccl_count<double><<<nb, kCclBlock, 0, st>>>((const Vec2<double>*)c->psi, parent, flag, n0,
+                                                    n1, comp, chunk, partial);
+    else
+      k_ccl_count<float><<<nb, kCclBlock, 0, st>>>((const Vec2<float>*)c->psi, parent, flag, n0, n1,
+                                                   comp, chunk, partial);
+  }
+  k_sum_pairs<<<1, 32, 0, st>>>(partial, nb, out);
+  CU(cudaPeekAtLastError());
+  double h[2] = {0.0, 0.0};
+  CU(cudaMemcpyAsync(h, out, sizeof h, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  *mass = h[0];
+  *nodes = (long long)h[1];
+  return LBM_OK;
+}
+
 int lbm_mean_pressure(lbm_ctx* c, int z0, int z1, double* P) {
   if (int rc = check_ctx(c)) return rc;
   if (c->slab && c->slab_phase != 2)

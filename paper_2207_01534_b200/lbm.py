@@ -20,7 +20,7 @@ LBM_OK, LBM_EINVAL, LBM_ENOFLUID, LBM_ESOLIDOPEN, LBM_ENOMEM, LBM_ECUDA, LBM_ENO
 SYMBOLS = [
     "lbm_create", "lbm_destroy", "lbm_set_density", "lbm_set_populations", "lbm_get_populations",
     "lbm_set_boundary", "lbm_step", "lbm_sync", "lbm_get_macroscopic", "lbm_diagnostics",
-    "lbm_saturation", "lbm_trapped_volume", "lbm_mean_pressure", "lbm_num_fluid", "lbm_num_wall_solid",
+    "lbm_saturation", "lbm_trapped_volume", "lbm_trapped_volume_static", "lbm_mean_pressure", "lbm_num_fluid", "lbm_num_wall_solid",
     "lbm_memory_bytes", "lbm_set_profiling", "lbm_last_step_profile", "lbm_last_error",
     "lbm_build_index",
     "lbm_options_default", "lbm_create_opt", "lbm_create_slab_opt", "lbm_step_info",
@@ -85,6 +85,8 @@ def load():
     lib.lbm_diagnostics.argtypes = [P, D, D]
     lib.lbm_saturation.argtypes = [P, I, I, I, D]
     lib.lbm_trapped_volume.argtypes = [P, I, I, I, C.POINTER(LL), D]
+    lib.lbm_trapped_volume_static.argtypes = [P, I, I, I, C.POINTER(LL), D]
+    lib.lbm_trapped_volume_static.restype = I
     lib.lbm_mean_pressure.argtypes = [P, I, I, D]
     lib.lbm_num_fluid.argtypes = [P]
     lib.lbm_num_fluid.restype = LL
@@ -399,6 +401,14 @@ class Lbm:
         m = C.c_double()
         _chk(load().lbm_trapped_volume(self._h, int(comp), int(z0), int(z1), C.byref(n),
                                        C.byref(m)), "lbm_trapped_volume")
+        return n.value, m.value
+
+    def trapped_volume_static(self, comp, z0=0, z1=None):
+        z1 = self.shape[0] if z1 is None else z1
+        n = C.c_longlong()
+        m = C.c_double()
+        _chk(load().lbm_trapped_volume_static(self._h, int(comp), int(z0), int(z1), C.byref(n),
+                                              C.byref(m)), "lbm_trapped_volume_static")
         return n.value, m.value
 
     def mean_pressure(self, z0=0, z1=None):
