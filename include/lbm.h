@@ -73,7 +73,9 @@ enum { LBM_INDEX_16 = 0, LBM_INDEX_BITS = 1 };
 typedef struct {
   int index;        /* neighbour index of the fused pass: LBM_INDEX_16 (default) 16-bit tile-relative
                        rows, 37 B per node; LBM_INDEX_BITS per-row bitmasks + prefix ids, 0.5 B per
-                       voxel + 4 B per node (low-memory option, ~2.5 % slower)                      */
+                       voxel + 4 B per node and per wall solid; also replaces the virtual-solid pass's
+                       72 B gather lists (low-memory option: index memory 141 -> 8 B per node on the
+                       256^3 rock; step ~4 % slower)                                                */
   int graph;        /* -1 (default) replay a captured CUDA graph of 16 steps on boxes of
                        <= 600 000 fluid nodes, 0 never, 1 always                                    */
   int pdl;          /* 1 (default) programmatic dependent launch of the three passes    */
@@ -99,7 +101,8 @@ void lbm_destroy(lbm_ctx* c);
 /* What lbm_create chose: info[0] index form (LBM_INDEX_16 / LBM_INDEX_BITS; a box edge above
  * 1024 falls back to LBM_INDEX_16), [1] 1 if lbm_step replays CUDA graphs, [2] pdl, [3] reverse,
  * [4] share of the psi lines stored with evict_last priority, in 1/1000, [5] tiles that read the
- * int32 index rows instead of the 16-bit ones, [6], [7] reserved (0). */
+ * int32 index rows instead of the 16-bit ones, [6] 1 if the virtual-solid pass reads the geometric
+ * index, [7] reserved (0). */
 int lbm_step_info(lbm_ctx* c, int info[8]);
 
 /* f_i^sigma = w_i * rho_sigma (reading R11); dense double arrays of nx*ny*nz.  Also records the

@@ -175,7 +175,8 @@ int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Ind
   return 0;
 }
 
-int build_bitindex(const Geometry& g, long long psi_wall_base, BitIndex& out) {
+int build_bitindex(const Geometry& g, long long psi_wall_base, BitIndex& out,
+                   bool with_fluid_coord) {
   if (g.nf <= 0 || g.vox2id.empty()) return -1;
   if (g.nx > 1024 || g.ny > 1024 || g.nz > 1024) return -1;
   const int nx = g.nx, W = (nx + 31) / 32;
@@ -183,7 +184,8 @@ int build_bitindex(const Geometry& g, long long psi_wall_base, BitIndex& out) {
   try {
     out.words = W;
     out.rec.assign((size_t)rows * W * 4, 0);
-    out.coord.assign((size_t)nf, 0);
+    out.coord.assign(with_fluid_coord ? (size_t)nf : 0, 0);
+    out.wall_coord.assign((size_t)g.nw, 0);
 #pragma omp parallel for schedule(static)
     for (long long r = 0; r < rows; ++r) {
       const int32_t* id = &g.vox2id[(size_t)r * nx];
@@ -202,9 +204,11 @@ int build_bitindex(const Geometry& g, long long psi_wall_base, BitIndex& out) {
         rec[4 * w + 2] = (uint32_t)next_f; rec[4 * w + 3] = (uint32_t)next_w;
       }
       const int y = (int)(r % g.ny), z = (int)(r / g.ny);
-      for (int x = 0; x < nx; ++x)
-        if (id[x] >= 0 && id[x] < nf)
-          out.coord[id[x]] = (uint32_t)x | ((uint32_t)y << 10) | ((uint32_t)z << 20);
+      for (int x = 0; x < nx; ++x) {
+        const uint32_t c = (uint32_t)x | ((uint32_t)y << 10) | ((uint32_t)z << 20);
+        if (id[x] >= nf) out.wall_coord[id[x] - nf] = c;
+        else if (id[x] >= 0 && with_fluid_coord) out.coord[id[x]] = c;
+      }
     }
   } catch (const std::bad_alloc&) {
     return -4;

@@ -68,10 +68,13 @@ int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Ind
 struct BitIndex {
   int words = 0;                    // 32-voxel words per row
   std::vector<uint32_t> rec;        // [nz*ny][words][4]
-  std::vector<uint32_t> coord;      // [nf]
+  std::vector<uint32_t> coord;      // [nf]  x | y << 10 | z << 20 of fluid node n
+  std::vector<uint32_t> wall_coord; // [nw]  the same of wall solid w (the wall pass's whole index)
 };
 // psi_wall_base = psi index of wall solid 0.  -1 if a box edge exceeds 1024.
-int build_bitindex(const Geometry& g, long long psi_wall_base, BitIndex& out);
+// with_fluid_coord = false: coord stays empty (only the wall pass reads the index)
+int build_bitindex(const Geometry& g, long long psi_wall_base, BitIndex& out,
+                   bool with_fluid_coord = true);
 
 // Returns 0, or -1 bad arguments, -2 no fluid voxel, -3 solid on an open plane or its interior
 // neighbour plane (z in {0,1,nz-2,nz-1}), -4 out of memory.  `with_tables` = also fill nbr,

@@ -173,6 +173,89 @@ __global__ void __launch_bounds__(256) k_wallpsi(Vec2<T>* __restrict__ psi,
   store_vec2(psi + wall_base + w, o, l2_keep_policy(keep_psi));
 }
 
+// direction index of (dx, dy, dz), or -1 if that offset is not a D3Q19 direction
+__host__ __device__ constexpr int dir_of(int dx, int dy, int dz) {
+  for (int i = 0; i < Q; ++i)
+    if (ex(i) == dx && ey(i) == dy && ez(i) == dz) return i;
+  return -1;
+}
+
+// a2 with the geometric index (geometry.hpp BitIndex) instead of the 72 B gather list per wall
+// solid: 4 B of packed coordinates per wall solid; the fluid neighbours' ids come from the per-row
+// records {fluid bitmask, wall bitmask, id of the first fluid node of the word, ...} -- id =
+// first id + popcount of the mask below x' -- which are 0.5 B per voxel and cache-resident
+// (consecutive wall solids share their 9 rows).  All of that is static and runs BEFORE the
+// dependency wait, beside the draining density pass.  z wraps periodically: a wall solid is never
+// within two planes of an open plane, and at a slab's cut ends the outermost halo plane's values
+// are never read (as with the lists).  Same sums in the same order as k_wallpsi: bit-identical.
+template <typename T>
+__global__ void __launch_bounds__(256, 8) k_wallpsi_bits(Vec2<T>* __restrict__ psi,
+                                                      const uint32_t* __restrict__ wall_coord,
+                                                      const uint4* __restrict__ bits,
+                                                      const T* __restrict__ inv_den,
+                                                      size_t wall_base, int nw, int nx, int ny,
+                                                      int nz, int words, T chiA, T chiB,
+                                                      float keep_psi) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool live = w < nw;
+  const uint32_t cw = live ? wall_coord[w] : 0u;
+  const int x = (int)(cw & 1023u), y = (int)((cw >> 10) & 1023u), z = (int)(cw >> 20);
+  int word[3];
+  uint32_t bit[3], below[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {  // ex = d - 1, periodic in x
+    int xx = x + d - 1;
+    xx = xx < 0 ? nx - 1 : (xx == nx ? 0 : xx);
+    word[d] = xx >> 5;
+    bit[d] = (uint32_t)xx & 31u;
+    below[d] = (1u << bit[d]) - 1u;
+  }
+  int id[Q];
+#pragma unroll
+  for (int dz = -1; dz <= 1; ++dz) {
+    int zz = z + dz;
+    zz = zz < 0 ? nz - 1 : (zz == nz ? 0 : zz);
+#pragma unroll
+    for (int dy = -1; dy <= 1; ++dy) {
+      int yy = y + dy;
+      yy = yy < 0 ? ny - 1 : (yy == ny ? 0 : yy);
+      const uint4* row = bits + (size_t)(zz * ny + yy) * words;
+      // the three x-neighbours of a row almost always lie in one 32-voxel word
+      const bool need_m = dir_of(-1, dy, dz) > 0, need_c = dir_of(0, dy, dz) > 0,
+                 need_p = dir_of(1, dy, dz) > 0;
+      uint4 qc = __ldg(row + word[1]);
+      if (need_m) {
+        const uint4 q = word[0] == word[1] ? qc : __ldg(row + word[0]);
+        id[dir_of(-1, dy, dz) > 0 ? dir_of(-1, dy, dz) : 0] =
+            (live && ((q.x >> bit[0]) & 1u)) ? (int)(q.z + __popc(q.x & below[0])) : -1;
+      }
+      if (need_c)
+        id[dir_of(0, dy, dz) > 0 ? dir_of(0, dy, dz) : 0] =
+            (live && ((qc.x >> bit[1]) & 1u)) ? (int)(qc.z + __popc(qc.x & below[1])) : -1;
+      if (need_p) {
+        const uint4 q = word[2] == word[1] ? qc : __ldg(row + word[2]);
+        id[dir_of(1, dy, dz) > 0 ? dir_of(1, dy, dz) : 0] =
+            (live && ((q.x >> bit[2]) & 1u)) ? (int)(q.z + __popc(q.x & below[2])) : -1;
+      }
+    }
+  }
+  const T s = live ? inv_den[w] : T(0);
+  pdl_wait();     // everything above is static; psi comes from the density pass
+  pdl_trigger();  // as k_wallpsi: the fused pass may stage its first tiles beside this kernel
+  if (!live) return;
+  T na = T(0), nb = T(0);
+#pragma unroll
+  for (int i = 1; i < Q; ++i) {
+    if (id[i] >= 0) {
+      const Vec2<T> p = psi[id[i]];
+      na = fma_rn(wgt<T>(i), p.a, na);
+      nb = fma_rn(wgt<T>(i), p.b, nb);
+    }
+  }
+  Vec2<T> o; o.a = mul_rn(mul_rn(chiA, na), s); o.b = mul_rn(mul_rn(chiB, nb), s);
+  store_vec2(psi + wall_base + w, o, l2_keep_policy(keep_psi));
+}
+
 // ---------------------------------------------------------------------------------------------
 // Per-node mixture quantities shared by the collide kernel and the macroscopic getter.
 // a3: F_sigma = -G rho_sigma sum_i w_i Psi_sigmabar(x+e_i) e_i + rho_sigma g

@@ -109,7 +109,10 @@ struct lbm_ctx {
                             // 2 = geometric bitmask index (lbm_options.index = LBM_INDEX_BITS;
                             // geometry.hpp BitIndex)
   uint32_t* bit_rec = nullptr;       // [nz*ny][bit_words][4]
-  uint32_t* bit_coord = nullptr;     // [npad]
+  uint32_t* bit_coord = nullptr;     // [npad]  (only with the geometric index of the fused pass)
+  uint32_t* wall_coord = nullptr;    // [nw]    packed coordinates of the wall solids
+  int wall_bits = 0;        // 1: the wall pass reads the geometric index (k_wallpsi_bits; with
+                            // LBM_INDEX_BITS), 0: the int32 gather lists
   int bit_words = 0;
   uint16_t* nbr16 = nullptr;         // [18][npad]
   int* nbr16_meta = nullptr;         // [tiles][kIdxMeta]
@@ -167,7 +170,7 @@ struct lbm_ctx {
     lbm_shim_free(nbr16_meta);
     lbm_shim_free(halo_slots); lbm_shim_free(halo_send); lbm_shim_free(halo_recv);
     lbm_shim_free(ccl);
-    lbm_shim_free(bit_rec); lbm_shim_free(bit_coord);
+    lbm_shim_free(bit_rec); lbm_shim_free(bit_coord); lbm_shim_free(wall_coord);
   }
 };
 
@@ -299,9 +302,15 @@ void launch_wall(lbm_ctx* c, cudaStream_t st) {
   if (c->nw <= 0) return;
   const bool pdl = c->pdl && !c->prof;
   Timed t(c, st, 1);
-  launch_k(pdl, k_wallpsi<T>, blocks(c->nw, 256), 256, 0, st, (Vec2<T>*)c->psi,
-           (const int*)c->wall_nbr, (const T*)c->wall_inv_den, c->npad, c->nw, c->nwpad,
-           (T)(1.0 + c->p.xi), (T)(1.0 - c->p.xi), c->keep_psi);
+  if (c->wall_bits)
+    launch_k(pdl, k_wallpsi_bits<T>, blocks(c->nw, 256), 256, 0, st, (Vec2<T>*)c->psi,
+             (const uint32_t*)c->wall_coord, (const uint4*)c->bit_rec, (const T*)c->wall_inv_den,
+             c->npad, c->nw, c->nx, c->ny, c->nz, c->bit_words, (T)(1.0 + c->p.xi),
+             (T)(1.0 - c->p.xi), c->keep_psi);
+  else
+    launch_k(pdl, k_wallpsi<T>, blocks(c->nw, 256), 256, 0, st, (Vec2<T>*)c->psi,
+             (const int*)c->wall_nbr, (const T*)c->wall_inv_den, c->npad, c->nw, c->nwpad,
+             (T)(1.0 + c->p.xi), (T)(1.0 - c->p.xi), c->keep_psi);
 }
 
 // a1 + a2.  Slab mode: the density pass (lbm_slab_density) and the psi halo exchange are the
@@ -593,7 +602,13 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   const size_t fbytes = (size_t)2 * 19 * c->npad * c->esz;
   const size_t psibytes = (c->npad + c->nwpad) * 2 * c->esz;  // wall part starts at npad
   const size_t nbrbytes = (size_t)18 * c->npad * sizeof(int);
-  const size_t wnbrbytes = (size_t)18 * c->nwpad * sizeof(int);
+  // LBM_INDEX_BITS (the low-memory option): both the fused pass and the wall pass read the
+  // geometric index; the int32 gather lists of the wall pass are then not allocated
+  lbmgeo::BitIndex bix;  // upload source until the sync below
+  const bool have_bits = c->idx16 == 2 && lbmgeo::build_bitindex(g, (long long)c->npad, bix) == 0;
+  if (!have_bits) c->idx16 = 1;   // a box edge above 1024: the packed coordinates do not fit
+  c->wall_bits = have_bits && g.nw > 0;
+  const size_t wnbrbytes = c->wall_bits ? 0 : (size_t)18 * c->nwpad * sizeof(int);
   const size_t frozenbytes = p->z_open ? (size_t)2 * 2 * 5 * c->np * c->esz : 0;
   c->diag_blocks = 148 * 8;
   c->f[0] = lbm_shim_alloc(fbytes);
@@ -643,8 +658,9 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   }
   for (int i = 0; i < 18; ++i) {
     up(c->nbr + (size_t)i * c->npad, g.nbr.data() + (size_t)i * g.nf, g.nf * sizeof(int));
-    up(c->wall_nbr + (size_t)i * c->nwpad, g.wall_nbr.data() + (size_t)i * g.nw,
-       g.nw * sizeof(int));
+    if (!c->wall_bits)
+      up(c->wall_nbr + (size_t)i * c->nwpad, g.wall_nbr.data() + (size_t)i * g.nw,
+         g.nw * sizeof(int));
   }
   up(c->node_vox_d, g.node_vox.data(), g.nf * sizeof(int));
   std::vector<float> invf;
@@ -663,22 +679,25 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   up(c->nbr16, i16.nbr16.data(), i16.nbr16.size() * sizeof(uint16_t));
   up(c->nbr16_meta, i16.meta.data(), i16.meta.size() * sizeof(int32_t));
   c->bytes[2] += (long long)(i16.nbr16.size() * 2 + i16.meta.size() * 4);
-  lbmgeo::BitIndex bix;  // upload source until the sync below
-  if (c->idx16 == 2) {
-    if (lbmgeo::build_bitindex(g, (long long)c->npad, bix) != 0) {
-      c->idx16 = 1;   // a box edge above 1024: the packed coordinates do not fit
-    } else {
-      c->bit_words = bix.words;
-      c->bit_rec = (uint32_t*)lbm_shim_alloc(bix.rec.size() * sizeof(uint32_t));
-      c->bit_coord = (uint32_t*)lbm_shim_alloc(c->npad * sizeof(uint32_t));
-      if (!c->bit_rec || !c->bit_coord) {
-        delete c;
-        return fail(LBM_ENOMEM, "device allocation failed (bit index)");
-      }
+  if (have_bits) {
+    c->bit_words = bix.words;
+    c->bit_rec = (uint32_t*)lbm_shim_alloc(bix.rec.size() * sizeof(uint32_t));
+    if (c->idx16 == 2) c->bit_coord = (uint32_t*)lbm_shim_alloc(c->npad * sizeof(uint32_t));
+    if (c->wall_bits) c->wall_coord = (uint32_t*)lbm_shim_alloc(bix.wall_coord.size() * sizeof(uint32_t));
+    if (!c->bit_rec || (c->idx16 == 2 && !c->bit_coord) || (c->wall_bits && !c->wall_coord)) {
+      delete c;
+      return fail(LBM_ENOMEM, "device allocation failed (bit index)");
+    }
+    up(c->bit_rec, bix.rec.data(), bix.rec.size() * sizeof(uint32_t));
+    c->bytes[2] += (long long)(bix.rec.size() * 4);
+    if (c->idx16 == 2) {
       if (e == cudaSuccess) e = cudaMemsetAsync(c->bit_coord, 0, c->npad * sizeof(uint32_t), st);
-      up(c->bit_rec, bix.rec.data(), bix.rec.size() * sizeof(uint32_t));
       up(c->bit_coord, bix.coord.data(), bix.coord.size() * sizeof(uint32_t));
-      c->bytes[2] += (long long)(bix.rec.size() * 4 + c->npad * 4);
+      c->bytes[2] += (long long)(c->npad * 4);
+    }
+    if (c->wall_bits) {
+      up(c->wall_coord, bix.wall_coord.data(), bix.wall_coord.size() * sizeof(uint32_t));
+      c->bytes[2] += (long long)(bix.wall_coord.size() * 4);
     }
   }
   lbmgeo::Halo halo;  // declared here: its lists are upload sources until the sync below
@@ -800,7 +819,7 @@ int lbm_step_info(lbm_ctx* c, int info[8]) {
   info[2] = c->pdl; info[3] = c->reverse;
   info[4] = (int)(c->keep_psi * 1000.f + 0.5f);
   info[5] = (int)std::min<long long>(c->wide_tiles, 2147483647LL);
-  info[6] = 0; info[7] = 0;
+  info[6] = c->wall_bits; info[7] = 0;
   return LBM_OK;
 }
 

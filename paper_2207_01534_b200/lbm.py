@@ -359,7 +359,7 @@ class Lbm:
         _chk(load().lbm_step_info(self._h, v), "lbm_step_info")
         return {"index": {LBM_INDEX_16: "16", LBM_INDEX_BITS: "bits"}[v[0]], "graph": bool(v[1]),
                 "pdl": bool(v[2]), "reverse": bool(v[3]), "keep_psi": v[4] / 1000.0,
-                "wide_tiles": v[5]}
+                "wide_tiles": v[5], "wall_index": "bits" if v[6] else "lists"}
 
     def sync(self):
         _chk(load().lbm_sync(self._h), "lbm_sync")
