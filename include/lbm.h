@@ -74,8 +74,9 @@ typedef struct {
   int index;        /* neighbour index of the fused pass: LBM_INDEX_16 (default) 16-bit tile-relative
                        rows, 37 B per node; LBM_INDEX_BITS per-row bitmasks + prefix ids, 0.5 B per
                        voxel + 4 B per node and per wall solid; also replaces the virtual-solid pass's
-                       72 B gather lists (low-memory option: index memory 141 -> 8 B per node on the
-                       256^3 rock; step ~4 % slower)                                                */
+                       72 B gather lists, and the 16-bit rows are not built (low-memory option: index
+                       memory 140 -> 85 B per node on the 256^3 rock, what remains being the int32
+                       rows the getters read; step ~5 % slower)                                     */
   int graph;        /* -1 (default) replay a captured CUDA graph of 16 steps on boxes of
                        <= 600 000 fluid nodes, 0 never, 1 always                                    */
   int pdl;          /* 1 (default) programmatic dependent launch of the three passes    */

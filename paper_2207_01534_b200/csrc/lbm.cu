@@ -644,12 +644,14 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   if (e == cudaSuccess && frozenbytes) e = cudaMemsetAsync(c->frozen, 0, frozenbytes, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->nbr, 0, nbrbytes, st);
   // Re-base wall ids from nf+w to npad+w so that the wall part of psi starts on a tile boundary.
-  lbmgeo::Index16 i16;
-  if (lbmgeo::build_index16(g, (long long)c->npad, c->npad, i16) != 0) {
-    delete c;
-    return fail(LBM_ENOMEM, "index16 build failed");
+  lbmgeo::Index16 i16;   // not built with LBM_INDEX_BITS: the fused pass then never reads it
+  if (c->idx16 != 2) {
+    if (lbmgeo::build_index16(g, (long long)c->npad, c->npad, i16) != 0) {
+      delete c;
+      return fail(LBM_ENOMEM, "index16 build failed");
+    }
+    c->wide_tiles = i16.wide_tiles;
   }
-  c->wide_tiles = i16.wide_tiles;
   {
     const int32_t shift = (int32_t)(c->npad - (size_t)g.nf);
     const int32_t nf32 = (int32_t)g.nf;
@@ -670,15 +672,17 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   } else {
     up(c->wall_inv_den, g.wall_inv_den.data(), g.nw * sizeof(double));
   }
-  c->nbr16 = (uint16_t*)lbm_shim_alloc(i16.nbr16.size() * sizeof(uint16_t));
-  c->nbr16_meta = (int*)lbm_shim_alloc(i16.meta.size() * sizeof(int32_t) + 16);
-  if (!c->nbr16 || !c->nbr16_meta) {
-    delete c;
-    return fail(LBM_ENOMEM, "device allocation failed (index16)");
+  if (c->idx16 != 2) {
+    c->nbr16 = (uint16_t*)lbm_shim_alloc(i16.nbr16.size() * sizeof(uint16_t));
+    c->nbr16_meta = (int*)lbm_shim_alloc(i16.meta.size() * sizeof(int32_t) + 16);
+    if (!c->nbr16 || !c->nbr16_meta) {
+      delete c;
+      return fail(LBM_ENOMEM, "device allocation failed (index16)");
+    }
+    up(c->nbr16, i16.nbr16.data(), i16.nbr16.size() * sizeof(uint16_t));
+    up(c->nbr16_meta, i16.meta.data(), i16.meta.size() * sizeof(int32_t));
+    c->bytes[2] += (long long)(i16.nbr16.size() * 2 + i16.meta.size() * 4);
   }
-  up(c->nbr16, i16.nbr16.data(), i16.nbr16.size() * sizeof(uint16_t));
-  up(c->nbr16_meta, i16.meta.data(), i16.meta.size() * sizeof(int32_t));
-  c->bytes[2] += (long long)(i16.nbr16.size() * 2 + i16.meta.size() * 4);
   if (have_bits) {
     c->bit_words = bix.words;
     c->bit_rec = (uint32_t*)lbm_shim_alloc(bix.rec.size() * sizeof(uint32_t));
