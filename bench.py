@@ -186,8 +186,10 @@ def ncu_traffic(workload_name, kernel):
     sha = source_sha16()
     with open(path) as fh:
         for line in fh:
-            f = [x.strip() for x in line.split(",")]
-            if len(f) >= 4 and f[0] == sha and f[1] == workload_name and f[2] == kernel:
+            if line.startswith("#"):
+                continue
+            f = [x.strip() for x in line.split(", ")]     # kernel names hold commas, no ", "
+            if len(f) == 4 and f[0] == sha and f[1] == workload_name and f[2] == kernel:
                 return float(f[3])
     return None
 

@@ -54,3 +54,23 @@ def test_mode_selection(monkeypatch):
     assert (a.shard, a.config, a.gpus) == ("replicas", 4, 8)
     src = open(os.path.join(ROOT, "bench.py")).read()
     assert 'shard = a.shard or ("slab" if world > 1 else "replicas")' in src
+
+
+def test_roofline_traffic_is_keyed_by_the_build():
+    """bench.py reports roofline.traffic only from an ncu capture of the build it runs
+    (profiles/ncu_traffic.csv keyed by the source hash), never a number of another build."""
+    sys.path.insert(0, ROOT)
+    import bench
+    sha = bench.source_sha16()
+    assert len(sha) == 16
+    rows = [l for l in open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) if not l.startswith("#")]
+    assert rows and all(len(l.split(", ")) == 4 for l in rows)
+    k = "k_collide_stream_bulk<float,128,7,1,1>"
+    got = bench.ncu_traffic("cfg4_grf_256_imbibition", k)
+    mine = [l for l in rows if l.startswith(sha)]
+    if mine:
+        assert got is not None and 1.3e9 < got < 1.7e9      # 312 B x N_f = 1.352 GB + index
+    else:
+        assert got is None
+    assert bench.ncu_traffic("cfg5_spherepack_512_throughput", k) is None
+    assert bench.ncu_traffic(None, k) is None
