@@ -248,6 +248,9 @@ class SlabLbm:
     #    kind 2 = cluster flags of the trapped-volume query (8,9 -> 10,11)
     def _exchange_start(self, kind):
         b = 4 * kind
+        if self.native:     # one grouped ncclSend/ncclRecv round inside the library, in stream order
+            self.sims[0].slab_exchange(kind)
+            return []
         if self._ring is not None:
             buf = self._buf[0]
             return self._ring.start(buf[b], buf[b + 1], buf[b + 2], buf[b + 3])

@@ -453,6 +453,8 @@ def test_native_slab_step_ring_of_one(k, bits):
     ref.step(25)
     want = [ref.get_populations(s) for s in (0, 1)]
     want_sat = ref.saturation(1)
+    want_trapped = ref.trapped_volume(0)
+    want_p = ref.mean_pressure(0, c["mask"].shape[0])
     ref.close()
     for native in (True, False):
         s = SlabLbm(c["mask"], c["params"], rank=0, world=1, native=native)
@@ -464,6 +466,8 @@ def test_native_slab_step_ring_of_one(k, bits):
         for comp in (0, 1):
             assert np.array_equal(s.get_populations(comp), want[comp]), (native, comp)
         assert s.saturation(1) == want_sat
+        assert s.trapped_volume(0) == want_trapped      # cluster flags cross the (self-)cut by kind 2
+        assert abs(s.mean_pressure(0, c["mask"].shape[0]) - want_p) < 1e-12
         s.close()
 
 
