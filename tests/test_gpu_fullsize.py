@@ -129,3 +129,40 @@ def test_config5_at_256_elementwise_100_steps():
     cfg = make_config(5, size=256)
     assert cfg["mask"].shape == (256, 256, 256)
     _elementwise_fp32(cfg, 100)
+
+
+def _elementwise_fp64(cfg, steps):
+    """fp64 validation build against the oracle: every population of both components, 1e-10."""
+    o = LbmRef(cfg["mask"], cfg["params"])
+    g = Lbm(cfg["mask"], cfg["params"])
+    o.set_density(cfg["rhoA"], cfg["rhoB"])
+    g.set_density(cfg["rhoA"], cfg["rhoB"])
+    o.step(steps)
+    g.step(steps)
+    fl = cfg["mask"] == 0
+    worst = 0.0
+    for s in (0, 1):
+        a, b = g.get_populations(s)[:, fl], o.get_populations(s)[:, fl]
+        worst = max(worst, float((np.abs(a - b) / np.abs(b)).max()))
+    m_o, _ = o.diagnostics()
+    m_g, _ = g.diagnostics()
+    o.close()
+    g.close()
+    assert worst <= 1e-10, worst
+    assert np.max(np.abs(m_g - m_o) / m_o) <= 1e-12
+
+
+def test_config2_full_size_fp64_200_steps():
+    """north_star: "the fp64 GPU build must match to within 1e-10 relative on every population
+    after 200 steps" -- config 2 at its full 64^3 size (walls, wetting)."""
+    cfg = make_config(2, xi=0.3, storage_bits=64)
+    assert cfg["mask"].shape == (64, 64, 64)
+    _elementwise_fp64(cfg, 200)
+
+
+def test_config3_full_size_fp64_200_steps():
+    """The same bar on config 3 at its full 128^3 size: sphere pack, velocity inlet on A, pressure
+    outlet on B (NEEM planes, frozen inward populations), 200 steps."""
+    cfg = make_config(3, storage_bits=64)
+    assert cfg["mask"].shape == (128, 128, 128)
+    _elementwise_fp64(cfg, 200)
