@@ -13,9 +13,12 @@
  *      Zou-He variant (kinds 3-4, R31): pinned by its defining properties and a fixed point
  *      (tests/test_oracle_zouhe.py).  The mirrored psi neighbours beyond a plane (R12 iv, the
  *      one statement PAPER.md L113 prints: psi(x+e_14) = psi(x+e_13)) are pinned by the exact
- *      cancellation of the plane-normal force they imply (tests/test_oracle_diag_open.py).  What
- *      stays a READING of a garbled passage -- parity unpinned -- is R12 iii: which velocity NEEM
- *      extrapolates (the bare mixture velocity); neither the paper nor the mathematics fixes it.
+ *      cancellation of the plane-normal force they imply (tests/test_oracle_diag_open.py); that
+ *      NEEM's equilibrium is taken at the COMMON velocity of Eq. (8), not a component's own, by
+ *      reading the model's equilibrium off the collision step itself (tests/test_oracle_neem.py).
+ *      What stays a READING -- parity unpinned -- is one detail of R12 iii: that velocity is the
+ *      bare mixture velocity, without the F/2 shift of R3, also where the force at the interior
+ *      neighbour is not zero; the paper prints nothing that fixes it.
  * No blocking, fusion or reordering: five plain loop nests over the dense box.
  */
 #include "lbmref.h"

@@ -13,8 +13,9 @@
  * Open planes (lbmref_step with z_open=1): the NEEM formula, the frozen rule, the Zou-He
  * variant and the psi mirror across the planes are pinned by identities,
  * fixed points and an exact force cancellation (tests/test_oracle_neem.py, _zouhe.py,
- * _diag_open.py).  PARITY UNPINNED: one choice the garbled passage PAPER.md L147-157 leaves
- * open -- which velocity NEEM extrapolates (reading R12 iii: the bare mixture velocity).
+ * _diag_open.py), and so is the choice of the common velocity of Eq. (8) for NEEM's
+ * equilibrium.  PARITY UNPINNED: one detail the garbled passage PAPER.md L147-157 leaves open
+ * -- that velocity carries no F/2 shift where the force is not zero (reading R12 iii).
  *
  * Layout: dense arrays are indexed idx = x + nx*(y + ny*z); populations are
  * f[i*nvox + idx] per component with the direction order returned by lbmref_lattice.

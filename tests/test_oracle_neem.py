@@ -109,3 +109,48 @@ def test_neem_moving_uniform_flow_is_a_fixed_point():
         o.step(30)
         for s in range(2):
             assert np.max(np.abs(o.get_populations(s) - f0[s])) < 1e-15
+
+
+def test_neem_extrapolates_the_collision_operators_nonequilibrium_part():
+    """Reading R12 iii without retyping anything: ref. [6] extrapolates f - f^eq, and the model has
+    ONE equilibrium -- Eq. (2) at the common velocity of Eq. (8), the one its
+    collision relaxes to.  That equilibrium is read off the oracle's own collision operator (which
+    the shear-wave and Poiseuille pins fix independently): with no forces (G = 0, g = 0) and
+    tau_A = tau_B = tau, Eq. (1) is f* = f - (f - f^eq)/tau, so f^eq = f - tau (f - f*), and f* of a
+    node sits, after streaming, at its neighbours.  Because Eq. (2) is linear in the density at
+    fixed velocity, f^eq(rho_b, u_f) = (rho_b / rho_sigma(x_f)) f^eq_sigma(x_f), and NEEM reads
+        f(x_b) = (rho_b / rho(x_f)) f^eq(x_f) + f(x_f) - f^eq(x_f)
+    with nothing typed here but that linearity.  The two components are given different momenta,
+    so an extrapolation at a component's own velocity j_sigma/rho_sigma fails by O(1e-3)."""
+    shape = (8, 4, 5)
+    nz = shape[0]
+    tau = 0.8
+    mask = np.zeros(shape, np.uint8)
+    p = _params(G=0.0, tau=(tau, tau), xi=0.0)
+    o = LbmRef(mask, p)
+    rng = np.random.Generator(np.random.PCG64(12))
+    f0 = _random_pops(shape, 12)
+    f0[0] = f0[0] * (1.0 + 0.05 * Ef[:, 2].reshape(19, 1, 1, 1))      # A drifts up, B down:
+    f0[1] = f0[1] * (1.0 - 0.05 * Ef[:, 0].reshape(19, 1, 1, 1))      # different momenta
+    for s in range(2):
+        o.set_populations(s, f0[s])
+    o.step(1)
+    f = [o.get_populations(s) for s in range(2)]          # complete state at t+1, planes fixed
+    ua = np.tensordot(Ef.T, f[0][:, 1], axes=(1, 0)) / f[0][:, 1].sum(0)
+    ub = np.tensordot(Ef.T, f[1][:, 1], axes=(1, 0)) / f[1][:, 1].sum(0)
+    assert np.abs(ua - ub).max() > 1e-2                    # the discrimination is real
+    # the model's equilibrium of that state, from the collision operator of a periodic copy
+    q = LbmRef(mask, _params(G=0.0, tau=(tau, tau), xi=0.0, z_open=0))
+    for s in range(2):
+        q.set_populations(s, f[s])
+    q.step(1)
+    g = [q.get_populations(s) for s in range(2)]
+    for zb, zf, dc, rho_b in ((0, 1, 0, 1.03), (nz - 1, nz - 2, 1, 0.97)):
+        fstar = np.empty_like(f[dc][:, zf])
+        for i in range(19):                                # f*_i(x) travelled to x + e_i
+            fstar[i] = np.roll(g[dc][i], (-E[i][2], -E[i][1], -E[i][0]), (0, 1, 2))[zf]
+        feq = f[dc][:, zf] - tau * (f[dc][:, zf] - fstar)
+        rho_f = f[dc][:, zf].sum(0)
+        assert np.abs(feq.sum(0) - rho_f).max() < 1e-14    # it is an equilibrium of that density
+        want = (rho_b / rho_f) * feq + f[dc][:, zf] - feq
+        assert np.abs(f[dc][:, zb] - want).max() < 1e-14
