@@ -477,3 +477,47 @@ def test_get_macroscopic_validates_output_arrays():
         with pytest.raises(ValueError):
             g.get_macroscopic(fields=("rhoA",), out={"rhoA": bad})
     g.close()
+
+
+def test_neem_extrapolates_the_collision_operators_nonequilibrium_part_on_gpu():
+    """The oracle pin of reading R12 iii (tests/test_oracle_neem.py), through the C ABI in fp64: on
+    a force-free state with different component momenta, the plane populations NEEM writes equal
+    (rho_b / rho(x_f)) f^eq(x_f) + f(x_f) - f^eq(x_f) with f^eq read off the library's own collision
+    step of a z-periodic copy: f^eq = f - tau (f - f*)."""
+    W = np.array([1 / 3] + [1 / 18] * 6 + [1 / 36] * 12)
+    E = np.array([(0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1),
+                  (1, 1, 0), (-1, 1, 0), (1, -1, 0), (-1, -1, 0), (1, 0, 1), (-1, 0, 1), (1, 0, -1),
+                  (-1, 0, -1), (0, 1, 1), (0, -1, 1), (0, 1, -1), (0, -1, -1)])
+    shape = (8, 4, 5)
+    nz, tau = shape[0], 0.8
+    mask = np.zeros(shape, np.uint8)
+    rng = np.random.Generator(np.random.PCG64(12))
+    f0 = []
+    for s in range(2):
+        rho = rng.uniform(0.3, 1.0, shape)
+        f0.append(np.stack([W[i] * rho * (1.0 + 0.2 * rng.uniform(-1, 1, shape)) for i in range(19)]))
+    f0[0] = f0[0] * (1.0 + 0.05 * E[:, 2].reshape(19, 1, 1, 1))
+    f0[1] = f0[1] * (1.0 - 0.05 * E[:, 0].reshape(19, 1, 1, 1))
+    p = default_params(G=0.0, tau=(tau, tau), xi=0.0, z_open=1, inlet_kind=1, inlet_comp=0,
+                       inlet_rho=1.03, outlet_kind=1, outlet_comp=1, outlet_rho=0.97,
+                       storage_bits=64)
+    g = Lbm(mask, p)
+    for s in range(2):
+        g.set_populations(s, f0[s])
+    g.step(1)
+    f = [g.get_populations(s) for s in range(2)]
+    g.close()
+    q = Lbm(mask, dict(p, z_open=0))
+    for s in range(2):
+        q.set_populations(s, f[s])
+    q.step(1)
+    h = [q.get_populations(s) for s in range(2)]
+    q.close()
+    for zb, zf, dc, rho_b in ((0, 1, 0, 1.03), (nz - 1, nz - 2, 1, 0.97)):
+        fstar = np.empty_like(f[dc][:, zf])
+        for i in range(19):
+            fstar[i] = np.roll(h[dc][i], (-E[i][2], -E[i][1], -E[i][0]), (0, 1, 2))[zf]
+        feq = f[dc][:, zf] - tau * (f[dc][:, zf] - fstar)
+        rho_f = f[dc][:, zf].sum(0)
+        want = (rho_b / rho_f) * feq + f[dc][:, zf] - feq
+        assert np.abs(f[dc][:, zb] - want).max() < 1e-14
