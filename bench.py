@@ -52,6 +52,8 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
                     help="lbm_options field, e.g. --opt index=bits --opt graph=0 (repeatable)")
+    ap.add_argument("--clock-interval-ms", type=float, default=2.0,
+                    help="NVML sampling period of clocks and throttle reasons during the timed region")
     ap.add_argument("--no-single", action="store_true",
                     help="sharded run: skip the unsharded reference timing on rank 0")
     ap.add_argument("--shard", default=None, choices=["replicas", "slab"],
@@ -116,8 +118,9 @@ def time_oracle(cfg, steps, warmup, budget_s=15.0):
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
-    def __init__(self, index):
+    def __init__(self, index, interval=0.002):
         super().__init__(daemon=True)
+        self.interval = interval   # a 20-step timed region is 7 ms: sample every 2 ms
         self.index, self.stop_flag, self.samples, self.reasons, self.max_mhz = index, False, [], set(), None
         try:
             import pynvml
@@ -146,7 +149,7 @@ class ClockSampler(threading.Thread):
                         self.reasons.add(name)
             except Exception:
                 pass
-            time.sleep(0.001)   # a 20-step timed region is 7 ms: sample every millisecond or so
+            time.sleep(self.interval)
 
     def result(self):
         s = sorted(self.samples)
@@ -248,7 +251,7 @@ def run_ours(args):
     # ---- device-resident throughput: W warm-up steps, then exactly K steps between events
     sim.step(W)
     barrier()
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(local, args.clock_interval_ms * 1e-3)
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
@@ -381,7 +384,7 @@ def run_slab(args):
     sim.step(W)
     barrier()
     one.set_profiling(False)             # restarts the launch counter
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(local, args.clock_interval_ms * 1e-3)
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
