@@ -51,7 +51,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
-                    help="lbm_options field, e.g. --opt index=bits --opt graph=0 (repeatable)")
+                    help="lbm_options field, e.g. --opt graph=0 --opt keep_psi_mb=0 (repeatable)")
     ap.add_argument("--clock-interval-ms", type=float, default=2.0,
                     help="NVML sampling period of clocks and throttle reasons during the timed region")
     ap.add_argument("--no-single", action="store_true",

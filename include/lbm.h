@@ -69,14 +69,7 @@ typedef struct {
 /* Execution options (plain data, copied by lbm_create_opt; every combination computes the same
  * numbers bit for bit -- tests/test_gpu_parity.py -- they select how the step is scheduled).
  * lbm_options_default fills in the defaults; lbm_create uses them. */
-enum { LBM_INDEX_16 = 0, LBM_INDEX_BITS = 1 };
 typedef struct {
-  int index;        /* neighbour index of the fused pass: LBM_INDEX_16 (default) 16-bit tile-relative
-                       rows, 37 B per node; LBM_INDEX_BITS per-row bitmasks + prefix ids, 0.5 B per
-                       voxel + 4 B per node and per wall solid; also replaces the virtual-solid pass's
-                       72 B gather lists, and the 16-bit rows are not built (low-memory option: index
-                       memory 140 -> 85 B per node on the 256^3 rock, what remains being the int32
-                       rows the getters read; step ~5 % slower)                                     */
   int graph;        /* -1 (default) replay a captured CUDA graph of 16 steps on boxes of
                        <= 600 000 fluid nodes, 0 never, 1 always                                    */
   int pdl;          /* 1 (default) programmatic dependent launch of the three passes    */
@@ -99,11 +92,10 @@ int lbm_create_opt(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int nz,
 /* Synchronises the device (kernels of the context may be in flight on any stream it was used
  * from), then releases everything.  NULL is allowed. */
 void lbm_destroy(lbm_ctx* c);
-/* What lbm_create chose: info[0] index form (LBM_INDEX_16 / LBM_INDEX_BITS; a box edge above
- * 1024 falls back to LBM_INDEX_16), [1] 1 if lbm_step replays CUDA graphs, [2] pdl, [3] reverse,
- * [4] share of the psi lines stored with evict_last priority, in 1/1000, [5] tiles that read the
- * int32 index rows instead of the 16-bit ones, [6] 1 if the virtual-solid pass reads the geometric
- * index, [7] reserved (0). */
+/* What lbm_create chose: info[1] 1 if lbm_step replays CUDA graphs, [2] pdl, [3] reverse,
+ * [4] share of the psi lines stored with evict_last priority, in 1/1000, [5] tiles that read
+ * int32 ids from the compact wide-tile table instead of the 16-bit rows; [0], [6], [7] reserved
+ * (0). */
 int lbm_step_info(lbm_ctx* c, int info[8]);
 
 /* f_i^sigma = w_i * rho_sigma (reading R11); dense double arrays of nx*ny*nz.  Also records the

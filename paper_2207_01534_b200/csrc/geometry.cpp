@@ -169,46 +169,22 @@ int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Ind
       wide += is_wide ? 1 : 0;
     }
     out.wide_tiles = wide;
-  } catch (const std::bad_alloc&) {
-    return -4;
-  }
-  return 0;
-}
-
-int build_bitindex(const Geometry& g, long long psi_wall_base, BitIndex& out,
-                   bool with_fluid_coord) {
-  if (g.nf <= 0 || g.vox2id.empty()) return -1;
-  if (g.nx > 1024 || g.ny > 1024 || g.nz > 1024) return -1;
-  const int nx = g.nx, W = (nx + 31) / 32;
-  const long long rows = (long long)g.ny * g.nz, nf = g.nf;
-  try {
-    out.words = W;
-    out.rec.assign((size_t)rows * W * 4, 0);
-    out.coord.assign(with_fluid_coord ? (size_t)nf : 0, 0);
-    out.wall_coord.assign((size_t)g.nw, 0);
-#pragma omp parallel for schedule(static)
-    for (long long r = 0; r < rows; ++r) {
-      const int32_t* id = &g.vox2id[(size_t)r * nx];
-      uint32_t* rec = &out.rec[(size_t)r * W * 4];
-      // first fluid id / wall psi index at or after each word: walk the row backwards
-      long long next_f = 0, next_w = 0;
-      for (int w = W - 1; w >= 0; --w) {
-        uint32_t fm = 0, wm = 0;
-        for (int b = std::min(31, nx - 1 - 32 * w); b >= 0; --b) {
-          const int32_t v = id[32 * w + b];
-          if (v < 0) continue;
-          if (v < nf) { fm |= 1u << b; next_f = v; }
-          else { wm |= 1u << b; next_w = psi_wall_base + (v - nf); }
+    // compact int32 table of the wide tiles (everything else is served by the 16-bit rows)
+    out.wide_rows.assign((size_t)wide * 18 * kIdxTile, 0);
+    long long pos = 0;
+    for (int t = 0; t < ntf; ++t) {
+      int32_t* m = &out.meta[(size_t)t * kIdxMeta];
+      if (!m[36]) continue;
+      m[37] = (int32_t)pos;
+      const long long n0 = (long long)t * kIdxTile, n1 = std::min<long long>(nf, n0 + kIdxTile);
+      for (int i = 0; i < 18; ++i)
+        for (long long n = n0; n < n1; ++n) {
+          const int32_t raw = g.nbr[(size_t)i * nf + n];
+          int32_t id = raw < 0 ? -raw - 1 : raw;
+          if (id >= nf) id = (int32_t)(psi_wall_base + (id - nf));
+          out.wide_rows[((size_t)pos * 18 + i) * kIdxTile + (n - n0)] = raw < 0 ? -id - 1 : id;
         }
-        rec[4 * w] = fm; rec[4 * w + 1] = wm;
-        rec[4 * w + 2] = (uint32_t)next_f; rec[4 * w + 3] = (uint32_t)next_w;
-      }
-      const int y = (int)(r % g.ny), z = (int)(r / g.ny);
-      for (int x = 0; x < nx; ++x) {
-        const uint32_t c = (uint32_t)x | ((uint32_t)y << 10) | ((uint32_t)z << 20);
-        if (id[x] >= nf) out.wall_coord[id[x] - nf] = c;
-        else if (id[x] >= 0 && with_fluid_coord) out.coord[id[x]] = c;
-      }
+      ++pos;
     }
   } catch (const std::bad_alloc&) {
     return -4;

@@ -47,34 +47,18 @@ struct Geometry {
 // meta[t][36] = 1 marks a "wide" tile (some offset range does not fit 15 bits, e.g. a periodic
 // wrap inside the tile): the kernel then reads the tile's int32 rows instead.
 constexpr int kIdxTile = 128;
-constexpr int kIdxMeta = 40;  // ints per tile: 18 fluid bases, 18 wall bases, wide flag, 3 pad
+constexpr int kIdxMeta = 40;  // ints per tile: 18 fluid bases, 18 wall bases, wide flag, wide-table position, 2 pad
 struct Index16 {
   std::vector<uint16_t> nbr16;  // [18][stride]
   std::vector<int32_t> meta;    // [ntf][kIdxMeta]
+  std::vector<int32_t> wide_rows;  // [wide_tiles][18][kIdxTile]: the int32 ids (psi indices, open-plane
+                                   // sign included) of the wide tiles only; meta[t][37] = a wide
+                                   // tile's position in this table
   size_t stride = 0;
   long long wide_tiles = 0;
 };
 // psi_wall_base = psi index of wall solid 0 (npad); stride = row stride of nbr16 (>= ntf*kIdxTile)
 int build_index16(const Geometry& g, long long psi_wall_base, size_t stride, Index16& out);
-
-// Geometric ("bitmask") form of the neighbour index: nothing is stored per (node, direction).
-// Per x-row (y, z) and per 32-voxel word w of the row one 16-byte record
-//   { fluid bitmask, wall-solid bitmask, id of the first fluid node at or after the word,
-//     psi index of the first wall solid at or after the word }
-// (ids inside a row are consecutive in both numberings), plus 4 B of packed coordinates per fluid
-// node (x | y << 10 | z << 20).  The neighbour (x', y', z') of a node is then
-//   fluid:  rec.fid0 + popc(rec.fmask & below(x'))     wall solid:  rec.wid0 + popc(rec.wmask & below(x'))
-// 0.5 B per voxel of table (cache-resident: 8 MB for 256^3) + 4 B per node instead of 36 B per node.
-struct BitIndex {
-  int words = 0;                    // 32-voxel words per row
-  std::vector<uint32_t> rec;        // [nz*ny][words][4]
-  std::vector<uint32_t> coord;      // [nf]  x | y << 10 | z << 20 of fluid node n
-  std::vector<uint32_t> wall_coord; // [nw]  the same of wall solid w (the wall pass's whole index)
-};
-// psi_wall_base = psi index of wall solid 0.  -1 if a box edge exceeds 1024.
-// with_fluid_coord = false: coord stays empty (only the wall pass reads the index)
-int build_bitindex(const Geometry& g, long long psi_wall_base, BitIndex& out,
-                   bool with_fluid_coord = true);
 
 // Returns 0, or -1 bad arguments, -2 no fluid voxel, -3 solid on an open plane or its interior
 // neighbour plane (z in {0,1,nz-2,nz-1}), -4 out of memory.  `with_tables` = also fill nbr,

@@ -173,89 +173,6 @@ __global__ void __launch_bounds__(256) k_wallpsi(Vec2<T>* __restrict__ psi,
   store_vec2(psi + wall_base + w, o, l2_keep_policy(keep_psi));
 }
 
-// direction index of (dx, dy, dz), or -1 if that offset is not a D3Q19 direction
-__host__ __device__ constexpr int dir_of(int dx, int dy, int dz) {
-  for (int i = 0; i < Q; ++i)
-    if (ex(i) == dx && ey(i) == dy && ez(i) == dz) return i;
-  return -1;
-}
-
-// a2 with the geometric index (geometry.hpp BitIndex) instead of the 72 B gather list per wall
-// solid: 4 B of packed coordinates per wall solid; the fluid neighbours' ids come from the per-row
-// records {fluid bitmask, wall bitmask, id of the first fluid node of the word, ...} -- id =
-// first id + popcount of the mask below x' -- which are 0.5 B per voxel and cache-resident
-// (consecutive wall solids share their 9 rows).  All of that is static and runs BEFORE the
-// dependency wait, beside the draining density pass.  z wraps periodically: a wall solid is never
-// within two planes of an open plane, and at a slab's cut ends the outermost halo plane's values
-// are never read (as with the lists).  Same sums in the same order as k_wallpsi: bit-identical.
-template <typename T>
-__global__ void __launch_bounds__(256, 8) k_wallpsi_bits(Vec2<T>* __restrict__ psi,
-                                                      const uint32_t* __restrict__ wall_coord,
-                                                      const uint4* __restrict__ bits,
-                                                      const T* __restrict__ inv_den,
-                                                      size_t wall_base, int nw, int nx, int ny,
-                                                      int nz, int words, T chiA, T chiB,
-                                                      float keep_psi) {
-  const int w = blockIdx.x * blockDim.x + threadIdx.x;
-  const bool live = w < nw;
-  const uint32_t cw = live ? wall_coord[w] : 0u;
-  const int x = (int)(cw & 1023u), y = (int)((cw >> 10) & 1023u), z = (int)(cw >> 20);
-  int word[3];
-  uint32_t bit[3], below[3];
-#pragma unroll
-  for (int d = 0; d < 3; ++d) {  // ex = d - 1, periodic in x
-    int xx = x + d - 1;
-    xx = xx < 0 ? nx - 1 : (xx == nx ? 0 : xx);
-    word[d] = xx >> 5;
-    bit[d] = (uint32_t)xx & 31u;
-    below[d] = (1u << bit[d]) - 1u;
-  }
-  int id[Q];
-#pragma unroll
-  for (int dz = -1; dz <= 1; ++dz) {
-    int zz = z + dz;
-    zz = zz < 0 ? nz - 1 : (zz == nz ? 0 : zz);
-#pragma unroll
-    for (int dy = -1; dy <= 1; ++dy) {
-      int yy = y + dy;
-      yy = yy < 0 ? ny - 1 : (yy == ny ? 0 : yy);
-      const uint4* row = bits + (size_t)(zz * ny + yy) * words;
-      // the three x-neighbours of a row almost always lie in one 32-voxel word
-      const bool need_m = dir_of(-1, dy, dz) > 0, need_c = dir_of(0, dy, dz) > 0,
-                 need_p = dir_of(1, dy, dz) > 0;
-      uint4 qc = __ldg(row + word[1]);
-      if (need_m) {
-        const uint4 q = word[0] == word[1] ? qc : __ldg(row + word[0]);
-        id[dir_of(-1, dy, dz) > 0 ? dir_of(-1, dy, dz) : 0] =
-            (live && ((q.x >> bit[0]) & 1u)) ? (int)(q.z + __popc(q.x & below[0])) : -1;
-      }
-      if (need_c)
-        id[dir_of(0, dy, dz) > 0 ? dir_of(0, dy, dz) : 0] =
-            (live && ((qc.x >> bit[1]) & 1u)) ? (int)(qc.z + __popc(qc.x & below[1])) : -1;
-      if (need_p) {
-        const uint4 q = word[2] == word[1] ? qc : __ldg(row + word[2]);
-        id[dir_of(1, dy, dz) > 0 ? dir_of(1, dy, dz) : 0] =
-            (live && ((q.x >> bit[2]) & 1u)) ? (int)(q.z + __popc(q.x & below[2])) : -1;
-      }
-    }
-  }
-  const T s = live ? inv_den[w] : T(0);
-  pdl_wait();     // everything above is static; psi comes from the density pass
-  pdl_trigger();  // as k_wallpsi: the fused pass may stage its first tiles beside this kernel
-  if (!live) return;
-  T na = T(0), nb = T(0);
-#pragma unroll
-  for (int i = 1; i < Q; ++i) {
-    if (id[i] >= 0) {
-      const Vec2<T> p = psi[id[i]];
-      na = fma_rn(wgt<T>(i), p.a, na);
-      nb = fma_rn(wgt<T>(i), p.b, nb);
-    }
-  }
-  Vec2<T> o; o.a = mul_rn(mul_rn(chiA, na), s); o.b = mul_rn(mul_rn(chiB, nb), s);
-  store_vec2(psi + wall_base + w, o, l2_keep_policy(keep_psi));
-}
-
 // ---------------------------------------------------------------------------------------------
 // Per-node mixture quantities shared by the collide kernel and the macroscopic getter.
 // a3: F_sigma = -G rho_sigma sum_i w_i Psi_sigmabar(x+e_i) e_i + rho_sigma g
@@ -616,10 +533,6 @@ struct Idx16 {
   int reverse;            // 1: CTA b takes tile gridDim-1-b
   int nact;               // nodes this pass updates: ids [0,nact).  = nf, except in slab mode, where
                           // the halo nodes [nact,nf) only receive pushes
-  // IDX = 2 (geometric index, geometry.hpp BitIndex): per-row-word records and packed coordinates
-  const uint4* bits;        // [nz*ny][words] {fluid mask, wall mask, first fluid id, first wall psi index}
-  const uint32_t* coord;    // [npad] x | y << 10 | z << 20
-  int nx, ny, nz, words;
   int tile0, split, tile1;  // tiles of this launch: position b < split -> tile0 + b, else
                             // tile1 + (b - split)  (whole pass: 0, grid, 0; slab mode: the boundary
                             // tiles of both faces in one launch, the interior in another)
@@ -677,7 +590,8 @@ __device__ __forceinline__ void stage_tile16(const TileSmem<T, TN, ALIAS> sm,
 // After the staged tile has arrived: decode this thread's column of the 16-bit rows into the
 // int32 form the tile function reads.  A neighbour beyond an open plane (reading R12 iv) is
 // recognised from the node's plane and e_z.  Rare "wide" tiles (an offset range does not fit 15
-// bits) take the int32 rows with a second round of bulk copies (one more phase of `bar`).
+// bits) take int32 ids from the compact wide-tile table with a second round of bulk copies (one
+// more phase of `bar`).
 // Called by every thread of the CTA.
 template <typename T, int TN, bool ALIAS>
 __device__ __forceinline__ void decode_tile16(const TileSmem<T, TN, ALIAS> sm,
@@ -690,8 +604,9 @@ __device__ __forceinline__ void decode_tile16(const TileSmem<T, TN, ALIAS> sm,
       if (elect_one()) {
         mbar_expect_tx(bar, (uint32_t)((size_t)18 * TN * sizeof(int)));
 #pragma unroll
-        for (int r = 0; r < 18; ++r)
-          bulk_g2s(sm.sid + (size_t)r * TN, nbr + (size_t)r * npad + t0, TN * sizeof(int), bar);
+        for (int r = 0; r < 18; ++r)   // nbr = the compact table of the wide tiles, [pos][18][TN]
+          bulk_g2s(sm.sid + (size_t)r * TN, nbr + ((size_t)sm.smeta[37] * 18 + r) * TN,
+                   TN * sizeof(int), bar);
       }
       __syncwarp();
     }
@@ -717,15 +632,16 @@ __device__ __forceinline__ void decode_tile16(const TileSmem<T, TN, ALIAS> sm,
 }
 
 // The fused pass (a3-a6): one CTA per tile.
-// IDX: 1 = 16-bit tile-relative rows (default), 2 = geometric (bitmask) index (low-memory option)
+// IDX: index form; 1 = 16-bit tile-relative rows (the only one left: the geometric index, 2, and
+// 8-bit rows were measured slower and removed)
 template <typename T, int TN, int MINB, bool REMAINDER, int IDX>
 __global__ void __launch_bounds__(TN, MINB)
     k_collide_stream_bulk(const T* __restrict__ fin, T* __restrict__ fout,
                           const Vec2<T>* __restrict__ psi, const int* __restrict__ nbr, int nf,
                           size_t npad, Consts<T> c, Idx16 ix) {
-  static_assert(IDX == 1 || IDX == 2, "index form");
+  static_assert(IDX == 1, "index form");
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  constexpr bool kAlias = IDX == 1 && MINB >= 7;
+  constexpr bool kAlias = MINB >= 7;
   const TileSmem<T, TN, kAlias> sm(smem_raw);
   __shared__ uint64_t bar;
   const int tid = threadIdx.x;
@@ -740,70 +656,14 @@ __global__ void __launch_bounds__(TN, MINB)
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // compiler-visible warp-uniform value
   const int n = (int)t0 + tid;
   uint32_t phase = 0;
-  if constexpr (IDX == 2) {
-    if (warp == 0) {
-      if (elect_one()) {
-        mbar_expect_tx(&bar, (uint32_t)((size_t)2 * Q * TN * sizeof(T)));
-#pragma unroll
-        for (int r = 0; r < Q; ++r)  // one row of TN (A, B) pairs per direction
-          bulk_g2s(sm.sf + (size_t)r * TN * 2, fin + ((size_t)r * npad + t0) * 2,
-                   2 * TN * sizeof(T), &bar);
-      }
-      __syncwarp();
-    }
-    // Neighbour ids from the geometry while the populations arrive: nothing below depends on the
-    // previous kernels (static tables), so it runs before the dependency wait.
-    {
-      const uint32_t cw = ix.coord[n];  // coord is npad long, zero beyond nf
-      const int x = (int)(cw & 1023u), y = (int)((cw >> 10) & 1023u), z = (int)(cw >> 20);
-      int word[3];
-      uint32_t below[3], bit[3];
-#pragma unroll
-      for (int d = 0; d < 3; ++d) {  // ex = d - 1, periodic in x
-        int xx = x + d - 1;
-        xx = xx < 0 ? ix.nx - 1 : (xx == ix.nx ? 0 : xx);
-        word[d] = xx >> 5;
-        bit[d] = (uint32_t)xx & 31u;
-        below[d] = (1u << bit[d]) - 1u;
-      }
-      int yy[3], zz[3];
-      bool beyond[3];
-#pragma unroll
-      for (int d = 0; d < 3; ++d) {
-        int v = y + d - 1;
-        yy[d] = v < 0 ? ix.ny - 1 : (v == ix.ny ? 0 : v);
-        int w = z + d - 1;
-        beyond[d] = false;
-        if (w < 0) {
-          if (ix.np_lo) { beyond[d] = true; w = z + 1; } else w = ix.nz - 1;  // mirror (R12 iv) | wrap
-        } else if (w == ix.nz) {
-          if (ix.np_hi) { beyond[d] = true; w = z - 1; } else w = 0;
-        }
-        zz[d] = w;
-      }
-#pragma unroll
-      for (int i = 1; i < Q; ++i) {
-        const int dx = ex(i) + 1, dy = ey(i) + 1, dz = ez(i) + 1;
-        const uint4 q = __ldg(ix.bits + ((size_t)(zz[dz] * ix.ny + yy[dy]) * ix.words + word[dx]));
-        const bool fl = (q.x >> bit[dx]) & 1u;
-        int k = fl ? (int)(q.z + __popc(q.x & below[dx])) : (int)(q.w + __popc(q.y & below[dx]));
-        if (ez(i) != 0 && beyond[dz]) k = -k - 1;
-        sm.sid[(i - 1) * TN + tid] = k;
-      }
-    }
-    pdl_wait();
-    mbar_wait(&bar, phase);
-    phase ^= 1u;
-  } else {
-    if (warp == 0) stage_tile16<T, TN, kAlias>(sm, fin, ix, npad, tile, &bar);
-    // the bulk copies above read the populations (complete since the previous step; the density
-    // pass that fixed the open planes finished before the wall pass began) and the static index;
-    // psi and the wall psi are this step's
-    pdl_wait();
-    mbar_wait(&bar, phase);
-    phase ^= 1u;
-    decode_tile16<T, TN, kAlias>(sm, nbr, ix, npad, t0, n, tid, warp, &bar, phase);
-  }
+  if (warp == 0) stage_tile16<T, TN, kAlias>(sm, fin, ix, npad, tile, &bar);
+  // the bulk copies above read the populations (complete since the previous step; the density
+  // pass that fixed the open planes finished before the wall pass began) and the static index;
+  // psi and the wall psi are this step's
+  pdl_wait();
+  mbar_wait(&bar, phase);
+  phase ^= 1u;
+  decode_tile16<T, TN, kAlias>(sm, nbr, ix, npad, t0, n, tid, warp, &bar, phase);
   collide_tile_thread<T, TN, REMAINDER>(sm.sf, sm.sid, tid, n, n < ix.nact, fout, psi, nf, npad, c);
 }
 
@@ -1065,12 +925,31 @@ __global__ void k_compact_to_dense(const T* __restrict__ row, const int* __restr
   if (n < nf) dense[node_vox[n]] = (double)row[(size_t)n * stride];
 }
 
+// Neighbour ids for the kernels outside the time step (macroscopic getter, connected components):
+// decoded from the 16-bit rows exactly as the fused pass does, wide tiles from the compact table.
+struct NbrView {
+  const uint16_t* nbr16;    // [18][npad]
+  const int* meta;          // [tiles][kIdxMeta]
+  const int* wide;          // [wide tiles][18][128]
+  int np_lo, np_hi, nact;   // open planes, as in Idx16
+};
+// psi index of x+e_i for node n, i = 1..18 (negative: -(mirror id + 1) beyond an open plane)
+__device__ __forceinline__ int nbr_id(const NbrView& v, size_t npad, int n, int i) {
+  const int* m = v.meta + (size_t)(n >> 7) * kIdxMeta;
+  if (m[36]) return v.wide[((size_t)m[37] * 18 + (i - 1)) * 128 + (n & 127)];
+  const int e = v.nbr16[(size_t)(i - 1) * npad + n];
+  int k = m[(e >> 15) * 18 + (i - 1)] + (e & 0x7fff);
+  if (ez(i) < 0 && n < v.np_lo) k = -k - 1;
+  if (ez(i) > 0 && n >= v.nact - v.np_hi) k = -k - 1;
+  return k;
+}
+
 // rho_sigma, u = u_eq, P = (rho_A+rho_B)/3 + (G/3) rho_A rho_B (Eq. 12, R13) into
 // compact double rows out[q][nf], q = rhoA, rhoB, ux, uy, uz, P.  Needs psi of the current state.
 template <typename T>
 __global__ void __launch_bounds__(256) k_macroscopic(const T* __restrict__ fin,
                                                      const Vec2<T>* __restrict__ psi,
-                                                     const int* __restrict__ nbr,
+                                                     NbrView nv,
                                                      double* __restrict__ out, int nf, size_t npad,
                                                      Consts<T> c) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
@@ -1078,7 +957,7 @@ __global__ void __launch_bounds__(256) k_macroscopic(const T* __restrict__ fin,
   int id[Q];
   id[0] = n;
 #pragma unroll
-  for (int i = 1; i < Q; ++i) id[i] = nbr[(size_t)(i - 1) * npad + n];
+  for (int i = 1; i < Q; ++i) id[i] = nbr_id(nv, npad, n, i);
   T fa[Q], fb[Q];
 #pragma unroll
   for (int i = 0; i < Q; ++i) {
@@ -1208,14 +1087,13 @@ __device__ __forceinline__ void ccl_unite(int* parent, int a, int b) {
 // one thread per fluid node: joins it to its +x, +y, +z neighbour of the same phase (each edge of
 // the graph is the forward edge of exactly one of its ends; the periodic wrap in z is the one
 // forward neighbour with a smaller id, and a neighbour beyond an open plane is negative)
-__global__ void __launch_bounds__(256) k_ccl_unite(const int* __restrict__ nbr, int nf, size_t npad,
-                                                   int* parent) {
+__global__ void __launch_bounds__(256) k_ccl_unite(NbrView nv, int nf, size_t npad, int* parent) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
   if (n >= nf || __ldcg(parent + n) < 0) return;
 #pragma unroll
   for (int i = 1; i <= 5; i += 2) {
     static_assert(ex(1) == 1 && ey(3) == 1 && ez(5) == 1, "forward axis directions");
-    const int m = nbr[(size_t)(i - 1) * npad + n];
+    const int m = nbr_id(nv, npad, n, i);
     if (m < 0 || m >= nf || (i == 5 && m <= n)) continue;
     if (__ldcg(parent + m) < 0) continue;
     ccl_unite(parent, n, m);

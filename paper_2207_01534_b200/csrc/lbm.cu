@@ -93,7 +93,7 @@ struct lbm_ctx {
   std::vector<int32_t> zstart;  // [nz+1] first fluid id of every z-plane (host copy, used by queries)
   void* f[2] = {nullptr, nullptr};                // two buffers of [19][npad][2 comps] T
   void* psi = nullptr;                            // [nf+nw] Vec2<T>
-  int* nbr = nullptr;                             // [18][npad]
+  int* nbr_wide = nullptr;                        // [wide tiles][18][128] int32 ids of the wide tiles
   int* wall_nbr = nullptr;                        // [18][nwpad]
   void* wall_inv_den = nullptr;                   // [nw] T
   int* node_vox_d = nullptr;                      // [nf]
@@ -105,15 +105,6 @@ struct lbm_ctx {
   bool open_pending = false;  // the open-plane fix of the last step has not been applied yet (it
                               // is folded into the next density pass, or applied by a getter)
   int num_sms = 148;
-  int idx16 = 1;            // index the fused pass reads: 1 = 16-bit tile-relative rows (default),
-                            // 2 = geometric bitmask index (lbm_options.index = LBM_INDEX_BITS;
-                            // geometry.hpp BitIndex)
-  uint32_t* bit_rec = nullptr;       // [nz*ny][bit_words][4]
-  uint32_t* bit_coord = nullptr;     // [npad]  (only with the geometric index of the fused pass)
-  uint32_t* wall_coord = nullptr;    // [nw]    packed coordinates of the wall solids
-  int wall_bits = 0;        // 1: the wall pass reads the geometric index (k_wallpsi_bits; with
-                            // LBM_INDEX_BITS), 0: the int32 gather lists
-  int bit_words = 0;
   uint16_t* nbr16 = nullptr;         // [18][npad]
   int* nbr16_meta = nullptr;         // [tiles][kIdxMeta]
   long long wide_tiles = 0;
@@ -163,14 +154,14 @@ struct lbm_ctx {
     if (comm_stream) cudaStreamDestroy(comm_stream);
     for (auto& e : comm_ev) if (e) cudaEventDestroy(e);
     for (auto& e : prof_events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
-    lbm_shim_free(f[0]); lbm_shim_free(f[1]); lbm_shim_free(psi); lbm_shim_free(nbr);
+    lbm_shim_free(f[0]); lbm_shim_free(f[1]); lbm_shim_free(psi);
+    lbm_shim_free(nbr_wide);
     lbm_shim_free(wall_nbr); lbm_shim_free(wall_inv_den); lbm_shim_free(node_vox_d);
     lbm_shim_free(frozen); lbm_shim_free(partial); lbm_shim_free(diag_out);
     lbm_shim_free(nbr16);
     lbm_shim_free(nbr16_meta);
     lbm_shim_free(halo_slots); lbm_shim_free(halo_send); lbm_shim_free(halo_recv);
     lbm_shim_free(ccl);
-    lbm_shim_free(bit_rec); lbm_shim_free(bit_coord); lbm_shim_free(wall_coord);
   }
 };
 
@@ -198,6 +189,17 @@ OpenPlane<T> make_open(const lbm_params& p, const int (&open_end)[2]) {
   o.rho[0] = (T)p.inlet_rho; o.rho[1] = (T)p.outlet_rho;
   o.uz[0] = (T)p.inlet_uz; o.uz[1] = (T)0;
   return o;
+}
+
+NbrView make_view(const lbm_ctx* c) {
+  NbrView v;
+  v.nbr16 = (const uint16_t*)c->nbr16;
+  v.meta = c->nbr16_meta;
+  v.wide = c->nbr_wide;
+  v.np_lo = c->open_end[0] ? c->np : 0;
+  v.np_hi = c->open_end[1] ? c->np : 0;
+  v.nact = c->nact;
+  return v;
 }
 
 cudaStream_t cur_stream() { return (cudaStream_t)lbm_shim_stream(); }
@@ -302,15 +304,9 @@ void launch_wall(lbm_ctx* c, cudaStream_t st) {
   if (c->nw <= 0) return;
   const bool pdl = c->pdl && !c->prof;
   Timed t(c, st, 1);
-  if (c->wall_bits)
-    launch_k(pdl, k_wallpsi_bits<T>, blocks(c->nw, 256), 256, 0, st, (Vec2<T>*)c->psi,
-             (const uint32_t*)c->wall_coord, (const uint4*)c->bit_rec, (const T*)c->wall_inv_den,
-             c->npad, c->nw, c->nx, c->ny, c->nz, c->bit_words, (T)(1.0 + c->p.xi),
-             (T)(1.0 - c->p.xi), c->keep_psi);
-  else
-    launch_k(pdl, k_wallpsi<T>, blocks(c->nw, 256), 256, 0, st, (Vec2<T>*)c->psi,
-             (const int*)c->wall_nbr, (const T*)c->wall_inv_den, c->npad, c->nw, c->nwpad,
-             (T)(1.0 + c->p.xi), (T)(1.0 - c->p.xi), c->keep_psi);
+  launch_k(pdl, k_wallpsi<T>, blocks(c->nw, 256), 256, 0, st, (Vec2<T>*)c->psi,
+           (const int*)c->wall_nbr, (const T*)c->wall_inv_den, c->npad, c->nw, c->nwpad,
+           (T)(1.0 + c->p.xi), (T)(1.0 - c->p.xi), c->keep_psi);
 }
 
 // a1 + a2.  Slab mode: the density pass (lbm_slab_density) and the psi halo exchange are the
@@ -353,9 +349,6 @@ void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
   ix.np_hi = c->open_end[1] ? c->np : 0;
   ix.reverse = c->reverse;
   ix.nact = c->nact;
-  ix.bits = (const uint4*)c->bit_rec;
-  ix.coord = c->bit_coord;
-  ix.nx = c->nx; ix.ny = c->ny; ix.nz = c->nz; ix.words = c->bit_words;
   static_assert(TN == 128 || TN == 256, "tile ranges below are in units of 128 ids");
   const int per = TN / 128;                      // slab tile ranges are kept in 128-id tiles
   unsigned grid = blocks(c->nact, TN);
@@ -375,7 +368,7 @@ void launch_bulk(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaStre
   // density pass (which may have rewritten the open planes of fin) is complete and visible.
   launch_k(c->pdl && !c->prof && c->nw > 0, k_collide_stream_bulk<T, TN, MINB, kRemainder, IDX>,
            grid, TN, smem, st, fin, fout, (const Vec2<T>*)c->psi,
-           (const int*)c->nbr, c->nf, c->npad, k, ix);
+           (const int*)c->nbr_wide, c->nf, c->npad, k, ix);
 }
 
 template <typename T>
@@ -384,11 +377,9 @@ void launch_collide(lbm_ctx* c, const T* fin, T* fout, const Consts<T>& k, cudaS
   // fp32: 128-node tiles, 7 CTAs per SM at 72 registers (6 and 8 CTAs, 64- and 256-node tiles were
   // measured slower); fp64 validation build: 2 CTAs per SM
   if constexpr (sizeof(T) == 4) {
-    if (c->idx16 == 2) launch_bulk<T, 128, 7, 2>(c, fin, fout, k, st, part);
-    else launch_bulk<T, 128, 7, 1>(c, fin, fout, k, st, part);
+    launch_bulk<T, 128, 7, 1>(c, fin, fout, k, st, part);
   } else {
-    if (c->idx16 == 2) launch_bulk<T, 128, 2, 2>(c, fin, fout, k, st, part);
-    else launch_bulk<T, 128, 2, 1>(c, fin, fout, k, st, part);
+    launch_bulk<T, 128, 2, 1>(c, fin, fout, k, st, part);
   }
 }
 
@@ -523,7 +514,6 @@ int lbm_build_index(const uint8_t* solid, int nx, int ny, int nz, int z_open, in
 
 void lbm_options_default(lbm_options* o) {
   if (!o) return;
-  o->index = LBM_INDEX_16;
   o->graph = -1;
   o->pdl = 1;
   o->reverse = 1;
@@ -531,8 +521,6 @@ void lbm_options_default(lbm_options* o) {
 }
 
 static int validate_options(const lbm_options* o) {
-  if (o->index != LBM_INDEX_16 && o->index != LBM_INDEX_BITS)
-    return fail(LBM_EINVAL, "options.index must be LBM_INDEX_16 or LBM_INDEX_BITS");
   if (o->graph < -1 || o->graph > 1) return fail(LBM_EINVAL, "options.graph must be -1, 0 or 1");
   if ((o->pdl != 0 && o->pdl != 1) || (o->reverse != 0 && o->reverse != 1))
     return fail(LBM_EINVAL, "options.pdl and options.reverse must be 0 or 1");
@@ -588,7 +576,6 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   c->pdl = o.pdl;
   c->graph_mode = o.graph;
   c->keep_psi_mb = o.keep_psi_mb;
-  c->idx16 = o.index == LBM_INDEX_BITS ? 2 : 1;
   c->npad = pad256(g.nf); c->nwpad = pad64(g.nw);
   // pair-slot indices i * npad + k and psi indices npad + w are 32-bit
   if ((size_t)19 * c->npad >= ((size_t)1 << 31) || c->npad + c->nwpad >= ((size_t)1 << 31)) {
@@ -601,27 +588,19 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   cudaStream_t st = use_stream(c);
   const size_t fbytes = (size_t)2 * 19 * c->npad * c->esz;
   const size_t psibytes = (c->npad + c->nwpad) * 2 * c->esz;  // wall part starts at npad
-  const size_t nbrbytes = (size_t)18 * c->npad * sizeof(int);
-  // LBM_INDEX_BITS (the low-memory option): both the fused pass and the wall pass read the
-  // geometric index; the int32 gather lists of the wall pass are then not allocated
-  lbmgeo::BitIndex bix;  // upload source until the sync below
-  const bool have_bits = c->idx16 == 2 && lbmgeo::build_bitindex(g, (long long)c->npad, bix) == 0;
-  if (!have_bits) c->idx16 = 1;   // a box edge above 1024: the packed coordinates do not fit
-  c->wall_bits = have_bits && g.nw > 0;
-  const size_t wnbrbytes = c->wall_bits ? 0 : (size_t)18 * c->nwpad * sizeof(int);
+  const size_t wnbrbytes = (size_t)18 * c->nwpad * sizeof(int);
   const size_t frozenbytes = p->z_open ? (size_t)2 * 2 * 5 * c->np * c->esz : 0;
   c->diag_blocks = 148 * 8;
   c->f[0] = lbm_shim_alloc(fbytes);
   c->f[1] = lbm_shim_alloc(fbytes);
   c->psi = lbm_shim_alloc(psibytes);
-  c->nbr = (int*)lbm_shim_alloc(nbrbytes);
   c->wall_nbr = (int*)lbm_shim_alloc(wnbrbytes ? wnbrbytes : 4);
   c->wall_inv_den = lbm_shim_alloc(g.nw ? g.nw * c->esz : 4);
   c->node_vox_d = (int*)lbm_shim_alloc(g.nf * sizeof(int));
   c->frozen = lbm_shim_alloc(frozenbytes ? frozenbytes : 4);
   c->partial = (double*)lbm_shim_alloc((size_t)c->diag_blocks * kDiagVals * sizeof(double));
   c->diag_out = (double*)lbm_shim_alloc(8 * sizeof(double));
-  if (!c->f[0] || !c->f[1] || !c->psi || !c->nbr || !c->wall_nbr || !c->wall_inv_den ||
+  if (!c->f[0] || !c->f[1] || !c->psi || !c->wall_nbr || !c->wall_inv_den ||
       !c->node_vox_d || !c->frozen || !c->partial || !c->diag_out) {
     delete c;
     return fail(LBM_ENOMEM, "device allocation failed (populations need %zu bytes per buffer)",
@@ -632,7 +611,7 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   c->keep_psi = c->keep_psi_mb > 0
                     ? (float)std::min(1.0, (double)c->keep_psi_mb * 1048576.0 / (double)psibytes)
                     : 0.f;
-  c->bytes[2] = (long long)(nbrbytes + wnbrbytes + g.nw * c->esz + g.nf * sizeof(int));
+  c->bytes[2] = (long long)(wnbrbytes + g.nw * c->esz + g.nf * sizeof(int));
   c->bytes[3] = (long long)(frozenbytes + c->diag_blocks * kDiagVals * 8 + 64);
   cudaError_t e = cudaSuccess;
   auto up = [&](void* dst, const void* src, size_t bytes) {
@@ -642,26 +621,17 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   if (e == cudaSuccess) e = cudaMemsetAsync(c->f[1], 0, fbytes, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->psi, 0, psibytes, st);
   if (e == cudaSuccess && frozenbytes) e = cudaMemsetAsync(c->frozen, 0, frozenbytes, st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(c->nbr, 0, nbrbytes, st);
-  // Re-base wall ids from nf+w to npad+w so that the wall part of psi starts on a tile boundary.
-  lbmgeo::Index16 i16;   // not built with LBM_INDEX_BITS: the fused pass then never reads it
-  if (c->idx16 != 2) {
+  // (wall ids are stored as psi indices npad + w: the wall part of psi starts on a tile boundary)
+  lbmgeo::Index16 i16;
+  {
     if (lbmgeo::build_index16(g, (long long)c->npad, c->npad, i16) != 0) {
       delete c;
       return fail(LBM_ENOMEM, "index16 build failed");
     }
     c->wide_tiles = i16.wide_tiles;
   }
-  {
-    const int32_t shift = (int32_t)(c->npad - (size_t)g.nf);
-    const int32_t nf32 = (int32_t)g.nf;
-    for (auto& v : g.nbr)
-      if (v >= nf32) v += shift;
-  }
   for (int i = 0; i < 18; ++i) {
-    up(c->nbr + (size_t)i * c->npad, g.nbr.data() + (size_t)i * g.nf, g.nf * sizeof(int));
-    if (!c->wall_bits)
-      up(c->wall_nbr + (size_t)i * c->nwpad, g.wall_nbr.data() + (size_t)i * g.nw,
+    up(c->wall_nbr + (size_t)i * c->nwpad, g.wall_nbr.data() + (size_t)i * g.nw,
          g.nw * sizeof(int));
   }
   up(c->node_vox_d, g.node_vox.data(), g.nf * sizeof(int));
@@ -672,7 +642,7 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
   } else {
     up(c->wall_inv_den, g.wall_inv_den.data(), g.nw * sizeof(double));
   }
-  if (c->idx16 != 2) {
+  {
     c->nbr16 = (uint16_t*)lbm_shim_alloc(i16.nbr16.size() * sizeof(uint16_t));
     c->nbr16_meta = (int*)lbm_shim_alloc(i16.meta.size() * sizeof(int32_t) + 16);
     if (!c->nbr16 || !c->nbr16_meta) {
@@ -682,27 +652,13 @@ static int create_impl(lbm_ctx** out, const uint8_t* solid, int nx, int ny, int 
     up(c->nbr16, i16.nbr16.data(), i16.nbr16.size() * sizeof(uint16_t));
     up(c->nbr16_meta, i16.meta.data(), i16.meta.size() * sizeof(int32_t));
     c->bytes[2] += (long long)(i16.nbr16.size() * 2 + i16.meta.size() * 4);
-  }
-  if (have_bits) {
-    c->bit_words = bix.words;
-    c->bit_rec = (uint32_t*)lbm_shim_alloc(bix.rec.size() * sizeof(uint32_t));
-    if (c->idx16 == 2) c->bit_coord = (uint32_t*)lbm_shim_alloc(c->npad * sizeof(uint32_t));
-    if (c->wall_bits) c->wall_coord = (uint32_t*)lbm_shim_alloc(bix.wall_coord.size() * sizeof(uint32_t));
-    if (!c->bit_rec || (c->idx16 == 2 && !c->bit_coord) || (c->wall_bits && !c->wall_coord)) {
+    c->nbr_wide = (int*)lbm_shim_alloc(i16.wide_rows.size() * sizeof(int32_t) + 16);
+    if (!c->nbr_wide) {
       delete c;
-      return fail(LBM_ENOMEM, "device allocation failed (bit index)");
+      return fail(LBM_ENOMEM, "device allocation failed (wide-tile table)");
     }
-    up(c->bit_rec, bix.rec.data(), bix.rec.size() * sizeof(uint32_t));
-    c->bytes[2] += (long long)(bix.rec.size() * 4);
-    if (c->idx16 == 2) {
-      if (e == cudaSuccess) e = cudaMemsetAsync(c->bit_coord, 0, c->npad * sizeof(uint32_t), st);
-      up(c->bit_coord, bix.coord.data(), bix.coord.size() * sizeof(uint32_t));
-      c->bytes[2] += (long long)(c->npad * 4);
-    }
-    if (c->wall_bits) {
-      up(c->wall_coord, bix.wall_coord.data(), bix.wall_coord.size() * sizeof(uint32_t));
-      c->bytes[2] += (long long)(bix.wall_coord.size() * 4);
-    }
+    up(c->nbr_wide, i16.wide_rows.data(), i16.wide_rows.size() * sizeof(int32_t));
+    c->bytes[2] += (long long)(i16.wide_rows.size() * 4);
   }
   lbmgeo::Halo halo;  // declared here: its lists are upload sources until the sync below
   if (c->slab) {
@@ -818,12 +774,12 @@ int lbm_create_slab_opt(lbm_ctx** out, const uint8_t* solid_local, int nx, int n
 int lbm_step_info(lbm_ctx* c, int info[8]) {
   if (!c || !info) return fail(LBM_EINVAL, "NULL argument");
   const bool graph = c->graph_mode == 1 || (c->graph_mode < 0 && c->nf <= kGraphAutoNodes);
-  info[0] = c->idx16 == 2 ? LBM_INDEX_BITS : LBM_INDEX_16;
+  info[0] = 0;
   info[1] = graph && !c->slab ? 1 : 0;
   info[2] = c->pdl; info[3] = c->reverse;
   info[4] = (int)(c->keep_psi * 1000.f + 0.5f);
   info[5] = (int)std::min<long long>(c->wide_tiles, 2147483647LL);
-  info[6] = c->wall_bits; info[7] = 0;
+  info[6] = 0; info[7] = 0;
   return LBM_OK;
 }
 
@@ -919,7 +875,7 @@ int lbm_slab_ccl_begin(lbm_ctx* c, int comp, int mark_lo, int mark_hi) {
     k_ccl_init<double><<<g, 256, 0, st>>>((const Vec2<double>*)c->psi, na, comp, parent, flag);
   else
     k_ccl_init<float><<<g, 256, 0, st>>>((const Vec2<float>*)c->psi, na, comp, parent, flag);
-  k_ccl_unite<<<g, 256, 0, st>>>(c->nbr, na, c->npad, parent);   // ids >= na (halo) are skipped
+  k_ccl_unite<<<g, 256, 0, st>>>(make_view(c), na, c->npad, parent);   // ids >= na (halo) are skipped
   k_ccl_flatten<<<g, 256, 0, st>>>(na, parent);
   const int a1 = mark_lo ? c->edge_plane[0] : 0, b0 = mark_hi ? na - c->edge_plane[1] : na;
   if (a1 + (na - b0) > 0)
@@ -1319,12 +1275,12 @@ int lbm_get_macroscopic(lbm_ctx* c, double* rhoA, double* rhoB, double* ux, doub
   if (c->bits == 64) {
     launch_psi<double>(c, st);
     k_macroscopic<double><<<blocks(na, 256), 256, 0, st>>>(
-        (const double*)c->f[c->cur], (const Vec2<double>*)c->psi, c->nbr, (double*)m.p, na,
+        (const double*)c->f[c->cur], (const Vec2<double>*)c->psi, make_view(c), (double*)m.p, na,
         c->npad, make_consts<double>(c->p));
   } else {
     launch_psi<float>(c, st);
     k_macroscopic<float><<<blocks(na, 256), 256, 0, st>>>(
-        (const float*)c->f[c->cur], (const Vec2<float>*)c->psi, c->nbr, (double*)m.p, na,
+        (const float*)c->f[c->cur], (const Vec2<float>*)c->psi, make_view(c), (double*)m.p, na,
         c->npad, make_consts<float>(c->p));
   }
   }
@@ -1424,7 +1380,7 @@ int lbm_trapped_volume(lbm_ctx* c, int comp, int z0, int z1, long long* nodes, d
     k_ccl_init<double><<<g, 256, 0, st>>>((const Vec2<double>*)c->psi, nf, comp, parent, flag);
   else
     k_ccl_init<float><<<g, 256, 0, st>>>((const Vec2<float>*)c->psi, nf, comp, parent, flag);
-  k_ccl_unite<<<g, 256, 0, st>>>(c->nbr, nf, c->npad, parent);
+  k_ccl_unite<<<g, 256, 0, st>>>(make_view(c), nf, c->npad, parent);
   k_ccl_flatten<<<g, 256, 0, st>>>(nf, parent);
   const int a0 = c->zstart[0], a1 = c->zstart[1], b0 = c->zstart[nz - 1], b1 = c->zstart[nz];
   if ((a1 - a0) + (b1 - b0) > 0)
@@ -1502,7 +1458,7 @@ int lbm_trapped_volume_static(lbm_ctx* c, int comp, int z0, int z1, long long* n
     k_ccl_init<double><<<g, 256, 0, st>>>((const Vec2<double>*)c->psi, nf, comp, parent, flag);
   else
     k_ccl_init<float><<<g, 256, 0, st>>>((const Vec2<float>*)c->psi, nf, comp, parent, flag);
-  k_ccl_unite<<<g, 256, 0, st>>>(c->nbr, nf, c->npad, parent);
+  k_ccl_unite<<<g, 256, 0, st>>>(make_view(c), nf, c->npad, parent);
   k_ccl_flatten<<<g, 256, 0, st>>>(nf, parent);
   const int a0 = c->zstart[0], a1 = c->zstart[1], b0 = c->zstart[nz - 1], b1 = c->zstart[nz];
   if ((a1 - a0) + (b1 - b0) > 0)

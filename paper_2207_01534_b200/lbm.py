@@ -46,12 +46,9 @@ class lbm_params(C.Structure):
 
 
 class lbm_options(C.Structure):
-    _fields_ = [("index", C.c_int), ("graph", C.c_int), ("pdl", C.c_int), ("reverse", C.c_int),
+    _fields_ = [("graph", C.c_int), ("pdl", C.c_int), ("reverse", C.c_int),
                 ("keep_psi_mb", C.c_int)]
 
-
-LBM_INDEX_16, LBM_INDEX_BITS = 0, 1
-_INDEX = {"16": LBM_INDEX_16, "bits": LBM_INDEX_BITS}
 
 _lib = None
 
@@ -158,12 +155,10 @@ def make_params(p):
 
 def make_options(o=None):
     """dict -> lbm_options: the library's defaults (lbm_options_default) with the given fields
-    replaced; index may be "16" | "bits"."""
+    replaced."""
     s = lbm_options()
     load().lbm_options_default(C.byref(s))
     for k, v in (o or {}).items():
-        if k == "index" and isinstance(v, str):
-            v = _INDEX[v]
         if k not in dict(lbm_options._fields_):
             raise KeyError(f"unknown option {k!r}")
         setattr(s, k, int(v))
@@ -357,9 +352,8 @@ class Lbm:
     def step_info(self):
         v = (C.c_int * 8)()
         _chk(load().lbm_step_info(self._h, v), "lbm_step_info")
-        return {"index": {LBM_INDEX_16: "16", LBM_INDEX_BITS: "bits"}[v[0]], "graph": bool(v[1]),
-                "pdl": bool(v[2]), "reverse": bool(v[3]), "keep_psi": v[4] / 1000.0,
-                "wide_tiles": v[5], "wall_index": "bits" if v[6] else "lists"}
+        return {"graph": bool(v[1]), "pdl": bool(v[2]), "reverse": bool(v[3]),
+                "keep_psi": v[4] / 1000.0, "wide_tiles": v[5]}
 
     def sync(self):
         _chk(load().lbm_sync(self._h), "lbm_sync")

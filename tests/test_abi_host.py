@@ -165,18 +165,18 @@ def test_library_has_no_global_knobs():
 
 
 def test_options_struct_and_defaults():
-    assert C.sizeof(lbm.lbm_options) == 20
+    assert C.sizeof(lbm.lbm_options) == 16
     o = lbm.make_options()
-    assert (o.index, o.graph, o.pdl, o.reverse, o.keep_psi_mb) == (0, -1, 1, 1, 48)
-    o = lbm.make_options({"index": "bits", "graph": 0})
-    assert (o.index, o.graph) == (1, 0)
+    assert (o.graph, o.pdl, o.reverse, o.keep_psi_mb) == (-1, 1, 1, 48)
+    o = lbm.make_options({"reverse": 0, "graph": 0})
+    assert (o.reverse, o.graph) == (0, 0)
     with pytest.raises(KeyError):
         lbm.make_options({"tile": 1287})
     # bad option values are rejected before any device is needed
     h = C.c_void_p()
     m = np.zeros((4, 4, 4), np.uint8)
     ps = lbm.make_params(default_params())
-    for bad in ({"index": 5}, {"graph": 3}, {"pdl": 2}, {"keep_psi_mb": -1}):
+    for bad in ({"reverse": 5}, {"graph": 3}, {"pdl": 2}, {"keep_psi_mb": -1}):
         po = lbm.make_options(bad)
         rc = lbm.load().lbm_create_opt(C.byref(h), m.ctypes.data, 4, 4, 4, C.byref(ps), C.byref(po))
         assert rc == binding.LBM_EINVAL

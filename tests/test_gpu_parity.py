@@ -315,20 +315,18 @@ def test_velocity_inlet_on_component_b_and_extreme_parameters_fp64():
 
 @pytest.mark.parametrize("bits", [64, 32])
 def test_execution_options_are_bit_identical(bits):
-    """lbm_options select how the step is scheduled and which index form the fused pass reads --
-    never what is computed: the geometric (bitmask) index, forward tile order, no programmatic
-    dependent launch, no L2 priority for psi, CUDA-graph replay all give the default path's
-    populations bit for bit (fp64 and fp32 builds), and those match the oracle."""
+    """lbm_options select how the step is scheduled -- never what is computed: forward tile order,
+    no programmatic dependent launch, no L2 priority for psi, CUDA-graph replay all give the default
+    path's populations bit for bit (fp64 and fp32 builds), and those match the oracle."""
     c = make_config(3, size=32, storage_bits=bits)
     sims = {}
-    for name, opt in (("prod", None), ("bits", {"index": "bits"}), ("fwd", {"reverse": 0}),
+    for name, opt in (("prod", None), ("fwd", {"reverse": 0}),
                       ("nopdl", {"pdl": 0}), ("nokeep", {"keep_psi_mb": 0}), ("graph", {"graph": 1}),
                       ("nograph", {"graph": 0})):
         g = Lbm(c["mask"], c["params"], options=opt)
         g.set_density(c["rhoA"], c["rhoB"])
         g.step(30)
         info = g.step_info()
-        assert info["index"] == ("bits" if name == "bits" else "16")
         assert info["pdl"] == (name != "nopdl") and info["reverse"] == (name != "fwd")
         sims[name] = [g.get_populations(s) for s in (0, 1)]
         g.close()
@@ -347,7 +345,7 @@ def test_execution_options_are_bit_identical(bits):
 def test_options_are_validated():
     from paper_2207_01534_b200 import LbmError
     c = make_config(1, size=8)
-    for bad in ({"index": 7}, {"graph": 2}, {"pdl": 3}, {"reverse": -1}, {"keep_psi_mb": -5}):
+    for bad in ({"graph": 2}, {"pdl": 3}, {"reverse": -1}, {"keep_psi_mb": -5}):
         with pytest.raises(LbmError) as e:
             Lbm(c["mask"], c["params"], options=bad)
         assert e.value.code == -1
@@ -521,3 +519,31 @@ def test_neem_extrapolates_the_collision_operators_nonequilibrium_part_on_gpu():
         rho_f = f[dc][:, zf].sum(0)
         want = (rho_b / rho_f) * feq + f[dc][:, zf] - feq
         assert np.abs(f[dc][:, zb] - want).max() < 1e-14
+
+
+def test_getters_decode_the_tile_index_including_wide_tiles():
+    """lbm_get_macroscopic and the connected-component query read neighbour ids through the same
+    16-bit rows as the fused pass (no separate int32 table); tiles whose offsets do not fit 15 bits
+    ("wide": periodic wraps inside a tile) read the compact wide-tile table.  Forces, hence
+    velocities, see every neighbour id: fp64 fields against the oracle on boxes made of wide
+    tiles, after a few steps."""
+    rng = np.random.Generator(np.random.PCG64(77))
+    wide_seen = 0
+    for shape, solid in (((1, 40, 41), 0.2), ((3, 1, 5), 0.0), ((2, 2, 2), 0.0), ((40, 40, 40), 0.35),
+                         ((6, 300, 7), 0.3)):
+        mask = (rng.uniform(size=shape) < solid).astype(np.uint8)
+        rA = rng.uniform(0.1, 1.0, shape)
+        rB = rng.uniform(0.1, 1.0, shape)
+        p = default_params(G=1.5, tau=(1.0, 0.8), xi=0.2, accel=(1e-5, 0, 2e-5), storage_bits=64)
+        o, g = LbmRef(mask, p), Lbm(mask, p)
+        for s in (o, g):
+            s.set_density(rA, rB)
+            s.step(3)
+        wide_seen += g.step_info()["wide_tiles"]
+        mo, mg = o.get_macroscopic(), g.get_macroscopic()
+        for k in ("rhoA", "rhoB", "ux", "uy", "uz", "P"):
+            assert np.max(np.abs(mg[k] - mo[k])) < 1e-12, (shape, k)
+        for comp in (0, 1):
+            assert g.trapped_volume(comp)[0] == o.trapped_volume(comp)[0]
+        g.close()
+    assert wide_seen > 0

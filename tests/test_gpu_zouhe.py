@@ -96,8 +96,8 @@ def test_zou_he_properties_through_the_cuda_path():
 
 
 def test_zou_he_all_step_paths_agree():
-    """The geometric index, forward tile order, graph replay and plain launches run the same
-    arithmetic as the default path (bit-identical).  All share the open-plane code."""
+    """Forward tile order, graph replay and plain launches run the same arithmetic as the default
+    path (bit-identical).  All share the open-plane code."""
     c = make_config(4, size=40, storage_bits=64)
     p = dict(c["params"], inlet_kind=3, outlet_kind=3)
 
@@ -110,7 +110,7 @@ def test_zou_he_all_step_paths_agree():
         return f
 
     base = run()
-    for opt in ({"index": "bits"}, {"reverse": 0}, {"graph": 1}, {"graph": 0, "pdl": 0}):
+    for opt in ({"reverse": 0}, {"graph": 1}, {"graph": 0, "pdl": 0}):
         other = run(opt)
         for s in (0, 1):
             assert np.array_equal(base[s], other[s]), opt
